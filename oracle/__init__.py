@@ -1,0 +1,131 @@
+"""oracle -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+ctypes front end to ``gemm_oracle.c``: the plain fp64 CPU statement of
+``C = A @ B`` (Listing 2) used to judge the CUDA path.
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s
+``cpu_baseline`` / ``--impl reference`` legs may import this package.  It
+imports nothing from ``paper_2606_15991_b200`` and that package imports
+nothing from here.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "gemm_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle_gemm.so")
+_lib = None
+
+_i64 = ctypes.c_int64
+_u16p = ctypes.POINTER(ctypes.c_uint16)
+_f64p = ctypes.POINTER(ctypes.c_double)
+_f32p = ctypes.POINTER(ctypes.c_float)
+_i64p = ctypes.POINTER(ctypes.c_int64)
+
+
+def build(force: bool = False) -> str:
+    """Compile gemm_oracle.c with gcc (x86-64-v3: runs on any AVX2 host)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O3", "-march=x86-64-v3", "-std=c11", "-fPIC", "-shared",
+               "-pthread", "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True, cwd=_HERE)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        lib.oracle_gemm.restype = ctypes.c_int
+        lib.oracle_gemm.argtypes = [_u16p, _u16p, _f64p, _f64p, _i64, _i64, _i64, _i64, _i64,
+                                    _i64, ctypes.c_int, _i64, _i64, _i64]
+        lib.oracle_gemm_sampled.restype = ctypes.c_int
+        lib.oracle_gemm_sampled.argtypes = [_u16p, _u16p, _i64p, _i64p, _i64, _f64p, _f64p,
+                                            _i64, _i64, _i64, _i64, _i64]
+        lib.oracle_bf16_decode_array.restype = None
+        lib.oracle_bf16_decode_array.argtypes = [_u16p, _f64p, _i64]
+        lib.oracle_bf16_encode_array.restype = None
+        lib.oracle_bf16_encode_array.argtypes = [_f32p, _u16p, _i64]
+        _lib = lib
+    return _lib
+
+
+def default_threads() -> int:
+    return max(1, len(os.sched_getaffinity(0)))
+
+
+def _as_u16_2d(x, name):
+    x = np.asarray(x)
+    if x.dtype != np.uint16 or x.ndim != 2:
+        raise TypeError(f"{name} must be a 2-D uint16 array of bf16 bit patterns")
+    if x.strides[1] != 2 or x.strides[0] % 2 or x.strides[0] < 2 * x.shape[1]:
+        x = np.ascontiguousarray(x)
+    return x
+
+
+def gemm(A, B, threads: int | None = None, blocks=(0, 0, 0)):
+    """Full fp64 GEMM.  A: (M,K) uint16 bf16 bits, B: (K,N).  Row strides are
+    taken from the arrays (padded leading dimensions are honoured).
+    Returns (C, S) float64 (M,N): C = A@B and S = |A|@|B|."""
+    A = _as_u16_2d(A, "A")
+    B = _as_u16_2d(B, "B")
+    M, K = A.shape
+    K2, N = B.shape
+    if K != K2:
+        raise ValueError("inner dimensions differ")
+    C = np.empty((M, N), dtype=np.float64)
+    S = np.empty((M, N), dtype=np.float64)
+    lda = A.strides[0] // 2 if M > 1 else max(K, 1)
+    ldb = B.strides[0] // 2 if K > 1 else max(N, 1)
+    lda, ldb = max(lda, K), max(ldb, N)
+    rc = _load().oracle_gemm(A.ctypes.data_as(_u16p), B.ctypes.data_as(_u16p),
+                             C.ctypes.data_as(_f64p), S.ctypes.data_as(_f64p),
+                             M, N, K, lda, ldb, max(N, 1),
+                             default_threads() if threads is None else int(threads),
+                             int(blocks[0]), int(blocks[1]), int(blocks[2]))
+    if rc != 0:
+        raise RuntimeError(f"oracle_gemm failed ({rc})")
+    return C, S
+
+
+def gemm_sampled(A, B, rows, cols):
+    """Dot products for the listed output elements: returns (c, s) float64."""
+    A = _as_u16_2d(A, "A")
+    B = _as_u16_2d(B, "B")
+    M, K = A.shape
+    _, N = B.shape
+    rows = np.ascontiguousarray(rows, dtype=np.int64)
+    cols = np.ascontiguousarray(cols, dtype=np.int64)
+    n = rows.shape[0]
+    c = np.empty(n, dtype=np.float64)
+    s = np.empty(n, dtype=np.float64)
+    lda = max(A.strides[0] // 2 if M > 1 else K, K)
+    ldb = max(B.strides[0] // 2 if K > 1 else N, N)
+    rc = _load().oracle_gemm_sampled(A.ctypes.data_as(_u16p), B.ctypes.data_as(_u16p),
+                                     rows.ctypes.data_as(_i64p), cols.ctypes.data_as(_i64p), n,
+                                     c.ctypes.data_as(_f64p), s.ctypes.data_as(_f64p),
+                                     M, N, K, lda, ldb)
+    if rc != 0:
+        raise RuntimeError(f"oracle_gemm_sampled failed ({rc})")
+    return c, s
+
+
+def bf16_decode(bits):
+    """uint16 bf16 bit patterns -> float64 values (exact)."""
+    bits = np.ascontiguousarray(bits, dtype=np.uint16)
+    out = np.empty(bits.shape, dtype=np.float64)
+    _load().oracle_bf16_decode_array(bits.ctypes.data_as(_u16p), out.ctypes.data_as(_f64p), bits.size)
+    return out
+
+
+def bf16_encode(x):
+    """float32 -> uint16 bf16 bit patterns, round to nearest even."""
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    out = np.empty(x.shape, dtype=np.uint16)
+    _load().oracle_bf16_encode_array(x.ctypes.data_as(_f32p), out.ctypes.data_as(_u16p), x.size)
+    return out
