@@ -1,0 +1,170 @@
+/*
+ * tile_gemm.h -- C ABI of libtilegemm.so: dense BF16 GEMM  C = A * B  with fp32
+ * accumulation on one NVIDIA B200 (sm_100a), plus its M=1 decode GEMV and the
+ * shape selector between them.
+ *
+ * Operation (Listing 2 "gemm_persistent"): z = x * y where z is
+ * split into disjoint output tiles, each owned by exactly one tile program at a
+ * time, x and y are shared read-only, the accumulator starts
+ * at zero, all K tiles are summed and each
+ * tile is stored once.  Edge tiles are legal: loads past the
+ * tensor read as zero and stores past it are masked.  Every
+ * shape / stride / pointer check is a *launch precondition*: it runs once at
+ * this host entry before any work is queued and returns an error with its own
+ * message; the device K loop contains no checks.
+ *
+ *     C[i*ldc + j] = round_out( sum_{k<K} A[i*lda + k] * B[k*ldb + j] )
+ *
+ * alpha = 1, beta = 0 (C is never read).  A is M x K and B is K x N, both
+ * row-major bf16 (raw 16-bit patterns); products are exact, sums are carried in
+ * fp32 in an unspecified but fixed order (results are bitwise reproducible run
+ * to run for a given shape); round_out is identity for fp32 output and
+ * round-to-nearest-even for bf16 output.  Only C[0..M) x [0..N) is written;
+ * padding columns (j >= N when ldc > N) and everything else stay untouched.
+ *
+ * Conventions for every entry point below
+ *   - lda, ldb, ldc are row strides in ELEMENTS (not bytes).
+ *   - A, B, C are DEVICE pointers on the current CUDA device unless the entry
+ *     says "host".  The caller owns them; the library keeps no reference after
+ *     the work completes.  Calls are asynchronous: they return after enqueueing
+ *     on `stream` (a cudaStream_t passed as void*; NULL = legacy default stream)
+ *     and never synchronise; buffers must stay valid until the stream reaches
+ *     the work.  Internal state: a per-stream grow-only repack workspace and a
+ *     tensor-map cache, both released by tile_gemm_shutdown().
+ *   - Return value 0 = success; otherwise a TILE_GEMM_E_* code.  On any error
+ *     nothing is enqueued and C is untouched.  tile_gemm_last_error() holds the
+ *     detailed message of the calling thread's last failure.
+ *   - No CPU fallback exists: on a machine without an sm_100 device compute
+ *     entries fail with TILE_GEMM_E_DEVICE.
+ *   - Degenerate extents (reading c8): M == 0 or N == 0 is a
+ *     successful no-op; K == 0 writes zeros to C[0..M) x [0..N).
+ *   - Base-pointer / stride alignment to 16 bytes is NOT a precondition: rows
+ *     that TMA cannot address are first copied into an aligned workspace
+ *     (TILE_GEMM_PATH_GEMM_REPACK) and misaligned C is written with clipped
+ *     st.global stores from the epilogue.
+ */
+#ifndef TILE_GEMM_H_
+#define TILE_GEMM_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* out_dtype */
+#define TILE_GEMM_OUT_F32 0
+#define TILE_GEMM_OUT_BF16 1
+
+/* status codes */
+#define TILE_GEMM_OK 0
+#define TILE_GEMM_E_NULL 1        /* NULL A/B/C with a non-empty extent                    */
+#define TILE_GEMM_E_EXTENT 2      /* negative M, N or K                                    */
+#define TILE_GEMM_E_LDA 3         /* lda < K                                               */
+#define TILE_GEMM_E_LDB 4         /* ldb < N                                               */
+#define TILE_GEMM_E_LDC 5         /* ldc < N                                               */
+#define TILE_GEMM_E_DTYPE 6       /* out_dtype is neither F32 nor BF16                     */
+#define TILE_GEMM_E_ALIGN 7       /* A/B not 2-byte aligned, or C not element aligned      */
+#define TILE_GEMM_E_ALIAS 8       /* C's byte range overlaps A's or B's      */
+#define TILE_GEMM_E_OVERFLOW 9    /* byte offsets overflow int64 or tile counts int32      */
+#define TILE_GEMM_E_DEVICE 10     /* no CUDA device, or the device is not sm_100           */
+#define TILE_GEMM_E_CUDA 11       /* a CUDA runtime/driver call failed (code in message)   */
+#define TILE_GEMM_E_PATH 12       /* force_path unknown or not applicable to this shape    */
+#define TILE_GEMM_E_INTERNAL 13
+#define TILE_GEMM_NUM_STATUS 14
+
+/* execution paths (what the selector returns / what force_path accepts) */
+#define TILE_GEMM_PATH_AUTO 0         /* force_path only                                      */
+#define TILE_GEMM_PATH_GEMM_TMA 1     /* tcgen05 GEMM, A and B read in place through TMA      */
+#define TILE_GEMM_PATH_GEMM_REPACK 2  /* same kernel after copying A and/or B to aligned rows */
+#define TILE_GEMM_PATH_GEMV 3         /* M == 1 HBM-bound weight-streaming kernel             */
+#define TILE_GEMM_PATH_ZERO 4         /* K == 0: C <- 0                                       */
+#define TILE_GEMM_PATH_NOOP 5         /* M == 0 or N == 0                                     */
+
+/*
+ * The GEMM (Listing 2).  Validates, selects a path
+ * (tile_gemm_select) and enqueues it on `stream`.
+ */
+int tile_gemm(const void* A, const void* B, void* C,
+              int64_t M, int64_t N, int64_t K,
+              int64_t lda, int64_t ldb, int64_t ldc,
+              int out_dtype, void* stream);
+
+/*
+ * Same, with the path forced (tests / measurements): TILE_GEMM_PATH_AUTO,
+ * _GEMM_TMA (fails with E_PATH when A or B is not TMA-addressable), _GEMM_REPACK
+ * (always legal for K > 0) or _GEMV (requires M == 1).
+ */
+int tile_gemm_ex(const void* A, const void* B, void* C,
+                 int64_t M, int64_t N, int64_t K,
+                 int64_t lda, int64_t ldb, int64_t ldc,
+                 int out_dtype, void* stream, int force_path);
+
+/*
+ * Launch preconditions + shape selector as a pure host function (PAPER.md:200:
+ * "runs once per launch before any work is queued"; tile shapes
+ * chosen per size).  Never dereferences A/B/C and makes no CUDA call.
+ * Returns the TILE_GEMM_PATH_* the auto selector takes (> 0), or the NEGATED
+ * status code (-TILE_GEMM_E_*) when a precondition fails.
+ */
+int tile_gemm_select(int64_t M, int64_t N, int64_t K,
+                     int64_t lda, int64_t ldb, int64_t ldc,
+                     const void* A, const void* B, const void* C, int out_dtype);
+
+/*
+ * End-to-end convenience entry on HOST buffers (pageable or pinned): copies A
+ * and B to the device, runs tile_gemm, copies C[0..M) x [0..N) back (row pitch
+ * ldc) and synchronises before returning.  Device staging buffers are grow-only
+ * and owned by the library.  This is the call bench.py's `e2e` figure times.
+ */
+int tile_gemm_host(const void* A_host, const void* B_host, void* C_host,
+                   int64_t M, int64_t N, int64_t K,
+                   int64_t lda, int64_t ldb, int64_t ldc, int out_dtype);
+
+/*
+ * Debug: run the GEMM kernel's own persistent schedule and epilogue (no loads,
+ * no MMAs) and write, for every element of an M x N int32 matrix `owner`
+ * (device, row stride ld_owner), the value (tile_index << 8) | cta_index of the
+ * CTA that owns the element's output tile.  "Each sub-tensor has exactly one
+ * owner": tests check the map is the documented function and
+ * covers [0,M) x [0,N) exactly once.  K only selects the tile configuration.
+ */
+int tile_gemm_debug_owner_map(int32_t* owner, int64_t M, int64_t N, int64_t K,
+                              int64_t ld_owner, int out_dtype, void* stream);
+
+/*
+ * Describes the tile configuration the GEMM path uses for a shape, so that a
+ * host program can rebuild the owner map: out[0]=BM (rows per CTA),
+ * out[1]=BN (columns per tile), out[2]=cta_group (1 or 2: CTAs per tile, tile
+ * rows = BM*cta_group), out[3]=number of CTAs launched, out[4]=GROUP_M (tile
+ * rows per raster group), out[5]=pipeline stages, out[6]=BK, out[7]=reserved.
+ * Needs a CUDA device (SM count).  Returns a status code.
+ */
+int tile_gemm_query_config(int64_t M, int64_t N, int64_t K, int out_dtype, int32_t out[8]);
+
+/*
+ * Tuning / test overrides, process-global, not thread-safe against concurrent
+ * tile_gemm calls.  key: 0 = GEMM config (0 auto, 1 = 1-CTA 128x128, 2 = 1-CTA
+ * 128x256, 3 = 2-CTA 256x256), 1 = GEMM GROUP_M (0 auto), 2 = GEMM max CTAs
+ * (0 = all SMs), 3 = GEMV split-K (0 auto), 4 = GEMV columns-per-CTA selector
+ * (0 auto), 5 = reserved.  Returns 0 or E_PATH for an unknown key.
+ */
+int tile_gemm_set_tuning(int key, int value);
+
+/* Number of kernels this library has launched in this process (all paths). */
+int64_t tile_gemm_launch_count(void);
+
+/* Static, human-readable name of a status code. */
+const char* tile_gemm_status_string(int status);
+
+/* Thread-local detailed message of the calling thread's last failing call. */
+const char* tile_gemm_last_error(void);
+
+/* Frees workspaces, staging buffers and the tensor-map cache.  The caller must
+ * have synchronised all streams that ran library work. */
+int tile_gemm_shutdown(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TILE_GEMM_H_ */

@@ -14,6 +14,7 @@ def __getattr__(name):
     # the CUDA library has not been built (e.g. the oracle's CPU tests).
     if name == "binding" or name.startswith("tile_gemm") or name in (
         "TileGemmError", "load_library", "PATH_NAMES", "OUT_F32", "OUT_BF16"):
-        from . import binding as _b
+        import importlib
+        _b = importlib.import_module(__name__ + ".binding")
         return _b if name == "binding" else getattr(_b, name)
     raise AttributeError(name)

@@ -1,0 +1,222 @@
+"""ctypes binding of libtilegemm.so (include/tile_gemm.h) -- argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels.  There is no CPU
+fallback: if the shared library cannot be found or built, ``load_library``
+raises, and on a machine without an sm_100 device every compute entry returns
+``TILE_GEMM_E_DEVICE`` which is raised as ``TileGemmError``.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+from . import build as _build
+
+OUT_F32 = 0
+OUT_BF16 = 1
+
+PATH_AUTO, PATH_GEMM_TMA, PATH_GEMM_REPACK, PATH_GEMV, PATH_ZERO, PATH_NOOP = range(6)
+PATH_NAMES = {PATH_AUTO: "auto", PATH_GEMM_TMA: "gemm_tma", PATH_GEMM_REPACK: "gemm_repack",
+              PATH_GEMV: "gemv", PATH_ZERO: "zero", PATH_NOOP: "noop"}
+
+(E_OK, E_NULL, E_EXTENT, E_LDA, E_LDB, E_LDC, E_DTYPE, E_ALIGN, E_ALIAS, E_OVERFLOW, E_DEVICE,
+ E_CUDA, E_PATH, E_INTERNAL) = range(14)
+
+TUNE_GEMM_CONFIG, TUNE_GEMM_GROUP_M, TUNE_GEMM_MAX_CTAS, TUNE_GEMV_SPLIT, TUNE_GEMV_VARIANT = range(5)
+
+EXPORTS = ("tile_gemm", "tile_gemm_ex", "tile_gemm_select", "tile_gemm_host",
+           "tile_gemm_debug_owner_map", "tile_gemm_query_config", "tile_gemm_set_tuning",
+           "tile_gemm_launch_count", "tile_gemm_status_string", "tile_gemm_last_error",
+           "tile_gemm_shutdown")
+
+_lib = None
+_i64 = ctypes.c_int64
+_vp = ctypes.c_void_p
+_int = ctypes.c_int
+
+
+class TileGemmError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"tile_gemm status {status}: {message}")
+        self.status = status
+        self.message = message
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def load_library():
+    """Loads (building first if the in-tree .so is missing or stale and nvcc exists)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if not os.path.exists(path) or _build.needs_build():
+        try:
+            _build.build()
+        except Exception as exc:  # no nvcc here and no prebuilt library: fail loudly
+            if not os.path.exists(path):
+                raise RuntimeError(
+                    f"libtilegemm.so is missing and could not be built ({exc}); "
+                    "the CUDA path has no fallback") from exc
+    lib = ctypes.CDLL(path)
+    g = [_vp, _vp, _vp, _i64, _i64, _i64, _i64, _i64, _i64, _int]
+    lib.tile_gemm.argtypes = g + [_vp]
+    lib.tile_gemm.restype = _int
+    lib.tile_gemm_ex.argtypes = g + [_vp, _int]
+    lib.tile_gemm_ex.restype = _int
+    lib.tile_gemm_select.argtypes = [_i64] * 6 + [_vp, _vp, _vp, _int]
+    lib.tile_gemm_select.restype = _int
+    lib.tile_gemm_host.argtypes = g
+    lib.tile_gemm_host.restype = _int
+    lib.tile_gemm_debug_owner_map.argtypes = [_vp, _i64, _i64, _i64, _i64, _int, _vp]
+    lib.tile_gemm_debug_owner_map.restype = _int
+    lib.tile_gemm_query_config.argtypes = [_i64, _i64, _i64, _int, ctypes.POINTER(ctypes.c_int32)]
+    lib.tile_gemm_query_config.restype = _int
+    lib.tile_gemm_set_tuning.argtypes = [_int, _int]
+    lib.tile_gemm_set_tuning.restype = _int
+    lib.tile_gemm_launch_count.argtypes = []
+    lib.tile_gemm_launch_count.restype = _i64
+    lib.tile_gemm_status_string.argtypes = [_int]
+    lib.tile_gemm_status_string.restype = ctypes.c_char_p
+    lib.tile_gemm_last_error.argtypes = []
+    lib.tile_gemm_last_error.restype = ctypes.c_char_p
+    lib.tile_gemm_shutdown.argtypes = []
+    lib.tile_gemm_shutdown.restype = _int
+    _lib = lib
+    return lib
+
+
+def _check(status: int):
+    if status != 0:
+        raise TileGemmError(status, tile_gemm_last_error())
+
+
+def _stream_handle(stream) -> int:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream) if hasattr(stream, "cuda_stream") else int(stream)
+
+
+def _ld(t: torch.Tensor) -> int:
+    if t.dim() != 2 or (t.shape[1] > 1 and t.stride(1) != 1):
+        raise ValueError("expected a 2-D row-major tensor (unit column stride)")
+    return int(t.stride(0)) if t.shape[0] > 1 else max(int(t.stride(0)), int(t.shape[1]), 1)
+
+
+def tile_gemm_status_string(status: int) -> str:
+    return load_library().tile_gemm_status_string(int(status)).decode()
+
+
+def tile_gemm_last_error() -> str:
+    return load_library().tile_gemm_last_error().decode()
+
+
+def tile_gemm_launch_count() -> int:
+    return int(load_library().tile_gemm_launch_count())
+
+
+def tile_gemm_set_tuning(key: int, value: int) -> None:
+    _check(load_library().tile_gemm_set_tuning(int(key), int(value)))
+
+
+def tile_gemm_shutdown() -> None:
+    _check(load_library().tile_gemm_shutdown())
+
+
+def tile_gemm_raw(A: int, B: int, C: int, M, N, K, lda, ldb, ldc, out_dtype, stream: int = 0,
+                  force_path: int = PATH_AUTO) -> int:
+    """Raw pointer form; returns the status code instead of raising."""
+    return int(load_library().tile_gemm_ex(_vp(A), _vp(B), _vp(C), M, N, K, lda, ldb, ldc,
+                                           int(out_dtype), _vp(stream), int(force_path)))
+
+
+def tile_gemm_select(M, N, K, lda, ldb, ldc, A: int = 256, B: int = 1 << 40, C: int = 1 << 41,
+                     out_dtype: int = OUT_F32) -> int:
+    """Pure host: path id (> 0) or the negated status of the failing precondition."""
+    return int(load_library().tile_gemm_select(M, N, K, lda, ldb, ldc, _vp(A), _vp(B), _vp(C), int(out_dtype)))
+
+
+def tile_gemm(A: torch.Tensor, B: torch.Tensor, C: torch.Tensor | None = None, out_dtype=None,
+              stream=None, force_path: int = PATH_AUTO) -> torch.Tensor:
+    """C = A @ B on the current CUDA device.  A: (M,K) bf16, B: (K,N) bf16, row-major (any row
+    stride); C: (M,N) fp32 or bf16, allocated if None.  Asynchronous on `stream`."""
+    if A.dtype != torch.bfloat16 or B.dtype != torch.bfloat16:
+        raise TypeError("A and B must be torch.bfloat16")
+    M, K = A.shape
+    K2, N = B.shape
+    if K != K2:
+        raise ValueError("inner dimensions differ")
+    if C is None:
+        dt = torch.float32 if out_dtype in (None, OUT_F32, torch.float32) else torch.bfloat16
+        C = torch.empty((M, N), dtype=dt, device=A.device)
+    if C.dtype not in (torch.float32, torch.bfloat16) or tuple(C.shape) != (M, N):
+        raise TypeError("C must be an (M,N) float32 or bfloat16 tensor")
+    od = OUT_F32 if C.dtype == torch.float32 else OUT_BF16
+    st = load_library().tile_gemm_ex(_vp(A.data_ptr()), _vp(B.data_ptr()), _vp(C.data_ptr()), M, N, K,
+                                     _ld(A), _ld(B), _ld(C), od, _vp(_stream_handle(stream)),
+                                     int(force_path))
+    _check(st)
+    return C
+
+
+def tile_gemm_host(A_bits, B_bits, C_out, lda=None, ldb=None, ldc=None):
+    """End-to-end on HOST numpy arrays: A_bits (M,K) uint16, B_bits (K,N) uint16 bf16 patterns,
+    C_out (M,N) float32 or uint16 (bf16 patterns), all C-contiguous rows."""
+    import numpy as np
+    M, K = A_bits.shape
+    _, N = B_bits.shape
+    od = OUT_F32 if C_out.dtype == np.float32 else OUT_BF16
+    lda = lda or max(A_bits.strides[0] // 2, K, 1)
+    ldb = ldb or max(B_bits.strides[0] // 2, N, 1)
+    ldc = ldc or max(C_out.strides[0] // C_out.itemsize, N, 1)
+    st = load_library().tile_gemm_host(_vp(A_bits.ctypes.data), _vp(B_bits.ctypes.data), _vp(C_out.ctypes.data),
+                                       M, N, K, lda, ldb, ldc, od)
+    _check(st)
+    return C_out
+
+
+def tile_gemm_host_raw(A: int, B: int, C: int, M, N, K, lda, ldb, ldc, out_dtype) -> int:
+    return int(load_library().tile_gemm_host(_vp(A), _vp(B), _vp(C), M, N, K, lda, ldb, ldc, int(out_dtype)))
+
+
+def tile_gemm_query_config(M, N, K, out_dtype=OUT_F32) -> dict:
+    out = (ctypes.c_int32 * 8)()
+    _check(load_library().tile_gemm_query_config(M, N, K, int(out_dtype), out))
+    return {"BM": out[0], "BN": out[1], "cta_group": out[2], "ctas": out[3], "group_m": out[4],
+            "stages": out[5], "BK": out[6]}
+
+
+def tile_gemm_debug_owner_map(M, N, K, out_dtype=OUT_F32, ld_owner=None, stream=None, device="cuda"):
+    ld = int(ld_owner or N)
+    owner = torch.full((M, ld), -1, dtype=torch.int32, device=device)
+    _check(load_library().tile_gemm_debug_owner_map(_vp(owner.data_ptr()), M, N, K, ld, int(out_dtype),
+                                                    _vp(_stream_handle(stream))))
+    return owner
+
+
+def expected_owner_map(M, N, cfg: dict):
+    """Host restatement of the kernel's tile -> owner function (csrc/gemm_kernel.cuh,
+    tile_coords + round-robin over clusters) for the owner-map test."""
+    import numpy as np
+    tile_m = cfg["BM"] * cfg["cta_group"]
+    tiles_m = -(-M // tile_m)
+    tiles_n = -(-N // cfg["BN"])
+    clusters = cfg["ctas"] // cfg["cta_group"]
+    own = np.full((M, N), -1, dtype=np.int64)
+    for t in range(tiles_m * tiles_n):
+        per_group = cfg["group_m"] * tiles_n
+        g = t // per_group
+        first_m = g * cfg["group_m"]
+        rows = min(cfg["group_m"], tiles_m - first_m)
+        r = t - g * per_group
+        tm, tn = first_m + r % rows, r // rows
+        cluster = t % clusters
+        for rank in range(cfg["cta_group"]):
+            cta = cluster * cfg["cta_group"] + rank
+            r0 = (tm * cfg["cta_group"] + rank) * cfg["BM"]
+            own[r0:r0 + cfg["BM"], tn * cfg["BN"]:(tn + 1) * cfg["BN"]] = (t << 8) | cta
+    return own

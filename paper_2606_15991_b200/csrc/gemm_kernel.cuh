@@ -1,0 +1,327 @@
+// Persistent, warp-specialised tcgen05 GEMM for sm_100a:  C = A * B, bf16 in, fp32 accumulate.
+//
+// What it computes: Listing 2 of the paper -- for each owned output tile,
+// zero accumulator, sum over all K tiles of mma(x[bid_m,k], y[k,bid_n]), one store.  The
+// schedule below is this build's own (the paper's tile shapes are not printed):
+//
+//   * one CTA (CG=1) or one CTA pair (CG=2, cta_group::2) owns exactly one output tile at a
+//     time; tile -> owner is the pure function `tile_coords` + round-robin over clusters
+//     ("each sub-tensor has exactly one owner");
+//   * warp 0 : TMA producer  -- A box 64(k) x 128(m), B boxes 64(n) x 64(k), 128B swizzle,
+//              out-of-bounds elements arrive as zeros (edge tiles), so the K loop
+//              carries no bounds checks at all;
+//   * warp 1 : MMA issuer    -- one thread, tcgen05.mma kind::f16 (bf16 x bf16 -> fp32 in TMEM),
+//              A K-major, B MN-major (row-major K x N), tcgen05.commit frees smem stages;
+//   * warp 2 : TMEM allocator (2 accumulator stages of BN columns);
+//   * warps 4-7: epilogue    -- tcgen05.ld TMEM -> registers -> (fp32 | RNE bf16) -> swizzled smem
+//              -> TMA store (clipped at M,N by the tensor map) or, when C is not 16-byte
+//              addressable, clipped st.global from the staged tile.
+//   The accumulator is double buffered so tile i's epilogue overlaps tile i+1's main loop.
+#pragma once
+#include "ptx.cuh"
+
+namespace tg {
+
+constexpr int GEMM_BM = 128;      // rows per CTA (UMMA M = 128 * CG)
+constexpr int GEMM_BK = 64;       // one 128-byte swizzle row of bf16
+constexpr int GEMM_UMMA_K = 16;   // K per tcgen05.mma for 16-bit inputs
+constexpr int GEMM_THREADS = 256;
+constexpr int GEMM_EPI_WARP0 = 4;
+constexpr uint32_t GEMM_EPI_BUF_BYTES = 32 * 128;   // 32 rows x 128 B per warp per buffer
+
+struct GemmParams {
+    int32_t M, N, K;
+    int32_t tiles_m, tiles_n;   // tile grid; a tile is (GEMM_BM*CG) x BN
+    int32_t group_m;            // raster group height in tiles
+    int32_t num_k_tiles;
+    int32_t out_bf16;           // 0: fp32 C, 1: bf16 C
+    int32_t tma_store;          // 1: TMA store, 0: clipped st.global
+    int32_t owner_mode;         // debug: write (tile << 8 | cta) instead of values
+    void* C;
+    int64_t ldc;                // elements
+};
+
+// Tile index -> tile coordinates.  Grouped raster: tiles are numbered down the rows of a
+// group of `group_m` tile rows, then across columns, so that concurrently running tiles share
+// A row panels and B column panels in L2.  Pure function, also evaluated on the host.
+__host__ __device__ __forceinline__ void tile_coords(int t, int tiles_m, int tiles_n, int group_m, int& tm,
+                                                     int& tn) {
+    const int per_group = group_m * tiles_n;
+    const int g = t / per_group;
+    const int first_m = g * group_m;
+    const int rows = (tiles_m - first_m) < group_m ? (tiles_m - first_m) : group_m;
+    const int r = t - g * per_group;
+    tm = first_m + r % rows;
+    tn = r / rows;
+}
+
+template <int CG, int BN, int STAGES>
+struct GemmSmem {
+    static constexpr uint32_t A_BYTES = GEMM_BM * GEMM_BK * 2;
+    static constexpr uint32_t B_COLS = BN / CG;                 // B columns loaded by each CTA
+    static constexpr uint32_t B_BOXES = B_COLS / 64;
+    static constexpr uint32_t B_BOX_BYTES = 64 * GEMM_BK * 2;   // 64 k-rows x 128 B
+    static constexpr uint32_t B_BYTES = B_BOXES * B_BOX_BYTES;
+    static constexpr uint32_t STAGE_BYTES = A_BYTES + B_BYTES;
+    static constexpr uint32_t EPI_OFF = STAGES * STAGE_BYTES;
+    static constexpr uint32_t EPI_BYTES = 4 * 2 * GEMM_EPI_BUF_BYTES;
+    static constexpr uint32_t BAR_OFF = EPI_OFF + EPI_BYTES;
+    static constexpr uint32_t NUM_BARS = 2 * STAGES + 4;
+    static constexpr uint32_t TMEM_PTR_OFF = BAR_OFF + NUM_BARS * 8;
+    static constexpr uint32_t TOTAL = TMEM_PTR_OFF + 16 + 1024;   // + slack for 1024 B alignment
+};
+
+template <int CG, int BN, int STAGES>
+__global__ void __launch_bounds__(GEMM_THREADS, 1)
+gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b,
+                    const __grid_constant__ CUtensorMap tmap_c, const GemmParams p) {
+    using L = GemmSmem<CG, BN, STAGES>;
+    static_assert(CG == 1 || CG == 2, "cta_group is 1 or 2");
+    static_assert(BN == 128 || BN == 256, "accumulator width");
+    static_assert(L::TOTAL <= 232448, "exceeds 227 KB of shared memory");
+
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
+
+    const uint32_t warp = threadIdx.x >> 5;
+    const uint32_t lane = threadIdx.x & 31;
+    const uint32_t rank = (CG == 2) ? cluster_ctarank() : 0u;
+    const int first_tile = (CG == 2) ? (int)cluster_id_x() : (int)blockIdx.x;
+    const int tile_stride = (CG == 2) ? (int)num_clusters_x() : (int)gridDim.x;
+    const int total_tiles = p.tiles_m * p.tiles_n;
+
+    const uint32_t bar_base = smem_base + L::BAR_OFF;
+    auto full_bar = [&](uint32_t s) { return bar_base + s * 8u; };
+    auto empty_bar = [&](uint32_t s) { return bar_base + (STAGES + s) * 8u; };
+    auto tmem_full_bar = [&](uint32_t a) { return bar_base + (2 * STAGES + a) * 8u; };
+    auto tmem_empty_bar = [&](uint32_t a) { return bar_base + (2 * STAGES + 2 + a) * 8u; };
+    volatile uint32_t* tmem_ptr_gen = reinterpret_cast<volatile uint32_t*>(smem_gen + L::TMEM_PTR_OFF);
+
+    // ------------------------------------------------------------------ one-time setup
+    if (warp == 0 && elect_one()) {
+        prefetch_tmap(&tmap_a);
+        prefetch_tmap(&tmap_b);
+        prefetch_tmap(&tmap_c);
+    }
+    if (warp == 1 && elect_one()) {
+        for (uint32_t s = 0; s < STAGES; ++s) {
+            mbar_init(full_bar(s), 1);    // producer's arrive.expect_tx (+ TMA transaction bytes)
+            mbar_init(empty_bar(s), 1);   // one tcgen05.commit
+        }
+        for (uint32_t a = 0; a < 2; ++a) {
+            mbar_init(tmem_full_bar(a), 1);           // one tcgen05.commit
+            mbar_init(tmem_empty_bar(a), 4 * CG);     // lane 0 of every epilogue warp of the pair
+        }
+        fence_mbar_init();
+    }
+    if (warp == 2) {
+        tmem_alloc<CG>(smem_base + L::TMEM_PTR_OFF, 2 * BN);
+        tmem_relinquish<CG>();
+    }
+    tc_fence_before();
+    if constexpr (CG == 2) cluster_sync(); else __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_ptr_gen;
+
+    // ------------------------------------------------------------------ warp roles
+    if (warp == 0) {
+        // ===== TMA producer (one lane) =====
+        if (elect_one()) {
+            uint32_t stage = 0, phase = 0;
+            for (int t = first_tile; t < total_tiles; t += tile_stride) {
+                int tm, tn;
+                tile_coords(t, p.tiles_m, p.tiles_n, p.group_m, tm, tn);
+                const int m0 = (tm * CG + (int)rank) * GEMM_BM;
+                const int n0 = tn * BN + (int)rank * (int)L::B_COLS;
+                for (int kt = 0; kt < p.num_k_tiles; ++kt) {
+                    mbar_wait(empty_bar(stage), phase ^ 1u);
+                    const uint32_t sa = smem_base + stage * L::STAGE_BYTES;
+                    const uint32_t sb = sa + L::A_BYTES;
+                    const int k0 = kt * GEMM_BK;
+                    if constexpr (CG == 1) {
+                        mbar_arrive_expect_tx(full_bar(stage), L::STAGE_BYTES);
+                        tma_load_2d(sa, &tmap_a, full_bar(stage), k0, m0);
+#pragma unroll
+                        for (uint32_t b = 0; b < L::B_BOXES; ++b)
+                            tma_load_2d(sb + b * L::B_BOX_BYTES, &tmap_b, full_bar(stage), n0 + (int)b * 64, k0);
+                    } else {
+                        // both CTAs' bytes are counted on the leader's barrier
+                        const uint32_t lead_bar = map_to_cta(full_bar(stage), 0);
+                        if (rank == 0) mbar_arrive_expect_tx(full_bar(stage), 2 * L::STAGE_BYTES);
+                        tma_load_2d_cg2(sa, &tmap_a, lead_bar, k0, m0);
+#pragma unroll
+                        for (uint32_t b = 0; b < L::B_BOXES; ++b)
+                            tma_load_2d_cg2(sb + b * L::B_BOX_BYTES, &tmap_b, lead_bar, n0 + (int)b * 64, k0);
+                    }
+                    if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                }
+            }
+        }
+        __syncwarp();
+    } else if (warp == 1) {
+        // ===== MMA issuer (one lane of the leader CTA) =====
+        if (rank == 0 && elect_one()) {
+            // instruction descriptor: D=f32, A=B=bf16, A K-major, B MN-major, N = BN, M = 128*CG
+            constexpr uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | (0u << 15) | (1u << 16) |
+                                       ((uint32_t)(BN >> 3) << 17) | ((uint32_t)((GEMM_BM * CG) >> 4) << 24);
+            // smem descriptors (version 1, SWIZZLE_128B):
+            //   A (K-major):  LBO unused (=1), SBO = 1024 B between 8-row groups
+            //   B (MN-major): LBO = one 64-column box (8192 B), SBO = 1024 B between 8-k groups
+            constexpr uint64_t desc_hi = (uint64_t(1) << 46) | (uint64_t(2) << 61);
+            constexpr uint64_t a_desc_base = desc_hi | (uint64_t(1) << 16) | (uint64_t(1024 >> 4) << 32);
+            constexpr uint64_t b_desc_base =
+                desc_hi | (uint64_t(L::B_BOX_BYTES >> 4) << 16) | (uint64_t(1024 >> 4) << 32);
+            uint32_t stage = 0, phase = 0, acc = 0, acc_phase = 0;
+            for (int t = first_tile; t < total_tiles; t += tile_stride) {
+                mbar_wait(tmem_empty_bar(acc), acc_phase ^ 1u);
+                tc_fence_after();
+                const uint32_t d_tmem = tmem_base + acc * BN;
+                for (int kt = 0; kt < p.num_k_tiles; ++kt) {
+                    mbar_wait(full_bar(stage), phase);
+                    tc_fence_after();
+                    const uint32_t sa = smem_base + stage * L::STAGE_BYTES;
+                    const uint32_t sb = sa + L::A_BYTES;
+                    const uint64_t a_desc = a_desc_base | (uint64_t)((sa & 0x3FFFFu) >> 4);
+                    const uint64_t b_desc = b_desc_base | (uint64_t)((sb & 0x3FFFFu) >> 4);
+#pragma unroll
+                    for (int k = 0; k < GEMM_BK / GEMM_UMMA_K; ++k) {
+                        // A: +16 elements along K = +32 B inside the swizzled row;
+                        // B: +16 k-rows of 128 B = +2048 B
+                        umma_bf16<CG>(d_tmem, a_desc + (uint64_t)(k * 2), b_desc + (uint64_t)(k * 128), idesc,
+                                      (uint32_t)((kt | k) != 0));
+                    }
+                    umma_commit<CG>(empty_bar(stage));   // smem stage reusable once these MMAs retire
+                    if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                }
+                umma_commit<CG>(tmem_full_bar(acc));     // accumulator ready for the epilogue
+                acc ^= 1u;
+                if (acc == 0) acc_phase ^= 1u;
+            }
+        }
+        __syncwarp();
+    } else if (warp >= GEMM_EPI_WARP0) {
+        // ===== epilogue: TMEM -> registers -> smem -> global =====
+        const uint32_t ew = warp - GEMM_EPI_WARP0;             // TMEM lane quarter of this warp
+        const uint32_t buf0 = smem_base + L::EPI_OFF + ew * 2u * GEMM_EPI_BUF_BYTES;
+        uint8_t* buf0_gen = smem_gen + L::EPI_OFF + ew * 2u * GEMM_EPI_BUF_BYTES;
+        const int cols_per_chunk = p.out_bf16 ? 64 : 32;       // 128 B of C per row per chunk
+        const int num_chunks = BN / cols_per_chunk;
+        uint32_t acc = 0, acc_phase = 0, buf = 0;
+        for (int t = first_tile; t < total_tiles; t += tile_stride) {
+            int tm, tn;
+            tile_coords(t, p.tiles_m, p.tiles_n, p.group_m, tm, tn);
+            const int m0 = (tm * CG + (int)rank) * GEMM_BM + (int)ew * 32;   // first row of this warp
+            const int n_tile = tn * BN;
+            mbar_wait(tmem_full_bar(acc), acc_phase);
+            tc_fence_after();
+            const uint32_t t_acc = tmem_base + ((ew * 32u) << 16) + acc * BN;
+            const uint32_t owner_val = ((uint32_t)t << 8) | (uint32_t)blockIdx.x;
+            for (int c = 0; c < num_chunks; ++c) {
+                const int n0 = n_tile + c * cols_per_chunk;
+                if (m0 >= p.M || n0 >= p.N) continue;   // chunk entirely outside C (warp-uniform)
+                // staging buffer `buf` must no longer be read by an earlier TMA store
+                if (lane == 0) tma_store_wait_read<1>();
+                __syncwarp();
+                const uint32_t sbuf = buf0 + buf * GEMM_EPI_BUF_BYTES;
+                const uint32_t row_addr = sbuf + lane * 128u;
+                const uint32_t sw = lane & 7u;
+                if (p.out_bf16) {
+                    uint32_t v0[32], v1[32];
+                    tmem_ld_32x32(t_acc + (uint32_t)(c * 64), v0);
+                    tmem_ld_32x32(t_acc + (uint32_t)(c * 64 + 32), v1);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (uint32_t j = 0; j < 4; ++j) {   // 16-byte chunk j holds columns 8j..8j+7
+                        st_shared_v4(row_addr + ((j ^ sw) << 4),
+                                     pack_bf16x2(__uint_as_float(v0[8 * j + 0]), __uint_as_float(v0[8 * j + 1])),
+                                     pack_bf16x2(__uint_as_float(v0[8 * j + 2]), __uint_as_float(v0[8 * j + 3])),
+                                     pack_bf16x2(__uint_as_float(v0[8 * j + 4]), __uint_as_float(v0[8 * j + 5])),
+                                     pack_bf16x2(__uint_as_float(v0[8 * j + 6]), __uint_as_float(v0[8 * j + 7])));
+                        st_shared_v4(row_addr + (((j + 4) ^ sw) << 4),
+                                     pack_bf16x2(__uint_as_float(v1[8 * j + 0]), __uint_as_float(v1[8 * j + 1])),
+                                     pack_bf16x2(__uint_as_float(v1[8 * j + 2]), __uint_as_float(v1[8 * j + 3])),
+                                     pack_bf16x2(__uint_as_float(v1[8 * j + 4]), __uint_as_float(v1[8 * j + 5])),
+                                     pack_bf16x2(__uint_as_float(v1[8 * j + 6]), __uint_as_float(v1[8 * j + 7])));
+                    }
+                } else {
+                    uint32_t v[32];
+                    tmem_ld_32x32(t_acc + (uint32_t)(c * 32), v);
+                    tmem_ld_wait();
+                    if (p.owner_mode) {
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) v[i] = owner_val;
+                    }
+#pragma unroll
+                    for (uint32_t j = 0; j < 8; ++j)     // 16-byte chunk j holds columns 4j..4j+3
+                        st_shared_v4(row_addr + ((j ^ sw) << 4), v[4 * j + 0], v[4 * j + 1], v[4 * j + 2],
+                                     v[4 * j + 3]);
+                }
+                if (p.tma_store) {
+                    fence_proxy_async_smem();
+                    __syncwarp();
+                    if (lane == 0) {
+                        tma_store_2d(&tmap_c, sbuf, n0, m0);   // clipped at (N, M) by the tensor map
+                        tma_store_commit();
+                    }
+                } else {
+                    // C rows are not 16-byte addressable: clipped, row-coalesced stores from smem
+                    __syncwarp();
+                    const uint8_t* sgen = buf0_gen + buf * GEMM_EPI_BUF_BYTES;
+                    const int rows = (p.M - m0) < 32 ? (p.M - m0) : 32;
+                    if (p.out_bf16) {
+                        uint16_t* Cb = reinterpret_cast<uint16_t*>(p.C);
+                        for (int r = 0; r < rows; ++r) {
+#pragma unroll
+                            for (int h = 0; h < 2; ++h) {
+                                const int e = (int)lane + 32 * h;   // column within the chunk
+                                if (n0 + e < p.N) {
+                                    const uint32_t off = (uint32_t)r * 128u +
+                                                         ((((uint32_t)e >> 3) ^ ((uint32_t)r & 7u)) << 4) +
+                                                         ((uint32_t)e & 7u) * 2u;
+                                    Cb[(int64_t)(m0 + r) * p.ldc + n0 + e] =
+                                        *reinterpret_cast<const uint16_t*>(sgen + off);
+                                }
+                            }
+                        }
+                    } else {
+                        uint32_t* Cf = reinterpret_cast<uint32_t*>(p.C);
+                        for (int r = 0; r < rows; ++r) {
+                            const int e = (int)lane;
+                            if (n0 + e < p.N) {
+                                const uint32_t off = (uint32_t)r * 128u +
+                                                     ((((uint32_t)e >> 2) ^ ((uint32_t)r & 7u)) << 4) +
+                                                     ((uint32_t)e & 3u) * 4u;
+                                Cf[(int64_t)(m0 + r) * p.ldc + n0 + e] =
+                                    *reinterpret_cast<const uint32_t*>(sgen + off);
+                            }
+                        }
+                    }
+                    __syncwarp();
+                }
+                buf ^= 1u;
+            }
+            // all TMEM reads of this accumulator stage are complete: hand it back to the MMA warp
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) {
+                if constexpr (CG == 1) mbar_arrive(tmem_empty_bar(acc));
+                else mbar_arrive_cluster(map_to_cta(tmem_empty_bar(acc), 0));
+            }
+            acc ^= 1u;
+            if (acc == 0) acc_phase ^= 1u;
+        }
+        if (lane == 0) tma_store_wait_all<0>();
+        __syncwarp();
+    }
+
+    // ------------------------------------------------------------------ teardown
+    tc_fence_before();
+    if constexpr (CG == 2) cluster_sync(); else __syncthreads();
+    if (warp == 2) {
+        tc_fence_after();
+        tmem_dealloc<CG>(tmem_base, 2 * BN);
+    }
+}
+
+}  // namespace tg

@@ -1,0 +1,235 @@
+// M = 1 decode GEMV for sm_100a:  y_j = sum_k x_k * B[k][j], bf16 in, fp32 accumulate.
+//
+// The same definition as the GEMM at M = 1, where the work is HBM-bound
+// (decode roofline R = beta / (W + Kbar)): every weight is read exactly once, so
+// the kernels only have to keep enough bytes in flight and waste none.  No tensor cores.
+//
+//   gemv_tma_kernel : B rows are 16-byte addressable.  One producer warp streams 64(k) x 256(n)
+//                     tiles (32 KB) through a shared-memory ring with TMA + mbarriers; TMA zero
+//                     fill handles the K and N tails.  Eight consumer warps each own 8 rows of a
+//                     tile, lanes own 8 consecutive columns (one conflict-free 16-byte LDS per row).
+//   gemv_ldg_kernel : generic fallback (any alignment): direct global loads, 16-byte when VEC.
+//
+// Split-K: gridDim.y CTAs (one thread-block cluster along y) share a column block; partial sums
+// are combined through distributed shared memory in a fixed order (thread -> warp -> cluster
+// rank), so results are bitwise reproducible and need no global workspace or atomics.
+#pragma once
+#include "ptx.cuh"
+
+namespace tg {
+
+constexpr int GEMV_COLS = 256;          // columns per CTA (32 lanes x 8)
+constexpr int GEMV_TILE_K = 64;         // rows per TMA tile
+constexpr int GEMV_CONSUMER_WARPS = 8;
+constexpr int GEMV_TMA_THREADS = (GEMV_CONSUMER_WARPS + 1) * 32;
+constexpr uint32_t GEMV_TILE_BYTES = GEMV_TILE_K * GEMV_COLS * 2;   // 32 KB
+
+struct GemvParams {
+    const uint16_t* x;
+    const uint16_t* B;
+    void* y;
+    int32_t N, K;
+    int64_t ldb;
+    int32_t k_per_cta;   // rows per split-K slice (multiple of GEMV_TILE_K)
+    int32_t out_bf16;
+};
+
+__device__ __forceinline__ float bf16_bits_to_f32(uint16_t h) { return __uint_as_float(((uint32_t)h) << 16); }
+
+__device__ __forceinline__ void fma8(float (&acc)[8], const uint4& w, float xr) {
+    acc[0] = fmaf(__uint_as_float(w.x << 16), xr, acc[0]);
+    acc[1] = fmaf(__uint_as_float(w.x & 0xffff0000u), xr, acc[1]);
+    acc[2] = fmaf(__uint_as_float(w.y << 16), xr, acc[2]);
+    acc[3] = fmaf(__uint_as_float(w.y & 0xffff0000u), xr, acc[3]);
+    acc[4] = fmaf(__uint_as_float(w.z << 16), xr, acc[4]);
+    acc[5] = fmaf(__uint_as_float(w.z & 0xffff0000u), xr, acc[5]);
+    acc[6] = fmaf(__uint_as_float(w.w << 16), xr, acc[6]);
+    acc[7] = fmaf(__uint_as_float(w.w & 0xffff0000u), xr, acc[7]);
+}
+
+__device__ __forceinline__ uint16_t f32_to_bf16_rne(float f) {
+    uint16_t r;
+    asm("cvt.rn.bf16.f32 %0, %1;" : "=h"(r) : "f"(f));
+    return r;
+}
+
+// Combine the per-thread partial sums of one CTA (warps ordered along K) and of the split-K
+// cluster, then write this CTA's share of the 256 output columns.
+//   red  : smem [nwarps][256] floats, part : smem [256] floats
+template <int NWARPS>
+__device__ __forceinline__ void gemv_reduce_and_store(const float (&acc)[8], float* red, float* part,
+                                                      uint32_t cwarp, uint32_t lane, bool is_consumer,
+                                                      const GemvParams& p, int n0) {
+    if (is_consumer) {
+#pragma unroll
+        for (int e = 0; e < 8; ++e) red[cwarp * GEMV_COLS + lane * 8 + e] = acc[e];
+    }
+    __syncthreads();
+    const uint32_t tid = threadIdx.x;
+    if (tid < GEMV_COLS) {
+        float s = 0.f;
+#pragma unroll
+        for (int w = 0; w < NWARPS; ++w) s += red[w * GEMV_COLS + tid];   // fixed order
+        part[tid] = s;
+    }
+    const uint32_t nsplit = gridDim.y;
+    if (nsplit > 1) cluster_sync(); else __syncthreads();
+    const uint32_t rank = blockIdx.y;   // cluster spans the whole y extent
+    if (tid < GEMV_COLS && (tid % nsplit) == rank) {
+        float s = 0.f;
+        if (nsplit > 1) {
+            const uint32_t a = smem_u32(&part[tid]);
+            for (uint32_t q = 0; q < nsplit; ++q) s += ld_dsmem_f32(map_to_cta(a, q));   // fixed order
+        } else {
+            s = part[tid];
+        }
+        const int col = n0 + (int)tid;
+        if (col < p.N) {
+            if (p.out_bf16) reinterpret_cast<uint16_t*>(p.y)[col] = f32_to_bf16_rne(s);
+            else reinterpret_cast<float*>(p.y)[col] = s;
+        }
+    }
+    if (nsplit > 1) cluster_sync();   // peers may still be reading this CTA's `part`
+}
+
+template <int STAGES>
+__global__ void __launch_bounds__(GEMV_TMA_THREADS)
+gemv_tma_kernel(const __grid_constant__ CUtensorMap tmap_b, const GemvParams p) {
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 127u) & ~127u;
+    uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
+    // layout: STAGES tiles | red [8][256] f32 | part [256] f32 | barriers
+    constexpr uint32_t RED_OFF = STAGES * GEMV_TILE_BYTES;
+    constexpr uint32_t PART_OFF = RED_OFF + GEMV_CONSUMER_WARPS * GEMV_COLS * 4;
+    constexpr uint32_t BAR_OFF = PART_OFF + GEMV_COLS * 4;
+    float* red = reinterpret_cast<float*>(smem_gen + RED_OFF);
+    float* part = reinterpret_cast<float*>(smem_gen + PART_OFF);
+    auto full_bar = [&](uint32_t s) { return smem_base + BAR_OFF + s * 8u; };
+    auto empty_bar = [&](uint32_t s) { return smem_base + BAR_OFF + (STAGES + s) * 8u; };
+
+    const uint32_t warp = threadIdx.x >> 5;
+    const uint32_t lane = threadIdx.x & 31;
+    const int n0 = (int)blockIdx.x * GEMV_COLS;
+    const int k_begin = (int)blockIdx.y * p.k_per_cta;
+    const int k_end = min(p.K, k_begin + p.k_per_cta);
+    const int ntiles = k_end > k_begin ? (k_end - k_begin + GEMV_TILE_K - 1) / GEMV_TILE_K : 0;
+
+    if (threadIdx.x == 0) {
+        prefetch_tmap(&tmap_b);
+        for (uint32_t s = 0; s < STAGES; ++s) {
+            mbar_init(full_bar(s), 1);
+            mbar_init(empty_bar(s), GEMV_CONSUMER_WARPS);
+        }
+        fence_mbar_init();
+    }
+    __syncthreads();
+
+    float acc[8];
+#pragma unroll
+    for (int e = 0; e < 8; ++e) acc[e] = 0.f;
+
+    if (warp == GEMV_CONSUMER_WARPS) {
+        // ===== producer =====
+        if (elect_one()) {
+            uint32_t stage = 0, phase = 0;
+            for (int it = 0; it < ntiles; ++it) {
+                mbar_wait(empty_bar(stage), phase ^ 1u);
+                mbar_arrive_expect_tx(full_bar(stage), GEMV_TILE_BYTES);
+                tma_load_2d(smem_base + stage * GEMV_TILE_BYTES, &tmap_b, full_bar(stage), n0,
+                            k_begin + it * GEMV_TILE_K);
+                if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+            }
+        }
+        __syncwarp();
+    } else {
+        // ===== consumers: warp w owns rows 8w..8w+7 of every tile =====
+        auto load_x = [&](int it) -> float {
+            const int k = k_begin + it * GEMV_TILE_K + (int)warp * 8 + (int)(lane & 7u);
+            return (it < ntiles && k < p.K) ? bf16_bits_to_f32(__ldg(p.x + k)) : 0.f;
+        };
+        uint32_t stage = 0, phase = 0;
+        float xv_next = load_x(0);
+        for (int it = 0; it < ntiles; ++it) {
+            const float xv = xv_next;
+            xv_next = load_x(it + 1);
+            mbar_wait(full_bar(stage), phase);
+            const uint8_t* tile = smem_gen + stage * GEMV_TILE_BYTES + warp * 8u * (GEMV_COLS * 2) + lane * 16u;
+            uint4 w[8];
+#pragma unroll
+            for (int r = 0; r < 8; ++r) w[r] = *reinterpret_cast<const uint4*>(tile + r * (GEMV_COLS * 2));
+#pragma unroll
+            for (int r = 0; r < 8; ++r) fma8(acc, w[r], __shfl_sync(0xffffffffu, xv, r));
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty_bar(stage));
+            if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+        }
+    }
+    gemv_reduce_and_store<GEMV_CONSUMER_WARPS>(acc, red, part, warp, lane, warp < GEMV_CONSUMER_WARPS, p, n0);
+}
+
+// Generic fallback: no alignment requirement on B when VEC == false.
+template <bool VEC>
+__global__ void __launch_bounds__(256)
+gemv_ldg_kernel(const GemvParams p) {
+    __shared__ float red[8 * GEMV_COLS];
+    __shared__ float part[GEMV_COLS];
+    const uint32_t warp = threadIdx.x >> 5;
+    const uint32_t lane = threadIdx.x & 31;
+    const int n0 = (int)blockIdx.x * GEMV_COLS;
+    const int col0 = n0 + (int)lane * 8;
+    const int k_begin = (int)blockIdx.y * p.k_per_cta;
+    const int k_end = min(p.K, k_begin + p.k_per_cta);
+    // warp w takes a contiguous share of the CTA's K slice
+    const int len = max(0, k_end - k_begin);
+    const int per_warp = (len + 7) / 8;
+    const int wb = k_begin + (int)warp * per_warp;
+    const int we = min(k_end, wb + per_warp);
+    const int ncols = min(8, p.N - col0);   // <= 0: this lane owns no column
+
+    float acc[8];
+#pragma unroll
+    for (int e = 0; e < 8; ++e) acc[e] = 0.f;
+
+    auto load_row = [&](int k) -> uint4 {
+        uint4 w = make_uint4(0u, 0u, 0u, 0u);
+        const uint16_t* src = p.B + (int64_t)k * p.ldb + col0;
+        if (VEC && ncols == 8) {
+            asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
+                         : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w)
+                         : "l"(src));
+        } else if (ncols > 0) {
+            uint32_t h[8];
+#pragma unroll
+            for (int e = 0; e < 8; ++e) h[e] = (e < ncols) ? (uint32_t)__ldg(src + e) : 0u;
+            w.x = h[0] | (h[1] << 16);
+            w.y = h[2] | (h[3] << 16);
+            w.z = h[4] | (h[5] << 16);
+            w.w = h[6] | (h[7] << 16);
+        }
+        return w;
+    };
+
+    for (int k0 = wb; k0 < we; k0 += 32) {
+        const int kk = k0 + (int)lane;
+        const float xv = (kk < we) ? bf16_bits_to_f32(__ldg(p.x + kk)) : 0.f;
+        const int nrows = min(32, we - k0);
+        if (nrows == 32) {
+#pragma unroll
+            for (int r0 = 0; r0 < 32; r0 += 8) {
+                uint4 w[8];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) w[u] = load_row(k0 + r0 + u);
+#pragma unroll
+                for (int u = 0; u < 8; ++u) fma8(acc, w[u], __shfl_sync(0xffffffffu, xv, r0 + u));
+            }
+        } else {
+            for (int r = 0; r < nrows; ++r) {
+                const uint4 w = load_row(k0 + r);
+                fma8(acc, w, __shfl_sync(0xffffffffu, xv, r));
+            }
+        }
+    }
+    gemv_reduce_and_store<8>(acc, red, part, warp, lane, true, p, n0);
+}
+
+}  // namespace tg

@@ -1,0 +1,634 @@
+// Host entry of libtilegemm.so: launch preconditions, shape selector, tensor-map cache,
+// workspaces and kernel launches.  See include/tile_gemm.h for the contract.
+//
+// "An obligation becomes a launch precondition when every operand is known at launch ... The
+// check moves into the generated launcher, runs once per launch before any work is queued, and
+// returns an error on failure".  Everything validated here is exactly what lets
+// the device K loops run without a single bounds check.
+#include "../../include/tile_gemm.h"
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <atomic>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <unordered_map>
+
+#include "aux_kernels.cuh"
+#include "gemm_kernel.cuh"
+#include "gemv_kernel.cuh"
+
+namespace {
+
+// ------------------------------------------------------------------ errors
+thread_local char g_err[640] = "";
+
+int fail(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+const char* const kStatusNames[TILE_GEMM_NUM_STATUS] = {
+    "ok",
+    "null pointer with a non-empty extent",
+    "negative extent",
+    "lda < K",
+    "ldb < N",
+    "ldc < N",
+    "unknown out_dtype",
+    "pointer not aligned to its element size",
+    "C overlaps A or B",
+    "extent overflow",
+    "no sm_100 CUDA device",
+    "CUDA call failed",
+    "path not applicable",
+    "internal error",
+};
+
+std::atomic<int64_t> g_launches{0};
+std::atomic<int> g_tune[8];
+
+// ------------------------------------------------------------------ preconditions + selector
+struct Plan {
+    int path = 0;
+    int esize = 4;
+    int64_t a_bytes = 0, b_bytes = 0, c_bytes = 0;   // byte spans of the three operands
+    bool a_tma = false, b_tma = false, c_tma = false;
+};
+
+bool span_bytes(int64_t rows, int64_t cols, int64_t ld, int64_t esize, int64_t* out) {
+    if (rows == 0 || cols == 0) { *out = 0; return true; }
+    int64_t t;
+    if (__builtin_mul_overflow(rows - 1, ld, &t)) return false;
+    if (__builtin_add_overflow(t, cols, &t)) return false;
+    if (__builtin_mul_overflow(t, esize, &t)) return false;
+    *out = t;
+    return true;
+}
+
+bool overlaps(const void* p, int64_t pn, const void* q, int64_t qn) {
+    if (pn == 0 || qn == 0) return false;
+    const uintptr_t a = (uintptr_t)p, b = (uintptr_t)q;
+    return a < b + (uintptr_t)qn && b < a + (uintptr_t)pn;
+}
+
+int check_and_select(const void* A, const void* B, const void* C, int64_t M, int64_t N, int64_t K, int64_t lda,
+                     int64_t ldb, int64_t ldc, int out_dtype, Plan* plan) {
+    if (M < 0 || N < 0 || K < 0)
+        return fail(TILE_GEMM_E_EXTENT, "negative extent: M=%lld N=%lld K=%lld", (long long)M, (long long)N,
+                    (long long)K);
+    if (out_dtype != TILE_GEMM_OUT_F32 && out_dtype != TILE_GEMM_OUT_BF16)
+        return fail(TILE_GEMM_E_DTYPE, "out_dtype=%d is neither TILE_GEMM_OUT_F32 (0) nor TILE_GEMM_OUT_BF16 (1)",
+                    out_dtype);
+    if (lda < K) return fail(TILE_GEMM_E_LDA, "lda=%lld < K=%lld", (long long)lda, (long long)K);
+    if (ldb < N) return fail(TILE_GEMM_E_LDB, "ldb=%lld < N=%lld", (long long)ldb, (long long)N);
+    if (ldc < N) return fail(TILE_GEMM_E_LDC, "ldc=%lld < N=%lld", (long long)ldc, (long long)N);
+    const int64_t lim = (int64_t)INT32_MAX - 1024;
+    if (M > lim || N > lim || K > lim)
+        return fail(TILE_GEMM_E_OVERFLOW, "extent above 2^31-1025: M=%lld N=%lld K=%lld", (long long)M, (long long)N,
+                    (long long)K);
+    plan->esize = (out_dtype == TILE_GEMM_OUT_BF16) ? 2 : 4;
+    if (!span_bytes(M, K, lda, 2, &plan->a_bytes) || !span_bytes(K, N, ldb, 2, &plan->b_bytes) ||
+        !span_bytes(M, N, ldc, plan->esize, &plan->c_bytes))
+        return fail(TILE_GEMM_E_OVERFLOW, "operand byte span overflows int64");
+    if (lda > (int64_t(1) << 38) || ldb > (int64_t(1) << 38) || ldc > (int64_t(1) << 38))
+        return fail(TILE_GEMM_E_OVERFLOW, "row stride above 2^38 elements");
+    const int64_t tiles = ((M + 127) / 128) * ((N + 127) / 128);
+    if (tiles > lim) return fail(TILE_GEMM_E_OVERFLOW, "output tile count %lld overflows int32", (long long)tiles);
+    if (M == 0 || N == 0) { plan->path = TILE_GEMM_PATH_NOOP; return TILE_GEMM_OK; }
+    if (C == nullptr) return fail(TILE_GEMM_E_NULL, "C is NULL but M*N > 0");
+    if (K > 0 && A == nullptr) return fail(TILE_GEMM_E_NULL, "A is NULL but M*K > 0");
+    if (K > 0 && B == nullptr) return fail(TILE_GEMM_E_NULL, "B is NULL but K*N > 0");
+    if (((uintptr_t)A & 1) || ((uintptr_t)B & 1))
+        return fail(TILE_GEMM_E_ALIGN, "A (%p) or B (%p) is not 2-byte aligned", A, B);
+    if ((uintptr_t)C & (uintptr_t)(plan->esize - 1))
+        return fail(TILE_GEMM_E_ALIGN, "C (%p) is not %d-byte aligned", C, plan->esize);
+    if (overlaps(C, plan->c_bytes, A, plan->a_bytes))
+        return fail(TILE_GEMM_E_ALIAS, "C [%p,+%lld) overlaps A [%p,+%lld): the output must be exclusively owned", C,
+                    (long long)plan->c_bytes, A, (long long)plan->a_bytes);
+    if (overlaps(C, plan->c_bytes, B, plan->b_bytes))
+        return fail(TILE_GEMM_E_ALIAS, "C [%p,+%lld) overlaps B [%p,+%lld): the output must be exclusively owned", C,
+                    (long long)plan->c_bytes, B, (long long)plan->b_bytes);
+    // TMA addressability: 16-byte aligned base and 16-byte multiple row pitch
+    plan->a_tma = (((uintptr_t)A & 15) == 0) && (lda % 8 == 0);
+    plan->b_tma = (((uintptr_t)B & 15) == 0) && (ldb % 8 == 0);
+    plan->c_tma = (((uintptr_t)C & 15) == 0) && ((ldc * plan->esize) % 16 == 0);
+    if (K == 0) plan->path = TILE_GEMM_PATH_ZERO;
+    else if (M == 1) plan->path = TILE_GEMM_PATH_GEMV;
+    else plan->path = (plan->a_tma && plan->b_tma) ? TILE_GEMM_PATH_GEMM_TMA : TILE_GEMM_PATH_GEMM_REPACK;
+    return TILE_GEMM_OK;
+}
+
+// ------------------------------------------------------------------ device
+struct DevInfo {
+    bool probed = false;
+    int status = TILE_GEMM_E_DEVICE;
+    int sms = 0;
+};
+DevInfo g_dev[64];
+std::mutex g_mu;
+
+#define CUDA_TRY(expr)                                                                              \
+    do {                                                                                            \
+        cudaError_t e_ = (expr);                                                                    \
+        if (e_ != cudaSuccess)                                                                      \
+            return fail(TILE_GEMM_E_CUDA, "%s failed: %s (%d)", #expr, cudaGetErrorString(e_), (int)e_); \
+    } while (0)
+
+int current_device(int* dev, int* sms) {
+    int d = -1;
+    cudaError_t e = cudaGetDevice(&d);
+    if (e != cudaSuccess || d < 0 || d >= 64)
+        return fail(TILE_GEMM_E_DEVICE, "no usable CUDA device: %s; this library has no CPU fallback",
+                    cudaGetErrorString(e));
+    std::lock_guard<std::mutex> lk(g_mu);
+    DevInfo& di = g_dev[d];
+    if (!di.probed) {
+        int major = 0, minor = 0, sms_ = 0;
+        cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, d);
+        cudaDeviceGetAttribute(&minor, cudaDevAttrComputeCapabilityMinor, d);
+        cudaDeviceGetAttribute(&sms_, cudaDevAttrMultiProcessorCount, d);
+        di.probed = true;
+        di.sms = sms_;
+        di.status = (major == 10 && minor == 0) ? TILE_GEMM_OK : TILE_GEMM_E_DEVICE;
+        if (di.status != TILE_GEMM_OK)
+            snprintf(g_err, sizeof g_err, "device %d is sm_%d%d; the kernels are built for sm_100a only", d, major,
+                     minor);
+    }
+    if (di.status != TILE_GEMM_OK) {
+        if (g_err[0] == 0) snprintf(g_err, sizeof g_err, "device %d is not sm_100", d);
+        return di.status;
+    }
+    *dev = d;
+    *sms = di.sms;
+    return TILE_GEMM_OK;
+}
+
+// ------------------------------------------------------------------ tensor maps
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn g_encode = nullptr;
+
+struct MapKey {
+    uintptr_t p;
+    uint64_t d0, d1, pitch;
+    uint32_t b0, b1, dtype, swizzle;
+    bool operator==(const MapKey& o) const {
+        return p == o.p && d0 == o.d0 && d1 == o.d1 && pitch == o.pitch && b0 == o.b0 && b1 == o.b1 &&
+               dtype == o.dtype && swizzle == o.swizzle;
+    }
+};
+struct MapKeyHash {
+    size_t operator()(const MapKey& k) const {
+        uint64_t h = 1469598103934665603ull;
+        const uint64_t v[6] = {k.p, k.d0, k.d1, k.pitch, ((uint64_t)k.b0 << 32) | k.b1,
+                               ((uint64_t)k.dtype << 32) | k.swizzle};
+        for (uint64_t x : v) { h ^= x; h *= 1099511628211ull; }
+        return (size_t)h;
+    }
+};
+std::unordered_map<MapKey, CUtensorMap, MapKeyHash> g_maps;
+
+// 2-D row-major tensor [d1 rows][d0 cols] of `esize`-byte elements with row pitch `pitch` bytes.
+int get_tensor_map(CUtensorMap* out, const void* base, int dtype_bytes, bool is_float32, uint64_t d0, uint64_t d1,
+                   uint64_t pitch, uint32_t b0, uint32_t b1, bool swizzle128) {
+    MapKey key{(uintptr_t)base, d0, d1, pitch, b0, b1, (uint32_t)(is_float32 ? 4 : dtype_bytes),
+               (uint32_t)swizzle128};
+    std::lock_guard<std::mutex> lk(g_mu);
+    auto it = g_maps.find(key);
+    if (it != g_maps.end()) { *out = it->second; return TILE_GEMM_OK; }
+    if (!g_encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+        if (e != cudaSuccess || fn == nullptr || qres != cudaDriverEntryPointSuccess)
+            return fail(TILE_GEMM_E_CUDA, "cuTensorMapEncodeTiled entry point unavailable: %s", cudaGetErrorString(e));
+        g_encode = (EncodeTiledFn)fn;
+    }
+    const cuuint64_t dims[2] = {d0, d1};
+    const cuuint64_t strides[1] = {pitch};
+    const cuuint32_t box[2] = {b0, b1};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUtensorMapDataType dt = is_float32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16;
+    CUtensorMap m;
+    CUresult r = g_encode(&m, dt, 2, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                          swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+                          CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS)
+        return fail(TILE_GEMM_E_CUDA,
+                    "cuTensorMapEncodeTiled failed (%d) for base=%p dims=(%llu,%llu) pitch=%llu box=(%u,%u)", (int)r,
+                    base, (unsigned long long)d0, (unsigned long long)d1, (unsigned long long)pitch, b0, b1);
+    if (g_maps.size() > 8192) g_maps.clear();
+    g_maps.emplace(key, m);
+    *out = m;
+    return TILE_GEMM_OK;
+}
+
+// ------------------------------------------------------------------ workspaces
+struct Buf {
+    void* p = nullptr;
+    size_t n = 0;
+};
+std::unordered_map<uint64_t, Buf> g_ws;   // (device, stream) -> repack workspace
+Buf g_stage[3];                            // tile_gemm_host staging (A, B, C)
+cudaStream_t g_host_stream = nullptr;
+
+int grow(Buf& b, size_t need) {
+    if (b.n >= need) return TILE_GEMM_OK;
+    if (b.p) CUDA_TRY(cudaFree(b.p));   // cudaFree synchronises: no in-flight user remains
+    b.p = nullptr;
+    b.n = 0;
+    const size_t sz = (need + ((size_t)1 << 20) - 1) & ~(((size_t)1 << 20) - 1);
+    CUDA_TRY(cudaMalloc(&b.p, sz));
+    b.n = sz;
+    return TILE_GEMM_OK;
+}
+
+int workspace_for(int dev, cudaStream_t s, size_t need, void** out) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    Buf& b = g_ws[((uint64_t)dev << 56) ^ (uint64_t)(uintptr_t)s];
+    int rc = grow(b, need);
+    if (rc) return rc;
+    *out = b.p;
+    return TILE_GEMM_OK;
+}
+
+// ------------------------------------------------------------------ GEMM launch
+struct GemmConfig {
+    int id;       // 1: 1-CTA 128x128, 2: 1-CTA 128x256, 3: 2-CTA 256x256
+    int cg, bn, stages;
+};
+const GemmConfig kConfigs[4] = {{0, 0, 0, 0}, {1, 1, 128, 6}, {2, 1, 256, 4}, {3, 2, 256, 6}};
+
+GemmConfig choose_config(int64_t M, int64_t N, int sms) {
+    const int forced = g_tune[0].load();
+    if (forced >= 1 && forced <= 3) return kConfigs[forced];
+    const int64_t t3 = ((M + 255) / 256) * ((N + 255) / 256);
+    if (t3 >= sms / 2) return kConfigs[3];
+    const int64_t t2 = ((M + 127) / 128) * ((N + 255) / 256);
+    if (t2 * 4 >= (int64_t)sms * 3) return kConfigs[2];
+    return kConfigs[1];
+}
+
+struct GemmLaunch {
+    GemmConfig cfg;
+    tg::GemmParams p;
+    int ctas;
+};
+
+void plan_gemm(int64_t M, int64_t N, int64_t K, int out_bf16, int sms, GemmLaunch* gl) {
+    gl->cfg = choose_config(M, N, sms);
+    const int tile_m = tg::GEMM_BM * gl->cfg.cg;
+    tg::GemmParams& p = gl->p;
+    memset(&p, 0, sizeof p);
+    p.M = (int32_t)M; p.N = (int32_t)N; p.K = (int32_t)K;
+    p.tiles_m = (int32_t)((M + tile_m - 1) / tile_m);
+    p.tiles_n = (int32_t)((N + gl->cfg.bn - 1) / gl->cfg.bn);
+    int gm = g_tune[1].load();
+    if (gm <= 0) gm = (gl->cfg.cg == 2) ? 8 : 16;
+    p.group_m = gm < p.tiles_m ? gm : p.tiles_m;
+    p.num_k_tiles = (int32_t)((K + tg::GEMM_BK - 1) / tg::GEMM_BK);
+    p.out_bf16 = out_bf16;
+    int64_t units = (int64_t)p.tiles_m * p.tiles_n;
+    int max_units = sms / gl->cfg.cg;
+    const int cap = g_tune[2].load();
+    if (cap > 0 && cap / gl->cfg.cg >= 1 && cap / gl->cfg.cg < max_units) max_units = cap / gl->cfg.cg;
+    if (units > max_units) units = max_units;
+    gl->ctas = (int)units * gl->cfg.cg;
+}
+
+template <int CG, int BN, int STAGES>
+int launch_gemm_inst(const CUtensorMap& ta, const CUtensorMap& tb, const CUtensorMap& tc, const tg::GemmParams& p,
+                     int ctas, cudaStream_t s, int dev) {
+    using L = tg::GemmSmem<CG, BN, STAGES>;
+    auto kern = tg::gemm_tcgen05_kernel<CG, BN, STAGES>;
+    static bool configured[64] = {};
+    if (!configured[dev]) {
+        CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::TOTAL));
+        configured[dev] = true;
+    }
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof cfg);
+    cfg.gridDim = dim3((unsigned)ctas, 1, 1);
+    cfg.blockDim = dim3(tg::GEMM_THREADS, 1, 1);
+    cfg.dynamicSmemBytes = L::TOTAL;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CG;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, ta, tb, tc, p));
+    g_launches.fetch_add(1);
+    return TILE_GEMM_OK;
+}
+
+int launch_gemm(const GemmLaunch& gl, const CUtensorMap& ta, const CUtensorMap& tb, const CUtensorMap& tc,
+                cudaStream_t s, int dev) {
+    switch (gl.cfg.id) {
+        case 1: return launch_gemm_inst<1, 128, 6>(ta, tb, tc, gl.p, gl.ctas, s, dev);
+        case 2: return launch_gemm_inst<1, 256, 4>(ta, tb, tc, gl.p, gl.ctas, s, dev);
+        case 3: return launch_gemm_inst<2, 256, 6>(ta, tb, tc, gl.p, gl.ctas, s, dev);
+    }
+    return fail(TILE_GEMM_E_INTERNAL, "unknown GEMM config %d", gl.cfg.id);
+}
+
+int c_tensor_map(CUtensorMap* tc, void* C, int64_t M, int64_t N, int64_t ldc, int out_bf16) {
+    // one epilogue chunk: 32 rows x 128 bytes, 128B-swizzled in shared memory
+    return get_tensor_map(tc, C, out_bf16 ? 2 : 4, !out_bf16, (uint64_t)N, (uint64_t)M,
+                          (uint64_t)ldc * (out_bf16 ? 2 : 4), out_bf16 ? 64u : 32u, 32u, true);
+}
+
+int run_gemm(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_t K, int64_t lda, int64_t ldb,
+             int64_t ldc, int out_dtype, cudaStream_t s, const Plan& plan, bool force_repack, int dev, int sms) {
+    const int out_bf16 = out_dtype == TILE_GEMM_OUT_BF16;
+    const bool rep_a = force_repack || !plan.a_tma;
+    const bool rep_b = force_repack || !plan.b_tma;
+    const uint16_t* Ap = (const uint16_t*)A;
+    const uint16_t* Bp = (const uint16_t*)B;
+    if (rep_a || rep_b) {
+        const int64_t lda2 = (K + 7) & ~int64_t(7), ldb2 = (N + 7) & ~int64_t(7);
+        const size_t a_sz = rep_a ? (((size_t)M * lda2 * 2 + 255) & ~(size_t)255) : 0;
+        const size_t b_sz = rep_b ? (((size_t)K * ldb2 * 2 + 255) & ~(size_t)255) : 0;
+        void* ws = nullptr;
+        int rc = workspace_for(dev, s, a_sz + b_sz, &ws);
+        if (rc) return rc;
+        if (rep_a) {
+            const int64_t chunks = M * (lda2 >> 3);
+            const int blocks = (int)((chunks + 255) / 256 < 148 * 16 ? (chunks + 255) / 256 : 148 * 16);
+            tg::repack_rows_kernel<<<blocks, 256, 0, s>>>(Ap, lda, (uint16_t*)ws, lda2, M, K);
+            CUDA_TRY(cudaGetLastError());
+            g_launches.fetch_add(1);
+            Ap = (const uint16_t*)ws;
+            lda = lda2;
+        }
+        if (rep_b) {
+            uint16_t* dst = (uint16_t*)((char*)ws + a_sz);
+            const int64_t chunks = K * (ldb2 >> 3);
+            const int blocks = (int)((chunks + 255) / 256 < 148 * 16 ? (chunks + 255) / 256 : 148 * 16);
+            tg::repack_rows_kernel<<<blocks, 256, 0, s>>>(Bp, ldb, dst, ldb2, K, N);
+            CUDA_TRY(cudaGetLastError());
+            g_launches.fetch_add(1);
+            Bp = dst;
+            ldb = ldb2;
+        }
+    }
+    GemmLaunch gl;
+    plan_gemm(M, N, K, out_bf16, sms, &gl);
+    gl.p.tma_store = plan.c_tma ? 1 : 0;
+    gl.p.C = C;
+    gl.p.ldc = ldc;
+    CUtensorMap ta, tb, tc;
+    int rc = get_tensor_map(&ta, Ap, 2, false, (uint64_t)K, (uint64_t)M, (uint64_t)lda * 2, 64u, 128u, true);
+    if (rc) return rc;
+    rc = get_tensor_map(&tb, Bp, 2, false, (uint64_t)N, (uint64_t)K, (uint64_t)ldb * 2, 64u, 64u, true);
+    if (rc) return rc;
+    if (plan.c_tma) {
+        rc = c_tensor_map(&tc, C, M, N, ldc, out_bf16);
+        if (rc) return rc;
+    } else {
+        tc = ta;   // never dereferenced by the clipped st.global epilogue; must still be a valid map
+    }
+    return launch_gemm(gl, ta, tb, tc, s, dev);
+}
+
+// ------------------------------------------------------------------ GEMV launch
+int run_gemv(const void* x, const void* B, void* y, int64_t N, int64_t K, int64_t ldb, int out_dtype, cudaStream_t s,
+             const Plan& plan, int sms) {
+    tg::GemvParams p;
+    p.x = (const uint16_t*)x;
+    p.B = (const uint16_t*)B;
+    p.y = y;
+    p.N = (int32_t)N;
+    p.K = (int32_t)K;
+    p.ldb = ldb;
+    p.out_bf16 = out_dtype == TILE_GEMM_OUT_BF16;
+    int variant = g_tune[4].load();   // 0 auto, 1 TMA, 2 LDG 16-byte, 3 LDG scalar
+    if (!plan.b_tma) variant = 3;
+    else if (variant < 1 || variant > 3) variant = 1;
+    const int64_t xblocks = (N + tg::GEMV_COLS - 1) / tg::GEMV_COLS;
+    // split-K: as many slices as keep every CTA co-resident (2 per SM) with >= 2 tiles each
+    int split = g_tune[3].load();
+    if (split <= 0) {
+        split = 1;
+        const int64_t slots = (int64_t)sms * 2;
+        for (int c = 2; c <= 8; ++c)
+            if (xblocks * c <= slots && K / c >= 2 * tg::GEMV_TILE_K) split = c;
+    }
+    if (split > 8) split = 8;
+    int64_t kper = (K + split - 1) / split;
+    kper = (kper + tg::GEMV_TILE_K - 1) / tg::GEMV_TILE_K * tg::GEMV_TILE_K;
+    split = (int)((K + kper - 1) / kper);
+    p.k_per_cta = (int32_t)kper;
+
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof cfg);
+    cfg.gridDim = dim3((unsigned)xblocks, (unsigned)split, 1);
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 1;
+    attr[0].val.clusterDim.y = (unsigned)split;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    if (variant == 1) {
+        constexpr int STAGES = 3;
+        constexpr uint32_t smem = STAGES * tg::GEMV_TILE_BYTES + tg::GEMV_CONSUMER_WARPS * tg::GEMV_COLS * 4 +
+                                  tg::GEMV_COLS * 4 + 2 * STAGES * 8 + 128;
+        auto kern = tg::gemv_tma_kernel<STAGES>;
+        static bool configured = false;
+        if (!configured) {
+            CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            configured = true;
+        }
+        CUtensorMap tb;
+        int rc = get_tensor_map(&tb, B, 2, false, (uint64_t)N, (uint64_t)K, (uint64_t)ldb * 2, (uint32_t)tg::GEMV_COLS,
+                                (uint32_t)tg::GEMV_TILE_K, false);
+        if (rc) return rc;
+        cfg.blockDim = dim3(tg::GEMV_TMA_THREADS, 1, 1);
+        cfg.dynamicSmemBytes = smem;
+        CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, tb, p));
+    } else {
+        cfg.blockDim = dim3(256, 1, 1);
+        cfg.dynamicSmemBytes = 0;
+        if (variant == 2) CUDA_TRY(cudaLaunchKernelEx(&cfg, tg::gemv_ldg_kernel<true>, p));
+        else CUDA_TRY(cudaLaunchKernelEx(&cfg, tg::gemv_ldg_kernel<false>, p));
+    }
+    g_launches.fetch_add(1);
+    return TILE_GEMM_OK;
+}
+
+int run_zero(void* C, int64_t M, int64_t N, int64_t ldc, int esize, cudaStream_t s) {
+    const int64_t total = M * N;
+    const int blocks = (int)((total + 255) / 256 < 148 * 8 ? (total + 255) / 256 : 148 * 8);
+    tg::zero_fill_kernel<<<blocks, 256, 0, s>>>(C, M, N, ldc, esize);
+    CUDA_TRY(cudaGetLastError());
+    g_launches.fetch_add(1);
+    return TILE_GEMM_OK;
+}
+
+}  // namespace
+
+// ====================================================================== C ABI
+extern "C" {
+
+int tile_gemm_select(int64_t M, int64_t N, int64_t K, int64_t lda, int64_t ldb, int64_t ldc, const void* A,
+                     const void* B, const void* C, int out_dtype) {
+    Plan plan;
+    const int rc = check_and_select(A, B, C, M, N, K, lda, ldb, ldc, out_dtype, &plan);
+    return rc ? -rc : plan.path;
+}
+
+int tile_gemm_ex(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_t K, int64_t lda, int64_t ldb,
+                 int64_t ldc, int out_dtype, void* stream, int force_path) {
+    Plan plan;
+    int rc = check_and_select(A, B, C, M, N, K, lda, ldb, ldc, out_dtype, &plan);
+    if (rc) return rc;
+    if (force_path < TILE_GEMM_PATH_AUTO || force_path > TILE_GEMM_PATH_GEMV)
+        return fail(TILE_GEMM_E_PATH, "force_path=%d is not AUTO, GEMM_TMA, GEMM_REPACK or GEMV", force_path);
+    if (plan.path == TILE_GEMM_PATH_NOOP) return TILE_GEMM_OK;
+    int path = plan.path;
+    if (force_path != TILE_GEMM_PATH_AUTO && path != TILE_GEMM_PATH_ZERO) {
+        if (force_path == TILE_GEMM_PATH_GEMV && M != 1)
+            return fail(TILE_GEMM_E_PATH, "the GEMV path needs M == 1 (M=%lld)", (long long)M);
+        if (force_path == TILE_GEMM_PATH_GEMM_TMA && !(plan.a_tma && plan.b_tma))
+            return fail(TILE_GEMM_E_PATH, "GEMM_TMA needs 16-byte aligned A/B with lda, ldb multiples of 8");
+        path = force_path;
+    }
+    int dev = 0, sms = 0;
+    rc = current_device(&dev, &sms);
+    if (rc) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    switch (path) {
+        case TILE_GEMM_PATH_ZERO: return run_zero(C, M, N, ldc, plan.esize, s);
+        case TILE_GEMM_PATH_GEMV: return run_gemv(A, B, C, N, K, ldb, out_dtype, s, plan, sms);
+        case TILE_GEMM_PATH_GEMM_TMA:
+            return run_gemm(A, B, C, M, N, K, lda, ldb, ldc, out_dtype, s, plan, false, dev, sms);
+        case TILE_GEMM_PATH_GEMM_REPACK:   // forced: repack both operands; auto: only what TMA cannot address
+            return run_gemm(A, B, C, M, N, K, lda, ldb, ldc, out_dtype, s, plan,
+                            force_path == TILE_GEMM_PATH_GEMM_REPACK, dev, sms);
+    }
+    return fail(TILE_GEMM_E_INTERNAL, "unhandled path %d", path);
+}
+
+int tile_gemm(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_t K, int64_t lda, int64_t ldb,
+              int64_t ldc, int out_dtype, void* stream) {
+    return tile_gemm_ex(A, B, C, M, N, K, lda, ldb, ldc, out_dtype, stream, TILE_GEMM_PATH_AUTO);
+}
+
+int tile_gemm_host(const void* A_host, const void* B_host, void* C_host, int64_t M, int64_t N, int64_t K,
+                   int64_t lda, int64_t ldb, int64_t ldc, int out_dtype) {
+    Plan plan;
+    int rc = check_and_select(A_host, B_host, C_host, M, N, K, lda, ldb, ldc, out_dtype, &plan);
+    if (rc) return rc;
+    if (plan.path == TILE_GEMM_PATH_NOOP) return TILE_GEMM_OK;
+    int dev = 0, sms = 0;
+    rc = current_device(&dev, &sms);
+    if (rc) return rc;
+    {
+        std::lock_guard<std::mutex> lk(g_mu);
+        if (!g_host_stream) CUDA_TRY(cudaStreamCreateWithFlags(&g_host_stream, cudaStreamNonBlocking));
+        if ((rc = grow(g_stage[0], (size_t)plan.a_bytes + 16))) return rc;
+        if ((rc = grow(g_stage[1], (size_t)plan.b_bytes + 16))) return rc;
+        if ((rc = grow(g_stage[2], (size_t)plan.c_bytes + 16))) return rc;
+    }
+    cudaStream_t s = g_host_stream;
+    if (plan.a_bytes) CUDA_TRY(cudaMemcpyAsync(g_stage[0].p, A_host, (size_t)plan.a_bytes, cudaMemcpyHostToDevice, s));
+    if (plan.b_bytes) CUDA_TRY(cudaMemcpyAsync(g_stage[1].p, B_host, (size_t)plan.b_bytes, cudaMemcpyHostToDevice, s));
+    rc = tile_gemm(g_stage[0].p, g_stage[1].p, g_stage[2].p, M, N, K, lda, ldb, ldc, out_dtype, (void*)s);
+    if (rc) return rc;
+    CUDA_TRY(cudaMemcpy2DAsync(C_host, (size_t)ldc * plan.esize, g_stage[2].p, (size_t)ldc * plan.esize,
+                               (size_t)N * plan.esize, (size_t)M, cudaMemcpyDeviceToHost, s));
+    CUDA_TRY(cudaStreamSynchronize(s));
+    return TILE_GEMM_OK;
+}
+
+int tile_gemm_query_config(int64_t M, int64_t N, int64_t K, int out_dtype, int32_t out[8]) {
+    if (M <= 0 || N <= 0 || K < 0 || !out) return fail(TILE_GEMM_E_EXTENT, "query needs M, N > 0, K >= 0");
+    int dev = 0, sms = 0;
+    int rc = current_device(&dev, &sms);
+    if (rc) return rc;
+    GemmLaunch gl;
+    plan_gemm(M, N, K, out_dtype == TILE_GEMM_OUT_BF16, sms, &gl);
+    out[0] = tg::GEMM_BM;
+    out[1] = gl.cfg.bn;
+    out[2] = gl.cfg.cg;
+    out[3] = gl.ctas;
+    out[4] = gl.p.group_m;
+    out[5] = gl.cfg.stages;
+    out[6] = tg::GEMM_BK;
+    out[7] = 0;
+    return TILE_GEMM_OK;
+}
+
+int tile_gemm_debug_owner_map(int32_t* owner, int64_t M, int64_t N, int64_t K, int64_t ld_owner, int out_dtype,
+                              void* stream) {
+    if (M <= 0 || N <= 0 || K < 0) return fail(TILE_GEMM_E_EXTENT, "owner map needs M, N > 0, K >= 0");
+    if (!owner) return fail(TILE_GEMM_E_NULL, "owner is NULL");
+    if (ld_owner < N) return fail(TILE_GEMM_E_LDC, "ld_owner=%lld < N=%lld", (long long)ld_owner, (long long)N);
+    if ((uintptr_t)owner & 3) return fail(TILE_GEMM_E_ALIGN, "owner (%p) is not 4-byte aligned", (void*)owner);
+    int dev = 0, sms = 0;
+    int rc = current_device(&dev, &sms);
+    if (rc) return rc;
+    GemmLaunch gl;
+    plan_gemm(M, N, K, out_dtype == TILE_GEMM_OUT_BF16, sms, &gl);
+    gl.p.num_k_tiles = 0;   // same schedule and epilogue, no loads and no MMAs
+    gl.p.out_bf16 = 0;      // the map itself is written through the 32-bit epilogue
+    gl.p.owner_mode = 1;
+    gl.p.C = owner;
+    gl.p.ldc = ld_owner;
+    const bool c_tma = (((uintptr_t)owner & 15) == 0) && ((ld_owner * 4) % 16 == 0);
+    gl.p.tma_store = c_tma ? 1 : 0;
+    CUtensorMap tc;
+    if (c_tma) {
+        rc = c_tensor_map(&tc, owner, M, N, ld_owner, 0);
+    } else {
+        // any valid descriptor: it is prefetched but never used by the clipped-store epilogue
+        static void* dummy = nullptr;
+        if (!dummy) CUDA_TRY(cudaMalloc(&dummy, 32 * 128));
+        rc = get_tensor_map(&tc, dummy, 4, true, 32, 32, 128, 32u, 32u, true);
+    }
+    if (rc) return rc;
+    return launch_gemm(gl, tc, tc, tc, (cudaStream_t)stream, dev);
+}
+
+int tile_gemm_set_tuning(int key, int value) {
+    if (key < 0 || key >= 8) return fail(TILE_GEMM_E_PATH, "unknown tuning key %d", key);
+    g_tune[key].store(value);
+    return TILE_GEMM_OK;
+}
+
+int64_t tile_gemm_launch_count(void) { return g_launches.load(); }
+
+const char* tile_gemm_status_string(int status) {
+    if (status < 0 || status >= TILE_GEMM_NUM_STATUS) return "unknown status";
+    return kStatusNames[status];
+}
+
+const char* tile_gemm_last_error(void) { return g_err; }
+
+int tile_gemm_shutdown(void) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    for (auto& kv : g_ws)
+        if (kv.second.p) cudaFree(kv.second.p);
+    g_ws.clear();
+    for (Buf& b : g_stage) {
+        if (b.p) cudaFree(b.p);
+        b = Buf();
+    }
+    if (g_host_stream) { cudaStreamDestroy(g_host_stream); g_host_stream = nullptr; }
+    g_maps.clear();
+    return TILE_GEMM_OK;
+}
+
+}  // extern "C"
