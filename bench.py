@@ -1,0 +1,412 @@
+#!/usr/bin/env python
+"""bench.py -- headline measurement of the tile_gemm hot path on B200.
+
+    python bench.py --gpus N --steps K --warmup W            # this build (CUDA path, C ABI)
+    python bench.py --impl reference --steps K --warmup W    # the fp64 CPU oracle, timed as it stands
+
+One JSON line on stdout (rank 0).  A "step" is one call of tile_gemm on BASELINE.json's
+config[2] -- the 8192^3 BF16 GEMM with bf16 output the metric is quoted on -- which runs the
+whole GEMM path per call: launch preconditions (a1), selector (a2), persistent tile map (a3),
+TMA K-loop loads (a4), tcgen05 MMAs (a5), epilogue (a6).  The M=1 decode path (a7, config[4]:
+256 GEMVs over distinct 62.4 GB of weights) and the prefill projections (config[3]) are timed in
+the same run and reported under "gemv" / "prefill" with their own rooflines.
+
+N > 1: one process per GPU (torchrun), every rank runs the same independent problem (no
+data-path collective exists for this path), time = max over ranks, value = sum of the work.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "bf16_gemm_tflops"
+UNIT = "TFLOP/s"
+WORKLOAD = "cfg3: BF16 GEMM M=N=K=8192, A~N(0,1), B~N(0,1/K), fp32 accumulate, bf16 output, seed 2"
+L2_NOTE = "inputs 256 MiB per step > 126 MB L2; 4 rotating A/B/C sets so no step re-reads the previous step's data"
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return {"hbm_gbs": float(d["hbm_gbs"]), "bf16_tflops": float(d["bf16_tflops"]),
+                "bf16_tflops_sustained": float(d.get("bf16_tflops_sustained", d["bf16_tflops"])),
+                "source": "measured"}
+    # B200_PROFILING.md fallback
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "source": "fallback"}
+
+
+def ncu_traffic(key):
+    """Per-launch DRAM bytes of the dominant kernel from the committed ncu capture, or None."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f).get(key)
+    return None
+
+
+# ---------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """Samples SM clock, power and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        self.samples, self.reasons, self.stop_flag, self.thread = [], set(), False, None
+        self.max_mhz = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _loop(self):
+        nv = self.nv
+        names = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "sw_thermal_slowdown": 0x20,
+                 "hw_thermal_slowdown": 0x40, "hw_power_brake": 0x80}
+        while not self.stop_flag:
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(0.002)
+
+    def __enter__(self):
+        if self.nv:
+            self.thread = threading.Thread(target=self._loop, daemon=True)
+            self.thread.start()
+        return self
+
+    def __exit__(self, *a):
+        self.stop_flag = True
+        if self.thread:
+            self.thread.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ---------------------------------------------------------------------------- CPU oracle legs
+def oracle_gemm_sample(rows, seed=2):
+    """The oracle as it stands on a slab of cfg3: `rows` rows of A against all of B."""
+    import oracle
+    rng = np.random.default_rng([seed, 99])
+    from paper_2606_15991_b200 import workloads as wl
+    K = N = 8192
+    a = wl.f32_to_bf16_bits(rng.standard_normal((rows, K), dtype=np.float32))
+    b = wl.f32_to_bf16_bits(rng.standard_normal((K, N), dtype=np.float32) * np.float32(K ** -0.5))
+    oracle.gemm(a[:8], b)   # touch pages / load the library
+    t0 = time.perf_counter()
+    oracle.gemm(a, b)
+    dt = time.perf_counter() - t0
+    return 2.0 * rows * N * K / dt / 1e12, dt
+
+
+def cpu_baseline_leg(target_seconds=12.0):
+    import oracle
+    cores = oracle.default_threads()
+    tf, dt = oracle_gemm_sample(64)
+    rows = int(max(64, min(2048, 64 * target_seconds / max(dt, 1e-3))))
+    rows -= rows % 8
+    tf, dt = oracle_gemm_sample(rows)
+    return {"value": tf, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"oracle.gemm (fp64, C and S) on rows [0,{rows}) of cfg3 x all 8192 columns, K=8192; "
+                      f"{dt:.1f} s wall on {cores} threads"}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    oracle.build()
+    cores = oracle.default_threads()
+    _, dt8 = oracle_gemm_sample(32)
+    budget = 150.0 / max(1, args.steps + args.warmup)
+    rows = int(max(8, min(512, 32 * budget / max(dt8, 1e-3))))
+    rows -= rows % 8
+    for _ in range(args.warmup):
+        oracle_gemm_sample(rows)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_gemm_sample(rows)
+    # oracle_gemm_sample times only the oracle call; re-measure wall inclusive of input generation
+    wall = time.perf_counter() - t0
+    tf = np.mean([oracle_gemm_sample(rows)[0] for _ in range(1)]) if args.steps == 0 else None
+    # per-step oracle time measured precisely
+    per = [oracle_gemm_sample(rows)[1] for _ in range(max(1, min(3, args.steps)))]
+    ms = float(np.median(per)) * 1e3
+    value = 2.0 * rows * 8192 * 8192 / (ms * 1e-3) / 1e12
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "sample": f"each step = oracle.gemm on a {rows}-row slab (all N, all K)"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": f"{rows} rows x 8192 cols x K=8192 per step, {wall:.1f} s for the timed steps"},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ---------------------------------------------------------------------------- CUDA legs
+def time_region(fn_step, steps, stream_sync, dist_barrier):
+    """barrier+sync, K steps between two CUDA events on the launching stream, sync+barrier."""
+    import torch
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    dist_barrier()
+    stream_sync()
+    e0.record()
+    for i in range(steps):
+        fn_step(i)
+    e1.record()
+    stream_sync()
+    dist_barrier()
+    return e0.elapsed_time(e1)   # ms
+
+
+def bench_gemm(tg, wl, torch, case, steps, warmup, sets, tdist, sampler=None):
+    dev = torch.device("cuda", torch.cuda.current_device())
+    g = torch.Generator(device=dev)
+    g.manual_seed(1000 + case.seed[0])
+    out_dt = torch.bfloat16 if case.out_dtype == "bf16" else torch.float32
+    bufs = []
+    for _ in range(sets):
+        A = torch.empty((case.M, case.K), dtype=torch.bfloat16, device=dev).normal_(0, case.sigma_a, generator=g)
+        B = torch.empty((case.K, case.N), dtype=torch.bfloat16, device=dev).normal_(0, case.sigma_b, generator=g)
+        C = torch.empty((case.M, case.N), dtype=out_dt, device=dev)
+        bufs.append((A, B, C))
+
+    def step(i):
+        A, B, C = bufs[i % sets]
+        tg.tile_gemm(A, B, C)
+
+    for i in range(warmup):
+        step(i)
+    torch.cuda.synchronize()
+    l0 = tg.tile_gemm_launch_count()
+    if sampler is not None:
+        with sampler:
+            ms = time_region(step, steps, torch.cuda.synchronize, tdist.barrier)
+    else:
+        ms = time_region(step, steps, torch.cuda.synchronize, tdist.barrier)
+    launches = tg.tile_gemm_launch_count() - l0
+    ms = tdist.max_over_ranks(ms)
+    return ms / steps, launches, bufs
+
+
+def bench_e2e(tg, wl, torch, case, steps):
+    """Same metric through the C ABI with HOST buffers: H2D of A and B, GEMM, D2H of C per step."""
+    rng = np.random.default_rng(77)
+    esz = 2 if case.out_dtype == "bf16" else 4
+    A = torch.empty((case.M, case.K), dtype=torch.bfloat16).pin_memory()
+    B = torch.empty((case.K, case.N), dtype=torch.bfloat16).pin_memory()
+    C = torch.empty((case.M, case.N), dtype=torch.bfloat16 if esz == 2 else torch.float32).pin_memory()
+    A.copy_(torch.from_numpy(rng.standard_normal((case.M, case.K), dtype=np.float32)).to(torch.bfloat16))
+    B.copy_((torch.from_numpy(rng.standard_normal((case.K, case.N), dtype=np.float32)) * case.sigma_b).to(torch.bfloat16))
+    od = tg.OUT_BF16 if esz == 2 else tg.OUT_F32
+
+    def call():
+        rc = tg.tile_gemm_host_raw(A.data_ptr(), B.data_ptr(), C.data_ptr(), case.M, case.N, case.K,
+                                   case.K, case.N, case.N, od)
+        if rc != 0:
+            raise tg.TileGemmError(rc, tg.tile_gemm_last_error())
+
+    call()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        call()   # synchronous: returns after the D2H copy completed
+    dt = (time.perf_counter() - t0) / steps
+    h2d = (case.M * case.K + case.K * case.N) * 2
+    d2h = case.M * case.N * esz
+    tg.tile_gemm_shutdown()   # release the staging buffers
+    return dt, h2d, d2h, float(C.float().abs().mean())
+
+
+def bench_decode(tg, wl, torch, passes, warmup, layers, tdist):
+    """config[4]: 4 projections x `layers` layers, every weight in its own buffer."""
+    dev = torch.device("cuda", torch.cuda.current_device())
+    g = torch.Generator(device=dev)
+    g.manual_seed(4)
+    items = []
+    for layer in range(layers):
+        for (K, N) in wl.QWEN3_32B:
+            W = torch.empty((K, N), dtype=torch.bfloat16, device=dev).normal_(0, 0.02, generator=g)
+            x = torch.empty((1, K), dtype=torch.bfloat16, device=dev).normal_(0, 1.0, generator=g)
+            y = torch.empty((1, N), dtype=torch.bfloat16, device=dev)
+            items.append((x, W, y))
+    alg_bytes = sum(2 * K * N + 2 * K + 2 * N for (K, N) in wl.QWEN3_32B) * layers
+
+    def one_pass(_):
+        for x, W, y in items:
+            tg.tile_gemm(x, W, y)
+
+    for i in range(warmup):
+        one_pass(i)
+    torch.cuda.synchronize()
+    l0 = tg.tile_gemm_launch_count()
+    ms = time_region(one_pass, passes, torch.cuda.synchronize, tdist.barrier)
+    launches = tg.tile_gemm_launch_count() - l0
+    ms = tdist.max_over_ranks(ms) / passes
+    # per-shape kernel time (events around each projection class, one extra pass)
+    per_shape = {}
+    for p, (K, N) in enumerate(wl.QWEN3_32B):
+        sel = items[p::4]
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for x, W, y in sel:
+            tg.tile_gemm(x, W, y)
+        e1.record()
+        torch.cuda.synchronize()
+        t = e0.elapsed_time(e1) / len(sel)
+        per_shape[f"K{K}_N{N}"] = {"us": t * 1e3, "gbs": (2 * K * N + 2 * K + 2 * N) / (t * 1e-3) / 1e9}
+    # CUDA-graph replay of the same pass (decode engines replay a recorded step)
+    graph_ms = None
+    try:
+        graph = torch.cuda.CUDAGraph()
+        s = torch.cuda.Stream()
+        with torch.cuda.stream(s):
+            one_pass(0)
+            s.synchronize()
+            with torch.cuda.graph(graph, stream=s):
+                one_pass(0)
+        torch.cuda.synchronize()
+        graph.replay()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(passes):
+            graph.replay()
+        e1.record()
+        torch.cuda.synchronize()
+        graph_ms = e0.elapsed_time(e1) / passes
+    except Exception as exc:  # reported, never silently substituted for the headline
+        graph_ms = None
+        sys.stderr.write(f"[bench] graph replay variant unavailable: {exc}\n")
+    return ms, alg_bytes, launches, per_shape, graph_ms, len(items)
+
+
+def run_cuda(args):
+    import torch
+    from paper_2606_15991_b200 import binding as tg
+    from paper_2606_15991_b200 import dist as tdist
+    from paper_2606_15991_b200 import workloads as wl
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback); use --impl reference for the oracle")
+    rank, local_rank, world = tdist.init()
+    torch.cuda.set_device(local_rank)
+    tg.load_library()
+    peaks = measured_peaks()
+    case = wl.CFG3
+    flops = 2.0 * case.M * case.N * case.K
+
+    sampler = ClockSampler(local_rank)
+    ms_step, launches, bufs = bench_gemm(tg, wl, torch, case, args.steps, args.warmup, 4, tdist, sampler)
+    clocks = sampler.summary()
+    value = world * flops / (ms_step * 1e-3) / 1e12
+    per_gpu = flops / (ms_step * 1e-3) / 1e12
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "l2": L2_NOTE, "tile_config": tg.tile_gemm_query_config(case.M, case.N, case.K, tg.OUT_BF16),
+                   "parallelism": f"{world} independent replicas, no collective"},
+        "clocks": clocks,
+        "gpu_launches": int(launches * world),
+        "roofline": {"bound": "tensor", "achieved": per_gpu, "peak": peaks["bf16_tflops"], "unit": "TFLOP/s",
+                     "frac": per_gpu / peaks["bf16_tflops"], "traffic": ncu_traffic("gemm_8192_dram_bytes"),
+                     "peak_source": f"{peaks['source']} cuBLAS bf16 burst (MEASURED_PEAKS.json)",
+                     "frac_of_sustained": per_gpu / peaks["bf16_tflops_sustained"],
+                     "frac_of_nominal_2250": per_gpu / 2250.0,
+                     "kernel": "gemm_tcgen05_kernel<2,256,6>", "algorithmic_flops_per_launch": flops},
+    }
+    del bufs
+    torch.cuda.empty_cache()
+
+    if rank == 0 and not args.no_e2e:
+        dt, h2d, d2h, _ = bench_e2e(tg, wl, torch, case, max(2, min(args.steps, 5)))
+        line["e2e"] = {"value": flops / dt / 1e12, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                       "d2h_bytes_per_step": d2h, "ms_per_step": dt * 1e3,
+                       "api": "tile_gemm_host (pinned host A,B,C; H2D + GEMM + D2H per step)"}
+    tdist.barrier()
+
+    if not args.headline_only:
+        # config[3]: prefill projections
+        pre = {}
+        tot_ms, tot_fl = 0.0, 0.0
+        for c in wl.CFG4:
+            ms, _, b = bench_gemm(tg, wl, torch, c, max(5, args.steps // 4), 3, 2, tdist)
+            del b
+            torch.cuda.empty_cache()
+            fl = 2.0 * c.M * c.N * c.K
+            pre[c.name] = {"ms": ms, "tflops": fl / (ms * 1e-3) / 1e12}
+            tot_ms += ms
+            tot_fl += fl
+        pre["aggregate_tflops"] = tot_fl / (tot_ms * 1e-3) / 1e12
+        pre["frac_of_measured_peak"] = pre["aggregate_tflops"] / peaks["bf16_tflops"]
+        line["prefill"] = pre
+        # config[4]: decode GEMV sequence
+        ms, alg_bytes, gl, per_shape, graph_ms, n = bench_decode(tg, wl, torch, args.decode_passes, 2,
+                                                                 args.decode_layers, tdist)
+        gbs = alg_bytes / (ms * 1e-3) / 1e9
+        line["gemv"] = {
+            "metric": "decode_gemv_hbm_gbs", "value": gbs * world, "unit": "GB/s", "ms_per_pass": ms,
+            "launches_per_pass": n, "layers": args.decode_layers, "algorithmic_bytes_per_pass": alg_bytes,
+            "per_shape": per_shape,
+            "graph_replay": None if graph_ms is None else {"ms_per_pass": graph_ms,
+                                                           "gbs": alg_bytes / (graph_ms * 1e-3) / 1e9},
+            "roofline": {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                         "frac": gbs / peaks["hbm_gbs"], "traffic": ncu_traffic("gemv_gate_up_dram_bytes"),
+                         "peak_source": f"{peaks['source']} copy bandwidth (MEASURED_PEAKS.json)",
+                         "frac_of_8000": gbs / 8000.0, "kernel": "gemv_tma_kernel<3>"},
+        }
+    if rank == 0:
+        if not args.no_cpu_baseline and world == 1:
+            line["cpu_baseline"] = cpu_baseline_leg()
+        print(json.dumps(line), flush=True)
+    tdist.barrier()
+    tdist.shutdown()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--decode-passes", type=int, default=5)
+    ap.add_argument("--decode-layers", type=int, default=64)
+    ap.add_argument("--headline-only", action="store_true", help="skip the prefill and decode legs")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_cuda(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

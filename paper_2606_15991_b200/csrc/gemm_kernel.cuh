@@ -207,6 +207,10 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
         uint8_t* buf0_gen = smem_gen + L::EPI_OFF + ew * 2u * GEMM_EPI_BUF_BYTES;
         const int cols_per_chunk = p.out_bf16 ? 64 : 32;       // 128 B of C per row per chunk
         const int num_chunks = BN / cols_per_chunk;
+        // TMA stores clip at 16-byte granularity along a row (measured on B200): when N is not a
+        // multiple of 16 bytes of elements the chunk containing column N-1 takes the clipped
+        // st.global path so that C[i][N..] is never written.
+        const bool ragged_n = (p.N % (p.out_bf16 ? 8 : 4)) != 0;
         uint32_t acc = 0, acc_phase = 0, buf = 0;
         for (int t = first_tile; t < total_tiles; t += tile_stride) {
             int tm, tn;
@@ -257,7 +261,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
                         st_shared_v4(row_addr + ((j ^ sw) << 4), v[4 * j + 0], v[4 * j + 1], v[4 * j + 2],
                                      v[4 * j + 3]);
                 }
-                if (p.tma_store) {
+                if (p.tma_store && !(ragged_n && n0 + cols_per_chunk > p.N)) {
                     fence_proxy_async_smem();
                     __syncwarp();
                     if (lane == 0) {
@@ -298,6 +302,9 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
                         }
                     }
                     __syncwarp();
+                    // keep one bulk group per chunk so that wait_group.read<1> above always
+                    // refers to the buffer written two chunks ago
+                    if (lane == 0) tma_store_commit();
                 }
                 buf ^= 1u;
             }

@@ -1,0 +1,67 @@
+"""Comparison gates between the CUDA path and the fp64 oracle.
+
+contract gate   |C_gpu - C_ref| <= 2^-5 * S                         (BASELINE.json north_star)
+tight gate      fp32 out: |err| <= 2K * 2^-24 * S
+                bf16 out: |err| <= 2^-8 * |C_ref| + 2K * 2^-24 * S
+bit-exact       fp32 out, integer-valued inputs: identical bits after -0 -> +0
+
+The tight gates are derived from the arithmetic: any fp32 summation
+order of K exact products has error <= (K-1) * 2^-24 * S to first order, doubled as allowance;
+RNE to bf16 adds at most half an ulp = 2^-9 * |C| (2^-8 used).  rel_rms = ||C_gpu - C_ref||_F /
+||C_ref||_F must stay below 2^-16 + (K/16) * 2^-24 for fp32 output (2^-8 for bf16): the tensor
+core adds each K=16 step into the fp32 accumulator with truncation, a bias of up to one ulp of
+the running sum per step.  The contract gate alone is
+nearly vacuous on random data, so every test enforces both.
+"""
+import numpy as np
+
+CONTRACT = 2.0 ** -5
+
+
+def check_close(got, ref, S, K, out_dtype, what=""):
+    got = np.asarray(got, dtype=np.float64)
+    err = np.abs(got - ref)
+    assert not np.isnan(got).any(), f"{what}: NaN in output"
+    contract = err <= CONTRACT * S + 1e-300
+    assert contract.all(), f"{what}: contract gate violated at {np.argwhere(~contract)[:5].tolist()}"
+    acc = 2.0 * max(K, 1) * 2.0 ** -24 * S
+    tight = acc + 1e-300 if out_dtype == "f32" else 2.0 ** -8 * np.abs(ref) + acc + 1e-300
+    bad = err > tight
+    assert not bad.any(), (f"{what}: tight gate violated at {np.argwhere(bad)[:5].tolist()} "
+                           f"max err/S={np.max(err / np.maximum(S, 1e-300)):.3g}")
+    denom = np.linalg.norm(ref)
+    rel_rms = np.linalg.norm(got - ref) / denom if denom > 0 else 0.0
+    # fp32: 2^-16 floor plus one truncation of <= 1 ulp(running sum) per K=16 tensor-core step
+    # (the tcgen05 accumulator adds with truncation, not RNE; measured 2.95e-5 at K=25600).
+    rms_gate = (2.0 ** -16 + (max(K, 1) / 16.0) * 2.0 ** -24) if out_dtype == "f32" else 2.0 ** -8
+    assert rel_rms <= rms_gate, f"{what}: rel_rms={rel_rms:.3g} > {rms_gate:.3g}"
+    return {"max_err_over_S": float(np.max(err / np.maximum(S, 1e-300))), "rel_rms": float(rel_rms),
+            "checked": int(err.size)}
+
+
+def check_bit_exact(got_f32, ref_f64, what=""):
+    got = np.asarray(got_f32, dtype=np.float32)
+    want = np.asarray(ref_f64).astype(np.float32)
+    assert np.array_equal(want.astype(np.float64), ref_f64), f"{what}: reference not exact in fp32"
+    g = (got + np.float32(0.0)).view(np.uint32)   # -0 -> +0
+    w = (want + np.float32(0.0)).view(np.uint32)
+    bad = g != w
+    assert not bad.any(), f"{what}: {int(bad.sum())} elements differ, first at {np.argwhere(bad)[:5].tolist()}"
+
+
+def freivalds_rows(C_gpu_f64, a64, b64, seed=0):
+    """|C r - A (B r)| <= 2^-14 * ||C_i||_2 for every row, r in {+-1}^N (and columns likewise)."""
+    rng = np.random.default_rng([seed, 15485863])
+    M, N = C_gpu_f64.shape
+    r = rng.choice([-1.0, 1.0], size=N)
+    lhs = C_gpu_f64 @ r
+    rhs = a64 @ (b64 @ r)
+    tol = 2.0 ** -14 * np.linalg.norm(C_gpu_f64, axis=1) + 1e-30
+    bad = np.abs(lhs - rhs) > tol
+    assert not bad.any(), f"Freivalds row test failed for rows {np.where(bad)[0][:8].tolist()}"
+    c = rng.choice([-1.0, 1.0], size=M)
+    lhs = c @ C_gpu_f64
+    rhs = (c @ a64) @ b64
+    tol = 2.0 ** -14 * np.linalg.norm(C_gpu_f64, axis=0) + 1e-30
+    bad = np.abs(lhs - rhs) > tol
+    assert not bad.any(), f"Freivalds column test failed for columns {np.where(bad)[0][:8].tolist()}"

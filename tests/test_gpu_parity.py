@@ -1,0 +1,367 @@
+"""Parity of the CUDA path (through the C ABI) against the fp64 oracle, on a B200.
+
+Covers BASELINE.json's five configs at full size in the launch configuration bench.py times,
+plus the extra cases SURVEY.md 8(c) asks for: one-hot inputs per tile configuration, integer
+ragged / large-K shapes bit-exact, canary-filled C, owner map, force_path sweep, determinism,
+degenerate extents and the host-buffer entry.
+"""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2606_15991_b200 import binding as tg
+from paper_2606_15991_b200 import workloads as wl
+from parity import check_bit_exact, check_close, freivalds_rows
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+CANARY_F32 = 0x7FC0DEAD
+CANARY_BF16 = 0x7FD5
+
+
+@pytest.fixture(autouse=True)
+def _reset_tuning():
+    yield
+    for key in range(5):
+        tg.tile_gemm_set_tuning(key, 0)
+    torch.cuda.synchronize()
+
+
+def device_operand(bits, pad_cols=0, misalign_elems=0):
+    """bf16 operand on the device with `pad_cols` extra (NaN) columns per row and an optional
+    element offset of the base pointer; returns a strided view."""
+    r, c = bits.shape
+    ld = c + pad_cols
+    flat = torch.full((r * ld + misalign_elems + 8,), float("nan"), dtype=torch.bfloat16, device=DEV)
+    view = flat[misalign_elems:misalign_elems + r * ld].view(r, ld)[:, :c]
+    view.copy_(wl.bits_to_torch(bits, DEV))
+    return view
+
+
+class CanaryC:
+    """C with guard rows above/below and padding columns, all canary filled."""
+
+    def __init__(self, M, N, out, pad_cols=0, guard=8, misalign_elems=0):
+        self.M, self.N, self.out, self.guard = M, N, out, guard
+        self.ld = N + pad_cols
+        rows = M + 2 * guard
+        if out == "f32":
+            self.raw = torch.full((rows * self.ld + misalign_elems + 4,), 0, dtype=torch.int32, device=DEV)
+            self.raw.fill_(np.int32(CANARY_F32))
+            self.dtype, self.canary = torch.float32, np.uint32(CANARY_F32)
+        else:
+            self.raw = torch.full((rows * self.ld + misalign_elems + 8,), 0, dtype=torch.int16, device=DEV)
+            self.raw.fill_(np.int16(CANARY_BF16))
+            self.dtype, self.canary = torch.bfloat16, np.uint16(CANARY_BF16)
+        self.full = self.raw[misalign_elems:misalign_elems + rows * self.ld].view(rows, self.ld)
+        self.C = self.full[guard:guard + M, :N].view(self.dtype)
+
+    def check(self, what=""):
+        """Guards untouched, every inside element overwritten.  Returns C as float64."""
+        host = self.full.cpu().numpy()
+        bits = host.view(np.uint32 if self.out == "f32" else np.uint16)
+        g = self.guard
+        outside = np.ones(bits.shape, dtype=bool)
+        outside[g:g + self.M, :self.N] = False
+        touched = outside & (bits != self.canary)
+        assert not touched.any(), (f"{what}: {int(touched.sum())} elements written outside C[0:M,0:N], "
+                                   f"first at (row-guard, col) {(np.argwhere(touched)[:5] - [g, 0]).tolist()}")
+        inside = bits[g:g + self.M, :self.N]
+        assert not (inside == self.canary).any(), f"{what}: some elements of C were never written"
+        if self.out == "f32":
+            return inside.view(np.float32).astype(np.float64)
+        return oracle.bf16_decode(np.ascontiguousarray(inside))
+
+
+def run_case(a_bits, b_bits, out="f32", pads=(0, 0, 0), force=tg.PATH_AUTO, misalign=(0, 0, 0), what=""):
+    M, K = a_bits.shape
+    N = b_bits.shape[1]
+    A = device_operand(a_bits, pads[0], misalign[0])
+    B = device_operand(b_bits, pads[1], misalign[1])
+    cc = CanaryC(M, N, out, pads[2], misalign_elems=misalign[2])
+    tg.tile_gemm(A, B, cc.C, force_path=force)
+    torch.cuda.synchronize()
+    return cc.check(what)
+
+
+def rne_bf16(x64):
+    """Library RNE (torch) of fp32 values to bf16, back as float64."""
+    t = torch.from_numpy(np.asarray(x64, dtype=np.float32)).to(torch.bfloat16)
+    return t.to(torch.float64).numpy()
+
+
+# ------------------------------------------------------------------ library actually loaded
+def test_native_library_is_loaded_and_launches():
+    tg.load_library()
+    maps = open("/proc/self/maps").read()
+    assert "libtilegemm.so" in maps
+    before = tg.tile_gemm_launch_count()
+    a, b = wl.make_inputs(wl.CFG1)
+    run_case(a, b)
+    assert tg.tile_gemm_launch_count() > before
+
+
+# ------------------------------------------------------------------ config 1
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3])
+def test_cfg1_bit_exact(cfg):
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMM_CONFIG, cfg)
+    a, b = wl.make_inputs(wl.CFG1)
+    ref, _ = oracle.gemm(a, b)
+    got = run_case(a, b, "f32", what=f"cfg1 config={cfg}")
+    check_bit_exact(got, ref, f"cfg1 config={cfg}")
+    got = run_case(a, b, "bf16", what=f"cfg1 bf16 config={cfg}")
+    assert np.array_equal(got, rne_bf16(ref))
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_one_hot_rows_and_columns(cfg):
+    """a_{i,pi(i)} = 1 gives C_i. = B_{pi(i)}. exactly: any k-pairing, transposition, swizzle or
+    descriptor error in the tensor-core path shows up as a wrong row/column."""
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMM_CONFIG, cfg)
+    rng = np.random.default_rng(cfg)
+    M, N, K = 384, 640, 448
+    pi = rng.integers(0, K, size=M)
+    A = np.zeros((M, K), np.float32)
+    A[np.arange(M), pi] = 1.0
+    bb = wl.f32_to_bf16_bits(rng.standard_normal((K, N)).astype(np.float32))
+    got = run_case(wl.f32_to_bf16_bits(A), bb, what="one-hot rows")
+    assert np.array_equal(got, oracle.bf16_decode(bb)[pi])
+    pj = rng.integers(0, K, size=N)
+    Bm = np.zeros((K, N), np.float32)
+    Bm[pj, np.arange(N)] = 1.0
+    ab = wl.f32_to_bf16_bits(rng.standard_normal((M, K)).astype(np.float32))
+    got = run_case(ab, wl.f32_to_bf16_bits(Bm), what="one-hot columns")
+    assert np.array_equal(got, oracle.bf16_decode(ab)[:, pj])
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+@pytest.mark.parametrize("K", [1, 63, 64, 65, 257])
+def test_all_ones_any_k(cfg, K):
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMM_CONFIG, cfg)
+    M, N = 130, 264
+    ones = lambda r, c: wl.f32_to_bf16_bits(np.ones((r, c), np.float32))
+    got = run_case(ones(M, K), ones(K, N), "f32", what="all ones")
+    assert np.all(got == K)
+    got = run_case(ones(M, K), ones(K, N), "bf16", what="all ones bf16")
+    assert np.all(got == rne_bf16(np.array([float(K)]))[0])
+
+
+# ------------------------------------------------------------------ config 2 (ragged, canary)
+LAYOUTS = {
+    "packed": ((0, 0, 0), (0, 0, 0)),                       # lda=769, ldb=ldc=1537: repack + st.global
+    "padded": ((776 - 769, 1544 - 1537, 1544 - 1537), (0, 0, 0)),   # TMA loads and TMA stores
+    "offset": ((776 - 769, 1544 - 1537, 1544 - 1537), (1, 3, 1)),   # 16-byte multiples, odd bases
+    "mixed": ((776 - 769, 0, 1544 - 1537), (0, 0, 0)),      # only B needs a repack
+}
+
+
+@pytest.mark.parametrize("layout", list(LAYOUTS))
+@pytest.mark.parametrize("out", ["f32", "bf16"])
+def test_cfg2_ragged_full_oracle_and_canary(layout, out):
+    pads, mis = LAYOUTS[layout]
+    a, b = wl.make_inputs(wl.CFG2)
+    ref, S = oracle.gemm(a, b)
+    got = run_case(a, b, out, pads=pads, misalign=mis, what=f"cfg2 {layout} {out}")
+    check_close(got, ref, S, wl.CFG2.K, out, f"cfg2 {layout} {out}")
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+@pytest.mark.parametrize("layout", ["packed", "padded"])
+def test_cfg2_shape_integer_inputs_bit_exact(cfg, layout):
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMM_CONFIG, cfg)
+    pads, mis = LAYOUTS[layout]
+    a, b = wl.make_inputs_custom(1023, 1537, 769, "int4", seed=21)
+    ref, _ = oracle.gemm(a, b)
+    got = run_case(a, b, "f32", pads=pads, misalign=mis, what=f"cfg2-int {layout} config={cfg}")
+    check_bit_exact(got, ref, f"cfg2-int {layout} config={cfg}")
+
+
+def test_force_path_sweep_agrees():
+    a, b = wl.make_inputs_custom(300, 520, 200, "int4", seed=5)
+    ref, _ = oracle.gemm(a, b)
+    for force in (tg.PATH_GEMM_TMA, tg.PATH_GEMM_REPACK):
+        got = run_case(a, b, "f32", force=force, what=f"force={force}")
+        check_bit_exact(got, ref, f"force={force}")
+    # M = 1 through the tensor-core path and through every GEMV variant
+    a, b = wl.make_inputs_custom(1, 1032, 520, "int4", seed=6)
+    ref, _ = oracle.gemm(a, b)
+    for force in (tg.PATH_GEMM_TMA, tg.PATH_GEMM_REPACK, tg.PATH_GEMV):
+        check_bit_exact(run_case(a, b, "f32", force=force), ref, f"M=1 force={force}")
+
+
+def test_large_k_integer_bit_exact():
+    a, b = wl.make_inputs_custom(512, 768, 8192, "int4", seed=8)
+    ref, _ = oracle.gemm(a, b)
+    check_bit_exact(run_case(a, b, "f32"), ref, "K=8192 ints")
+
+
+# ------------------------------------------------------------------ GEMV variants
+@pytest.mark.parametrize("variant", [1, 2, 3])
+@pytest.mark.parametrize("split", [0, 1, 3, 8])
+def test_gemv_variants_integer_bit_exact(variant, split):
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMV_VARIANT, variant)
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMV_SPLIT, split)
+    for (K, N, padb) in ((512, 1024, 0), (769, 1537, 7), (2000, 264, 0), (64, 8, 0), (1, 300, 4)):
+        a, b = wl.make_inputs_custom(1, N, K, "int4", seed=K + N)
+        ref, _ = oracle.gemm(a, b)
+        got = run_case(a, b, "f32", pads=(0, padb, 0), what=f"gemv v{variant} s{split} K={K} N={N}")
+        check_bit_exact(got, ref, f"gemv v{variant} s{split} K={K} N={N}")
+
+
+def test_gemv_unaligned_weights_take_scalar_path():
+    a, b = wl.make_inputs_custom(1, 1537, 769, "normal", seed=3)
+    ref, S = oracle.gemm(a, b)
+    for out in ("f32", "bf16"):
+        got = run_case(a, b, out, misalign=(1, 1, 1), what="gemv odd")
+        check_close(got, ref, S, 769, out, "gemv odd ldb / odd base")
+
+
+# ------------------------------------------------------------------ config 3 (headline)
+def test_cfg3_8192_sampled_freivalds_and_rounding_chain():
+    case = wl.CFG3
+    a, b = wl.make_inputs(case)
+    A, B = wl.bits_to_torch(a, DEV), wl.bits_to_torch(b, DEV)
+    C32 = torch.empty((case.M, case.N), dtype=torch.float32, device=DEV)
+    Cb = torch.empty((case.M, case.N), dtype=torch.bfloat16, device=DEV)
+    Cb2 = torch.empty_like(Cb)
+    tg.tile_gemm(A, B, C32)
+    tg.tile_gemm(A, B, Cb)
+    tg.tile_gemm(A, B, Cb2)
+    torch.cuda.synchronize()
+    assert torch.equal(Cb.view(torch.int16), Cb2.view(torch.int16)), "run-to-run bits differ"
+    # (ii) the bf16 result is RNE of the fp32 result bit for bit (same main loop)
+    assert torch.equal(C32.to(torch.bfloat16).view(torch.int16), Cb.view(torch.int16))
+    rows, cols = wl.stratified_samples(case.M, case.N, 128, seed=2)
+    assert rows.size == 4096
+    c_ref, s_ref = oracle.gemm_sampled(a, b, rows, cols)
+    got32 = C32[torch.from_numpy(rows).to(DEV), torch.from_numpy(cols).to(DEV)].cpu().numpy()
+    gotb = Cb[torch.from_numpy(rows).to(DEV), torch.from_numpy(cols).to(DEV)].float().cpu().numpy()
+    check_close(got32, c_ref, s_ref, case.K, "f32", "cfg3 fp32 samples")
+    check_close(gotb, c_ref, s_ref, case.K, "bf16", "cfg3 bf16 samples")
+    # (i) Freivalds on the full fp32 matrix
+    freivalds_rows(C32.cpu().numpy().astype(np.float64), oracle.bf16_decode(a), oracle.bf16_decode(b), seed=2)
+
+
+# ------------------------------------------------------------------ config 4 (prefill projections)
+@pytest.mark.parametrize("proj", [0, 1, 2, 3])
+def test_cfg4_prefill_sampled(proj):
+    case = wl.CFG4[proj]
+    a, b = wl.make_inputs(case)
+    A, B = wl.bits_to_torch(a, DEV), wl.bits_to_torch(b, DEV)
+    Cb = torch.empty((case.M, case.N), dtype=torch.bfloat16, device=DEV)
+    C32 = torch.empty((case.M, case.N), dtype=torch.float32, device=DEV)
+    tg.tile_gemm(A, B, Cb)
+    tg.tile_gemm(A, B, C32)
+    torch.cuda.synchronize()
+    assert torch.equal(C32.to(torch.bfloat16).view(torch.int16), Cb.view(torch.int16))
+    rows, cols = wl.uniform_samples(case.M, case.N, 4096, seed=proj)
+    c_ref, s_ref = oracle.gemm_sampled(a, b, rows, cols)
+    ri, ci = torch.from_numpy(rows).to(DEV), torch.from_numpy(cols).to(DEV)
+    check_close(Cb[ri, ci].float().cpu().numpy(), c_ref, s_ref, case.K, "bf16", case.name)
+    check_close(C32[ri, ci].cpu().numpy(), c_ref, s_ref, case.K, "f32", case.name + " fp32")
+    # Freivalds over a 1024-row band of the fp32 result (full width, all K)
+    band = slice(1024, 2048)
+    a64 = oracle.bf16_decode(a[band])
+    r = np.random.default_rng(proj).choice([-1.0, 1.0], size=case.N)
+    br = np.zeros(case.K)
+    for k0 in range(0, case.K, 1024):
+        br[k0:k0 + 1024] = oracle.bf16_decode(b[k0:k0 + 1024]) @ r
+    Cband = C32[band].cpu().numpy().astype(np.float64)
+    tol = 2.0 ** -14 * np.linalg.norm(Cband, axis=1)
+    assert np.all(np.abs(Cband @ r - a64 @ br) <= tol)
+
+
+# ------------------------------------------------------------------ config 5 (decode GEMV)
+def _cfg5_layers():
+    if os.environ.get("TILEGEMM_FULL_CFG5") == "1":
+        return list(range(wl.DECODE_LAYERS))
+    return [0, wl.DECODE_LAYERS - 1]
+
+
+def test_cfg5_decode_full_oracle():
+    """Every output of every checked GEMV against the oracle, in the auto launch configuration.
+    Default: layers {0, 63} x 4 projections (8 GEMVs, 1.95 GB of weights); TILEGEMM_FULL_CFG5=1
+    checks all 64 layers (256 GEMVs, 62.4 GB)."""
+    for layer in _cfg5_layers():
+        for proj in range(4):
+            case = wl.cfg5_case(layer, proj)
+            x, W = wl.make_inputs_device(case, DEV)
+            y = torch.empty((1, case.N), dtype=torch.bfloat16, device=DEV)
+            assert tg.tile_gemm_select(1, case.N, case.K, case.K, case.N, case.N) == tg.PATH_GEMV
+            tg.tile_gemm(x, W, y)
+            torch.cuda.synchronize()
+            ref, S = oracle.gemm(wl.torch_to_bits(x), wl.torch_to_bits(W))
+            check_close(y.float().cpu().numpy(), ref, S, case.K, "bf16", case.name)
+            del W
+
+
+# ------------------------------------------------------------------ ownership
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+@pytest.mark.parametrize("shape", [(1023, 1537), (256, 256), (4096, 5120), (130, 70)])
+def test_owner_map_is_the_documented_function(cfg, shape):
+    """Each output element is written by exactly one CTA, the one tile_coords assigns
+    (PAPER.md:163 'each sub-tensor has exactly one owner')."""
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMM_CONFIG, cfg)
+    M, N = shape
+    conf = tg.tile_gemm_query_config(M, N, 64)
+    for ld in (N, N + 3):
+        owner = tg.tile_gemm_debug_owner_map(M, N, 64, ld_owner=ld)
+        torch.cuda.synchronize()
+        host = owner.cpu().numpy()
+        assert np.all(host[:, N:] == -1), "padding columns were written"
+        want = tg.expected_owner_map(M, N, conf)
+        assert np.array_equal(host[:, :N].astype(np.int64), want)
+        ctas = np.unique(host[:, :N] & 0xFF)
+        assert ctas.max() < conf["ctas"]
+
+
+# ------------------------------------------------------------------ degenerate + errors
+def test_k_zero_writes_zeros_and_empty_is_noop():
+    for out in ("f32", "bf16"):
+        a = np.zeros((37, 0), np.uint16)
+        b = np.zeros((0, 53), np.uint16)
+        got = run_case(a, b, out, pads=(4, 3, 5), what="K=0")
+        assert np.all(got == 0)
+    C = torch.full((4, 4), 7.0, device=DEV)
+    A = torch.zeros((0, 4), dtype=torch.bfloat16, device=DEV)
+    B = torch.zeros((4, 4), dtype=torch.bfloat16, device=DEV)
+    assert tg.tile_gemm_raw(A.data_ptr(), B.data_ptr(), C.data_ptr(), 0, 4, 4, 4, 4, 4, 0) == 0
+    assert tg.tile_gemm_raw(A.data_ptr(), B.data_ptr(), C.data_ptr(), 4, 0, 4, 4, 4, 4, 0) == 0
+    torch.cuda.synchronize()
+    assert torch.all(C == 7.0)
+
+
+def test_precondition_failures_enqueue_nothing():
+    C = torch.full((8, 8), 3.0, device=DEV)
+    A = torch.ones((8, 8), dtype=torch.bfloat16, device=DEV)
+    B = torch.ones((8, 8), dtype=torch.bfloat16, device=DEV)
+    before = tg.tile_gemm_launch_count()
+    p = (A.data_ptr(), B.data_ptr(), C.data_ptr())
+    assert tg.tile_gemm_raw(*p, 8, 8, 8, 7, 8, 8, 0) == tg.E_LDA
+    assert tg.tile_gemm_raw(*p, 8, 8, 8, 8, 7, 8, 0) == tg.E_LDB
+    assert tg.tile_gemm_raw(*p, 8, 8, 8, 8, 8, 7, 0) == tg.E_LDC
+    assert tg.tile_gemm_raw(*p, 8, 8, 8, 8, 8, 8, 2) == tg.E_DTYPE
+    assert tg.tile_gemm_raw(A.data_ptr(), B.data_ptr(), A.data_ptr(), 8, 8, 8, 8, 8, 8, 1) == tg.E_ALIAS
+    assert tg.tile_gemm_raw(0, B.data_ptr(), C.data_ptr(), 8, 8, 8, 8, 8, 8, 0) == tg.E_NULL
+    assert tg.tile_gemm_raw(*p, 8, 8, 8, 8, 8, 8, 0, 0, tg.PATH_GEMV) == tg.E_PATH
+    torch.cuda.synchronize()
+    assert tg.tile_gemm_launch_count() == before
+    assert torch.all(C == 3.0)
+
+
+# ------------------------------------------------------------------ host-buffer entry (e2e)
+def test_host_entry_matches_oracle():
+    a, b = wl.make_inputs_custom(333, 520, 129, "normal", seed=12)
+    ref, S = oracle.gemm(a, b)
+    C = np.full((333, 528), np.float32(-77.0))
+    tg.tile_gemm_host(a, b, C[:, :520])
+    check_close(C[:, :520], ref, S, 129, "f32", "host entry")
+    assert np.all(C[:, 520:] == -77.0)
+    x, W = wl.make_inputs_custom(1, 2048, 1024, "normal", seed=13)
+    ref, S = oracle.gemm(x, W)
+    y = np.zeros((1, 2048), np.uint16)
+    tg.tile_gemm_host(x, W, y)
+    check_close(oracle.bf16_decode(y), ref, S, 1024, "bf16", "host entry gemv")

@@ -1,0 +1,151 @@
+"""CPU tests of the boundary: the C-ABI library loads and exports every symbol the header
+declares, launch preconditions and the selector behave as include/tile_gemm.h states (pure
+host, fake pointers, nothing dereferenced), the schedule function covers C exactly once, and
+the N>1 helpers work over gloo with world_size 2.  No compute call is made (no GPU here)."""
+import os
+import re
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_15991_b200 import binding as tg
+from paper_2606_15991_b200 import workloads as wl
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+A0, B0, C0 = 0x10000, 0x7000_0000_0000, 0x7100_0000_0000   # fake, well separated, 16-byte aligned
+
+
+def test_library_exports_every_declared_symbol():
+    header = open(os.path.join(ROOT, "include", "tile_gemm.h")).read()
+    declared = set(re.findall(r"\b(tile_gemm\w*)\s*\(", header))
+    assert declared == set(tg.EXPORTS), declared ^ set(tg.EXPORTS)
+    lib = tg.load_library()
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+def test_status_strings_are_distinct():
+    names = [tg.tile_gemm_status_string(i) for i in range(14)]
+    assert len(set(names)) == 14 and names[0] == "ok"
+    assert tg.tile_gemm_status_string(99) == "unknown status"
+
+
+def sel(M, N, K, lda=None, ldb=None, ldc=None, A=A0, B=B0, C=C0, out=tg.OUT_F32):
+    return tg.tile_gemm_select(M, N, K, K if lda is None else lda, N if ldb is None else ldb,
+                               N if ldc is None else ldc, A, B, C, out)
+
+
+def test_selector_paths_for_baseline_configs():
+    assert sel(256, 256, 256) == tg.PATH_GEMM_TMA
+    assert sel(1023, 1537, 769) == tg.PATH_GEMM_REPACK            # packed rows are not 16-byte multiples
+    assert sel(1023, 1537, 769, 776, 1544, 1544) == tg.PATH_GEMM_TMA
+    assert sel(8192, 8192, 8192, out=tg.OUT_BF16) == tg.PATH_GEMM_TMA
+    for (K, N) in wl.QWEN3_32B:
+        assert sel(4096, N, K, out=tg.OUT_BF16) == tg.PATH_GEMM_TMA
+        assert sel(1, N, K, out=tg.OUT_BF16) == tg.PATH_GEMV
+    assert sel(256, 256, 256, A=A0 + 2) == tg.PATH_GEMM_REPACK     # misaligned base
+    assert sel(1, 1537, 769) == tg.PATH_GEMV                       # GEMV needs no alignment
+    assert sel(5, 7, 0) == tg.PATH_ZERO
+    assert sel(0, 7, 3) == tg.PATH_NOOP and sel(7, 0, 3) == tg.PATH_NOOP
+
+
+@pytest.mark.parametrize("kwargs,code,fragment", [
+    (dict(M=-1, N=4, K=4), tg.E_EXTENT, "negative extent"),
+    (dict(M=4, N=4, K=4, lda=3), tg.E_LDA, "lda=3 < K=4"),
+    (dict(M=4, N=4, K=4, ldb=3), tg.E_LDB, "ldb=3 < N=4"),
+    (dict(M=4, N=4, K=4, ldc=3), tg.E_LDC, "ldc=3 < N=4"),
+    (dict(M=4, N=4, K=4, out=7), tg.E_DTYPE, "out_dtype=7"),
+    (dict(M=4, N=4, K=4, A=0), tg.E_NULL, "A is NULL"),
+    (dict(M=4, N=4, K=4, B=0), tg.E_NULL, "B is NULL"),
+    (dict(M=4, N=4, K=4, C=0), tg.E_NULL, "C is NULL"),
+    (dict(M=4, N=4, K=4, A=A0 + 1), tg.E_ALIGN, "2-byte aligned"),
+    (dict(M=4, N=4, K=4, C=C0 + 2), tg.E_ALIGN, "4-byte aligned"),
+    (dict(M=4, N=4, K=4, C=A0 + 8), tg.E_ALIAS, "overlaps A"),
+    (dict(M=4, N=4, K=4, C=B0), tg.E_ALIAS, "overlaps B"),
+    (dict(M=2 ** 31, N=4, K=4), tg.E_OVERFLOW, "extent above"),
+    (dict(M=2 ** 20, N=4, K=4, lda=2 ** 45), tg.E_OVERFLOW, "overflow"),
+])
+def test_each_precondition_has_its_own_error(kwargs, code, fragment):
+    """'each rejected on the host with its own message'."""
+    assert sel(**kwargs) == -code
+    assert fragment in tg.tile_gemm_last_error()
+
+
+def test_bf16_output_alignment_is_two_bytes():
+    assert sel(4, 4, 4, C=C0 + 2, out=tg.OUT_BF16) > 0
+    assert sel(4, 4, 4, C=C0 + 1, out=tg.OUT_BF16) == -tg.E_ALIGN
+
+
+def test_strided_operands_that_only_touch_do_not_alias():
+    a_bytes = (4 - 1) * 4 * 2 + 4 * 2
+    assert sel(4, 4, 4, C=A0 + a_bytes + 2, out=tg.OUT_BF16) > 0      # directly after A's span
+    assert sel(4, 4, 4, C=A0 + a_bytes - 2, out=tg.OUT_BF16) == -tg.E_ALIAS
+
+
+def test_compute_entries_fail_loudly_without_a_gpu():
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    rc = tg.tile_gemm_raw(A0, B0, C0, 4, 4, 4, 4, 4, 4, 0)
+    assert rc == tg.E_DEVICE
+    assert "no CPU fallback" in tg.tile_gemm_last_error()
+    rc = tg.tile_gemm_host_raw(A0, B0, C0, 4, 4, 4, 4, 4, 4, 0)
+    assert rc == tg.E_DEVICE
+
+
+def test_bad_force_path_and_tuning_key():
+    assert tg.tile_gemm_raw(A0, B0, C0, 4, 4, 4, 4, 4, 4, 0, 0, 9) == tg.E_PATH
+    with pytest.raises(tg.TileGemmError):
+        tg.tile_gemm_set_tuning(99, 0)
+
+
+@pytest.mark.parametrize("cfg", [
+    dict(BM=128, BN=128, cta_group=1, ctas=148, group_m=16),
+    dict(BM=128, BN=256, cta_group=1, ctas=56, group_m=16),
+    dict(BM=128, BN=256, cta_group=2, ctas=148, group_m=8),
+    dict(BM=128, BN=256, cta_group=2, ctas=8, group_m=3),
+])
+@pytest.mark.parametrize("shape", [(1023, 1537), (8192, 8192), (130, 70), (4096, 5120)])
+def test_schedule_function_covers_every_element_once(cfg, shape):
+    """The tile -> owner map restated on the host is a function onto [0,M) x [0,N): every
+    element has exactly one owning tile and CTA ids stay below the launched count."""
+    M, N = shape
+    own = tg.expected_owner_map(M, N, cfg)
+    assert own.min() >= 0
+    tile_m = cfg["BM"] * cfg["cta_group"]
+    tiles = -(-M // tile_m) * -(-N // cfg["BN"])
+    ids = np.unique(own >> 8)
+    assert ids.size == tiles and ids.max() == tiles - 1
+    assert (own & 0xFF).max() < cfg["ctas"]
+    # each tile id occupies one BM*cg x BN rectangle
+    t = int(ids[len(ids) // 2])
+    rr, cc = np.where((own >> 8) == t)
+    assert rr.max() - rr.min() < tile_m and cc.max() - cc.min() < cfg["BN"]
+
+
+def test_workload_shapes_match_baseline_json():
+    assert (wl.CFG1.M, wl.CFG1.N, wl.CFG1.K) == (256, 256, 256)
+    assert (wl.CFG2.M, wl.CFG2.N, wl.CFG2.K) == (1023, 1537, 769)
+    assert (wl.CFG3.M, wl.CFG3.N, wl.CFG3.K) == (8192, 8192, 8192)
+    assert [(c.K, c.N) for c in wl.CFG4] == [(5120, 10240), (5120, 8192), (5120, 51200), (25600, 5120)]
+    assert all(c.M == 4096 for c in wl.CFG4)
+    a, b = wl.make_inputs(wl.CFG1)
+    a2, _ = wl.make_inputs(wl.CFG1)
+    assert np.array_equal(a, a2)
+    vals = wl.bits_to_torch(a).float().numpy()
+    assert set(np.unique(vals)) <= set(range(-4, 5))
+    r, c = wl.stratified_samples(8192, 8192, 128, seed=2)
+    assert r.size == 4096 and len(set(zip((r // 128).tolist(), (c // 128).tolist()))) == 4096
+
+
+def test_gloo_world_size_two_bench_helpers():
+    """bench.py's N>1 plumbing (unit sharding, max-over-ranks timing) over gloo on CPU."""
+    script = os.path.join(ROOT, "tests", "gloo_worker.py")
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT="29541", PYTHONPATH=ROOT)
+    res = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2",
+                          "--master-addr", "127.0.0.1", "--master-port", "29541", script],
+                         env=env, capture_output=True, text=True, timeout=300)
+    assert res.returncode == 0, res.stdout + res.stderr
+    assert "GLOO_OK rank0" in res.stdout
