@@ -317,6 +317,10 @@ def run_cuda(args):
     rank, local_rank, world = tdist.init()
     torch.cuda.set_device(local_rank)
     tg.load_library()
+    if args.gemm_config:
+        tg.tile_gemm_set_tuning(tg.TUNE_GEMM_CONFIG, args.gemm_config)
+    if args.group_m:
+        tg.tile_gemm_set_tuning(tg.TUNE_GEMM_GROUP_M, args.group_m)
     peaks = measured_peaks()
     case = wl.CFG3
     flops = 2.0 * case.M * case.N * case.K
@@ -401,6 +405,8 @@ def main():
     ap.add_argument("--headline-only", action="store_true", help="skip the prefill and decode legs")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--gemm-config", type=int, default=0, help="force a GEMM tile config (tile_gemm_set_tuning key 0)")
+    ap.add_argument("--group-m", type=int, default=0, help="force the raster group height (tuning key 1)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
     if args.impl == "reference":

@@ -137,7 +137,7 @@ int tile_gemm_debug_owner_map(int32_t* owner, int64_t M, int64_t N, int64_t K,
  * host program can rebuild the owner map: out[0]=BM (rows per CTA),
  * out[1]=BN (columns per tile), out[2]=cta_group (1 or 2: CTAs per tile, tile
  * rows = BM*cta_group), out[3]=number of CTAs launched, out[4]=GROUP_M (tile
- * rows per raster group), out[5]=pipeline stages, out[6]=BK, out[7]=reserved.
+ * rows per raster group), out[5]=pipeline stages, out[6]=BK, out[7]=config id.
  * Needs a CUDA device (SM count).  Returns a status code.
  */
 int tile_gemm_query_config(int64_t M, int64_t N, int64_t K, int out_dtype, int32_t out[8]);
@@ -145,7 +145,7 @@ int tile_gemm_query_config(int64_t M, int64_t N, int64_t K, int out_dtype, int32
 /*
  * Tuning / test overrides, process-global, not thread-safe against concurrent
  * tile_gemm calls.  key: 0 = GEMM config (0 auto, 1 = 1-CTA 128x128, 2 = 1-CTA
- * 128x256, 3 = 2-CTA 256x256), 1 = GEMM GROUP_M (0 auto), 2 = GEMM max CTAs
+ * 128x256, 3 = 2-CTA 256x256, 4 = 2-CTA 256x512), 1 = GEMM GROUP_M (0 auto), 2 = GEMM max CTAs
  * (0 = all SMs), 3 = GEMV split-K (0 auto), 4 = GEMV columns-per-CTA selector
  * (0 auto), 5 = reserved.  Returns 0 or E_PATH for an unknown key.
  */

@@ -187,7 +187,7 @@ def tile_gemm_query_config(M, N, K, out_dtype=OUT_F32) -> dict:
     out = (ctypes.c_int32 * 8)()
     _check(load_library().tile_gemm_query_config(M, N, K, int(out_dtype), out))
     return {"BM": out[0], "BN": out[1], "cta_group": out[2], "ctas": out[3], "group_m": out[4],
-            "stages": out[5], "BK": out[6]}
+            "stages": out[5], "BK": out[6], "config": out[7]}
 
 
 def tile_gemm_debug_owner_map(M, N, K, out_dtype=OUT_F32, ld_owner=None, stream=None, device="cuda"):

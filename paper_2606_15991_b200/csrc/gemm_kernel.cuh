@@ -13,10 +13,15 @@
 //   * warp 1 : MMA issuer    -- one thread, tcgen05.mma kind::f16 (bf16 x bf16 -> fp32 in TMEM),
 //              A K-major, B MN-major (row-major K x N), tcgen05.commit frees smem stages;
 //   * warp 2 : TMEM allocator (2 accumulator stages of BN columns);
-//   * warps 4-7: epilogue    -- tcgen05.ld TMEM -> registers -> (fp32 | RNE bf16) -> swizzled smem
+//   * warps 4-11: epilogue   -- tcgen05.ld TMEM -> registers -> (fp32 | RNE bf16) -> swizzled smem
 //              -> TMA store (clipped at M,N by the tensor map) or, when C is not 16-byte
 //              addressable, clipped st.global from the staged tile.
-//   The accumulator is double buffered so tile i's epilogue overlaps tile i+1's main loop.
+//   TMEM holds two accumulator slots of BN columns.  NACC = 1: a tile is one slot wide and the
+//   slots alternate, so tile i's epilogue overlaps tile i+1's main loop.  NACC = 2: a tile is both
+//   slots wide (BM*CG x 2*BN, e.g. 256 x 512 for a CTA pair): every A stage feeds two MMAs, which
+//   cuts the L2 -> shared-memory fill traffic per FLOP by a quarter (the kernel is power bound on
+//   B200); each slot keeps its own full/empty barriers, so the next tile's
+//   main loop restarts on slot 0 while the epilogue still drains slot 1.
 #pragma once
 #include "ptx.cuh"
 
@@ -25,13 +30,13 @@ namespace tg {
 constexpr int GEMM_BM = 128;      // rows per CTA (UMMA M = 128 * CG)
 constexpr int GEMM_BK = 64;       // one 128-byte swizzle row of bf16
 constexpr int GEMM_UMMA_K = 16;   // K per tcgen05.mma for 16-bit inputs
-constexpr int GEMM_THREADS = 256;
+constexpr int GEMM_THREADS = 384;     // 4 control warps + 8 epilogue warps
 constexpr int GEMM_EPI_WARP0 = 4;
-constexpr uint32_t GEMM_EPI_BUF_BYTES = 32 * 128;   // 32 rows x 128 B per warp per buffer
+constexpr uint32_t GEMM_EPI_BUF_BYTES = 2 * 32 * 64;   // per epilogue warp: two buffers of 32 rows x 64 B
 
 struct GemmParams {
     int32_t M, N, K;
-    int32_t tiles_m, tiles_n;   // tile grid; a tile is (GEMM_BM*CG) x BN
+    int32_t tiles_m, tiles_n;   // tile grid; a tile is (GEMM_BM*CG) x (BN*NACC)
     int32_t group_m;            // raster group height in tiles
     int32_t num_k_tiles;
     int32_t out_bf16;           // 0: fp32 C, 1: bf16 C
@@ -55,29 +60,32 @@ __host__ __device__ __forceinline__ void tile_coords(int t, int tiles_m, int til
     tn = r / rows;
 }
 
-template <int CG, int BN, int STAGES>
+template <int CG, int BN, int STAGES, int NACC>
 struct GemmSmem {
     static constexpr uint32_t A_BYTES = GEMM_BM * GEMM_BK * 2;
-    static constexpr uint32_t B_COLS = BN / CG;                 // B columns loaded by each CTA
+    static constexpr uint32_t B_COLS = BN / CG;                 // B columns per accumulator slot loaded by each CTA
     static constexpr uint32_t B_BOXES = B_COLS / 64;
     static constexpr uint32_t B_BOX_BYTES = 64 * GEMM_BK * 2;   // 64 k-rows x 128 B
-    static constexpr uint32_t B_BYTES = B_BOXES * B_BOX_BYTES;
+    static constexpr uint32_t B_ACC_BYTES = B_BOXES * B_BOX_BYTES;
+    static constexpr uint32_t B_BYTES = NACC * B_ACC_BYTES;
     static constexpr uint32_t STAGE_BYTES = A_BYTES + B_BYTES;
     static constexpr uint32_t EPI_OFF = STAGES * STAGE_BYTES;
-    static constexpr uint32_t EPI_BYTES = 4 * 2 * GEMM_EPI_BUF_BYTES;
+    static constexpr uint32_t EPI_BYTES = 8 * GEMM_EPI_BUF_BYTES;
     static constexpr uint32_t BAR_OFF = EPI_OFF + EPI_BYTES;
     static constexpr uint32_t NUM_BARS = 2 * STAGES + 4;
     static constexpr uint32_t TMEM_PTR_OFF = BAR_OFF + NUM_BARS * 8;
     static constexpr uint32_t TOTAL = TMEM_PTR_OFF + 16 + 1024;   // + slack for 1024 B alignment
 };
 
-template <int CG, int BN, int STAGES>
+template <int CG, int BN, int STAGES, int NACC>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b,
                     const __grid_constant__ CUtensorMap tmap_c, const GemmParams p) {
-    using L = GemmSmem<CG, BN, STAGES>;
+    using L = GemmSmem<CG, BN, STAGES, NACC>;
     static_assert(CG == 1 || CG == 2, "cta_group is 1 or 2");
     static_assert(BN == 128 || BN == 256, "accumulator width");
+    static_assert(NACC == 1 || NACC == 2, "a tile is one or two accumulator slots wide");
+    constexpr int TILE_N = BN * NACC;
     static_assert(L::TOTAL <= 232448, "exceeds 227 KB of shared memory");
 
     extern __shared__ uint8_t smem_raw[];
@@ -111,7 +119,8 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
         }
         for (uint32_t a = 0; a < 2; ++a) {
             mbar_init(tmem_full_bar(a), 1);           // one tcgen05.commit
-            mbar_init(tmem_empty_bar(a), 4 * CG);     // lane 0 of every epilogue warp of the pair
+            // lane 0 of every epilogue warp of the pair that drains this slot
+            mbar_init(tmem_empty_bar(a), (NACC == 2 ? 4 : 8) * CG);
         }
         fence_mbar_init();
     }
@@ -133,7 +142,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
                 int tm, tn;
                 tile_coords(t, p.tiles_m, p.tiles_n, p.group_m, tm, tn);
                 const int m0 = (tm * CG + (int)rank) * GEMM_BM;
-                const int n0 = tn * BN + (int)rank * (int)L::B_COLS;
+                const int n0 = tn * TILE_N + (int)rank * (int)L::B_COLS;
                 for (int kt = 0; kt < p.num_k_tiles; ++kt) {
                     mbar_wait(empty_bar(stage), phase ^ 1u);
                     const uint32_t sa = smem_base + stage * L::STAGE_BYTES;
@@ -143,16 +152,22 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
                         mbar_arrive_expect_tx(full_bar(stage), L::STAGE_BYTES);
                         tma_load_2d(sa, &tmap_a, full_bar(stage), k0, m0);
 #pragma unroll
-                        for (uint32_t b = 0; b < L::B_BOXES; ++b)
-                            tma_load_2d(sb + b * L::B_BOX_BYTES, &tmap_b, full_bar(stage), n0 + (int)b * 64, k0);
+                        for (uint32_t j = 0; j < (uint32_t)NACC; ++j)
+#pragma unroll
+                            for (uint32_t b = 0; b < L::B_BOXES; ++b)
+                                tma_load_2d(sb + j * L::B_ACC_BYTES + b * L::B_BOX_BYTES, &tmap_b, full_bar(stage),
+                                            n0 + (int)j * BN + (int)b * 64, k0);
                     } else {
                         // both CTAs' bytes are counted on the leader's barrier
                         const uint32_t lead_bar = map_to_cta(full_bar(stage), 0);
                         if (rank == 0) mbar_arrive_expect_tx(full_bar(stage), 2 * L::STAGE_BYTES);
                         tma_load_2d_cg2(sa, &tmap_a, lead_bar, k0, m0);
 #pragma unroll
-                        for (uint32_t b = 0; b < L::B_BOXES; ++b)
-                            tma_load_2d_cg2(sb + b * L::B_BOX_BYTES, &tmap_b, lead_bar, n0 + (int)b * 64, k0);
+                        for (uint32_t j = 0; j < (uint32_t)NACC; ++j)
+#pragma unroll
+                            for (uint32_t b = 0; b < L::B_BOXES; ++b)
+                                tma_load_2d_cg2(sb + j * L::B_ACC_BYTES + b * L::B_BOX_BYTES, &tmap_b, lead_bar,
+                                                n0 + (int)j * BN + (int)b * 64, k0);
                     }
                     if (++stage == STAGES) { stage = 0; phase ^= 1u; }
                 }
@@ -172,151 +187,191 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
             constexpr uint64_t a_desc_base = desc_hi | (uint64_t(1) << 16) | (uint64_t(1024 >> 4) << 32);
             constexpr uint64_t b_desc_base =
                 desc_hi | (uint64_t(L::B_BOX_BYTES >> 4) << 16) | (uint64_t(1024 >> 4) << 32);
-            uint32_t stage = 0, phase = 0, acc = 0, acc_phase = 0;
-            for (int t = first_tile; t < total_tiles; t += tile_stride) {
-                mbar_wait(tmem_empty_bar(acc), acc_phase ^ 1u);
-                tc_fence_after();
-                const uint32_t d_tmem = tmem_base + acc * BN;
+            // slot use: NACC == 1 -> slot = tile iteration & 1 (phase flips every 2nd tile);
+            //           NACC == 2 -> both slots every tile (phase flips every tile)
+            uint32_t stage = 0, phase = 0, it = 0;
+            for (int t = first_tile; t < total_tiles; t += tile_stride, ++it) {
+                const uint32_t slot0 = (NACC == 2) ? 0u : (it & 1u);
+                const uint32_t acc_phase = (NACC == 2) ? (it & 1u) : ((it >> 1) & 1u);
                 for (int kt = 0; kt < p.num_k_tiles; ++kt) {
                     mbar_wait(full_bar(stage), phase);
                     tc_fence_after();
                     const uint32_t sa = smem_base + stage * L::STAGE_BYTES;
                     const uint32_t sb = sa + L::A_BYTES;
                     const uint64_t a_desc = a_desc_base | (uint64_t)((sa & 0x3FFFFu) >> 4);
-                    const uint64_t b_desc = b_desc_base | (uint64_t)((sb & 0x3FFFFu) >> 4);
 #pragma unroll
-                    for (int k = 0; k < GEMM_BK / GEMM_UMMA_K; ++k) {
-                        // A: +16 elements along K = +32 B inside the swizzled row;
-                        // B: +16 k-rows of 128 B = +2048 B
-                        umma_bf16<CG>(d_tmem, a_desc + (uint64_t)(k * 2), b_desc + (uint64_t)(k * 128), idesc,
-                                      (uint32_t)((kt | k) != 0));
+                    for (uint32_t j = 0; j < (uint32_t)NACC; ++j) {
+                        if (kt == 0) {   // the epilogue must have drained this slot
+                            mbar_wait(tmem_empty_bar(slot0 + j), acc_phase ^ 1u);
+                            tc_fence_after();
+                        }
+                        const uint32_t d_tmem = tmem_base + (slot0 + j) * BN;
+                        const uint64_t b_desc =
+                            b_desc_base | (uint64_t)(((sb + j * L::B_ACC_BYTES) & 0x3FFFFu) >> 4);
+#pragma unroll
+                        for (int k = 0; k < GEMM_BK / GEMM_UMMA_K; ++k) {
+                            // A: +16 elements along K = +32 B inside the swizzled row;
+                            // B: +16 k-rows of 128 B = +2048 B
+                            umma_bf16<CG>(d_tmem, a_desc + (uint64_t)(k * 2), b_desc + (uint64_t)(k * 128), idesc,
+                                          (uint32_t)((kt | k) != 0));
+                        }
+                        // accumulator slot ready for the epilogue after the last k-tile
+                        if (kt == p.num_k_tiles - 1) umma_commit<CG>(tmem_full_bar(slot0 + j));
                     }
                     umma_commit<CG>(empty_bar(stage));   // smem stage reusable once these MMAs retire
                     if (++stage == STAGES) { stage = 0; phase ^= 1u; }
                 }
-                umma_commit<CG>(tmem_full_bar(acc));     // accumulator ready for the epilogue
-                acc ^= 1u;
-                if (acc == 0) acc_phase ^= 1u;
+                if (p.num_k_tiles == 0) {   // owner-map mode: no MMAs, hand the slots over directly
+#pragma unroll
+                    for (uint32_t j = 0; j < (uint32_t)NACC; ++j) {
+                        mbar_wait(tmem_empty_bar(slot0 + j), acc_phase ^ 1u);
+                        umma_commit<CG>(tmem_full_bar(slot0 + j));
+                    }
+                }
             }
         }
         __syncwarp();
     } else if (warp >= GEMM_EPI_WARP0) {
         // ===== epilogue: TMEM -> registers -> smem -> global =====
-        const uint32_t ew = warp - GEMM_EPI_WARP0;             // TMEM lane quarter of this warp
-        const uint32_t buf0 = smem_base + L::EPI_OFF + ew * 2u * GEMM_EPI_BUF_BYTES;
-        uint8_t* buf0_gen = smem_gen + L::EPI_OFF + ew * 2u * GEMM_EPI_BUF_BYTES;
-        const int cols_per_chunk = p.out_bf16 ? 64 : 32;       // 128 B of C per row per chunk
-        const int num_chunks = BN / cols_per_chunk;
+        // Eight warps: warp e drains TMEM lane quarter (e & 3) -- the only lanes it may address --
+        // and column half (e >> 2) of the tile (NACC == 2: accumulator slot e >> 2).  The columns
+        // are walked in units of 32 (one tcgen05.ld.32x32b.x32); the load of unit u+1 is in
+        // flight while unit u is converted and staged; 64 bytes of C per row (one sub-chunk: 16 fp32
+        // or 32 bf16 columns) are staged 64B-swizzled and leave with one TMA store, double buffered.
+        const uint32_t ew = warp - GEMM_EPI_WARP0;
+        const uint32_t q = ew & 3u;
+        const uint32_t half = ew >> 2;
+        constexpr int WARP_COLS = TILE_N / 2;
+        constexpr int UNITS = WARP_COLS / 32;
+        // staging: two 2 KB buffers per warp, each 32 rows x 64 B, 64B-swizzled (16-byte slot c of row r
+        // sits at slot c ^ ((r >> 1) & 3): conflict-free st.shared.v4 and the layout the C tensor map expects)
+        const uint32_t sbuf0 = smem_base + L::EPI_OFF + ew * GEMM_EPI_BUF_BYTES;
+        const uint8_t* sgen0 = smem_gen + L::EPI_OFF + ew * GEMM_EPI_BUF_BYTES;
+        const uint32_t sw = (lane >> 1) & 3u;
+        const int out_bf16 = p.out_bf16;
+        const int sub_cols = out_bf16 ? 32 : 16;              // 64 B of C per row per sub-chunk
         // TMA stores clip at 16-byte granularity along a row (measured on B200): when N is not a
-        // multiple of 16 bytes of elements the chunk containing column N-1 takes the clipped
+        // multiple of 16 bytes of elements the sub-chunk containing column N-1 takes the clipped
         // st.global path so that C[i][N..] is never written.
-        const bool ragged_n = (p.N % (p.out_bf16 ? 8 : 4)) != 0;
-        uint32_t acc = 0, acc_phase = 0, buf = 0;
-        for (int t = first_tile; t < total_tiles; t += tile_stride) {
+        const bool ragged_n = (p.N % (out_bf16 ? 8 : 4)) != 0;
+        uint32_t it = 0, buf = 0;
+        for (int t = first_tile; t < total_tiles; t += tile_stride, ++it) {
             int tm, tn;
             tile_coords(t, p.tiles_m, p.tiles_n, p.group_m, tm, tn);
-            const int m0 = (tm * CG + (int)rank) * GEMM_BM + (int)ew * 32;   // first row of this warp
-            const int n_tile = tn * BN;
-            mbar_wait(tmem_full_bar(acc), acc_phase);
-            tc_fence_after();
-            const uint32_t t_acc = tmem_base + ((ew * 32u) << 16) + acc * BN;
+            const int m0 = (tm * CG + (int)rank) * GEMM_BM + (int)q * 32;    // first row of this warp
+            const int n_base = tn * TILE_N + (int)half * WARP_COLS;         // first column of this warp
             const uint32_t owner_val = ((uint32_t)t << 8) | (uint32_t)blockIdx.x;
-            for (int c = 0; c < num_chunks; ++c) {
-                const int n0 = n_tile + c * cols_per_chunk;
-                if (m0 >= p.M || n0 >= p.N) continue;   // chunk entirely outside C (warp-uniform)
-                // staging buffer `buf` must no longer be read by an earlier TMA store
+            const uint32_t acc = (NACC == 2) ? half : (it & 1u);
+            const uint32_t acc_phase = (NACC == 2) ? (it & 1u) : ((it >> 1) & 1u);
+            const uint32_t t_acc =
+                tmem_base + ((q * 32u) << 16) + acc * BN + ((NACC == 2) ? 0u : half * (uint32_t)WARP_COLS);
+            // units of this warp that intersect C (warp-uniform); the rest is never loaded or stored
+            int units = 0;
+            if (m0 < p.M && n_base < p.N) {
+                units = (p.N - n_base + 31) >> 5;
+                if (units > UNITS) units = UNITS;
+            }
+            mbar_wait_sleep(tmem_full_bar(acc), acc_phase);
+            tc_fence_after();
+
+            // stage 16 words (64 B) of this thread's row as columns [n0, n0 + sub_cols) and send them
+            auto emit = [&](uint32_t w0, uint32_t w1, uint32_t w2, uint32_t w3, uint32_t w4, uint32_t w5,
+                            uint32_t w6, uint32_t w7, uint32_t w8, uint32_t w9, uint32_t w10, uint32_t w11,
+                            uint32_t w12, uint32_t w13, uint32_t w14, uint32_t w15, int n0) {
+                if (n0 >= p.N) return;                         // warp-uniform
+                // the buffer written two sub-chunks ago must have been read by its TMA store
                 if (lane == 0) tma_store_wait_read<1>();
                 __syncwarp();
-                const uint32_t sbuf = buf0 + buf * GEMM_EPI_BUF_BYTES;
-                const uint32_t row_addr = sbuf + lane * 128u;
-                const uint32_t sw = lane & 7u;
-                if (p.out_bf16) {
-                    uint32_t v0[32], v1[32];
-                    tmem_ld_32x32(t_acc + (uint32_t)(c * 64), v0);
-                    tmem_ld_32x32(t_acc + (uint32_t)(c * 64 + 32), v1);
-                    tmem_ld_wait();
-#pragma unroll
-                    for (uint32_t j = 0; j < 4; ++j) {   // 16-byte chunk j holds columns 8j..8j+7
-                        st_shared_v4(row_addr + ((j ^ sw) << 4),
-                                     pack_bf16x2(__uint_as_float(v0[8 * j + 0]), __uint_as_float(v0[8 * j + 1])),
-                                     pack_bf16x2(__uint_as_float(v0[8 * j + 2]), __uint_as_float(v0[8 * j + 3])),
-                                     pack_bf16x2(__uint_as_float(v0[8 * j + 4]), __uint_as_float(v0[8 * j + 5])),
-                                     pack_bf16x2(__uint_as_float(v0[8 * j + 6]), __uint_as_float(v0[8 * j + 7])));
-                        st_shared_v4(row_addr + (((j + 4) ^ sw) << 4),
-                                     pack_bf16x2(__uint_as_float(v1[8 * j + 0]), __uint_as_float(v1[8 * j + 1])),
-                                     pack_bf16x2(__uint_as_float(v1[8 * j + 2]), __uint_as_float(v1[8 * j + 3])),
-                                     pack_bf16x2(__uint_as_float(v1[8 * j + 4]), __uint_as_float(v1[8 * j + 5])),
-                                     pack_bf16x2(__uint_as_float(v1[8 * j + 6]), __uint_as_float(v1[8 * j + 7])));
-                    }
-                } else {
-                    uint32_t v[32];
-                    tmem_ld_32x32(t_acc + (uint32_t)(c * 32), v);
-                    tmem_ld_wait();
-                    if (p.owner_mode) {
-#pragma unroll
-                        for (int i = 0; i < 32; ++i) v[i] = owner_val;
-                    }
-#pragma unroll
-                    for (uint32_t j = 0; j < 8; ++j)     // 16-byte chunk j holds columns 4j..4j+3
-                        st_shared_v4(row_addr + ((j ^ sw) << 4), v[4 * j + 0], v[4 * j + 1], v[4 * j + 2],
-                                     v[4 * j + 3]);
-                }
-                if (p.tma_store && !(ragged_n && n0 + cols_per_chunk > p.N)) {
+                const uint32_t sb = sbuf0 + buf * 2048u;
+                const uint32_t ra = sb + lane * 64u;
+                st_shared_v4(ra + ((0u ^ sw) << 4), w0, w1, w2, w3);
+                st_shared_v4(ra + ((1u ^ sw) << 4), w4, w5, w6, w7);
+                st_shared_v4(ra + ((2u ^ sw) << 4), w8, w9, w10, w11);
+                st_shared_v4(ra + ((3u ^ sw) << 4), w12, w13, w14, w15);
+                if (p.tma_store && !(ragged_n && n0 + sub_cols > p.N)) {
                     fence_proxy_async_smem();
                     __syncwarp();
                     if (lane == 0) {
-                        tma_store_2d(&tmap_c, sbuf, n0, m0);   // clipped at (N, M) by the tensor map
+                        tma_store_2d(&tmap_c, sb, n0, m0);     // clipped at (N, M) by the tensor map
                         tma_store_commit();
                     }
                 } else {
                     // C rows are not 16-byte addressable: clipped, row-coalesced stores from smem
                     __syncwarp();
-                    const uint8_t* sgen = buf0_gen + buf * GEMM_EPI_BUF_BYTES;
+                    const uint8_t* sg = sgen0 + buf * 2048u;
                     const int rows = (p.M - m0) < 32 ? (p.M - m0) : 32;
-                    if (p.out_bf16) {
+                    const int e = (int)lane;                   // column within the sub-chunk
+                    if (out_bf16) {
                         uint16_t* Cb = reinterpret_cast<uint16_t*>(p.C);
-                        for (int r = 0; r < rows; ++r) {
-#pragma unroll
-                            for (int h = 0; h < 2; ++h) {
-                                const int e = (int)lane + 32 * h;   // column within the chunk
-                                if (n0 + e < p.N) {
-                                    const uint32_t off = (uint32_t)r * 128u +
-                                                         ((((uint32_t)e >> 3) ^ ((uint32_t)r & 7u)) << 4) +
-                                                         ((uint32_t)e & 7u) * 2u;
-                                    Cb[(int64_t)(m0 + r) * p.ldc + n0 + e] =
-                                        *reinterpret_cast<const uint16_t*>(sgen + off);
-                                }
+                        if (n0 + e < p.N)
+                            for (int r = 0; r < rows; ++r) {
+                                const uint32_t off = (uint32_t)r * 64u +
+                                                     ((((uint32_t)e >> 3) ^ (((uint32_t)r >> 1) & 3u)) << 4) +
+                                                     ((uint32_t)e & 7u) * 2u;
+                                Cb[(int64_t)(m0 + r) * p.ldc + n0 + e] = *reinterpret_cast<const uint16_t*>(sg + off);
                             }
-                        }
                     } else {
                         uint32_t* Cf = reinterpret_cast<uint32_t*>(p.C);
-                        for (int r = 0; r < rows; ++r) {
-                            const int e = (int)lane;
-                            if (n0 + e < p.N) {
-                                const uint32_t off = (uint32_t)r * 128u +
-                                                     ((((uint32_t)e >> 2) ^ ((uint32_t)r & 7u)) << 4) +
-                                                     ((uint32_t)e & 3u) * 4u;
-                                Cf[(int64_t)(m0 + r) * p.ldc + n0 + e] =
-                                    *reinterpret_cast<const uint32_t*>(sgen + off);
+                        // 16 columns per row: lanes 0-15 take even rows, lanes 16-31 odd rows
+                        const int ec = e & 15;
+                        if (n0 + ec < p.N)
+                            for (int r = (e >> 4); r < rows; r += 2) {
+                                const uint32_t off = (uint32_t)r * 64u +
+                                                     ((((uint32_t)ec >> 2) ^ (((uint32_t)r >> 1) & 3u)) << 4) +
+                                                     ((uint32_t)ec & 3u) * 4u;
+                                Cf[(int64_t)(m0 + r) * p.ldc + n0 + ec] = *reinterpret_cast<const uint32_t*>(sg + off);
                             }
-                        }
                     }
                     __syncwarp();
-                    // keep one bulk group per chunk so that wait_group.read<1> above always
-                    // refers to the buffer written two chunks ago
-                    if (lane == 0) tma_store_commit();
+                    if (lane == 0) tma_store_commit();         // empty group: keeps wait_group.read<1> aligned
                 }
                 buf ^= 1u;
+            };
+            // one unit: `v` holds 32 consecutive columns of this thread's row
+            auto stage_unit = [&](uint32_t (&v)[32], int u) {
+                const int n0 = n_base + u * 32;
+                if (out_bf16) {
+#define TG_PK(i) pack_bf16x2(__uint_as_float(v[2 * (i)]), __uint_as_float(v[2 * (i) + 1]))
+                    emit(TG_PK(0), TG_PK(1), TG_PK(2), TG_PK(3), TG_PK(4), TG_PK(5), TG_PK(6), TG_PK(7), TG_PK(8),
+                         TG_PK(9), TG_PK(10), TG_PK(11), TG_PK(12), TG_PK(13), TG_PK(14), TG_PK(15), n0);
+#undef TG_PK
+                } else {
+                    if (p.owner_mode) {
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) v[i] = owner_val;
+                    }
+                    emit(v[0], v[1], v[2], v[3], v[4], v[5], v[6], v[7], v[8], v[9], v[10], v[11], v[12], v[13],
+                         v[14], v[15], n0);
+                    emit(v[16], v[17], v[18], v[19], v[20], v[21], v[22], v[23], v[24], v[25], v[26], v[27], v[28],
+                         v[29], v[30], v[31], n0 + 16);
+                }
+            };
+            // all TMEM reads of this accumulator slot are complete: hand it back to the MMA warp
+            auto release_tmem = [&]() {
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) {
+                    if constexpr (CG == 1) mbar_arrive(tmem_empty_bar(acc));
+                    else mbar_arrive_cluster(map_to_cta(tmem_empty_bar(acc), 0));
+                }
+            };
+
+            uint32_t va[32], vb[32];
+            if (units > 0) tmem_ld_32x32(t_acc, va);
+#pragma unroll 1
+            for (int u = 0; u < units; u += 2) {
+                tmem_ld_wait();                                            // va = unit u
+                if (u + 1 < units) tmem_ld_32x32(t_acc + (uint32_t)((u + 1) * 32), vb);
+                else release_tmem();
+                stage_unit(va, u);
+                if (u + 1 < units) {
+                    tmem_ld_wait();                                        // vb = unit u + 1
+                    if (u + 2 < units) tmem_ld_32x32(t_acc + (uint32_t)((u + 2) * 32), va);
+                    else release_tmem();
+                    stage_unit(vb, u + 1);
+                }
             }
-            // all TMEM reads of this accumulator stage are complete: hand it back to the MMA warp
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) {
-                if constexpr (CG == 1) mbar_arrive(tmem_empty_bar(acc));
-                else mbar_arrive_cluster(map_to_cta(tmem_empty_bar(acc), 0));
-            }
-            acc ^= 1u;
-            if (acc == 0) acc_phase ^= 1u;
+            if (units == 0) release_tmem();
         }
         if (lane == 0) tma_store_wait_all<0>();
         __syncwarp();

@@ -125,6 +125,26 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 #endif
 }
 
+// Long waits (an epilogue warp waiting for a whole main loop): back off between polls so the
+// waiting warps stay out of the issue slots.
+__device__ __forceinline__ void mbar_wait_sleep(uint32_t bar, uint32_t parity) {
+    if (mbar_try_wait(bar, parity)) return;
+#if TILEGEMM_WATCHDOG
+    const uint64_t t0 = global_timer_ns();
+    uint32_t spins = 0;
+#endif
+    while (!mbar_try_wait(bar, parity)) {
+        __nanosleep(64);
+#if TILEGEMM_WATCHDOG
+        if ((++spins & 0xfffu) == 0 && global_timer_ns() - t0 > 4000000000ull) {
+            printf("tilegemm watchdog: mbarrier wait timed out (block %d thread %d bar 0x%x parity %u)\n",
+                   (int)blockIdx.x, (int)threadIdx.x, bar, parity);
+            __trap();
+        }
+#endif
+    }
+}
+
 // ---------------------------------------------------------------- proxies / fences
 __device__ __forceinline__ void fence_proxy_async_smem() {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");

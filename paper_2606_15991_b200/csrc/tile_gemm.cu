@@ -198,9 +198,9 @@ std::unordered_map<MapKey, CUtensorMap, MapKeyHash> g_maps;
 
 // 2-D row-major tensor [d1 rows][d0 cols] of `esize`-byte elements with row pitch `pitch` bytes.
 int get_tensor_map(CUtensorMap* out, const void* base, int dtype_bytes, bool is_float32, uint64_t d0, uint64_t d1,
-                   uint64_t pitch, uint32_t b0, uint32_t b1, bool swizzle128) {
+                   uint64_t pitch, uint32_t b0, uint32_t b1, int swizzle_bytes) {
     MapKey key{(uintptr_t)base, d0, d1, pitch, b0, b1, (uint32_t)(is_float32 ? 4 : dtype_bytes),
-               (uint32_t)swizzle128};
+               (uint32_t)swizzle_bytes};
     std::lock_guard<std::mutex> lk(g_mu);
     auto it = g_maps.find(key);
     if (it != g_maps.end()) { *out = it->second; return TILE_GEMM_OK; }
@@ -219,7 +219,9 @@ int get_tensor_map(CUtensorMap* out, const void* base, int dtype_bytes, bool is_
     const CUtensorMapDataType dt = is_float32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16;
     CUtensorMap m;
     CUresult r = g_encode(&m, dt, 2, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                          swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
+                          swizzle_bytes == 128 ? CU_TENSOR_MAP_SWIZZLE_128B
+                          : swizzle_bytes == 64 ? CU_TENSOR_MAP_SWIZZLE_64B
+                                                : CU_TENSOR_MAP_SWIZZLE_NONE,
                           CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS)
         return fail(TILE_GEMM_E_CUDA,
@@ -262,15 +264,28 @@ int workspace_for(int dev, cudaStream_t s, size_t need, void** out) {
 
 // ------------------------------------------------------------------ GEMM launch
 struct GemmConfig {
-    int id;       // 1: 1-CTA 128x128, 2: 1-CTA 128x256, 3: 2-CTA 256x256
-    int cg, bn, stages;
+    int id;       // 1: 1-CTA 128x128, 2: 1-CTA 128x256, 3: 2-CTA 256x256, 4: 2-CTA 256x512
+    int cg, bn, stages, nacc;
+    int tile_n() const { return bn * nacc; }
 };
-const GemmConfig kConfigs[4] = {{0, 0, 0, 0}, {1, 1, 128, 6}, {2, 1, 256, 4}, {3, 2, 256, 6}};
+const GemmConfig kConfigs[5] = {{0, 0, 0, 0, 0}, {1, 1, 128, 6, 1}, {2, 1, 256, 4, 1}, {3, 2, 256, 6, 1},
+                                {4, 2, 256, 4, 2}};
+
+// ceil(tiles / slots) * slots / tiles: how much longer than perfectly divisible work the last
+// wave makes a persistent launch run
+double wave_waste(int64_t tiles, int64_t slots) {
+    const int64_t waves = (tiles + slots - 1) / slots;
+    return (double)(waves * slots) / (double)tiles;
+}
 
 GemmConfig choose_config(int64_t M, int64_t N, int sms) {
     const int forced = g_tune[0].load();
-    if (forced >= 1 && forced <= 3) return kConfigs[forced];
+    if (forced >= 1 && forced <= 4) return kConfigs[forced];
     const int64_t t3 = ((M + 255) / 256) * ((N + 255) / 256);
+    const int64_t t4 = ((M + 255) / 256) * ((N + 511) / 512);
+    // the 256x512 tile moves a quarter less operand data per FLOP (the kernel is power bound,
+    // DESIGN.md "Power"); take it unless its coarser wave quantisation costs more than that buys
+    if (t4 >= sms / 2 && wave_waste(t4, sms / 2) <= wave_waste(t3, sms / 2) * 1.06) return kConfigs[4];
     if (t3 >= sms / 2) return kConfigs[3];
     const int64_t t2 = ((M + 127) / 128) * ((N + 255) / 256);
     if (t2 * 4 >= (int64_t)sms * 3) return kConfigs[2];
@@ -290,7 +305,7 @@ void plan_gemm(int64_t M, int64_t N, int64_t K, int out_bf16, int sms, GemmLaunc
     memset(&p, 0, sizeof p);
     p.M = (int32_t)M; p.N = (int32_t)N; p.K = (int32_t)K;
     p.tiles_m = (int32_t)((M + tile_m - 1) / tile_m);
-    p.tiles_n = (int32_t)((N + gl->cfg.bn - 1) / gl->cfg.bn);
+    p.tiles_n = (int32_t)((N + gl->cfg.tile_n() - 1) / gl->cfg.tile_n());
     int gm = g_tune[1].load();
     if (gm <= 0) gm = (gl->cfg.cg == 2) ? 8 : 16;
     p.group_m = gm < p.tiles_m ? gm : p.tiles_m;
@@ -304,11 +319,11 @@ void plan_gemm(int64_t M, int64_t N, int64_t K, int out_bf16, int sms, GemmLaunc
     gl->ctas = (int)units * gl->cfg.cg;
 }
 
-template <int CG, int BN, int STAGES>
+template <int CG, int BN, int STAGES, int NACC>
 int launch_gemm_inst(const CUtensorMap& ta, const CUtensorMap& tb, const CUtensorMap& tc, const tg::GemmParams& p,
                      int ctas, cudaStream_t s, int dev) {
-    using L = tg::GemmSmem<CG, BN, STAGES>;
-    auto kern = tg::gemm_tcgen05_kernel<CG, BN, STAGES>;
+    using L = tg::GemmSmem<CG, BN, STAGES, NACC>;
+    auto kern = tg::gemm_tcgen05_kernel<CG, BN, STAGES, NACC>;
     static bool configured[64] = {};
     if (!configured[dev]) {
         CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::TOTAL));
@@ -335,17 +350,18 @@ int launch_gemm_inst(const CUtensorMap& ta, const CUtensorMap& tb, const CUtenso
 int launch_gemm(const GemmLaunch& gl, const CUtensorMap& ta, const CUtensorMap& tb, const CUtensorMap& tc,
                 cudaStream_t s, int dev) {
     switch (gl.cfg.id) {
-        case 1: return launch_gemm_inst<1, 128, 6>(ta, tb, tc, gl.p, gl.ctas, s, dev);
-        case 2: return launch_gemm_inst<1, 256, 4>(ta, tb, tc, gl.p, gl.ctas, s, dev);
-        case 3: return launch_gemm_inst<2, 256, 6>(ta, tb, tc, gl.p, gl.ctas, s, dev);
+        case 1: return launch_gemm_inst<1, 128, 6, 1>(ta, tb, tc, gl.p, gl.ctas, s, dev);
+        case 2: return launch_gemm_inst<1, 256, 4, 1>(ta, tb, tc, gl.p, gl.ctas, s, dev);
+        case 3: return launch_gemm_inst<2, 256, 6, 1>(ta, tb, tc, gl.p, gl.ctas, s, dev);
+        case 4: return launch_gemm_inst<2, 256, 4, 2>(ta, tb, tc, gl.p, gl.ctas, s, dev);
     }
     return fail(TILE_GEMM_E_INTERNAL, "unknown GEMM config %d", gl.cfg.id);
 }
 
 int c_tensor_map(CUtensorMap* tc, void* C, int64_t M, int64_t N, int64_t ldc, int out_bf16) {
-    // one epilogue chunk: 32 rows x 128 bytes, 128B-swizzled in shared memory
+    // one epilogue sub-chunk: 32 rows x 64 bytes, 64B-swizzled in shared memory
     return get_tensor_map(tc, C, out_bf16 ? 2 : 4, !out_bf16, (uint64_t)N, (uint64_t)M,
-                          (uint64_t)ldc * (out_bf16 ? 2 : 4), out_bf16 ? 64u : 32u, 32u, true);
+                          (uint64_t)ldc * (out_bf16 ? 2 : 4), out_bf16 ? 32u : 16u, 32u, 64);
 }
 
 int run_gemm(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_t K, int64_t lda, int64_t ldb,
@@ -388,9 +404,9 @@ int run_gemm(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_
     gl.p.C = C;
     gl.p.ldc = ldc;
     CUtensorMap ta, tb, tc;
-    int rc = get_tensor_map(&ta, Ap, 2, false, (uint64_t)K, (uint64_t)M, (uint64_t)lda * 2, 64u, 128u, true);
+    int rc = get_tensor_map(&ta, Ap, 2, false, (uint64_t)K, (uint64_t)M, (uint64_t)lda * 2, 64u, 128u, 128);
     if (rc) return rc;
-    rc = get_tensor_map(&tb, Bp, 2, false, (uint64_t)N, (uint64_t)K, (uint64_t)ldb * 2, 64u, 64u, true);
+    rc = get_tensor_map(&tb, Bp, 2, false, (uint64_t)N, (uint64_t)K, (uint64_t)ldb * 2, 64u, 64u, 128);
     if (rc) return rc;
     if (plan.c_tma) {
         rc = c_tensor_map(&tc, C, M, N, ldc, out_bf16);
@@ -453,7 +469,7 @@ int run_gemv(const void* x, const void* B, void* y, int64_t N, int64_t K, int64_
         }
         CUtensorMap tb;
         int rc = get_tensor_map(&tb, B, 2, false, (uint64_t)N, (uint64_t)K, (uint64_t)ldb * 2, (uint32_t)tg::GEMV_COLS,
-                                (uint32_t)tg::GEMV_TILE_K, false);
+                                (uint32_t)tg::GEMV_TILE_K, 0);
         if (rc) return rc;
         cfg.blockDim = dim3(tg::GEMV_TMA_THREADS, 1, 1);
         cfg.dynamicSmemBytes = smem;
@@ -561,13 +577,13 @@ int tile_gemm_query_config(int64_t M, int64_t N, int64_t K, int out_dtype, int32
     GemmLaunch gl;
     plan_gemm(M, N, K, out_dtype == TILE_GEMM_OUT_BF16, sms, &gl);
     out[0] = tg::GEMM_BM;
-    out[1] = gl.cfg.bn;
+    out[1] = gl.cfg.tile_n();
     out[2] = gl.cfg.cg;
     out[3] = gl.ctas;
     out[4] = gl.p.group_m;
     out[5] = gl.cfg.stages;
     out[6] = tg::GEMM_BK;
-    out[7] = 0;
+    out[7] = gl.cfg.id;
     return TILE_GEMM_OK;
 }
 
@@ -596,7 +612,7 @@ int tile_gemm_debug_owner_map(int32_t* owner, int64_t M, int64_t N, int64_t K, i
         // any valid descriptor: it is prefetched but never used by the clipped-store epilogue
         static void* dummy = nullptr;
         if (!dummy) CUDA_TRY(cudaMalloc(&dummy, 32 * 128));
-        rc = get_tensor_map(&tc, dummy, 4, true, 32, 32, 128, 32u, 32u, true);
+        rc = get_tensor_map(&tc, dummy, 4, true, 32, 32, 128, 16u, 32u, 64);
     }
     if (rc) return rc;
     return launch_gemm(gl, tc, tc, tc, (cudaStream_t)stream, dev);

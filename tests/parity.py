@@ -50,18 +50,21 @@ def check_bit_exact(got_f32, ref_f64, what=""):
 
 
 def freivalds_rows(C_gpu_f64, a64, b64, seed=0):
-    """|C r - A (B r)| <= 2^-14 * ||C_i||_2 for every row, r in {+-1}^N (and columns likewise)."""
+    """|C r - A (B r)| <= (2^-14 + K/16 * 2^-24) * ||C_i||_2 for every row, r in {+-1}^N (and
+    columns likewise)."""
     rng = np.random.default_rng([seed, 15485863])
     M, N = C_gpu_f64.shape
     r = rng.choice([-1.0, 1.0], size=N)
     lhs = C_gpu_f64 @ r
     rhs = a64 @ (b64 @ r)
-    tol = 2.0 ** -14 * np.linalg.norm(C_gpu_f64, axis=1) + 1e-30
+    K = a64.shape[1]
+    rel = 2.0 ** -14 + (K / 16.0) * 2.0 ** -24   # same K term as check_close's rel_rms gate
+    tol = rel * np.linalg.norm(C_gpu_f64, axis=1) + 1e-30
     bad = np.abs(lhs - rhs) > tol
     assert not bad.any(), f"Freivalds row test failed for rows {np.where(bad)[0][:8].tolist()}"
     c = rng.choice([-1.0, 1.0], size=M)
     lhs = c @ C_gpu_f64
     rhs = (c @ a64) @ b64
-    tol = 2.0 ** -14 * np.linalg.norm(C_gpu_f64, axis=0) + 1e-30
+    tol = rel * np.linalg.norm(C_gpu_f64, axis=0) + 1e-30
     bad = np.abs(lhs - rhs) > tol
     assert not bad.any(), f"Freivalds column test failed for columns {np.where(bad)[0][:8].tolist()}"

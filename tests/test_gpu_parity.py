@@ -105,7 +105,7 @@ def test_native_library_is_loaded_and_launches():
 
 
 # ------------------------------------------------------------------ config 1
-@pytest.mark.parametrize("cfg", [0, 1, 2, 3])
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3, 4])
 def test_cfg1_bit_exact(cfg):
     tg.tile_gemm_set_tuning(tg.TUNE_GEMM_CONFIG, cfg)
     a, b = wl.make_inputs(wl.CFG1)
@@ -116,7 +116,7 @@ def test_cfg1_bit_exact(cfg):
     assert np.array_equal(got, rne_bf16(ref))
 
 
-@pytest.mark.parametrize("cfg", [1, 2, 3])
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4])
 def test_one_hot_rows_and_columns(cfg):
     """a_{i,pi(i)} = 1 gives C_i. = B_{pi(i)}. exactly: any k-pairing, transposition, swizzle or
     descriptor error in the tensor-core path shows up as a wrong row/column."""
@@ -137,7 +137,7 @@ def test_one_hot_rows_and_columns(cfg):
     assert np.array_equal(got, oracle.bf16_decode(ab)[:, pj])
 
 
-@pytest.mark.parametrize("cfg", [1, 2, 3])
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4])
 @pytest.mark.parametrize("K", [1, 63, 64, 65, 257])
 def test_all_ones_any_k(cfg, K):
     tg.tile_gemm_set_tuning(tg.TUNE_GEMM_CONFIG, cfg)
@@ -168,7 +168,7 @@ def test_cfg2_ragged_full_oracle_and_canary(layout, out):
     check_close(got, ref, S, wl.CFG2.K, out, f"cfg2 {layout} {out}")
 
 
-@pytest.mark.parametrize("cfg", [1, 2, 3])
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4])
 @pytest.mark.parametrize("layout", ["packed", "padded"])
 def test_cfg2_shape_integer_inputs_bit_exact(cfg, layout):
     tg.tile_gemm_set_tuning(tg.TUNE_GEMM_CONFIG, cfg)
@@ -270,7 +270,9 @@ def test_cfg4_prefill_sampled(proj):
     for k0 in range(0, case.K, 1024):
         br[k0:k0 + 1024] = oracle.bf16_decode(b[k0:k0 + 1024]) @ r
     Cband = C32[band].cpu().numpy().astype(np.float64)
-    tol = 2.0 ** -14 * np.linalg.norm(Cband, axis=1)
+    # 2^-14 plus the K-dependent term of parity.check_close's rel_rms gate: the
+    # tensor core adds each K=16 step into the fp32 accumulator with truncation
+    tol = (2.0 ** -14 + (case.K / 16.0) * 2.0 ** -24) * np.linalg.norm(Cband, axis=1)
     assert np.all(np.abs(Cband @ r - a64 @ br) <= tol)
 
 
@@ -299,7 +301,7 @@ def test_cfg5_decode_full_oracle():
 
 
 # ------------------------------------------------------------------ ownership
-@pytest.mark.parametrize("cfg", [1, 2, 3])
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4])
 @pytest.mark.parametrize("shape", [(1023, 1537), (256, 256), (4096, 5120), (130, 70)])
 def test_owner_map_is_the_documented_function(cfg, shape):
     """Each output element is written by exactly one CTA, the one tile_coords assigns
