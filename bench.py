@@ -49,10 +49,13 @@ def measured_peaks():
 
 def ncu_traffic(key):
     """Per-launch DRAM bytes of the dominant kernel from the committed ncu capture, or None."""
-    path = os.path.join(ROOT, "profiles", "traffic.json")
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(path):
         with open(path) as f:
-            return json.load(f).get(key)
+            for line in f:
+                parts = line.strip().split(",")
+                if len(parts) >= 2 and parts[0] == key:
+                    return float(parts[1])
     return None
 
 
