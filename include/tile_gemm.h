@@ -73,6 +73,9 @@ extern "C" {
 #define TILE_GEMM_E_INTERNAL 13
 #define TILE_GEMM_NUM_STATUS 14
 
+/* internal flag behind tile_gemm_static_b */
+#define TILE_GEMM_FLAG_B_IMMUTABLE 1u
+
 /* execution paths (what the selector returns / what force_path accepts) */
 #define TILE_GEMM_PATH_AUTO 0         /* force_path only                                      */
 #define TILE_GEMM_PATH_GEMM_TMA 1     /* tcgen05 GEMM, A and B read in place through TMA      */
@@ -99,6 +102,20 @@ int tile_gemm_ex(const void* A, const void* B, void* C,
                  int64_t M, int64_t N, int64_t K,
                  int64_t lda, int64_t ldb, int64_t ldc,
                  int out_dtype, void* stream, int force_path);
+
+/*
+ * tile_gemm plus one promise from the caller: B holds weights -- no work that is
+ * still in flight when this call's kernel starts (earlier in `stream` or on any
+ * other stream) writes B.  The M == 1 path is launched with programmatic
+ * dependent launch in either entry; with this promise it streams weight tiles
+ * ahead of the wait on the previous kernel of the stream, so back-to-back
+ * decode projections (a recorded decode step) keep HBM
+ * busy across kernel boundaries.  A, C and every other rule are as in tile_gemm.
+ */
+int tile_gemm_static_b(const void* A, const void* B, void* C,
+                       int64_t M, int64_t N, int64_t K,
+                       int64_t lda, int64_t ldb, int64_t ldc,
+                       int out_dtype, void* stream);
 
 /*
  * Launch preconditions + shape selector as a pure host function (PAPER.md:200:
@@ -146,8 +163,14 @@ int tile_gemm_query_config(int64_t M, int64_t N, int64_t K, int out_dtype, int32
  * Tuning / test overrides, process-global, not thread-safe against concurrent
  * tile_gemm calls.  key: 0 = GEMM config (0 auto, 1 = 1-CTA 128x128, 2 = 1-CTA
  * 128x256, 3 = 2-CTA 256x256, 4 = 2-CTA 256x512), 1 = GEMM GROUP_M (0 auto), 2 = GEMM max CTAs
- * (0 = all SMs), 3 = GEMV split-K (0 auto), 4 = GEMV columns-per-CTA selector
- * (0 auto), 5 = reserved.  Returns 0 or E_PATH for an unknown key.
+ * (0 = all SMs; also caps the GEMV grid), 3 = split-K of the cluster GEMV
+ * (0 auto), 4 = GEMV kernel (0 auto = 4 when B is TMA-addressable, 1 = TMA ring +
+ * cluster split-K, 2 = 16-byte LDG, 3 = scalar LDG, 4 = TMA ring + interleaved
+ * split-K with ticketed fix-up), 5 = ring shape of kernel 4 (0 auto; 1..8 =
+ * {columns per CTA, rows per stage, stages, CTAs per SM}, table kGemvShapes in
+ * csrc/tile_gemm.cu), 6 = bit 0 disables programmatic dependent launch; key 3 also
+ * overrides kernel 4's split.  Returns 0 or
+ * E_PATH for an unknown key.
  */
 int tile_gemm_set_tuning(int key, int value);
 

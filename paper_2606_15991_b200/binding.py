@@ -24,9 +24,9 @@ PATH_NAMES = {PATH_AUTO: "auto", PATH_GEMM_TMA: "gemm_tma", PATH_GEMM_REPACK: "g
 (E_OK, E_NULL, E_EXTENT, E_LDA, E_LDB, E_LDC, E_DTYPE, E_ALIGN, E_ALIAS, E_OVERFLOW, E_DEVICE,
  E_CUDA, E_PATH, E_INTERNAL) = range(14)
 
-TUNE_GEMM_CONFIG, TUNE_GEMM_GROUP_M, TUNE_GEMM_MAX_CTAS, TUNE_GEMV_SPLIT, TUNE_GEMV_VARIANT = range(5)
+TUNE_GEMM_CONFIG, TUNE_GEMM_GROUP_M, TUNE_GEMM_MAX_CTAS, TUNE_GEMV_SPLIT, TUNE_GEMV_VARIANT, TUNE_GEMV_SHAPE, TUNE_FLAGS = range(7)
 
-EXPORTS = ("tile_gemm", "tile_gemm_ex", "tile_gemm_select", "tile_gemm_host",
+EXPORTS = ("tile_gemm", "tile_gemm_ex", "tile_gemm_static_b", "tile_gemm_select", "tile_gemm_host",
            "tile_gemm_debug_owner_map", "tile_gemm_query_config", "tile_gemm_set_tuning",
            "tile_gemm_launch_count", "tile_gemm_status_string", "tile_gemm_last_error",
            "tile_gemm_shutdown")
@@ -68,6 +68,8 @@ def load_library():
     lib.tile_gemm.restype = _int
     lib.tile_gemm_ex.argtypes = g + [_vp, _int]
     lib.tile_gemm_ex.restype = _int
+    lib.tile_gemm_static_b.argtypes = g + [_vp]
+    lib.tile_gemm_static_b.restype = _int
     lib.tile_gemm_select.argtypes = [_i64] * 6 + [_vp, _vp, _vp, _int]
     lib.tile_gemm_select.restype = _int
     lib.tile_gemm_host.argtypes = g
@@ -141,9 +143,10 @@ def tile_gemm_select(M, N, K, lda, ldb, ldc, A: int = 256, B: int = 1 << 40, C: 
 
 
 def tile_gemm(A: torch.Tensor, B: torch.Tensor, C: torch.Tensor | None = None, out_dtype=None,
-              stream=None, force_path: int = PATH_AUTO) -> torch.Tensor:
+              stream=None, force_path: int = PATH_AUTO, static_b: bool = False) -> torch.Tensor:
     """C = A @ B on the current CUDA device.  A: (M,K) bf16, B: (K,N) bf16, row-major (any row
-    stride); C: (M,N) fp32 or bf16, allocated if None.  Asynchronous on `stream`."""
+    stride); C: (M,N) fp32 or bf16, allocated if None.  Asynchronous on `stream`.
+    static_b=True calls tile_gemm_static_b (B holds weights nobody in flight writes)."""
     if A.dtype != torch.bfloat16 or B.dtype != torch.bfloat16:
         raise TypeError("A and B must be torch.bfloat16")
     M, K = A.shape
@@ -156,9 +159,15 @@ def tile_gemm(A: torch.Tensor, B: torch.Tensor, C: torch.Tensor | None = None, o
     if C.dtype not in (torch.float32, torch.bfloat16) or tuple(C.shape) != (M, N):
         raise TypeError("C must be an (M,N) float32 or bfloat16 tensor")
     od = OUT_F32 if C.dtype == torch.float32 else OUT_BF16
-    st = load_library().tile_gemm_ex(_vp(A.data_ptr()), _vp(B.data_ptr()), _vp(C.data_ptr()), M, N, K,
-                                     _ld(A), _ld(B), _ld(C), od, _vp(_stream_handle(stream)),
-                                     int(force_path))
+    if static_b:
+        if force_path != PATH_AUTO:
+            raise ValueError("static_b cannot be combined with force_path")
+        st = load_library().tile_gemm_static_b(_vp(A.data_ptr()), _vp(B.data_ptr()), _vp(C.data_ptr()), M, N, K,
+                                               _ld(A), _ld(B), _ld(C), od, _vp(_stream_handle(stream)))
+    else:
+        st = load_library().tile_gemm_ex(_vp(A.data_ptr()), _vp(B.data_ptr()), _vp(C.data_ptr()), M, N, K,
+                                         _ld(A), _ld(B), _ld(C), od, _vp(_stream_handle(stream)),
+                                         int(force_path))
     _check(st)
     return C
 

@@ -167,6 +167,209 @@ gemv_tma_kernel(const __grid_constant__ CUtensorMap tmap_b, const GemvParams p) 
     gemv_reduce_and_store<GEMV_CONSUMER_WARPS>(acc, red, part, warp, lane, warp < GEMV_CONSUMER_WARPS, p, n0);
 }
 
+// ---------------------------------------------------------------------------------------------
+// gemv_split_kernel: the default M = 1 kernel.  Grid (x, S): CTA (bx, s) owns column blocks
+// cb = bx, bx + gridDim.x, ... (256 columns each) and, inside each, the k-tiles kt = s, s + S,
+// s + 2S, ... (TILE_K rows each): *interleaved* split-K, so at any moment the S x gridDim.x CTAs
+// read one dense band of consecutive weight rows over the full row width -- the access pattern
+// HBM likes best (measured: equal contiguous runs per CTA scattered over the matrix lose 4-18 %).
+// All CTAs are co-resident and HBM-bound CTAs progress at equal rates, so equal tile counts per
+// CTA (+-1) finish together whatever the SM count.
+//
+// Split-K fix-up without clusters or float atomics: a CTA with S > 1 writes its 256 fp32 partial
+// sums to the workspace, takes a ticket on the column block, and the CTA that draws the last
+// ticket adds the S partials in slice order (fixed order: bitwise reproducible) and stores y.
+//
+// Programmatic dependent launch: every CTA signals launch_dependents at once, so the next kernel
+// of the stream is scheduled while this one runs (the launch leaves one CTA slot per SM free for
+// it); everything that touches x, y or the workspace sits behind griddepcontrol.wait.  With
+// GEMV_FLAG_B_IMMUTABLE (the caller promises that no work still in flight writes B: decode
+// weights) the producer fills its ring with weight tiles ahead of that wait, so HBM stays busy
+// across kernel boundaries.
+constexpr int GEMV_FLAG_B_IMMUTABLE = 1;
+
+struct GemvSplitParams {
+    const uint16_t* x;
+    void* y;
+    float* partials;      // [col_blocks][split][COLS]
+    uint32_t* tickets;    // [col_blocks], zero between launches
+    int32_t N, K;
+    int32_t k_tiles;      // ceil(K / TILE_K), >= split
+    int32_t col_blocks;
+    int32_t out_bf16;
+    int32_t flags;
+};
+
+__device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void griddep_launch_dependents() {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+__device__ __forceinline__ void consumer_bar_sync() {
+    asm volatile("bar.sync 1, %0;" ::"n"(GEMV_CONSUMER_WARPS * 32) : "memory");
+}
+__device__ __forceinline__ float ld_cg_f32(const float* p) {
+    float v;
+    asm volatile("ld.global.cg.f32 %0, [%1];" : "=f"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_cg_f32(float* p, float v) {
+    asm volatile("st.global.cg.f32 [%0], %1;" ::"l"(p), "f"(v) : "memory");
+}
+
+template <int COLS, int TILE_K, int STAGES>
+struct GemvSplitSmem {
+    static constexpr uint32_t BOX_BYTES = TILE_K * GEMV_COLS * 2;          // one TMA box: TILE_K rows x 256 columns
+    static constexpr uint32_t TILE_BYTES = (COLS / GEMV_COLS) * BOX_BYTES;
+    static constexpr uint32_t RED_OFF = STAGES * TILE_BYTES;
+    static constexpr uint32_t FLAG_OFF = RED_OFF + GEMV_CONSUMER_WARPS * COLS * 4;
+    static constexpr uint32_t BAR_OFF = FLAG_OFF + 16;
+    static constexpr uint32_t TOTAL = BAR_OFF + 2 * STAGES * 8 + 128;   // + slack for 128 B alignment
+};
+
+// COLS columns per CTA (NV = COLS / 256 TMA boxes side by side: a row segment of COLS * 2
+// contiguous bytes), TILE_K rows per ring stage.
+template <int COLS, int TILE_K, int STAGES, int MIN_CTAS>
+__global__ void __launch_bounds__(GEMV_TMA_THREADS, MIN_CTAS)
+gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const GemvSplitParams p) {
+    using L = GemvSplitSmem<COLS, TILE_K, STAGES>;
+    constexpr int NV = COLS / GEMV_COLS;                 // 16-byte vectors per lane per row
+    constexpr int RPW = TILE_K / GEMV_CONSUMER_WARPS;   // rows of a tile per consumer warp
+    static_assert(NV >= 1 && NV <= 4 && COLS % GEMV_COLS == 0, "COLS is 256, 512, 768 or 1024");
+    static_assert(RPW == 2 || RPW == 4 || RPW == 8, "TILE_K is 16, 32 or 64");
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 127u) & ~127u;
+    uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
+    float* red = reinterpret_cast<float*>(smem_gen + L::RED_OFF);
+    volatile uint32_t* s_last = reinterpret_cast<volatile uint32_t*>(smem_gen + L::FLAG_OFF);
+    auto full_bar = [&](uint32_t s) { return smem_base + L::BAR_OFF + s * 8u; };
+    auto empty_bar = [&](uint32_t s) { return smem_base + L::BAR_OFF + (STAGES + s) * 8u; };
+
+    const uint32_t warp = threadIdx.x >> 5;
+    const uint32_t lane = threadIdx.x & 31;
+    const int S = (int)gridDim.y, slice = (int)blockIdx.y;
+    const int KT = p.k_tiles;
+
+    if (threadIdx.x == 0) {
+        prefetch_tmap(&tmap_b);
+        for (uint32_t s = 0; s < STAGES; ++s) {
+            mbar_init(full_bar(s), 1);
+            mbar_init(empty_bar(s), GEMV_CONSUMER_WARPS);
+        }
+        fence_mbar_init();
+    }
+    __syncthreads();
+    griddep_launch_dependents();
+
+    if (warp == GEMV_CONSUMER_WARPS) {
+        // ===== producer =====
+        if (elect_one()) {
+            if (!(p.flags & GEMV_FLAG_B_IMMUTABLE)) griddep_wait();
+            uint32_t stage = 0, phase = 0;
+            for (int cb = (int)blockIdx.x; cb < p.col_blocks; cb += (int)gridDim.x)
+                for (int kt = slice; kt < KT; kt += S) {
+                    mbar_wait(empty_bar(stage), phase ^ 1u);
+                    mbar_arrive_expect_tx(full_bar(stage), L::TILE_BYTES);   // full boxes, even when clipped
+#pragma unroll
+                    for (int v = 0; v < NV; ++v)
+                        tma_load_2d(smem_base + stage * L::TILE_BYTES + v * L::BOX_BYTES, &tmap_b, full_bar(stage),
+                                    cb * COLS + v * GEMV_COLS, kt * TILE_K);
+                    if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                }
+        }
+        __syncwarp();
+        return;
+    }
+
+    // ===== consumers: warp w owns rows RPW*w .. RPW*w+RPW-1 of every tile; lane l owns columns
+    //       256 v + 8 l .. + 7 of every box v =====
+    griddep_wait();   // x may be the previous kernel's output; y and the workspace may still be in its use
+    const uint32_t tid = threadIdx.x;   // 0..255
+    auto load_x = [&](int kt_) -> float {
+        const int k = kt_ * TILE_K + (int)warp * RPW + (int)(lane & (RPW - 1));
+        return (kt_ < KT && k < p.K) ? bf16_bits_to_f32(__ldg(p.x + k)) : 0.f;
+    };
+    uint32_t stage = 0, phase = 0;
+    for (int cb = (int)blockIdx.x; cb < p.col_blocks; cb += (int)gridDim.x) {
+        float acc[NV][8];
+#pragma unroll
+        for (int v = 0; v < NV; ++v)
+#pragma unroll
+            for (int e = 0; e < 8; ++e) acc[v][e] = 0.f;
+        float xv_next = load_x(slice);
+        for (int kt = slice; kt < KT; kt += S) {
+            const float xv = xv_next;
+            xv_next = load_x(kt + S);
+            mbar_wait(full_bar(stage), phase);
+            const uint8_t* tile = smem_gen + stage * L::TILE_BYTES + warp * RPW * (GEMV_COLS * 2) + lane * 16u;
+            uint4 w[NV][RPW];
+#pragma unroll
+            for (int v = 0; v < NV; ++v)
+#pragma unroll
+                for (int r = 0; r < RPW; ++r)
+                    w[v][r] = *reinterpret_cast<const uint4*>(tile + v * L::BOX_BYTES + r * (GEMV_COLS * 2));
+#pragma unroll
+            for (int r = 0; r < RPW; ++r) {
+                const float xr = __shfl_sync(0xffffffffu, xv, r);
+#pragma unroll
+                for (int v = 0; v < NV; ++v) fma8(acc[v], w[v][r], xr);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty_bar(stage));
+            if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+        }
+        // ---- column block done for this slice: warps -> CTA -> (S > 1) slices ----
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+            float4* r4 = reinterpret_cast<float4*>(red + warp * COLS + v * GEMV_COLS + lane * 8);
+            r4[0] = make_float4(acc[v][0], acc[v][1], acc[v][2], acc[v][3]);
+            r4[1] = make_float4(acc[v][4], acc[v][5], acc[v][6], acc[v][7]);
+        }
+        consumer_bar_sync();
+        float s[NV];
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+            s[v] = 0.f;
+#pragma unroll
+            for (int w8 = 0; w8 < GEMV_CONSUMER_WARPS; ++w8) s[v] += red[w8 * COLS + v * GEMV_COLS + tid];   // fixed order
+        }
+        bool store = (S == 1);
+        if (!store) {
+            float* part = p.partials + (size_t)cb * S * COLS + tid;
+#pragma unroll
+            for (int v = 0; v < NV; ++v) st_cg_f32(part + (size_t)slice * COLS + v * GEMV_COLS, s[v]);
+            __threadfence();
+            consumer_bar_sync();
+            if (tid == 0) {
+                const uint32_t old = atomicAdd(p.tickets + cb, 1u);
+                const bool last = (old == (uint32_t)(S - 1));
+                if (last) p.tickets[cb] = 0u;   // every slice has arrived: re-arm for the next launch
+                *s_last = last ? 1u : 0u;
+            }
+            consumer_bar_sync();
+            if (*s_last) {
+                __threadfence();
+#pragma unroll
+                for (int v = 0; v < NV; ++v) {
+                    s[v] = 0.f;
+                    for (int q = 0; q < S; ++q) s[v] += ld_cg_f32(part + (size_t)q * COLS + v * GEMV_COLS);   // fixed order
+                }
+                store = true;
+            }
+        }
+        if (store) {
+#pragma unroll
+            for (int v = 0; v < NV; ++v) {
+                const int col = cb * COLS + v * GEMV_COLS + (int)tid;
+                if (col < p.N) {
+                    if (p.out_bf16) reinterpret_cast<uint16_t*>(p.y)[col] = f32_to_bf16_rne(s[v]);
+                    else reinterpret_cast<float*>(p.y)[col] = s[v];
+                }
+            }
+        }
+        consumer_bar_sync();   // red and s_last are free for the next column block
+    }
+}
+
 // Generic fallback: no alignment requirement on B when VEC == false.
 template <bool VEC>
 __global__ void __launch_bounds__(256)

@@ -262,6 +262,35 @@ int workspace_for(int dev, cudaStream_t s, size_t need, void** out) {
     return TILE_GEMM_OK;
 }
 
+// GEMV split-K workspace per (device, stream): fp32 partials [col_blocks][split][256] and one ticket per column
+// block (zero between launches: the CTA that draws the last ticket re-arms it).
+struct GemvWs {
+    Buf partials, tickets;
+};
+std::unordered_map<uint64_t, GemvWs> g_gemv_ws;
+
+int gemv_workspace_for(int dev, cudaStream_t s, size_t partial_bytes, size_t ticket_bytes, float** partials,
+                       uint32_t** tickets) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    GemvWs& w = g_gemv_ws[((uint64_t)dev << 56) ^ (uint64_t)(uintptr_t)s];
+    if (w.partials.n < partial_bytes || w.tickets.n < ticket_bytes) {
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(s, &cs) == cudaSuccess && cs != cudaStreamCaptureStatusNone)
+            return fail(TILE_GEMM_E_CUDA,
+                        "the GEMV workspace of this stream must grow during stream capture; run the shape once on "
+                        "the stream before capturing");
+        int rc = grow(w.partials, partial_bytes);
+        if (rc) return rc;
+        const size_t before = w.tickets.n;
+        rc = grow(w.tickets, ticket_bytes);
+        if (rc) return rc;
+        if (w.tickets.n != before) CUDA_TRY(cudaMemsetAsync(w.tickets.p, 0, w.tickets.n, s));
+    }
+    *partials = (float*)w.partials.p;
+    *tickets = (uint32_t*)w.tickets.p;
+    return TILE_GEMM_OK;
+}
+
 // ------------------------------------------------------------------ GEMM launch
 struct GemmConfig {
     int id;       // 1: 1-CTA 128x128, 2: 1-CTA 128x256, 3: 2-CTA 256x256, 4: 2-CTA 256x512
@@ -418,8 +447,99 @@ int run_gemm(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_
 }
 
 // ------------------------------------------------------------------ GEMV launch
+template <int COLS, int TILE_K, int STAGES, int MIN_CTAS>
+int launch_gemv_split(const void* B, int64_t N, int64_t K, int64_t ldb, tg::GemvSplitParams& p, int gx, int split,
+                      bool pdl, cudaStream_t s, int dev) {
+    using L = tg::GemvSplitSmem<COLS, TILE_K, STAGES>;
+    auto kern = tg::gemv_split_kernel<COLS, TILE_K, STAGES, MIN_CTAS>;
+    static bool configured[64] = {};
+    if (!configured[dev]) {
+        CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::TOTAL));
+        configured[dev] = true;
+    }
+    CUtensorMap tb;
+    int rc = get_tensor_map(&tb, B, 2, false, (uint64_t)N, (uint64_t)K, (uint64_t)ldb * 2, (uint32_t)tg::GEMV_COLS,
+                            (uint32_t)TILE_K, 0);
+    if (rc) return rc;
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof cfg);
+    cfg.gridDim = dim3((unsigned)gx, (unsigned)split, 1);
+    cfg.blockDim = dim3(tg::GEMV_TMA_THREADS, 1, 1);
+    cfg.dynamicSmemBytes = L::TOTAL;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = pdl ? 1 : 0;
+    CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, tb, p));
+    g_launches.fetch_add(1);
+    return TILE_GEMM_OK;
+}
+
+// ring shapes of the split kernel: {columns per CTA, rows per stage, stages, CTAs per SM}
+struct GemvShape { int cols, tile_k, stages, occ; };
+constexpr int kNumGemvShapes = 8;
+const GemvShape kGemvShapes[kNumGemvShapes + 1] = {{0, 0, 0, 0},     {256, 64, 2, 3}, {256, 64, 3, 2},
+                                                   {256, 32, 3, 4},  {512, 32, 3, 2}, {512, 32, 2, 3},
+                                                   {512, 16, 4, 3},  {1024, 16, 3, 2}, {512, 16, 3, 4}};
+
+// Default M = 1 kernel: interleaved split-K over a (column block, slice) grid (gemv_kernel.cuh).
+int run_gemv_split(const void* x, const void* B, void* y, int64_t N, int64_t K, int64_t ldb, int out_dtype,
+                   cudaStream_t s, int dev, int sms, unsigned flags) {
+    int shape = g_tune[5].load();
+    if (shape < 1 || shape > kNumGemvShapes) shape = 2;
+    const GemvShape gs = kGemvShapes[shape];
+    const int64_t col_blocks = (N + gs.cols - 1) / gs.cols;
+    const int64_t k_tiles = (K + gs.tile_k - 1) / gs.tile_k;
+    // CTA budget: all CTAs co-resident
+    int64_t budget = (int64_t)sms * gs.occ;
+    const int cap = g_tune[2].load();
+    if (cap > 0 && cap < budget) budget = cap;
+    int64_t gx = col_blocks < budget ? col_blocks : budget;
+    int64_t split = g_tune[3].load();
+    if (split <= 0) split = budget / gx;
+    if (split > k_tiles) split = k_tiles;
+    if (split > 65535) split = 65535;
+    if (split < 1) split = 1;
+    tg::GemvSplitParams p;
+    p.x = (const uint16_t*)x;
+    p.y = y;
+    p.N = (int32_t)N;
+    p.K = (int32_t)K;
+    p.k_tiles = (int32_t)k_tiles;
+    p.col_blocks = (int32_t)col_blocks;
+    p.out_bf16 = out_dtype == TILE_GEMM_OUT_BF16;
+    p.flags = (flags & TILE_GEMM_FLAG_B_IMMUTABLE) ? tg::GEMV_FLAG_B_IMMUTABLE : 0;
+    p.partials = nullptr;
+    p.tickets = nullptr;
+    if (split > 1) {
+        int rc = gemv_workspace_for(dev, s, (size_t)col_blocks * split * gs.cols * 4, (size_t)col_blocks * 4,
+                                    &p.partials, &p.tickets);
+        if (rc) return rc;
+    }
+    const bool pdl = (g_tune[6].load() & 1) == 0;
+#define TG_GEMV_CASE(id, C, T, ST, O) \
+    case id: return launch_gemv_split<C, T, ST, O>(B, N, K, ldb, p, (int)gx, (int)split, pdl, s, dev);
+    switch (shape) {
+        TG_GEMV_CASE(1, 256, 64, 2, 3)
+        TG_GEMV_CASE(2, 256, 64, 3, 2)
+        TG_GEMV_CASE(3, 256, 32, 3, 4)
+        TG_GEMV_CASE(4, 512, 32, 3, 2)
+        TG_GEMV_CASE(5, 512, 32, 2, 3)
+        TG_GEMV_CASE(6, 512, 16, 4, 3)
+        TG_GEMV_CASE(7, 1024, 16, 3, 2)
+        TG_GEMV_CASE(8, 512, 16, 3, 4)
+    }
+#undef TG_GEMV_CASE
+    return fail(TILE_GEMM_E_INTERNAL, "unknown GEMV ring shape %d", shape);
+}
+
 int run_gemv(const void* x, const void* B, void* y, int64_t N, int64_t K, int64_t ldb, int out_dtype, cudaStream_t s,
-             const Plan& plan, int sms) {
+             const Plan& plan, int dev, int sms, unsigned flags) {
+    int variant = g_tune[4].load();   // 0 auto, 1 TMA + cluster split-K, 2 LDG 16-byte, 3 LDG scalar, 4 interleaved split-K
+    if (plan.b_tma && (variant == 0 || variant == 4))
+        return run_gemv_split(x, B, y, N, K, ldb, out_dtype, s, dev, sms, flags);
     tg::GemvParams p;
     p.x = (const uint16_t*)x;
     p.B = (const uint16_t*)B;
@@ -428,7 +548,6 @@ int run_gemv(const void* x, const void* B, void* y, int64_t N, int64_t K, int64_
     p.K = (int32_t)K;
     p.ldb = ldb;
     p.out_bf16 = out_dtype == TILE_GEMM_OUT_BF16;
-    int variant = g_tune[4].load();   // 0 auto, 1 TMA, 2 LDG 16-byte, 3 LDG scalar
     if (!plan.b_tma) variant = 3;
     else if (variant < 1 || variant > 3) variant = 1;
     const int64_t xblocks = (N + tg::GEMV_COLS - 1) / tg::GEMV_COLS;
@@ -505,8 +624,11 @@ int tile_gemm_select(int64_t M, int64_t N, int64_t K, int64_t lda, int64_t ldb, 
     return rc ? -rc : plan.path;
 }
 
-int tile_gemm_ex(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_t K, int64_t lda, int64_t ldb,
-                 int64_t ldc, int out_dtype, void* stream, int force_path) {
+}  // extern "C"
+
+namespace {
+int gemm_entry(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_t K, int64_t lda, int64_t ldb,
+               int64_t ldc, int out_dtype, void* stream, int force_path, unsigned flags) {
     Plan plan;
     int rc = check_and_select(A, B, C, M, N, K, lda, ldb, ldc, out_dtype, &plan);
     if (rc) return rc;
@@ -527,7 +649,7 @@ int tile_gemm_ex(const void* A, const void* B, void* C, int64_t M, int64_t N, in
     cudaStream_t s = (cudaStream_t)stream;
     switch (path) {
         case TILE_GEMM_PATH_ZERO: return run_zero(C, M, N, ldc, plan.esize, s);
-        case TILE_GEMM_PATH_GEMV: return run_gemv(A, B, C, N, K, ldb, out_dtype, s, plan, sms);
+        case TILE_GEMM_PATH_GEMV: return run_gemv(A, B, C, N, K, ldb, out_dtype, s, plan, dev, sms, flags);
         case TILE_GEMM_PATH_GEMM_TMA:
             return run_gemm(A, B, C, M, N, K, lda, ldb, ldc, out_dtype, s, plan, false, dev, sms);
         case TILE_GEMM_PATH_GEMM_REPACK:   // forced: repack both operands; auto: only what TMA cannot address
@@ -535,6 +657,20 @@ int tile_gemm_ex(const void* A, const void* B, void* C, int64_t M, int64_t N, in
                             force_path == TILE_GEMM_PATH_GEMM_REPACK, dev, sms);
     }
     return fail(TILE_GEMM_E_INTERNAL, "unhandled path %d", path);
+}
+}  // namespace
+
+extern "C" {
+
+int tile_gemm_ex(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_t K, int64_t lda, int64_t ldb,
+                 int64_t ldc, int out_dtype, void* stream, int force_path) {
+    return gemm_entry(A, B, C, M, N, K, lda, ldb, ldc, out_dtype, stream, force_path, 0u);
+}
+
+int tile_gemm_static_b(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_t K, int64_t lda,
+                       int64_t ldb, int64_t ldc, int out_dtype, void* stream) {
+    return gemm_entry(A, B, C, M, N, K, lda, ldb, ldc, out_dtype, stream, TILE_GEMM_PATH_AUTO,
+                      TILE_GEMM_FLAG_B_IMMUTABLE);
 }
 
 int tile_gemm(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_t K, int64_t lda, int64_t ldb,
@@ -638,6 +774,11 @@ int tile_gemm_shutdown(void) {
     for (auto& kv : g_ws)
         if (kv.second.p) cudaFree(kv.second.p);
     g_ws.clear();
+    for (auto& kv : g_gemv_ws) {
+        if (kv.second.partials.p) cudaFree(kv.second.partials.p);
+        if (kv.second.tickets.p) cudaFree(kv.second.tickets.p);
+    }
+    g_gemv_ws.clear();
     for (Buf& b : g_stage) {
         if (b.p) cudaFree(b.p);
         b = Buf();

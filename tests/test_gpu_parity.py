@@ -25,7 +25,7 @@ CANARY_BF16 = 0x7FD5
 @pytest.fixture(autouse=True)
 def _reset_tuning():
     yield
-    for key in range(5):
+    for key in range(7):
         tg.tile_gemm_set_tuning(key, 0)
     torch.cuda.synchronize()
 
@@ -199,7 +199,7 @@ def test_large_k_integer_bit_exact():
 
 
 # ------------------------------------------------------------------ GEMV variants
-@pytest.mark.parametrize("variant", [1, 2, 3])
+@pytest.mark.parametrize("variant", [1, 2, 3, 4])
 @pytest.mark.parametrize("split", [0, 1, 3, 8])
 def test_gemv_variants_integer_bit_exact(variant, split):
     tg.tile_gemm_set_tuning(tg.TUNE_GEMV_VARIANT, variant)
@@ -209,6 +209,58 @@ def test_gemv_variants_integer_bit_exact(variant, split):
         ref, _ = oracle.gemm(a, b)
         got = run_case(a, b, "f32", pads=(0, padb, 0), what=f"gemv v{variant} s{split} K={K} N={N}")
         check_bit_exact(got, ref, f"gemv v{variant} s{split} K={K} N={N}")
+
+
+@pytest.mark.parametrize("shape", [1, 2, 3, 4, 5, 6, 7, 8])
+@pytest.mark.parametrize("cap", [0, 1, 3, 7, 100])
+@pytest.mark.parametrize("nopdl", [0, 1])
+def test_gemv_split_decompositions_integer_bit_exact(shape, cap, nopdl):
+    """The interleaved split-K kernel under every decomposition: one CTA looping over all column
+    blocks (cap=1), fewer CTAs than column blocks (cap 3, 7), deep splits with the ticketed fix-up
+    (cap 100 and the full budget); K and N tails; every ring shape; with and without programmatic
+    dependent launch."""
+    occ = shape
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMV_VARIANT, 4)
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMV_SHAPE, shape)
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMM_MAX_CTAS, cap)
+    tg.tile_gemm_set_tuning(tg.TUNE_FLAGS, nopdl)
+    for (K, N, padb) in ((512, 1024, 0), (769, 1537, 7), (2000, 264, 0), (64, 8, 0), (1, 300, 4), (4100, 2056, 0)):
+        a, b = wl.make_inputs_custom(1, N, K, "int4", seed=K + N)
+        ref, _ = oracle.gemm(a, b)
+        for rep in range(2):   # the second call finds the tickets re-armed by the first
+            got = run_case(a, b, "f32", pads=(0, padb, 0), what=f"flat occ{occ} cap{cap} K={K} N={N}")
+            check_bit_exact(got, ref, f"flat occ{occ} cap{cap} K={K} N={N} rep{rep}")
+
+
+@pytest.mark.parametrize("static_b", [False, True])
+def test_gemv_chain_is_stream_ordered_under_pdl(static_b):
+    """y of one GEMV is x of the next, launched back to back with programmatic dependent launch:
+    the bits must equal those of the same chain run with a synchronise after every launch, and every
+    link must match the oracle on the bits it was given."""
+    K = N = 2048
+    depth = 6
+    rng = np.random.default_rng(31)
+    Ws = [wl.bits_to_torch(wl.f32_to_bf16_bits((rng.standard_normal((K, N)) * K ** -0.5).astype(np.float32)), DEV)
+          for _ in range(depth)]
+    x0 = wl.bits_to_torch(wl.f32_to_bf16_bits(rng.standard_normal((1, K)).astype(np.float32)), DEV)
+
+    def chain(sync):
+        xs = [x0] + [torch.empty((1, N), dtype=torch.bfloat16, device=DEV) for _ in range(depth)]
+        for i in range(depth):
+            tg.tile_gemm(xs[i], Ws[i], xs[i + 1], static_b=static_b)
+            if sync:
+                torch.cuda.synchronize()
+        torch.cuda.synchronize()
+        return xs
+
+    want = chain(True)
+    for i in range(depth):
+        ref, S = oracle.gemm(wl.torch_to_bits(want[i]), wl.torch_to_bits(Ws[i]))
+        check_close(want[i + 1].float().cpu().numpy(), ref, S, K, "bf16", f"chain link {i}")
+    for rep in range(10):
+        got = chain(False)
+        for i in range(depth + 1):
+            assert torch.equal(got[i].view(torch.int16), want[i].view(torch.int16)), f"rep {rep} link {i}"
 
 
 def test_gemv_unaligned_weights_take_scalar_path():
