@@ -1,7 +1,9 @@
 """oracle -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
 
 ctypes front end to ``gemm_oracle.c``: the plain fp64 CPU statement of
-``C = A @ B`` (Listing 2) used to judge the CUDA path.
+``C = A @ B`` (Listing 2) used to judge the CUDA path, and to
+``ops_oracle.c``: the element-wise add of Listing 1 and the
+binary16 encoder.
 
 Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s
 ``cpu_baseline`` / ``--impl reference`` legs may import this package.  It
@@ -18,6 +20,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "gemm_oracle.c")
+_SRC_OPS = os.path.join(_HERE, "ops_oracle.c")
 _LIB = os.path.join(_HERE, "liboracle_gemm.so")
 _lib = None
 
@@ -29,10 +32,11 @@ _i64p = ctypes.POINTER(ctypes.c_int64)
 
 
 def build(force: bool = False) -> str:
-    """Compile gemm_oracle.c with gcc (x86-64-v3: runs on any AVX2 host)."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    """Compile gemm_oracle.c and ops_oracle.c with gcc (x86-64-v3: runs on any AVX2 host)."""
+    newest = max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_OPS))
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < newest:
         cmd = ["gcc", "-O3", "-march=x86-64-v3", "-std=c11", "-fPIC", "-shared",
-               "-pthread", "-o", _LIB, _SRC, "-lm"]
+               "-pthread", "-o", _LIB, _SRC, _SRC_OPS, "-lm"]
         subprocess.run(cmd, check=True, cwd=_HERE)
     return _LIB
 
@@ -47,6 +51,16 @@ def _load():
         lib.oracle_gemm_sampled.restype = ctypes.c_int
         lib.oracle_gemm_sampled.argtypes = [_u16p, _u16p, _i64p, _i64p, _i64, _f64p, _f64p,
                                             _i64, _i64, _i64, _i64, _i64]
+        lib.oracle_gemm_typed.restype = ctypes.c_int
+        lib.oracle_gemm_typed.argtypes = lib.oracle_gemm.argtypes + [ctypes.c_int]
+        lib.oracle_gemm_sampled_typed.restype = ctypes.c_int
+        lib.oracle_gemm_sampled_typed.argtypes = lib.oracle_gemm_sampled.argtypes + [ctypes.c_int]
+        lib.oracle_f16_decode_array.restype = None
+        lib.oracle_f16_decode_array.argtypes = [_u16p, _f64p, _i64]
+        lib.oracle_f16_encode_array.restype = None
+        lib.oracle_f16_encode_array.argtypes = [_f32p, _u16p, _i64]
+        lib.oracle_add_f32.restype = None
+        lib.oracle_add_f32.argtypes = [_f32p, _f32p, _f32p, _i64]
         lib.oracle_bf16_decode_array.restype = None
         lib.oracle_bf16_decode_array.argtypes = [_u16p, _f64p, _i64]
         lib.oracle_bf16_encode_array.restype = None
@@ -68,9 +82,13 @@ def _as_u16_2d(x, name):
     return x
 
 
-def gemm(A, B, threads: int | None = None, blocks=(0, 0, 0)):
-    """Full fp64 GEMM.  A: (M,K) uint16 bf16 bits, B: (K,N).  Row strides are
-    taken from the arrays (padded leading dimensions are honoured).
+IN_BF16, IN_F16 = 0, 1
+
+
+def gemm(A, B, threads: int | None = None, blocks=(0, 0, 0), in_dtype: int = IN_BF16):
+    """Full fp64 GEMM.  A: (M,K) uint16 bit patterns (bf16, or binary16 when
+    in_dtype == IN_F16), B: (K,N).  Row strides are taken from the arrays
+    (padded leading dimensions are honoured).
     Returns (C, S) float64 (M,N): C = A@B and S = |A|@|B|."""
     A = _as_u16_2d(A, "A")
     B = _as_u16_2d(B, "B")
@@ -83,17 +101,17 @@ def gemm(A, B, threads: int | None = None, blocks=(0, 0, 0)):
     lda = A.strides[0] // 2 if M > 1 else max(K, 1)
     ldb = B.strides[0] // 2 if K > 1 else max(N, 1)
     lda, ldb = max(lda, K), max(ldb, N)
-    rc = _load().oracle_gemm(A.ctypes.data_as(_u16p), B.ctypes.data_as(_u16p),
-                             C.ctypes.data_as(_f64p), S.ctypes.data_as(_f64p),
-                             M, N, K, lda, ldb, max(N, 1),
-                             default_threads() if threads is None else int(threads),
-                             int(blocks[0]), int(blocks[1]), int(blocks[2]))
+    rc = _load().oracle_gemm_typed(A.ctypes.data_as(_u16p), B.ctypes.data_as(_u16p),
+                                   C.ctypes.data_as(_f64p), S.ctypes.data_as(_f64p),
+                                   M, N, K, lda, ldb, max(N, 1),
+                                   default_threads() if threads is None else int(threads),
+                                   int(blocks[0]), int(blocks[1]), int(blocks[2]), int(in_dtype))
     if rc != 0:
         raise RuntimeError(f"oracle_gemm failed ({rc})")
     return C, S
 
 
-def gemm_sampled(A, B, rows, cols):
+def gemm_sampled(A, B, rows, cols, in_dtype: int = IN_BF16):
     """Dot products for the listed output elements: returns (c, s) float64."""
     A = _as_u16_2d(A, "A")
     B = _as_u16_2d(B, "B")
@@ -106,10 +124,10 @@ def gemm_sampled(A, B, rows, cols):
     s = np.empty(n, dtype=np.float64)
     lda = max(A.strides[0] // 2 if M > 1 else K, K)
     ldb = max(B.strides[0] // 2 if K > 1 else N, N)
-    rc = _load().oracle_gemm_sampled(A.ctypes.data_as(_u16p), B.ctypes.data_as(_u16p),
-                                     rows.ctypes.data_as(_i64p), cols.ctypes.data_as(_i64p), n,
-                                     c.ctypes.data_as(_f64p), s.ctypes.data_as(_f64p),
-                                     M, N, K, lda, ldb)
+    rc = _load().oracle_gemm_sampled_typed(A.ctypes.data_as(_u16p), B.ctypes.data_as(_u16p),
+                                           rows.ctypes.data_as(_i64p), cols.ctypes.data_as(_i64p), n,
+                                           c.ctypes.data_as(_f64p), s.ctypes.data_as(_f64p),
+                                           M, N, K, lda, ldb, int(in_dtype))
     if rc != 0:
         raise RuntimeError(f"oracle_gemm_sampled failed ({rc})")
     return c, s
@@ -129,3 +147,30 @@ def bf16_encode(x):
     out = np.empty(x.shape, dtype=np.uint16)
     _load().oracle_bf16_encode_array(x.ctypes.data_as(_f32p), out.ctypes.data_as(_u16p), x.size)
     return out
+
+
+def f16_decode(bits):
+    """uint16 IEEE binary16 bit patterns -> float64 values (exact)."""
+    bits = np.ascontiguousarray(bits, dtype=np.uint16)
+    out = np.empty(bits.shape, dtype=np.float64)
+    _load().oracle_f16_decode_array(bits.ctypes.data_as(_u16p), out.ctypes.data_as(_f64p), bits.size)
+    return out
+
+
+def f16_encode(x):
+    """float32 -> uint16 binary16 bit patterns, round to nearest even."""
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    out = np.empty(x.shape, dtype=np.uint16)
+    _load().oracle_f16_encode_array(x.ctypes.data_as(_f32p), out.ctypes.data_as(_u16p), x.size)
+    return out
+
+
+def add_f32(x, y):
+    """Listing 1: z_i = fl32(x_i + y_i) for two equal-length float32 vectors."""
+    x = np.ascontiguousarray(x, dtype=np.float32).ravel()
+    y = np.ascontiguousarray(y, dtype=np.float32).ravel()
+    if x.shape != y.shape:
+        raise ValueError("x and y differ in length")
+    z = np.empty_like(x)
+    _load().oracle_add_f32(x.ctypes.data_as(_f32p), y.ctypes.data_as(_f32p), z.ctypes.data_as(_f32p), x.size)
+    return z

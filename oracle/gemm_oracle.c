@@ -63,6 +63,27 @@ static inline double dec(uint16_t h)
 
 double oracle_bf16_decode(uint16_t h) { return dec(h); }
 
+/*
+ * IEEE binary16 ("f16", the precision the paper itself measures)
+ * bit pattern -> real value: sign s, exponent e (5 bits, bias 15), fraction m
+ * (10 bits).  e = 0: (-1)^s * m * 2^-24 (zero and subnormals); e = 31: infinity
+ * (m = 0) or NaN; otherwise (-1)^s * (1 + m/1024) * 2^(e-15).
+ */
+static inline double dec_f16(uint16_t h)
+{
+    const int s = h >> 15, e = (h >> 10) & 31, m = h & 1023;
+    double v;
+    if (e == 0) v = (double)m * 0x1p-24;
+    else if (e == 31) v = m ? NAN : INFINITY;
+    else v = ldexp(1.0 + (double)m * 0x1p-10, e - 15);
+    return s ? -v : v;
+}
+
+double oracle_f16_decode(uint16_t h) { return dec_f16(h); }
+
+/* element type of A and B: 0 = bf16 (BASELINE.json), 1 = f16 */
+static inline double dec_in(uint16_t h, const int f16) { return f16 ? dec_f16(h) : dec(h); }
+
 /* binary32 -> bf16, round to nearest even; NaN -> quiet NaN keeping the sign. */
 uint16_t oracle_bf16_encode(float f)
 {
@@ -84,19 +105,25 @@ void oracle_bf16_encode_array(const float *src, uint16_t *dst, int64_t n)
     for (int64_t i = 0; i < n; ++i) dst[i] = oracle_bf16_encode(src[i]);
 }
 
+void oracle_f16_decode_array(const uint16_t *src, double *dst, int64_t n)
+{
+    for (int64_t i = 0; i < n; ++i) dst[i] = dec_f16(src[i]);
+}
+
 typedef struct {
     const uint16_t *A, *B;
     double *C, *S;
     int64_t i_lo, i_hi, j_lo, j_hi, K, lda, ldb, ldc;
     int64_t MB, KB, NB;
+    int f16; /* input element type, see dec_in */
 } range_job;
 
 static inline int64_t min64(int64_t a, int64_t b) { return a < b ? a : b; }
 
-/* One thread's share: rows [i_lo,i_hi) x columns [j_lo,j_hi), all of K. */
-static void *run_range(void *arg)
+/* One thread's share: rows [i_lo,i_hi) x columns [j_lo,j_hi), all of K.  `f16` is a
+ * compile-time constant in both callers, so the decode is resolved outside the loops. */
+static inline void run_range_typed(const range_job *q, const int f16)
 {
-    const range_job *q = (const range_job *)arg;
     for (int64_t i = q->i_lo; i < q->i_hi; ++i)
         for (int64_t j = q->j_lo; j < q->j_hi; ++j) {
             q->C[i * q->ldc + j] = 0.0; /* tz = constant(ZERO) */
@@ -112,17 +139,24 @@ static void *run_range(void *arg)
                     double *c = q->C + i * q->ldc;
                     double *s = q->S + i * q->ldc;
                     for (int64_t k = k0; k < k1; ++k) {
-                        const double a = dec(q->A[i * q->lda + k]);
+                        const double a = dec_in(q->A[i * q->lda + k], f16);
                         const double aa = fabs(a);
                         const uint16_t *b = q->B + k * q->ldb;
                         for (int64_t j = j0; j < j1; ++j) {
-                            const double bv = dec(b[j]);
+                            const double bv = dec_in(b[j], f16);
                             c[j] += a * bv;        /* tz = mma(tx, ty, tz) */
                             s[j] += aa * fabs(bv); /* tolerance scale      */
                         }
                     }
                 }
             }
+}
+
+static void *run_range(void *arg)
+{
+    const range_job *q = (const range_job *)arg;
+    if (q->f16) run_range_typed(q, 1);
+    else run_range_typed(q, 0);
     return NULL;
 }
 
@@ -132,9 +166,10 @@ static void *run_range(void *arg)
  * threads <= 0 means 1.  MB/KB/NB <= 0 select 64/256/512.  Returns 0, or -1 on
  * a bad argument.
  */
-int oracle_gemm(const uint16_t *A, const uint16_t *B, double *C, double *S,
-                int64_t M, int64_t N, int64_t K, int64_t lda, int64_t ldb,
-                int64_t ldc, int threads, int64_t MB, int64_t KB, int64_t NB)
+int oracle_gemm_typed(const uint16_t *A, const uint16_t *B, double *C, double *S,
+                      int64_t M, int64_t N, int64_t K, int64_t lda, int64_t ldb,
+                      int64_t ldc, int threads, int64_t MB, int64_t KB, int64_t NB,
+                      int in_f16)
 {
     if (M < 0 || N < 0 || K < 0 || lda < K || ldb < N || ldc < N) return -1;
     if (M == 0 || N == 0) return 0;
@@ -152,14 +187,14 @@ int oracle_gemm(const uint16_t *A, const uint16_t *B, double *C, double *S,
         for (int t = 0; t < threads; ++t) {
             const int64_t lo = t * per, hi = min64(lo + per, M);
             if (lo >= hi) break;
-            jobs[n++] = (range_job){A, B, C, S, lo, hi, 0, N, K, lda, ldb, ldc, MB, KB, NB};
+            jobs[n++] = (range_job){A, B, C, S, lo, hi, 0, N, K, lda, ldb, ldc, MB, KB, NB, in_f16 != 0};
         }
     } else { /* few rows (the M=1 GEMV): disjoint column ranges */
         const int64_t per = (N + threads - 1) / threads;
         for (int t = 0; t < threads; ++t) {
             const int64_t lo = t * per, hi = min64(lo + per, N);
             if (lo >= hi) break;
-            jobs[n++] = (range_job){A, B, C, S, 0, M, lo, hi, K, lda, ldb, ldc, MB, KB, NB};
+            jobs[n++] = (range_job){A, B, C, S, 0, M, lo, hi, K, lda, ldb, ldc, MB, KB, NB, in_f16 != 0};
         }
     }
     if (n == 1) {
@@ -175,14 +210,22 @@ int oracle_gemm(const uint16_t *A, const uint16_t *B, double *C, double *S,
     return 0;
 }
 
+/* bf16 inputs (BASELINE.json's five configs). */
+int oracle_gemm(const uint16_t *A, const uint16_t *B, double *C, double *S,
+                int64_t M, int64_t N, int64_t K, int64_t lda, int64_t ldb,
+                int64_t ldc, int threads, int64_t MB, int64_t KB, int64_t NB)
+{
+    return oracle_gemm_typed(A, B, C, S, M, N, K, lda, ldb, ldc, threads, MB, KB, NB, 0);
+}
+
 /*
  * Sampled variant: for each listed (i,j) the two dot products over
  * k = 0..K-1, k ascending, directly from the definition.
  */
-int oracle_gemm_sampled(const uint16_t *A, const uint16_t *B, const int64_t *si,
-                        const int64_t *sj, int64_t nsamples, double *c_out,
-                        double *s_out, int64_t M, int64_t N, int64_t K,
-                        int64_t lda, int64_t ldb)
+int oracle_gemm_sampled_typed(const uint16_t *A, const uint16_t *B, const int64_t *si,
+                              const int64_t *sj, int64_t nsamples, double *c_out,
+                              double *s_out, int64_t M, int64_t N, int64_t K,
+                              int64_t lda, int64_t ldb, int in_f16)
 {
     if (M < 0 || N < 0 || K < 0 || lda < K || ldb < N) return -1;
     for (int64_t t = 0; t < nsamples; ++t) {
@@ -190,8 +233,8 @@ int oracle_gemm_sampled(const uint16_t *A, const uint16_t *B, const int64_t *si,
         if (i < 0 || i >= M || j < 0 || j >= N) return -1;
         double c = 0.0, s = 0.0;
         for (int64_t k = 0; k < K; ++k) {
-            const double a = dec(A[i * lda + k]);
-            const double b = dec(B[k * ldb + j]);
+            const double a = dec_in(A[i * lda + k], in_f16 != 0);
+            const double b = dec_in(B[k * ldb + j], in_f16 != 0);
             c += a * b;
             s += fabs(a) * fabs(b);
         }
@@ -199,4 +242,12 @@ int oracle_gemm_sampled(const uint16_t *A, const uint16_t *B, const int64_t *si,
         s_out[t] = s;
     }
     return 0;
+}
+
+int oracle_gemm_sampled(const uint16_t *A, const uint16_t *B, const int64_t *si,
+                        const int64_t *sj, int64_t nsamples, double *c_out,
+                        double *s_out, int64_t M, int64_t N, int64_t K,
+                        int64_t lda, int64_t ldb)
+{
+    return oracle_gemm_sampled_typed(A, B, si, sj, nsamples, c_out, s_out, M, N, K, lda, ldb, 0);
 }
