@@ -55,6 +55,11 @@ extern "C" {
 /* out_dtype */
 #define TILE_GEMM_OUT_F32 0
 #define TILE_GEMM_OUT_BF16 1
+#define TILE_GEMM_OUT_F16 2   /* IEEE binary16, RNE of the fp32 accumulator (tile_gemm_typed rows) */
+
+/* in_dtype of tile_gemm_typed: element type of A and B */
+#define TILE_GEMM_IN_BF16 0
+#define TILE_GEMM_IN_F16 1    /* IEEE binary16: the precision the paper measures */
 
 /* status codes */
 #define TILE_GEMM_OK 0
@@ -71,7 +76,8 @@ extern "C" {
 #define TILE_GEMM_E_CUDA 11       /* a CUDA runtime/driver call failed (code in message)   */
 #define TILE_GEMM_E_PATH 12       /* force_path unknown or not applicable to this shape    */
 #define TILE_GEMM_E_INTERNAL 13
-#define TILE_GEMM_NUM_STATUS 14
+#define TILE_GEMM_E_IN_DTYPE 14   /* in_dtype is neither BF16 nor F16                       */
+#define TILE_GEMM_NUM_STATUS 15
 
 /* internal flag behind tile_gemm_static_b */
 #define TILE_GEMM_FLAG_B_IMMUTABLE 1u
@@ -116,6 +122,34 @@ int tile_gemm_static_b(const void* A, const void* B, void* C,
                        int64_t M, int64_t N, int64_t K,
                        int64_t lda, int64_t ldb, int64_t ldc,
                        int out_dtype, void* stream);
+
+/*
+ * The same GEMM with the element types spelled out (the paper's
+ * own sweep, Figure 6b / PAPER.md:300, is in f16).  in_dtype = TILE_GEMM_IN_BF16
+ * or TILE_GEMM_IN_F16 is the type of BOTH A and B (raw 16-bit patterns either
+ * way); out_dtype = F32, BF16 or F16.  Same tensor-core instruction and rate for
+ * both input types (tcgen05 kind::f16), fp32 accumulation, one RNE rounding of the
+ * final accumulator for 16-bit outputs; all rules of tile_gemm apply, M == 1
+ * included.  Errors: those of tile_gemm plus TILE_GEMM_E_IN_DTYPE.
+ */
+int tile_gemm_typed(const void* A, const void* B, void* C,
+                    int64_t M, int64_t N, int64_t K,
+                    int64_t lda, int64_t ldb, int64_t ldc,
+                    int in_dtype, int out_dtype, void* stream);
+
+/*
+ * Element-wise add (Listing 1; measured at n = 2^28):
+ *     z[i] = fl32(x[i] + y[i])   for i in [0, n)
+ * one IEEE-754 binary32 addition per element (round to nearest even; NaN and
+ * infinities as the hardware FADD produces them).  x, y, z: DEVICE pointers to n
+ * contiguous floats, 4-byte aligned (16-byte aligned buffers take the 128-bit
+ * path); z is exclusively owned: its byte range may not overlap x's or y's
+ * (TILE_GEMM_E_ALIAS) while x and y may be the same buffer (shared
+ * reads).  Only z[0..n) is written.  n == 0 is a successful no-op.  Errors:
+ * E_EXTENT (n < 0), E_OVERFLOW (n > 2^40), E_NULL, E_ALIGN, E_ALIAS, E_DEVICE,
+ * E_CUDA; nothing is enqueued on error.  Asynchronous on `stream`.
+ */
+int tile_add_f32(const float* x, const float* y, float* z, int64_t n, void* stream);
 
 /*
  * Launch preconditions + shape selector as a pure host function (PAPER.md:200:
@@ -169,7 +203,8 @@ int tile_gemm_query_config(int64_t M, int64_t N, int64_t K, int out_dtype, int32
  * split-K with ticketed fix-up), 5 = ring shape of kernel 4 (0 auto; 1..8 =
  * {columns per CTA, rows per stage, stages, CTAs per SM}, table kGemvShapes in
  * csrc/tile_gemm.cu), 6 = bit 0 disables programmatic dependent launch; key 3 also
- * overrides kernel 4's split.  Returns 0 or
+ * overrides kernel 4's split, 7 = tile_add_f32 launch shape
+ * ((CTAs per SM) << 4 | vectors per thread in {1,2,4,8}; 0 auto).  Returns 0 or
  * E_PATH for an unknown key.
  */
 int tile_gemm_set_tuning(int key, int value);

@@ -16,17 +16,21 @@ from . import build as _build
 
 OUT_F32 = 0
 OUT_BF16 = 1
+OUT_F16 = 2
+IN_BF16 = 0
+IN_F16 = 1
 
 PATH_AUTO, PATH_GEMM_TMA, PATH_GEMM_REPACK, PATH_GEMV, PATH_ZERO, PATH_NOOP = range(6)
 PATH_NAMES = {PATH_AUTO: "auto", PATH_GEMM_TMA: "gemm_tma", PATH_GEMM_REPACK: "gemm_repack",
               PATH_GEMV: "gemv", PATH_ZERO: "zero", PATH_NOOP: "noop"}
 
 (E_OK, E_NULL, E_EXTENT, E_LDA, E_LDB, E_LDC, E_DTYPE, E_ALIGN, E_ALIAS, E_OVERFLOW, E_DEVICE,
- E_CUDA, E_PATH, E_INTERNAL) = range(14)
+ E_CUDA, E_PATH, E_INTERNAL, E_IN_DTYPE) = range(15)
 
-TUNE_GEMM_CONFIG, TUNE_GEMM_GROUP_M, TUNE_GEMM_MAX_CTAS, TUNE_GEMV_SPLIT, TUNE_GEMV_VARIANT, TUNE_GEMV_SHAPE, TUNE_FLAGS = range(7)
+TUNE_GEMM_CONFIG, TUNE_GEMM_GROUP_M, TUNE_GEMM_MAX_CTAS, TUNE_GEMV_SPLIT, TUNE_GEMV_VARIANT, TUNE_GEMV_SHAPE, TUNE_FLAGS, TUNE_ADD_SHAPE = range(8)
 
-EXPORTS = ("tile_gemm", "tile_gemm_ex", "tile_gemm_static_b", "tile_gemm_select", "tile_gemm_host",
+EXPORTS = ("tile_gemm", "tile_gemm_ex", "tile_gemm_static_b", "tile_gemm_typed", "tile_add_f32",
+           "tile_gemm_select", "tile_gemm_host",
            "tile_gemm_debug_owner_map", "tile_gemm_query_config", "tile_gemm_set_tuning",
            "tile_gemm_launch_count", "tile_gemm_status_string", "tile_gemm_last_error",
            "tile_gemm_shutdown")
@@ -70,6 +74,10 @@ def load_library():
     lib.tile_gemm_ex.restype = _int
     lib.tile_gemm_static_b.argtypes = g + [_vp]
     lib.tile_gemm_static_b.restype = _int
+    lib.tile_gemm_typed.argtypes = g[:-1] + [_int, _int, _vp]
+    lib.tile_gemm_typed.restype = _int
+    lib.tile_add_f32.argtypes = [_vp, _vp, _vp, _i64, _vp]
+    lib.tile_add_f32.restype = _int
     lib.tile_gemm_select.argtypes = [_i64] * 6 + [_vp, _vp, _vp, _int]
     lib.tile_gemm_select.restype = _int
     lib.tile_gemm_host.argtypes = g
@@ -144,22 +152,31 @@ def tile_gemm_select(M, N, K, lda, ldb, ldc, A: int = 256, B: int = 1 << 40, C: 
 
 def tile_gemm(A: torch.Tensor, B: torch.Tensor, C: torch.Tensor | None = None, out_dtype=None,
               stream=None, force_path: int = PATH_AUTO, static_b: bool = False) -> torch.Tensor:
-    """C = A @ B on the current CUDA device.  A: (M,K) bf16, B: (K,N) bf16, row-major (any row
-    stride); C: (M,N) fp32 or bf16, allocated if None.  Asynchronous on `stream`.
+    """C = A @ B on the current CUDA device.  A: (M,K), B: (K,N), both bf16 or both f16, row-major
+    (any row stride); C: (M,N) fp32, bf16 or f16, allocated if None.  Asynchronous on `stream`.
+    bf16 inputs with fp32/bf16 output go through tile_gemm_ex / tile_gemm_static_b, anything
+    involving f16 through tile_gemm_typed.
     static_b=True calls tile_gemm_static_b (B holds weights nobody in flight writes)."""
-    if A.dtype != torch.bfloat16 or B.dtype != torch.bfloat16:
-        raise TypeError("A and B must be torch.bfloat16")
+    if A.dtype != B.dtype or A.dtype not in (torch.bfloat16, torch.float16):
+        raise TypeError("A and B must both be torch.bfloat16 or both torch.float16")
     M, K = A.shape
     K2, N = B.shape
     if K != K2:
         raise ValueError("inner dimensions differ")
     if C is None:
-        dt = torch.float32 if out_dtype in (None, OUT_F32, torch.float32) else torch.bfloat16
+        dt = (torch.float32 if out_dtype in (None, OUT_F32, torch.float32)
+              else torch.float16 if out_dtype in (OUT_F16, torch.float16) else torch.bfloat16)
         C = torch.empty((M, N), dtype=dt, device=A.device)
-    if C.dtype not in (torch.float32, torch.bfloat16) or tuple(C.shape) != (M, N):
-        raise TypeError("C must be an (M,N) float32 or bfloat16 tensor")
-    od = OUT_F32 if C.dtype == torch.float32 else OUT_BF16
-    if static_b:
+    if C.dtype not in (torch.float32, torch.bfloat16, torch.float16) or tuple(C.shape) != (M, N):
+        raise TypeError("C must be an (M,N) float32, bfloat16 or float16 tensor")
+    od = {torch.float32: OUT_F32, torch.bfloat16: OUT_BF16, torch.float16: OUT_F16}[C.dtype]
+    if A.dtype == torch.float16 or od == OUT_F16:
+        if static_b or force_path != PATH_AUTO:
+            raise ValueError("static_b / force_path apply to the bf16 entries only")
+        st = load_library().tile_gemm_typed(_vp(A.data_ptr()), _vp(B.data_ptr()), _vp(C.data_ptr()), M, N, K,
+                                            _ld(A), _ld(B), _ld(C), IN_F16 if A.dtype == torch.float16 else IN_BF16,
+                                            od, _vp(_stream_handle(stream)))
+    elif static_b:
         if force_path != PATH_AUTO:
             raise ValueError("static_b cannot be combined with force_path")
         st = load_library().tile_gemm_static_b(_vp(A.data_ptr()), _vp(B.data_ptr()), _vp(C.data_ptr()), M, N, K,
@@ -170,6 +187,31 @@ def tile_gemm(A: torch.Tensor, B: torch.Tensor, C: torch.Tensor | None = None, o
                                          int(force_path))
     _check(st)
     return C
+
+
+def tile_gemm_typed_raw(A: int, B: int, C: int, M, N, K, lda, ldb, ldc, in_dtype, out_dtype, stream: int = 0) -> int:
+    """Raw pointer form of tile_gemm_typed; returns the status code instead of raising."""
+    return int(load_library().tile_gemm_typed(_vp(A), _vp(B), _vp(C), M, N, K, lda, ldb, ldc, int(in_dtype),
+                                              int(out_dtype), _vp(stream)))
+
+
+def tile_add_f32_raw(x: int, y: int, z: int, n: int, stream: int = 0) -> int:
+    return int(load_library().tile_add_f32(_vp(x), _vp(y), _vp(z), int(n), _vp(stream)))
+
+
+def tile_add_f32(x: torch.Tensor, y: torch.Tensor, z: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+    """z = x + y over contiguous float32 vectors on the current CUDA device (Listing 1)."""
+    if x.dtype != torch.float32 or y.dtype != torch.float32 or x.numel() != y.numel():
+        raise TypeError("x and y must be float32 tensors of equal length")
+    if not (x.is_contiguous() and y.is_contiguous()):
+        raise ValueError("x and y must be contiguous")
+    if z is None:
+        z = torch.empty_like(x)
+    if z.dtype != torch.float32 or z.numel() != x.numel() or not z.is_contiguous():
+        raise TypeError("z must be a contiguous float32 tensor of the same length")
+    _check(load_library().tile_add_f32(_vp(x.data_ptr()), _vp(y.data_ptr()), _vp(z.data_ptr()), x.numel(),
+                                       _vp(_stream_handle(stream))))
+    return z
 
 
 def tile_gemm_host(A_bits, B_bits, C_out, lda=None, ldb=None, ldc=None):

@@ -39,7 +39,9 @@ struct GemmParams {
     int32_t tiles_m, tiles_n;   // tile grid; a tile is (GEMM_BM*CG) x (BN*NACC)
     int32_t group_m;            // raster group height in tiles
     int32_t num_k_tiles;
-    int32_t out_bf16;           // 0: fp32 C, 1: bf16 C
+    int32_t out_16;             // 0: fp32 C, 1: 16-bit C (bf16, or f16 when out_f16)
+    int32_t out_f16;            // 16-bit C is IEEE binary16 instead of bf16
+    int32_t in_f16;             // A and B are IEEE binary16 instead of bf16 (PAPER.md:300 measures f16)
     int32_t tma_store;          // 1: TMA store, 0: clipped st.global
     int32_t owner_mode;         // debug: write (tile << 8 | cta) instead of values
     void* C;
@@ -177,9 +179,11 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
     } else if (warp == 1) {
         // ===== MMA issuer (one lane of the leader CTA) =====
         if (rank == 0 && elect_one()) {
-            // instruction descriptor: D=f32, A=B=bf16, A K-major, B MN-major, N = BN, M = 128*CG
-            constexpr uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | (0u << 15) | (1u << 16) |
-                                       ((uint32_t)(BN >> 3) << 17) | ((uint32_t)((GEMM_BM * CG) >> 4) << 24);
+            // instruction descriptor: D=f32, A=B=bf16|f16, A K-major, B MN-major, N = BN, M = 128*CG
+            // (A/B format field: 0 = f16, 1 = bf16; same kind::f16 instruction and rate)
+            const uint32_t ab_fmt = p.in_f16 ? 0u : 1u;
+            const uint32_t idesc = (1u << 4) | (ab_fmt << 7) | (ab_fmt << 10) | (0u << 15) | (1u << 16) |
+                                   ((uint32_t)(BN >> 3) << 17) | ((uint32_t)((GEMM_BM * CG) >> 4) << 24);
             // smem descriptors (version 1, SWIZZLE_128B):
             //   A (K-major):  LBO unused (=1), SBO = 1024 B between 8-row groups
             //   B (MN-major): LBO = one 64-column box (8192 B), SBO = 1024 B between 8-k groups
@@ -248,12 +252,13 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
         const uint32_t sbuf0 = smem_base + L::EPI_OFF + ew * GEMM_EPI_BUF_BYTES;
         const uint8_t* sgen0 = smem_gen + L::EPI_OFF + ew * GEMM_EPI_BUF_BYTES;
         const uint32_t sw = (lane >> 1) & 3u;
-        const int out_bf16 = p.out_bf16;
-        const int sub_cols = out_bf16 ? 32 : 16;              // 64 B of C per row per sub-chunk
+        const int out_16 = p.out_16;
+        const int out_f16 = p.out_f16;
+        const int sub_cols = out_16 ? 32 : 16;              // 64 B of C per row per sub-chunk
         // TMA stores clip at 16-byte granularity along a row (measured on B200): when N is not a
         // multiple of 16 bytes of elements the sub-chunk containing column N-1 takes the clipped
         // st.global path so that C[i][N..] is never written.
-        const bool ragged_n = (p.N % (out_bf16 ? 8 : 4)) != 0;
+        const bool ragged_n = (p.N % (out_16 ? 8 : 4)) != 0;
         uint32_t it = 0, buf = 0;
         for (int t = first_tile; t < total_tiles; t += tile_stride, ++it) {
             int tm, tn;
@@ -301,7 +306,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
                     const uint8_t* sg = sgen0 + buf * 2048u;
                     const int rows = (p.M - m0) < 32 ? (p.M - m0) : 32;
                     const int e = (int)lane;                   // column within the sub-chunk
-                    if (out_bf16) {
+                    if (out_16) {
                         uint16_t* Cb = reinterpret_cast<uint16_t*>(p.C);
                         if (n0 + e < p.N)
                             for (int r = 0; r < rows; ++r) {
@@ -330,8 +335,13 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
             // one unit: `v` holds 32 consecutive columns of this thread's row
             auto stage_unit = [&](uint32_t (&v)[32], int u) {
                 const int n0 = n_base + u * 32;
-                if (out_bf16) {
+                if (out_16 && !out_f16) {
 #define TG_PK(i) pack_bf16x2(__uint_as_float(v[2 * (i)]), __uint_as_float(v[2 * (i) + 1]))
+                    emit(TG_PK(0), TG_PK(1), TG_PK(2), TG_PK(3), TG_PK(4), TG_PK(5), TG_PK(6), TG_PK(7), TG_PK(8),
+                         TG_PK(9), TG_PK(10), TG_PK(11), TG_PK(12), TG_PK(13), TG_PK(14), TG_PK(15), n0);
+#undef TG_PK
+                } else if (out_16) {
+#define TG_PK(i) pack_f16x2(__uint_as_float(v[2 * (i)]), __uint_as_float(v[2 * (i) + 1]))
                     emit(TG_PK(0), TG_PK(1), TG_PK(2), TG_PK(3), TG_PK(4), TG_PK(5), TG_PK(6), TG_PK(7), TG_PK(8),
                          TG_PK(9), TG_PK(10), TG_PK(11), TG_PK(12), TG_PK(13), TG_PK(14), TG_PK(15), n0);
 #undef TG_PK

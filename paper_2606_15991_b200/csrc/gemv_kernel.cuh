@@ -14,6 +14,8 @@
 // are combined through distributed shared memory in a fixed order (thread -> warp -> cluster
 // rank), so results are bitwise reproducible and need no global workspace or atomics.
 #pragma once
+#include <cuda_fp16.h>
+
 #include "ptx.cuh"
 
 namespace tg {
@@ -31,12 +33,29 @@ struct GemvParams {
     int32_t N, K;
     int64_t ldb;
     int32_t k_per_cta;   // rows per split-K slice (multiple of GEMV_TILE_K)
-    int32_t out_bf16;
+    int32_t out_kind;    // 0: fp32 y, 1: bf16 y, 2: f16 y
 };
 
-__device__ __forceinline__ float bf16_bits_to_f32(uint16_t h) { return __uint_as_float(((uint32_t)h) << 16); }
+// 16-bit input element -> fp32 (exact).  F16 = false: bf16 is the upper half of a binary32;
+// F16 = true: IEEE binary16 (the paper's precision), one cvt per element.
+template <bool F16>
+__device__ __forceinline__ float in_bits_to_f32(uint16_t h) {
+    if constexpr (F16) return __half2float(__ushort_as_half(h));
+    else return __uint_as_float(((uint32_t)h) << 16);
+}
 
+template <bool F16>
 __device__ __forceinline__ void fma8(float (&acc)[8], const uint4& w, float xr) {
+    if constexpr (F16) {
+        const uint32_t u[4] = {w.x, w.y, w.z, w.w};
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&u[i]));
+            acc[2 * i] = fmaf(f.x, xr, acc[2 * i]);
+            acc[2 * i + 1] = fmaf(f.y, xr, acc[2 * i + 1]);
+        }
+        return;
+    }
     acc[0] = fmaf(__uint_as_float(w.x << 16), xr, acc[0]);
     acc[1] = fmaf(__uint_as_float(w.x & 0xffff0000u), xr, acc[1]);
     acc[2] = fmaf(__uint_as_float(w.y << 16), xr, acc[2]);
@@ -51,6 +70,13 @@ __device__ __forceinline__ uint16_t f32_to_bf16_rne(float f) {
     uint16_t r;
     asm("cvt.rn.bf16.f32 %0, %1;" : "=h"(r) : "f"(f));
     return r;
+}
+
+// y[col] = round_out(s): out_kind 0 fp32, 1 bf16 (RNE), 2 f16 (RNE)
+__device__ __forceinline__ void gemv_store(void* y, int col, float s, int out_kind) {
+    if (out_kind == 0) reinterpret_cast<float*>(y)[col] = s;
+    else if (out_kind == 1) reinterpret_cast<uint16_t*>(y)[col] = f32_to_bf16_rne(s);
+    else reinterpret_cast<uint16_t*>(y)[col] = __half_as_ushort(__float2half_rn(s));
 }
 
 // Combine the per-thread partial sums of one CTA (warps ordered along K) and of the split-K
@@ -84,15 +110,12 @@ __device__ __forceinline__ void gemv_reduce_and_store(const float (&acc)[8], flo
             s = part[tid];
         }
         const int col = n0 + (int)tid;
-        if (col < p.N) {
-            if (p.out_bf16) reinterpret_cast<uint16_t*>(p.y)[col] = f32_to_bf16_rne(s);
-            else reinterpret_cast<float*>(p.y)[col] = s;
-        }
+        if (col < p.N) gemv_store(p.y, col, s, p.out_kind);
     }
     if (nsplit > 1) cluster_sync();   // peers may still be reading this CTA's `part`
 }
 
-template <int STAGES>
+template <int STAGES, bool F16>
 __global__ void __launch_bounds__(GEMV_TMA_THREADS)
 gemv_tma_kernel(const __grid_constant__ CUtensorMap tmap_b, const GemvParams p) {
     extern __shared__ uint8_t smem_raw[];
@@ -145,7 +168,7 @@ gemv_tma_kernel(const __grid_constant__ CUtensorMap tmap_b, const GemvParams p) 
         // ===== consumers: warp w owns rows 8w..8w+7 of every tile =====
         auto load_x = [&](int it) -> float {
             const int k = k_begin + it * GEMV_TILE_K + (int)warp * 8 + (int)(lane & 7u);
-            return (it < ntiles && k < p.K) ? bf16_bits_to_f32(__ldg(p.x + k)) : 0.f;
+            return (it < ntiles && k < p.K) ? in_bits_to_f32<F16>(__ldg(p.x + k)) : 0.f;
         };
         uint32_t stage = 0, phase = 0;
         float xv_next = load_x(0);
@@ -158,7 +181,7 @@ gemv_tma_kernel(const __grid_constant__ CUtensorMap tmap_b, const GemvParams p) 
 #pragma unroll
             for (int r = 0; r < 8; ++r) w[r] = *reinterpret_cast<const uint4*>(tile + r * (GEMV_COLS * 2));
 #pragma unroll
-            for (int r = 0; r < 8; ++r) fma8(acc, w[r], __shfl_sync(0xffffffffu, xv, r));
+            for (int r = 0; r < 8; ++r) fma8<F16>(acc, w[r], __shfl_sync(0xffffffffu, xv, r));
             __syncwarp();
             if (lane == 0) mbar_arrive(empty_bar(stage));
             if (++stage == STAGES) { stage = 0; phase ^= 1u; }
@@ -196,7 +219,7 @@ struct GemvSplitParams {
     int32_t N, K;
     int32_t k_tiles;      // ceil(K / TILE_K), >= split
     int32_t col_blocks;
-    int32_t out_bf16;
+    int32_t out_kind;     // 0: fp32 y, 1: bf16 y, 2: f16 y
     int32_t flags;
 };
 
@@ -228,7 +251,7 @@ struct GemvSplitSmem {
 
 // COLS columns per CTA (NV = COLS / 256 TMA boxes side by side: a row segment of COLS * 2
 // contiguous bytes), TILE_K rows per ring stage.
-template <int COLS, int TILE_K, int STAGES, int MIN_CTAS>
+template <int COLS, int TILE_K, int STAGES, int MIN_CTAS, bool F16>
 __global__ void __launch_bounds__(GEMV_TMA_THREADS, MIN_CTAS)
 gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const GemvSplitParams p) {
     using L = GemvSplitSmem<COLS, TILE_K, STAGES>;
@@ -286,7 +309,7 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const GemvSplitPar
     const uint32_t tid = threadIdx.x;   // 0..255
     auto load_x = [&](int kt_) -> float {
         const int k = kt_ * TILE_K + (int)warp * RPW + (int)(lane & (RPW - 1));
-        return (kt_ < KT && k < p.K) ? bf16_bits_to_f32(__ldg(p.x + k)) : 0.f;
+        return (kt_ < KT && k < p.K) ? in_bits_to_f32<F16>(__ldg(p.x + k)) : 0.f;
     };
     uint32_t stage = 0, phase = 0;
     for (int cb = (int)blockIdx.x; cb < p.col_blocks; cb += (int)gridDim.x) {
@@ -311,7 +334,7 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const GemvSplitPar
             for (int r = 0; r < RPW; ++r) {
                 const float xr = __shfl_sync(0xffffffffu, xv, r);
 #pragma unroll
-                for (int v = 0; v < NV; ++v) fma8(acc[v], w[v][r], xr);
+                for (int v = 0; v < NV; ++v) fma8<F16>(acc[v], w[v][r], xr);
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(empty_bar(stage));
@@ -360,10 +383,7 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const GemvSplitPar
 #pragma unroll
             for (int v = 0; v < NV; ++v) {
                 const int col = cb * COLS + v * GEMV_COLS + (int)tid;
-                if (col < p.N) {
-                    if (p.out_bf16) reinterpret_cast<uint16_t*>(p.y)[col] = f32_to_bf16_rne(s[v]);
-                    else reinterpret_cast<float*>(p.y)[col] = s[v];
-                }
+                if (col < p.N) gemv_store(p.y, col, s[v], p.out_kind);
             }
         }
         consumer_bar_sync();   // red and s_last are free for the next column block
@@ -371,7 +391,7 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const GemvSplitPar
 }
 
 // Generic fallback: no alignment requirement on B when VEC == false.
-template <bool VEC>
+template <bool VEC, bool F16>
 __global__ void __launch_bounds__(256)
 gemv_ldg_kernel(const GemvParams p) {
     __shared__ float red[8 * GEMV_COLS];
@@ -414,7 +434,7 @@ gemv_ldg_kernel(const GemvParams p) {
 
     for (int k0 = wb; k0 < we; k0 += 32) {
         const int kk = k0 + (int)lane;
-        const float xv = (kk < we) ? bf16_bits_to_f32(__ldg(p.x + kk)) : 0.f;
+        const float xv = (kk < we) ? in_bits_to_f32<F16>(__ldg(p.x + kk)) : 0.f;
         const int nrows = min(32, we - k0);
         if (nrows == 32) {
 #pragma unroll
@@ -423,12 +443,12 @@ gemv_ldg_kernel(const GemvParams p) {
 #pragma unroll
                 for (int u = 0; u < 8; ++u) w[u] = load_row(k0 + r0 + u);
 #pragma unroll
-                for (int u = 0; u < 8; ++u) fma8(acc, w[u], __shfl_sync(0xffffffffu, xv, r0 + u));
+                for (int u = 0; u < 8; ++u) fma8<F16>(acc, w[u], __shfl_sync(0xffffffffu, xv, r0 + u));
             }
         } else {
             for (int r = 0; r < nrows; ++r) {
                 const uint4 w = load_row(k0 + r);
-                fma8(acc, w, __shfl_sync(0xffffffffu, xv, r));
+                fma8<F16>(acc, w, __shfl_sync(0xffffffffu, xv, r));
             }
         }
     }

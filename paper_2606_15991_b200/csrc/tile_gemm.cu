@@ -17,6 +17,7 @@
 #include <mutex>
 #include <unordered_map>
 
+#include "add_kernel.cuh"
 #include "aux_kernels.cuh"
 #include "gemm_kernel.cuh"
 #include "gemv_kernel.cuh"
@@ -49,6 +50,7 @@ const char* const kStatusNames[TILE_GEMM_NUM_STATUS] = {
     "CUDA call failed",
     "path not applicable",
     "internal error",
+    "unknown in_dtype",
 };
 
 std::atomic<int64_t> g_launches{0};
@@ -79,13 +81,17 @@ bool overlaps(const void* p, int64_t pn, const void* q, int64_t qn) {
 }
 
 int check_and_select(const void* A, const void* B, const void* C, int64_t M, int64_t N, int64_t K, int64_t lda,
-                     int64_t ldb, int64_t ldc, int out_dtype, Plan* plan) {
+                     int64_t ldb, int64_t ldc, int in_dtype, int out_dtype, Plan* plan) {
     if (M < 0 || N < 0 || K < 0)
         return fail(TILE_GEMM_E_EXTENT, "negative extent: M=%lld N=%lld K=%lld", (long long)M, (long long)N,
                     (long long)K);
-    if (out_dtype != TILE_GEMM_OUT_F32 && out_dtype != TILE_GEMM_OUT_BF16)
-        return fail(TILE_GEMM_E_DTYPE, "out_dtype=%d is neither TILE_GEMM_OUT_F32 (0) nor TILE_GEMM_OUT_BF16 (1)",
+    if (out_dtype != TILE_GEMM_OUT_F32 && out_dtype != TILE_GEMM_OUT_BF16 && out_dtype != TILE_GEMM_OUT_F16)
+        return fail(TILE_GEMM_E_DTYPE,
+                    "out_dtype=%d is none of TILE_GEMM_OUT_F32 (0), TILE_GEMM_OUT_BF16 (1), TILE_GEMM_OUT_F16 (2)",
                     out_dtype);
+    if (in_dtype != TILE_GEMM_IN_BF16 && in_dtype != TILE_GEMM_IN_F16)
+        return fail(TILE_GEMM_E_IN_DTYPE, "in_dtype=%d is neither TILE_GEMM_IN_BF16 (0) nor TILE_GEMM_IN_F16 (1)",
+                    in_dtype);
     if (lda < K) return fail(TILE_GEMM_E_LDA, "lda=%lld < K=%lld", (long long)lda, (long long)K);
     if (ldb < N) return fail(TILE_GEMM_E_LDB, "ldb=%lld < N=%lld", (long long)ldb, (long long)N);
     if (ldc < N) return fail(TILE_GEMM_E_LDC, "ldc=%lld < N=%lld", (long long)ldc, (long long)N);
@@ -93,7 +99,7 @@ int check_and_select(const void* A, const void* B, const void* C, int64_t M, int
     if (M > lim || N > lim || K > lim)
         return fail(TILE_GEMM_E_OVERFLOW, "extent above 2^31-1025: M=%lld N=%lld K=%lld", (long long)M, (long long)N,
                     (long long)K);
-    plan->esize = (out_dtype == TILE_GEMM_OUT_BF16) ? 2 : 4;
+    plan->esize = (out_dtype == TILE_GEMM_OUT_F32) ? 4 : 2;
     if (!span_bytes(M, K, lda, 2, &plan->a_bytes) || !span_bytes(K, N, ldb, 2, &plan->b_bytes) ||
         !span_bytes(M, N, ldc, plan->esize, &plan->c_bytes))
         return fail(TILE_GEMM_E_OVERFLOW, "operand byte span overflows int64");
@@ -327,7 +333,7 @@ struct GemmLaunch {
     int ctas;
 };
 
-void plan_gemm(int64_t M, int64_t N, int64_t K, int out_bf16, int sms, GemmLaunch* gl) {
+void plan_gemm(int64_t M, int64_t N, int64_t K, int in_dtype, int out_dtype, int sms, GemmLaunch* gl) {
     gl->cfg = choose_config(M, N, sms);
     const int tile_m = tg::GEMM_BM * gl->cfg.cg;
     tg::GemmParams& p = gl->p;
@@ -339,7 +345,9 @@ void plan_gemm(int64_t M, int64_t N, int64_t K, int out_bf16, int sms, GemmLaunc
     if (gm <= 0) gm = (gl->cfg.cg == 2) ? 8 : 16;
     p.group_m = gm < p.tiles_m ? gm : p.tiles_m;
     p.num_k_tiles = (int32_t)((K + tg::GEMM_BK - 1) / tg::GEMM_BK);
-    p.out_bf16 = out_bf16;
+    p.out_16 = out_dtype != TILE_GEMM_OUT_F32;
+    p.out_f16 = out_dtype == TILE_GEMM_OUT_F16;
+    p.in_f16 = in_dtype == TILE_GEMM_IN_F16;
     int64_t units = (int64_t)p.tiles_m * p.tiles_n;
     int max_units = sms / gl->cfg.cg;
     const int cap = g_tune[2].load();
@@ -387,15 +395,17 @@ int launch_gemm(const GemmLaunch& gl, const CUtensorMap& ta, const CUtensorMap& 
     return fail(TILE_GEMM_E_INTERNAL, "unknown GEMM config %d", gl.cfg.id);
 }
 
-int c_tensor_map(CUtensorMap* tc, void* C, int64_t M, int64_t N, int64_t ldc, int out_bf16) {
-    // one epilogue sub-chunk: 32 rows x 64 bytes, 64B-swizzled in shared memory
-    return get_tensor_map(tc, C, out_bf16 ? 2 : 4, !out_bf16, (uint64_t)N, (uint64_t)M,
-                          (uint64_t)ldc * (out_bf16 ? 2 : 4), out_bf16 ? 32u : 16u, 32u, 64);
+int c_tensor_map(CUtensorMap* tc, void* C, int64_t M, int64_t N, int64_t ldc, int out_16) {
+    // one epilogue sub-chunk: 32 rows x 64 bytes, 64B-swizzled in shared memory (a 16-bit C is
+    // described as bf16 whichever 16-bit format it holds: tiled TMA moves bits, it never converts)
+    return get_tensor_map(tc, C, out_16 ? 2 : 4, !out_16, (uint64_t)N, (uint64_t)M,
+                          (uint64_t)ldc * (out_16 ? 2 : 4), out_16 ? 32u : 16u, 32u, 64);
 }
 
 int run_gemm(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_t K, int64_t lda, int64_t ldb,
-             int64_t ldc, int out_dtype, cudaStream_t s, const Plan& plan, bool force_repack, int dev, int sms) {
-    const int out_bf16 = out_dtype == TILE_GEMM_OUT_BF16;
+             int64_t ldc, int in_dtype, int out_dtype, cudaStream_t s, const Plan& plan, bool force_repack, int dev,
+             int sms) {
+    const int out_16 = out_dtype != TILE_GEMM_OUT_F32;
     const bool rep_a = force_repack || !plan.a_tma;
     const bool rep_b = force_repack || !plan.b_tma;
     const uint16_t* Ap = (const uint16_t*)A;
@@ -428,7 +438,7 @@ int run_gemm(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_
         }
     }
     GemmLaunch gl;
-    plan_gemm(M, N, K, out_bf16, sms, &gl);
+    plan_gemm(M, N, K, in_dtype, out_dtype, sms, &gl);
     gl.p.tma_store = plan.c_tma ? 1 : 0;
     gl.p.C = C;
     gl.p.ldc = ldc;
@@ -438,7 +448,7 @@ int run_gemm(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_
     rc = get_tensor_map(&tb, Bp, 2, false, (uint64_t)N, (uint64_t)K, (uint64_t)ldb * 2, 64u, 64u, 128);
     if (rc) return rc;
     if (plan.c_tma) {
-        rc = c_tensor_map(&tc, C, M, N, ldc, out_bf16);
+        rc = c_tensor_map(&tc, C, M, N, ldc, out_16);
         if (rc) return rc;
     } else {
         tc = ta;   // never dereferenced by the clipped st.global epilogue; must still be a valid map
@@ -447,11 +457,11 @@ int run_gemm(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_
 }
 
 // ------------------------------------------------------------------ GEMV launch
-template <int COLS, int TILE_K, int STAGES, int MIN_CTAS>
+template <int COLS, int TILE_K, int STAGES, int MIN_CTAS, bool F16>
 int launch_gemv_split(const void* B, int64_t N, int64_t K, int64_t ldb, tg::GemvSplitParams& p, int gx, int split,
                       bool pdl, cudaStream_t s, int dev) {
     using L = tg::GemvSplitSmem<COLS, TILE_K, STAGES>;
-    auto kern = tg::gemv_split_kernel<COLS, TILE_K, STAGES, MIN_CTAS>;
+    auto kern = tg::gemv_split_kernel<COLS, TILE_K, STAGES, MIN_CTAS, F16>;
     static bool configured[64] = {};
     if (!configured[dev]) {
         CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::TOTAL));
@@ -485,8 +495,8 @@ const GemvShape kGemvShapes[kNumGemvShapes + 1] = {{0, 0, 0, 0},     {256, 64, 2
                                                    {512, 16, 4, 3},  {1024, 16, 3, 2}, {512, 16, 3, 4}};
 
 // Default M = 1 kernel: interleaved split-K over a (column block, slice) grid (gemv_kernel.cuh).
-int run_gemv_split(const void* x, const void* B, void* y, int64_t N, int64_t K, int64_t ldb, int out_dtype,
-                   cudaStream_t s, int dev, int sms, unsigned flags) {
+int run_gemv_split(const void* x, const void* B, void* y, int64_t N, int64_t K, int64_t ldb, int in_dtype,
+                   int out_dtype, cudaStream_t s, int dev, int sms, unsigned flags) {
     int shape = g_tune[5].load();
     if (shape < 1 || shape > kNumGemvShapes) shape = 2;
     const GemvShape gs = kGemvShapes[shape];
@@ -509,7 +519,7 @@ int run_gemv_split(const void* x, const void* B, void* y, int64_t N, int64_t K, 
     p.K = (int32_t)K;
     p.k_tiles = (int32_t)k_tiles;
     p.col_blocks = (int32_t)col_blocks;
-    p.out_bf16 = out_dtype == TILE_GEMM_OUT_BF16;
+    p.out_kind = out_dtype;
     p.flags = (flags & TILE_GEMM_FLAG_B_IMMUTABLE) ? tg::GEMV_FLAG_B_IMMUTABLE : 0;
     p.partials = nullptr;
     p.tickets = nullptr;
@@ -519,8 +529,11 @@ int run_gemv_split(const void* x, const void* B, void* y, int64_t N, int64_t K, 
         if (rc) return rc;
     }
     const bool pdl = (g_tune[6].load() & 1) == 0;
-#define TG_GEMV_CASE(id, C, T, ST, O) \
-    case id: return launch_gemv_split<C, T, ST, O>(B, N, K, ldb, p, (int)gx, (int)split, pdl, s, dev);
+    const bool f16 = in_dtype == TILE_GEMM_IN_F16;
+#define TG_GEMV_CASE(id, C, T, ST, O)                                                                        \
+    case id:                                                                                                 \
+        return f16 ? launch_gemv_split<C, T, ST, O, true>(B, N, K, ldb, p, (int)gx, (int)split, pdl, s, dev) \
+                   : launch_gemv_split<C, T, ST, O, false>(B, N, K, ldb, p, (int)gx, (int)split, pdl, s, dev);
     switch (shape) {
         TG_GEMV_CASE(1, 256, 64, 2, 3)
         TG_GEMV_CASE(2, 256, 64, 3, 2)
@@ -535,11 +548,12 @@ int run_gemv_split(const void* x, const void* B, void* y, int64_t N, int64_t K, 
     return fail(TILE_GEMM_E_INTERNAL, "unknown GEMV ring shape %d", shape);
 }
 
-int run_gemv(const void* x, const void* B, void* y, int64_t N, int64_t K, int64_t ldb, int out_dtype, cudaStream_t s,
-             const Plan& plan, int dev, int sms, unsigned flags) {
+int run_gemv(const void* x, const void* B, void* y, int64_t N, int64_t K, int64_t ldb, int in_dtype, int out_dtype,
+             cudaStream_t s, const Plan& plan, int dev, int sms, unsigned flags) {
+    const bool f16 = in_dtype == TILE_GEMM_IN_F16;
     int variant = g_tune[4].load();   // 0 auto, 1 TMA + cluster split-K, 2 LDG 16-byte, 3 LDG scalar, 4 interleaved split-K
     if (plan.b_tma && (variant == 0 || variant == 4))
-        return run_gemv_split(x, B, y, N, K, ldb, out_dtype, s, dev, sms, flags);
+        return run_gemv_split(x, B, y, N, K, ldb, in_dtype, out_dtype, s, dev, sms, flags);
     tg::GemvParams p;
     p.x = (const uint16_t*)x;
     p.B = (const uint16_t*)B;
@@ -547,7 +561,7 @@ int run_gemv(const void* x, const void* B, void* y, int64_t N, int64_t K, int64_
     p.N = (int32_t)N;
     p.K = (int32_t)K;
     p.ldb = ldb;
-    p.out_bf16 = out_dtype == TILE_GEMM_OUT_BF16;
+    p.out_kind = out_dtype;
     if (!plan.b_tma) variant = 3;
     else if (variant < 1 || variant > 3) variant = 1;
     const int64_t xblocks = (N + tg::GEMV_COLS - 1) / tg::GEMV_COLS;
@@ -580,12 +594,8 @@ int run_gemv(const void* x, const void* B, void* y, int64_t N, int64_t K, int64_
         constexpr int STAGES = 3;
         constexpr uint32_t smem = STAGES * tg::GEMV_TILE_BYTES + tg::GEMV_CONSUMER_WARPS * tg::GEMV_COLS * 4 +
                                   tg::GEMV_COLS * 4 + 2 * STAGES * 8 + 128;
-        auto kern = tg::gemv_tma_kernel<STAGES>;
-        static bool configured = false;
-        if (!configured) {
-            CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            configured = true;
-        }
+        auto kern = f16 ? tg::gemv_tma_kernel<STAGES, true> : tg::gemv_tma_kernel<STAGES, false>;
+        CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         CUtensorMap tb;
         int rc = get_tensor_map(&tb, B, 2, false, (uint64_t)N, (uint64_t)K, (uint64_t)ldb * 2, (uint32_t)tg::GEMV_COLS,
                                 (uint32_t)tg::GEMV_TILE_K, 0);
@@ -596,8 +606,9 @@ int run_gemv(const void* x, const void* B, void* y, int64_t N, int64_t K, int64_
     } else {
         cfg.blockDim = dim3(256, 1, 1);
         cfg.dynamicSmemBytes = 0;
-        if (variant == 2) CUDA_TRY(cudaLaunchKernelEx(&cfg, tg::gemv_ldg_kernel<true>, p));
-        else CUDA_TRY(cudaLaunchKernelEx(&cfg, tg::gemv_ldg_kernel<false>, p));
+        auto kern = variant == 2 ? (f16 ? tg::gemv_ldg_kernel<true, true> : tg::gemv_ldg_kernel<true, false>)
+                                 : (f16 ? tg::gemv_ldg_kernel<false, true> : tg::gemv_ldg_kernel<false, false>);
+        CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, p));
     }
     g_launches.fetch_add(1);
     return TILE_GEMM_OK;
@@ -620,7 +631,7 @@ extern "C" {
 int tile_gemm_select(int64_t M, int64_t N, int64_t K, int64_t lda, int64_t ldb, int64_t ldc, const void* A,
                      const void* B, const void* C, int out_dtype) {
     Plan plan;
-    const int rc = check_and_select(A, B, C, M, N, K, lda, ldb, ldc, out_dtype, &plan);
+    const int rc = check_and_select(A, B, C, M, N, K, lda, ldb, ldc, TILE_GEMM_IN_BF16, out_dtype, &plan);
     return rc ? -rc : plan.path;
 }
 
@@ -628,9 +639,9 @@ int tile_gemm_select(int64_t M, int64_t N, int64_t K, int64_t lda, int64_t ldb, 
 
 namespace {
 int gemm_entry(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_t K, int64_t lda, int64_t ldb,
-               int64_t ldc, int out_dtype, void* stream, int force_path, unsigned flags) {
+               int64_t ldc, int in_dtype, int out_dtype, void* stream, int force_path, unsigned flags) {
     Plan plan;
-    int rc = check_and_select(A, B, C, M, N, K, lda, ldb, ldc, out_dtype, &plan);
+    int rc = check_and_select(A, B, C, M, N, K, lda, ldb, ldc, in_dtype, out_dtype, &plan);
     if (rc) return rc;
     if (force_path < TILE_GEMM_PATH_AUTO || force_path > TILE_GEMM_PATH_GEMV)
         return fail(TILE_GEMM_E_PATH, "force_path=%d is not AUTO, GEMM_TMA, GEMM_REPACK or GEMV", force_path);
@@ -649,11 +660,11 @@ int gemm_entry(const void* A, const void* B, void* C, int64_t M, int64_t N, int6
     cudaStream_t s = (cudaStream_t)stream;
     switch (path) {
         case TILE_GEMM_PATH_ZERO: return run_zero(C, M, N, ldc, plan.esize, s);
-        case TILE_GEMM_PATH_GEMV: return run_gemv(A, B, C, N, K, ldb, out_dtype, s, plan, dev, sms, flags);
+        case TILE_GEMM_PATH_GEMV: return run_gemv(A, B, C, N, K, ldb, in_dtype, out_dtype, s, plan, dev, sms, flags);
         case TILE_GEMM_PATH_GEMM_TMA:
-            return run_gemm(A, B, C, M, N, K, lda, ldb, ldc, out_dtype, s, plan, false, dev, sms);
+            return run_gemm(A, B, C, M, N, K, lda, ldb, ldc, in_dtype, out_dtype, s, plan, false, dev, sms);
         case TILE_GEMM_PATH_GEMM_REPACK:   // forced: repack both operands; auto: only what TMA cannot address
-            return run_gemm(A, B, C, M, N, K, lda, ldb, ldc, out_dtype, s, plan,
+            return run_gemm(A, B, C, M, N, K, lda, ldb, ldc, in_dtype, out_dtype, s, plan,
                             force_path == TILE_GEMM_PATH_GEMM_REPACK, dev, sms);
     }
     return fail(TILE_GEMM_E_INTERNAL, "unhandled path %d", path);
@@ -664,12 +675,12 @@ extern "C" {
 
 int tile_gemm_ex(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_t K, int64_t lda, int64_t ldb,
                  int64_t ldc, int out_dtype, void* stream, int force_path) {
-    return gemm_entry(A, B, C, M, N, K, lda, ldb, ldc, out_dtype, stream, force_path, 0u);
+    return gemm_entry(A, B, C, M, N, K, lda, ldb, ldc, TILE_GEMM_IN_BF16, out_dtype, stream, force_path, 0u);
 }
 
 int tile_gemm_static_b(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_t K, int64_t lda,
                        int64_t ldb, int64_t ldc, int out_dtype, void* stream) {
-    return gemm_entry(A, B, C, M, N, K, lda, ldb, ldc, out_dtype, stream, TILE_GEMM_PATH_AUTO,
+    return gemm_entry(A, B, C, M, N, K, lda, ldb, ldc, TILE_GEMM_IN_BF16, out_dtype, stream, TILE_GEMM_PATH_AUTO,
                       TILE_GEMM_FLAG_B_IMMUTABLE);
 }
 
@@ -678,10 +689,54 @@ int tile_gemm(const void* A, const void* B, void* C, int64_t M, int64_t N, int64
     return tile_gemm_ex(A, B, C, M, N, K, lda, ldb, ldc, out_dtype, stream, TILE_GEMM_PATH_AUTO);
 }
 
+int tile_gemm_typed(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_t K, int64_t lda, int64_t ldb,
+                    int64_t ldc, int in_dtype, int out_dtype, void* stream) {
+    return gemm_entry(A, B, C, M, N, K, lda, ldb, ldc, in_dtype, out_dtype, stream, TILE_GEMM_PATH_AUTO, 0u);
+}
+
+int tile_add_f32(const float* x, const float* y, float* z, int64_t n, void* stream) {
+    if (n < 0) return fail(TILE_GEMM_E_EXTENT, "negative extent: n=%lld", (long long)n);
+    if (n == 0) return TILE_GEMM_OK;
+    if (n > (int64_t(1) << 40)) return fail(TILE_GEMM_E_OVERFLOW, "n=%lld above 2^40 elements", (long long)n);
+    if (!x || !y || !z) return fail(TILE_GEMM_E_NULL, "x (%p), y (%p) or z (%p) is NULL but n > 0", x, y, z);
+    if (((uintptr_t)x | (uintptr_t)y | (uintptr_t)z) & 3)
+        return fail(TILE_GEMM_E_ALIGN, "x (%p), y (%p) or z (%p) is not 4-byte aligned", x, y, z);
+    if (overlaps(z, n * 4, x, n * 4) || overlaps(z, n * 4, y, n * 4))
+        return fail(TILE_GEMM_E_ALIAS, "z [%p,+%lld) overlaps x (%p) or y (%p): the output must be exclusively owned",
+                    z, (long long)(n * 4), x, y);
+    int dev = 0, sms = 0;
+    int rc = current_device(&dev, &sms);
+    if (rc) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    const bool vec = ((((uintptr_t)x | (uintptr_t)y | (uintptr_t)z) & 15) == 0);
+    int per_sm = g_tune[7].load() >> 4, unroll = g_tune[7].load() & 15;
+    if (per_sm <= 0) per_sm = 8;
+    if (unroll != 1 && unroll != 2 && unroll != 4 && unroll != 8) unroll = 4;
+    if (vec) {
+        const int64_t tiles = ((n >> 2) + tg::ADD_THREADS * unroll - 1) / (tg::ADD_THREADS * unroll);
+        int64_t grid = (int64_t)sms * per_sm;
+        if (grid > tiles) grid = tiles;
+        if (grid < 1) grid = 1;
+        switch (unroll) {
+            case 1: tg::add_f32_vec_kernel<1><<<(unsigned)grid, tg::ADD_THREADS, 0, s>>>(x, y, z, n); break;
+            case 2: tg::add_f32_vec_kernel<2><<<(unsigned)grid, tg::ADD_THREADS, 0, s>>>(x, y, z, n); break;
+            case 4: tg::add_f32_vec_kernel<4><<<(unsigned)grid, tg::ADD_THREADS, 0, s>>>(x, y, z, n); break;
+            default: tg::add_f32_vec_kernel<8><<<(unsigned)grid, tg::ADD_THREADS, 0, s>>>(x, y, z, n); break;
+        }
+    } else {
+        int64_t grid = (n + tg::ADD_THREADS - 1) / tg::ADD_THREADS;
+        if (grid > (int64_t)sms * 8) grid = (int64_t)sms * 8;
+        tg::add_f32_scalar_kernel<<<(unsigned)grid, tg::ADD_THREADS, 0, s>>>(x, y, z, n);
+    }
+    CUDA_TRY(cudaGetLastError());
+    g_launches.fetch_add(1);
+    return TILE_GEMM_OK;
+}
+
 int tile_gemm_host(const void* A_host, const void* B_host, void* C_host, int64_t M, int64_t N, int64_t K,
                    int64_t lda, int64_t ldb, int64_t ldc, int out_dtype) {
     Plan plan;
-    int rc = check_and_select(A_host, B_host, C_host, M, N, K, lda, ldb, ldc, out_dtype, &plan);
+    int rc = check_and_select(A_host, B_host, C_host, M, N, K, lda, ldb, ldc, TILE_GEMM_IN_BF16, out_dtype, &plan);
     if (rc) return rc;
     if (plan.path == TILE_GEMM_PATH_NOOP) return TILE_GEMM_OK;
     int dev = 0, sms = 0;
@@ -711,7 +766,7 @@ int tile_gemm_query_config(int64_t M, int64_t N, int64_t K, int out_dtype, int32
     int rc = current_device(&dev, &sms);
     if (rc) return rc;
     GemmLaunch gl;
-    plan_gemm(M, N, K, out_dtype == TILE_GEMM_OUT_BF16, sms, &gl);
+    plan_gemm(M, N, K, TILE_GEMM_IN_BF16, out_dtype, sms, &gl);
     out[0] = tg::GEMM_BM;
     out[1] = gl.cfg.tile_n();
     out[2] = gl.cfg.cg;
@@ -733,9 +788,10 @@ int tile_gemm_debug_owner_map(int32_t* owner, int64_t M, int64_t N, int64_t K, i
     int rc = current_device(&dev, &sms);
     if (rc) return rc;
     GemmLaunch gl;
-    plan_gemm(M, N, K, out_dtype == TILE_GEMM_OUT_BF16, sms, &gl);
+    plan_gemm(M, N, K, TILE_GEMM_IN_BF16, out_dtype, sms, &gl);
     gl.p.num_k_tiles = 0;   // same schedule and epilogue, no loads and no MMAs
-    gl.p.out_bf16 = 0;      // the map itself is written through the 32-bit epilogue
+    gl.p.out_16 = 0;        // the map itself is written through the 32-bit epilogue
+    gl.p.out_f16 = 0;
     gl.p.owner_mode = 1;
     gl.p.C = owner;
     gl.p.ldc = ld_owner;

@@ -64,10 +64,35 @@ def f32_to_bf16_bits(x: np.ndarray) -> np.ndarray:
     return t.view(torch.int16).numpy().view(np.uint16)
 
 
-def bits_to_torch(bits: np.ndarray, device="cpu") -> torch.Tensor:
-    """uint16 bit patterns -> torch.bfloat16 tensor of the same shape."""
-    t = torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).view(torch.bfloat16)
+def bits_to_torch(bits: np.ndarray, device="cpu", dtype=torch.bfloat16) -> torch.Tensor:
+    """uint16 bit patterns -> torch.bfloat16 (or torch.float16) tensor of the same shape."""
+    t = torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).view(dtype)
     return t.to(device)
+
+
+def f32_to_f16_bits(x: np.ndarray) -> np.ndarray:
+    """float32 array -> uint16 IEEE binary16 bit patterns via numpy's RNE cast."""
+    return np.ascontiguousarray(x, dtype=np.float32).astype(np.float16).view(np.uint16)
+
+
+def make_inputs_f16(M, N, K, dist="normal", sigma_a=1.0, sigma_b=1.0, seed=0):
+    """f16 twin of make_inputs_custom (the paper's GEMM sweep is in f16)."""
+    rng = np.random.default_rng([int(seed), 7927])
+    a = f32_to_f16_bits(_draw(rng, (M, K), dist, sigma_a))
+    b = f32_to_f16_bits(_draw(rng, (K, N), dist, sigma_b))
+    return a, b
+
+
+def make_add_inputs(n: int, seed=0):
+    """Element-wise add (Listing 1; the paper fills x and y with ones and measures at n = 2^28):
+    seeded N(0,1) float32 vectors with every 16th element scaled by 2^+-20, so that sums round,
+    cancel and absorb."""
+    rng = np.random.default_rng([int(seed), 7933])
+    x = rng.standard_normal(n, dtype=np.float32)
+    y = rng.standard_normal(n, dtype=np.float32)
+    x[::16] *= np.float32(2.0 ** 20)
+    y[8::16] *= np.float32(2.0 ** -20)
+    return x, y
 
 
 def torch_to_bits(t: torch.Tensor) -> np.ndarray:

@@ -25,7 +25,7 @@ CANARY_BF16 = 0x7FD5
 @pytest.fixture(autouse=True)
 def _reset_tuning():
     yield
-    for key in range(7):
+    for key in range(8):
         tg.tile_gemm_set_tuning(key, 0)
     torch.cuda.synchronize()
 

@@ -1,0 +1,223 @@
+"""Parity of the SURVEY.md 8(f) rows (through the C ABI) against the oracle, on a B200:
+element-wise add (Listing 1; bit-exact, the paper fixes f32) and the GEMM with
+f16 inputs / f16 output (the paper's sweep is in f16; same gates as bf16)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2606_15991_b200 import binding as tg
+from paper_2606_15991_b200 import workloads as wl
+from parity import check_bit_exact, check_close, freivalds_rows
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+CANARY = 0x7FC0DEAD
+
+
+@pytest.fixture(autouse=True)
+def _reset_tuning():
+    yield
+    for key in range(8):
+        tg.tile_gemm_set_tuning(key, 0)
+    torch.cuda.synchronize()
+
+
+# ------------------------------------------------------------------ element-wise add
+def run_add(x, y, offset=(0, 0, 0)):
+    """x, y: host float32.  Buffers sit `offset` elements past a 256-byte aligned base, z between
+    canary guards.  Returns z (host) after checking the guards."""
+    n = x.size
+    G = 64
+
+    def dev(v, off):
+        buf = torch.zeros(n + off + 8, dtype=torch.float32, device=DEV)
+        view = buf[off:off + n]
+        view.copy_(torch.from_numpy(v))
+        return view
+
+    xd, yd = dev(x, offset[0]), dev(y, offset[1])
+    zraw = torch.empty(n + 2 * G + offset[2] + 8, dtype=torch.int32, device=DEV)
+    zraw.fill_(np.int32(CANARY))
+    zd = zraw[G + offset[2]:G + offset[2] + n].view(torch.float32)
+    tg.tile_add_f32(xd, yd, zd)
+    torch.cuda.synchronize()
+    bits = zraw.cpu().numpy().view(np.uint32)
+    lo = G + offset[2]
+    assert np.all(bits[:lo] == CANARY) and np.all(bits[lo + n:] == CANARY), "written outside z[0:n)"
+    return bits[lo:lo + n].view(np.float32).copy()
+
+
+def test_add_paper_example():
+    x = np.ones(1024, np.float32)
+    z = run_add(x, x.copy())
+    assert np.all(z == 2.0)
+
+
+@pytest.mark.parametrize("n", [1, 3, 4, 5, 1023, 1024, 4095, 4096, 4097, 100_003, 148 * 8 * 4096 + 4099, 1 << 22])
+@pytest.mark.parametrize("shape", [0, 8 * 16 + 1, 4 * 16 + 8, 16 * 16 + 2])
+def test_add_bit_exact_ragged_sizes(n, shape):
+    tg.tile_gemm_set_tuning(tg.TUNE_ADD_SHAPE, shape)
+    x, y = wl.make_add_inputs(n, seed=n)
+    z = run_add(x, y)
+    ref = oracle.add_f32(x, y)
+    assert np.array_equal(z.view(np.uint32), ref.view(np.uint32))
+
+
+@pytest.mark.parametrize("offset", [(1, 0, 0), (0, 2, 0), (0, 0, 3), (1, 1, 1), (4, 4, 4)])
+def test_add_unaligned_buffers(offset):
+    n = 70_001
+    x, y = wl.make_add_inputs(n, seed=11)
+    z = run_add(x, y, offset)
+    assert np.array_equal(z.view(np.uint32), oracle.add_f32(x, y).view(np.uint32))
+
+
+def test_add_ieee_cases_and_specials():
+    vals = np.array([1.0, 2.0 ** -24, 1.5 * 2.0 ** -23, 3.0, -3.0, 3.4028235e38, 2.0 ** 103, 1e-45, -1e-45,
+                     2.0 ** -126, 0.0, -0.0], np.float32)
+    x = np.repeat(vals, vals.size)
+    y = np.tile(vals, vals.size)
+    z = run_add(x, y)
+    ref = oracle.add_f32(x, y)
+    assert np.array_equal(z.view(np.uint32), ref.view(np.uint32))
+
+
+def test_add_full_size_sampled():
+    """n = 2^28, device-generated; the oracle checks 2^20 strided elements and a
+    checksum identity covers the rest: sum(z) over int32-valued inputs is exact."""
+    n = 1 << 28
+    g = torch.Generator(device=DEV)
+    g.manual_seed(28)
+    x = torch.empty(n, dtype=torch.float32, device=DEV).normal_(0, 1, generator=g)
+    y = torch.empty(n, dtype=torch.float32, device=DEV).normal_(0, 1, generator=g)
+    z = tg.tile_add_f32(x, y)
+    idx = torch.arange(0, n, 256, device=DEV) + torch.randint(0, 256, (n // 256,), device=DEV, generator=g)
+    xs, ys, zs = x[idx].cpu().numpy(), y[idx].cpu().numpy(), z[idx].cpu().numpy()
+    assert np.array_equal(zs.view(np.uint32), oracle.add_f32(xs, ys).view(np.uint32))
+    # small integers: every element and every partial sum exact, so sum(z) = sum(x) + sum(y) holds exactly
+    xi = torch.randint(-8, 9, (n,), device=DEV, generator=g).float()
+    yi = torch.randint(-8, 9, (n,), device=DEV, generator=g).float()
+    zi = tg.tile_add_f32(xi, yi)
+    assert int(zi.double().sum().item()) == int(xi.double().sum().item()) + int(yi.double().sum().item())
+    assert float(zi.abs().max().item()) <= 16.0
+
+
+def test_add_preconditions():
+    x = torch.zeros(64, dtype=torch.float32, device=DEV)
+    z = torch.full((64,), 7.0, dtype=torch.float32, device=DEV)
+    p, q = x.data_ptr(), z.data_ptr()
+    assert tg.tile_add_f32_raw(p, p, q, -1) == tg.E_EXTENT
+    assert tg.tile_add_f32_raw(p, 0, q, 8) == tg.E_NULL
+    assert tg.tile_add_f32_raw(p + 2, p, q, 8) == tg.E_ALIGN
+    assert tg.tile_add_f32_raw(p, p, p + 16, 8) == tg.E_ALIAS
+    assert tg.tile_add_f32_raw(p, p, q, 0) == tg.E_OK
+    assert tg.tile_add_f32_raw(p, p, q, 8) == tg.E_OK          # x and y may be the same buffer (shared reads)
+    torch.cuda.synchronize()
+    assert torch.all(z[:8] == 0) and torch.all(z[8:] == 7.0)
+
+
+# ------------------------------------------------------------------ f16 GEMM
+def run_f16(a_bits, b_bits, out, in_f16=True, pad=0):
+    M, K = a_bits.shape
+    N = b_bits.shape[1]
+    dt = torch.float16 if in_f16 else torch.bfloat16
+    A = torch.zeros((M, K + pad), dtype=dt, device=DEV)[:, :K]
+    B = torch.zeros((K, N + pad), dtype=dt, device=DEV)[:, :N]
+    A.copy_(wl.bits_to_torch(a_bits, DEV, dt))
+    B.copy_(wl.bits_to_torch(b_bits, DEV, dt))
+    odt = {"f32": torch.float32, "bf16": torch.bfloat16, "f16": torch.float16}[out]
+    Cfull = torch.full((M + 2, N + pad + 8), float("nan"), dtype=odt, device=DEV)
+    C = Cfull[1:M + 1, :N]
+    tg.tile_gemm(A, B, C)
+    torch.cuda.synchronize()
+    host = Cfull.cpu()
+    assert torch.isnan(host[0]).all() and torch.isnan(host[-1]).all() and torch.isnan(host[:, N:]).all(), \
+        "written outside C"
+    c = host[1:M + 1, :N].contiguous()
+    if out == "f32":
+        return c.numpy().astype(np.float64)
+    if out == "f16":
+        return oracle.f16_decode(c.view(torch.int16).numpy().view(np.uint16))
+    return oracle.bf16_decode(c.view(torch.int16).numpy().view(np.uint16))
+
+
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3, 4])
+def test_f16_integer_inputs_bit_exact(cfg):
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMM_CONFIG, cfg)
+    a, b = wl.make_inputs_f16(1023, 1537, 769, dist="int4", seed=21)
+    ref, _ = oracle.gemm(a, b, in_dtype=oracle.IN_F16)
+    got = run_f16(a, b, "f32")
+    check_bit_exact(got.astype(np.float32), ref, f"f16 ints cfg{cfg}")
+
+
+def test_f16_bits_are_not_read_as_bf16():
+    # 0x3C00 is 1.0 in f16 and 2^-7 in bf16; all-ones f16 inputs give C = K exactly
+    K = 2049
+    a = np.full((130, K), 0x3C00, np.uint16)
+    b = np.full((K, 70), 0x3C00, np.uint16)
+    assert np.all(run_f16(a, b, "f32") == K)
+    # binary16 spacing in [2048, 4096) is 2: 2049 is the tie between 2048 and 2050 -> even -> 2048
+    assert np.all(run_f16(a, b, "f16") == 2048)
+
+
+@pytest.mark.parametrize("out", ["f32", "f16", "bf16"])
+@pytest.mark.parametrize("pad", [0, 8, 3])
+def test_f16_ragged_full_oracle(out, pad):
+    a, b = wl.make_inputs_f16(1023, 1537, 769, seed=22)
+    b[5::97] = wl.f32_to_f16_bits(np.full(b[5::97].shape, 3e-6, np.float32))     # subnormal f16 inputs
+    ref, S = oracle.gemm(a, b, in_dtype=oracle.IN_F16)
+    got = run_f16(a, b, out, pad=pad)
+    check_close(got, ref, S, 769, out, f"f16 ragged out={out} pad={pad}")
+
+
+def test_bf16_inputs_with_f16_output():
+    a, b = wl.make_inputs_custom(300, 520, 1000, sigma_b=1000 ** -0.5, seed=23)
+    ref, S = oracle.gemm(a, b)
+    got = run_f16(a, b, "f16", in_f16=False)
+    check_close(got, ref, S, 1000, "f16", "bf16 in, f16 out")
+
+
+def test_f16_output_is_rne_of_the_fp32_result():
+    a, b = wl.make_inputs_f16(512, 768, 2048, sigma_b=2048 ** -0.5, seed=24)
+    b[:, ::5] = wl.f32_to_f16_bits(np.float32(1e-3) * wl.bits_to_torch(b[:, ::5], dtype=torch.float16).float().numpy())
+    c32 = run_f16(a, b, "f32").astype(np.float32)
+    dt = torch.float16
+    A, B = wl.bits_to_torch(a, DEV, dt), wl.bits_to_torch(b, DEV, dt)
+    C16 = tg.tile_gemm(A, B, out_dtype=tg.OUT_F16)
+    got = C16.cpu().view(torch.int16).numpy().view(np.uint16)
+    assert np.array_equal(got, oracle.f16_encode(c32))
+
+
+@pytest.mark.parametrize("K,N", [(5120, 10240), (769, 1537), (64, 8)])
+@pytest.mark.parametrize("out", ["f32", "f16"])
+def test_f16_gemv(K, N, out):
+    a, b = wl.make_inputs_f16(1, N, K, sigma_b=0.02, seed=25)
+    ref, S = oracle.gemm(a, b, in_dtype=oracle.IN_F16)
+    got = run_f16(a, b, out)
+    check_close(got, ref, S, K, out, f"f16 gemv K={K} N={N} out={out}")
+    ai, bi = wl.make_inputs_f16(1, N, K, dist="int4", seed=26)
+    refi, _ = oracle.gemm(ai, bi, in_dtype=oracle.IN_F16)
+    check_bit_exact(run_f16(ai, bi, "f32").astype(np.float32), refi, "f16 gemv ints")
+
+
+def test_f16_4096_sampled_and_freivalds():
+    M = N = K = 4096
+    a, b = wl.make_inputs_f16(M, N, K, sigma_b=K ** -0.5, seed=27)
+    dt = torch.float16
+    A, B = wl.bits_to_torch(a, DEV, dt), wl.bits_to_torch(b, DEV, dt)
+    C32 = tg.tile_gemm(A, B, out_dtype=tg.OUT_F32).cpu().numpy()
+    rows, cols = wl.stratified_samples(M, N, 128, seed=27)
+    c, s = oracle.gemm_sampled(a, b, rows, cols, in_dtype=oracle.IN_F16)
+    check_close(C32[rows, cols], c, s, K, "f32", "f16 4096 sampled")
+    freivalds_rows(C32.astype(np.float64), oracle.f16_decode(a), oracle.f16_decode(b), seed=27)
+    C16 = tg.tile_gemm(A, B, out_dtype=tg.OUT_F16).cpu().view(torch.int16).numpy().view(np.uint16)
+    assert np.array_equal(C16, oracle.f16_encode(C32))
+
+
+def test_typed_preconditions():
+    x = torch.zeros((8, 8), dtype=torch.float16, device=DEV)
+    c = torch.full((8, 8), 5.0, dtype=torch.float32, device=DEV)
+    assert tg.tile_gemm_typed_raw(x.data_ptr(), x.data_ptr(), c.data_ptr(), 8, 8, 8, 8, 8, 8, 5, tg.OUT_F32) == tg.E_IN_DTYPE
+    assert tg.tile_gemm_typed_raw(x.data_ptr(), x.data_ptr(), c.data_ptr(), 8, 8, 8, 8, 8, 8, tg.IN_F16, 3) == tg.E_DTYPE
+    torch.cuda.synchronize()
+    assert torch.all(c == 5.0)
