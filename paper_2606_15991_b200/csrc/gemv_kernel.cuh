@@ -210,6 +210,7 @@ gemv_tma_kernel(const __grid_constant__ CUtensorMap tmap_b, const GemvParams p) 
 // weights) the producer fills its ring with weight tiles ahead of that wait, so HBM stays busy
 // across kernel boundaries.
 constexpr int GEMV_FLAG_B_IMMUTABLE = 1;
+constexpr int GEMV_FLAG_X_TMA = 2;   // x is 16-byte aligned: its TILE_K-element slices ride the ring with the weight tiles
 
 struct GemvSplitParams {
     const uint16_t* x;
@@ -243,7 +244,8 @@ template <int COLS, int TILE_K, int STAGES>
 struct GemvSplitSmem {
     static constexpr uint32_t BOX_BYTES = TILE_K * GEMV_COLS * 2;          // one TMA box: TILE_K rows x 256 columns
     static constexpr uint32_t TILE_BYTES = (COLS / GEMV_COLS) * BOX_BYTES;
-    static constexpr uint32_t RED_OFF = STAGES * TILE_BYTES;
+    static constexpr uint32_t X_OFF = STAGES * TILE_BYTES;                 // per stage: TILE_K activations (128 B slots)
+    static constexpr uint32_t RED_OFF = X_OFF + STAGES * 128;
     static constexpr uint32_t FLAG_OFF = RED_OFF + GEMV_CONSUMER_WARPS * COLS * 4;
     static constexpr uint32_t BAR_OFF = FLAG_OFF + 16;
     static constexpr uint32_t TOTAL = BAR_OFF + 2 * STAGES * 8 + 128;   // + slack for 128 B alignment
@@ -253,7 +255,8 @@ struct GemvSplitSmem {
 // contiguous bytes), TILE_K rows per ring stage.
 template <int COLS, int TILE_K, int STAGES, int MIN_CTAS, bool F16>
 __global__ void __launch_bounds__(GEMV_TMA_THREADS, MIN_CTAS)
-gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const GemvSplitParams p) {
+gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_constant__ CUtensorMap tmap_x,
+                  const GemvSplitParams p) {
     using L = GemvSplitSmem<COLS, TILE_K, STAGES>;
     constexpr int NV = COLS / GEMV_COLS;                 // 16-byte vectors per lane per row
     constexpr int RPW = TILE_K / GEMV_CONSUMER_WARPS;   // rows of a tile per consumer warp
@@ -272,8 +275,10 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const GemvSplitPar
     const int S = (int)gridDim.y, slice = (int)blockIdx.y;
     const int KT = p.k_tiles;
 
+    const bool x_tma = (p.flags & GEMV_FLAG_X_TMA) != 0;
     if (threadIdx.x == 0) {
         prefetch_tmap(&tmap_b);
+        if (x_tma) prefetch_tmap(&tmap_x);
         for (uint32_t s = 0; s < STAGES; ++s) {
             mbar_init(full_bar(s), 1);
             mbar_init(empty_bar(s), GEMV_CONSUMER_WARPS);
@@ -284,20 +289,53 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const GemvSplitPar
     griddep_launch_dependents();
 
     if (warp == GEMV_CONSUMER_WARPS) {
-        // ===== producer =====
+        // ===== producer: one (column block, k-tile) unit per ring stage.  With x_tma the unit's
+        //       TILE_K activations land in the same stage on the same barrier, so the consumers
+        //       never wait on a global load of x =====
         if (elect_one()) {
-            if (!(p.flags & GEMV_FLAG_B_IMMUTABLE)) griddep_wait();
-            uint32_t stage = 0, phase = 0;
-            for (int cb = (int)blockIdx.x; cb < p.col_blocks; cb += (int)gridDim.x)
-                for (int kt = slice; kt < KT; kt += S) {
-                    mbar_wait(empty_bar(stage), phase ^ 1u);
-                    mbar_arrive_expect_tx(full_bar(stage), L::TILE_BYTES);   // full boxes, even when clipped
+            const uint32_t tx_bytes = L::TILE_BYTES + (x_tma ? (uint32_t)TILE_K * 2u : 0u);   // full boxes, even when clipped
+            auto issue_b = [&](uint32_t stage, int cb, int kt) {
+                mbar_arrive_expect_tx(full_bar(stage), tx_bytes);
 #pragma unroll
-                    for (int v = 0; v < NV; ++v)
-                        tma_load_2d(smem_base + stage * L::TILE_BYTES + v * L::BOX_BYTES, &tmap_b, full_bar(stage),
-                                    cb * COLS + v * GEMV_COLS, kt * TILE_K);
-                    if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                for (int v = 0; v < NV; ++v)
+                    tma_load_2d(smem_base + stage * L::TILE_BYTES + v * L::BOX_BYTES, &tmap_b, full_bar(stage),
+                                cb * COLS + v * GEMV_COLS, kt * TILE_K);
+            };
+            auto issue_x = [&](uint32_t stage, int kt) {
+                if (x_tma) tma_load_2d(smem_base + L::X_OFF + stage * 128u, &tmap_x, full_bar(stage), kt * TILE_K, 0);
+            };
+            auto next_unit = [&](int& cb, int& kt) {
+                kt += S;
+                if (kt >= KT) { kt = slice; cb += (int)gridDim.x; }
+            };
+            int cb = (int)blockIdx.x, kt = slice;
+            uint32_t stage = 0, phase = 0;
+            const bool have_work = cb < p.col_blocks && kt < KT;
+            if ((p.flags & GEMV_FLAG_B_IMMUTABLE) && have_work) {
+                // weights first: the ring fills while the previous kernel of the stream drains; x (which
+                // that kernel may have written) follows the dependency wait
+                int cb2 = cb, kt2 = kt;
+                uint32_t n_pre = 0;
+                for (; n_pre < (uint32_t)STAGES && cb2 < p.col_blocks; ++n_pre) {
+                    issue_b(n_pre, cb2, kt2);
+                    next_unit(cb2, kt2);
                 }
+                griddep_wait();
+                for (uint32_t i = 0; i < n_pre; ++i) {
+                    issue_x(i, kt);
+                    next_unit(cb, kt);
+                }
+                stage = n_pre % STAGES;
+                phase = n_pre / STAGES;
+            } else {
+                griddep_wait();
+            }
+            for (; cb < p.col_blocks; next_unit(cb, kt)) {
+                mbar_wait(empty_bar(stage), phase ^ 1u);
+                issue_b(stage, cb, kt);
+                issue_x(stage, kt);
+                if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+            }
         }
         __syncwarp();
         return;
@@ -307,9 +345,9 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const GemvSplitPar
     //       256 v + 8 l .. + 7 of every box v =====
     griddep_wait();   // x may be the previous kernel's output; y and the workspace may still be in its use
     const uint32_t tid = threadIdx.x;   // 0..255
-    auto load_x = [&](int kt_) -> float {
+    auto load_x = [&](int kt_) -> float {   // only when x is not TMA-addressable
         const int k = kt_ * TILE_K + (int)warp * RPW + (int)(lane & (RPW - 1));
-        return (kt_ < KT && k < p.K) ? in_bits_to_f32<F16>(__ldg(p.x + k)) : 0.f;
+        return (!x_tma && kt_ < KT && k < p.K) ? in_bits_to_f32<F16>(__ldg(p.x + k)) : 0.f;
     };
     uint32_t stage = 0, phase = 0;
     for (int cb = (int)blockIdx.x; cb < p.col_blocks; cb += (int)gridDim.x) {
@@ -330,11 +368,19 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const GemvSplitPar
 #pragma unroll
                 for (int r = 0; r < RPW; ++r)
                     w[v][r] = *reinterpret_cast<const uint4*>(tile + v * L::BOX_BYTES + r * (GEMV_COLS * 2));
+            float xrow[RPW];
+            if (x_tma) {   // this warp's RPW activations: broadcast reads of the stage's x slot
+                const uint16_t* xs = reinterpret_cast<const uint16_t*>(smem_gen + L::X_OFF + stage * 128u) + warp * RPW;
+#pragma unroll
+                for (int r = 0; r < RPW; ++r) xrow[r] = in_bits_to_f32<F16>(xs[r]);
+            } else {
+#pragma unroll
+                for (int r = 0; r < RPW; ++r) xrow[r] = __shfl_sync(0xffffffffu, xv, r);
+            }
 #pragma unroll
             for (int r = 0; r < RPW; ++r) {
-                const float xr = __shfl_sync(0xffffffffu, xv, r);
 #pragma unroll
-                for (int v = 0; v < NV; ++v) fma8<F16>(acc[v], w[v][r], xr);
+                for (int v = 0; v < NV; ++v) fma8<F16>(acc[v], w[v][r], xrow[r]);
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(empty_bar(stage));

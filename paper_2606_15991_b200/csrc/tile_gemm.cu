@@ -471,6 +471,13 @@ int launch_gemv_split(const void* B, int64_t N, int64_t K, int64_t ldb, tg::Gemv
     int rc = get_tensor_map(&tb, B, 2, false, (uint64_t)N, (uint64_t)K, (uint64_t)ldb * 2, (uint32_t)tg::GEMV_COLS,
                             (uint32_t)TILE_K, 0);
     if (rc) return rc;
+    // x as a [1][K] tensor with a TILE_K-element box: zero fill past K, like the weight rows
+    CUtensorMap tx = tb;
+    if (p.flags & tg::GEMV_FLAG_X_TMA) {
+        rc = get_tensor_map(&tx, p.x, 2, false, (uint64_t)K, 1, ((uint64_t)K * 2 + 15) & ~(uint64_t)15,
+                            (uint32_t)TILE_K, 1u, 0);
+        if (rc) return rc;
+    }
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof cfg);
     cfg.gridDim = dim3((unsigned)gx, (unsigned)split, 1);
@@ -482,7 +489,7 @@ int launch_gemv_split(const void* B, int64_t N, int64_t K, int64_t ldb, tg::Gemv
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = pdl ? 1 : 0;
-    CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, tb, p));
+    CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, tb, tx, p));
     g_launches.fetch_add(1);
     return TILE_GEMM_OK;
 }
@@ -521,6 +528,7 @@ int run_gemv_split(const void* x, const void* B, void* y, int64_t N, int64_t K, 
     p.col_blocks = (int32_t)col_blocks;
     p.out_kind = out_dtype;
     p.flags = (flags & TILE_GEMM_FLAG_B_IMMUTABLE) ? tg::GEMV_FLAG_B_IMMUTABLE : 0;
+    if ((((uintptr_t)x) & 15) == 0 && (g_tune[6].load() & 2) == 0) p.flags |= tg::GEMV_FLAG_X_TMA;
     p.partials = nullptr;
     p.tickets = nullptr;
     if (split > 1) {
@@ -694,6 +702,9 @@ int tile_gemm_typed(const void* A, const void* B, void* C, int64_t M, int64_t N,
     return gemm_entry(A, B, C, M, N, K, lda, ldb, ldc, in_dtype, out_dtype, stream, TILE_GEMM_PATH_AUTO, 0u);
 }
 
+// tile_add_f32 launch shape (measured on B200 at n = 2^28)
+constexpr int kAddDefaultPerSm = 255, kAddDefaultUnroll = 1, kAddDefaultMode = 1;
+
 int tile_add_f32(const float* x, const float* y, float* z, int64_t n, void* stream) {
     if (n < 0) return fail(TILE_GEMM_E_EXTENT, "negative extent: n=%lld", (long long)n);
     if (n == 0) return TILE_GEMM_OK;
@@ -708,21 +719,40 @@ int tile_add_f32(const float* x, const float* y, float* z, int64_t n, void* stre
     int rc = current_device(&dev, &sms);
     if (rc) return rc;
     cudaStream_t s = (cudaStream_t)stream;
-    const bool vec = ((((uintptr_t)x | (uintptr_t)y | (uintptr_t)z) & 15) == 0);
-    int per_sm = g_tune[7].load() >> 4, unroll = g_tune[7].load() & 15;
-    if (per_sm <= 0) per_sm = 8;
-    if (unroll != 1 && unroll != 2 && unroll != 4 && unroll != 8) unroll = 4;
+    const uintptr_t all = (uintptr_t)x | (uintptr_t)y | (uintptr_t)z;
+    const bool vec = (all & 15) == 0;
+    // tuning key 7: bits 0-3 vectors per thread, bits 4-11 CTAs per SM (255 = one tile per CTA),
+    // bits 12-15 mode (0 auto, 1 = 128-bit + hints, 2 = 128-bit plain, 3 = 256-bit + hints, 4 = 256-bit plain)
+    const int tune = g_tune[7].load();
+    int unroll = tune & 15, per_sm = (tune >> 4) & 255, mode = (tune >> 12) & 15;
+    if (per_sm <= 0) per_sm = kAddDefaultPerSm;
+    if (unroll != 1 && unroll != 2 && unroll != 4 && unroll != 8) unroll = kAddDefaultUnroll;
+    if (mode < 1 || mode > 4) mode = kAddDefaultMode;
+    if ((mode == 3 || mode == 4) && (all & 31)) mode -= 2;   // 256-bit accesses need 32-byte alignment
     if (vec) {
-        const int64_t tiles = ((n >> 2) + tg::ADD_THREADS * unroll - 1) / (tg::ADD_THREADS * unroll);
-        int64_t grid = (int64_t)sms * per_sm;
+        const int vw = mode >= 3 ? 8 : 4;
+        const int64_t tile = (int64_t)tg::ADD_THREADS * unroll * vw;
+        const int64_t tiles = (n + tile - 1) / tile;
+        int64_t grid = per_sm == 255 ? tiles : (int64_t)sms * per_sm;
         if (grid > tiles) grid = tiles;
+        if (grid > 0x7fffffff) grid = 0x7fffffff;
         if (grid < 1) grid = 1;
+#define TG_ADD_CASE(U, VW, H) tg::add_f32_vec_kernel<U, VW, H><<<(unsigned)grid, tg::ADD_THREADS, 0, s>>>(x, y, z, n)
+#define TG_ADD_MODE(U)                                      \
+    switch (mode) {                                         \
+        case 1: TG_ADD_CASE(U, 4, true); break;             \
+        case 2: TG_ADD_CASE(U, 4, false); break;            \
+        case 3: TG_ADD_CASE(U, 8, true); break;             \
+        default: TG_ADD_CASE(U, 8, false); break;           \
+    }
         switch (unroll) {
-            case 1: tg::add_f32_vec_kernel<1><<<(unsigned)grid, tg::ADD_THREADS, 0, s>>>(x, y, z, n); break;
-            case 2: tg::add_f32_vec_kernel<2><<<(unsigned)grid, tg::ADD_THREADS, 0, s>>>(x, y, z, n); break;
-            case 4: tg::add_f32_vec_kernel<4><<<(unsigned)grid, tg::ADD_THREADS, 0, s>>>(x, y, z, n); break;
-            default: tg::add_f32_vec_kernel<8><<<(unsigned)grid, tg::ADD_THREADS, 0, s>>>(x, y, z, n); break;
+            case 1: TG_ADD_MODE(1) break;
+            case 2: TG_ADD_MODE(2) break;
+            case 4: TG_ADD_MODE(4) break;
+            default: TG_ADD_MODE(8) break;
         }
+#undef TG_ADD_MODE
+#undef TG_ADD_CASE
     } else {
         int64_t grid = (n + tg::ADD_THREADS - 1) / tg::ADD_THREADS;
         if (grid > (int64_t)sms * 8) grid = (int64_t)sms * 8;
