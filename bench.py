@@ -317,6 +317,74 @@ def bench_decode(tg, wl, torch, passes, warmup, layers, tdist, static_b=True):
     return ms, alg_bytes, launches, per_shape, graph_ms, len(items), plain_ms
 
 
+def bench_add(tg, torch, n, steps, warmup, tdist):
+    """z = x + y over f32 at n = 2^28 (Listing 1).  12 B of HBM traffic per
+    element; the three 1 GiB vectors are far larger than L2."""
+    dev = torch.device("cuda", torch.cuda.current_device())
+    g = torch.Generator(device=dev)
+    g.manual_seed(28)
+    x = torch.empty(n, dtype=torch.float32, device=dev).normal_(0, 1, generator=g)
+    y = torch.empty(n, dtype=torch.float32, device=dev).normal_(0, 1, generator=g)
+    z = torch.empty(n, dtype=torch.float32, device=dev)
+    for _ in range(warmup):
+        tg.tile_add_f32(x, y, z)
+    ms = time_region(lambda i: tg.tile_add_f32(x, y, z), steps, torch.cuda.synchronize, tdist.barrier)
+    return tdist.max_over_ranks(ms) / steps
+
+
+def bench_sweep(tg, torch, sizes, tdist):
+    """the paper's Figure 6b sweep, M=N=K powers of two, f16 (the
+    paper's precision) and bf16, 16-bit output.  Per size: median of `reps` single-launch timings
+    (paper: medians) on rotating operand sets whose total exceeds L2 where the problem allows."""
+    dev = torch.device("cuda", torch.cuda.current_device())
+    out = {}
+    for dt_name, dt in (("f16", torch.float16), ("bf16", torch.bfloat16)):
+        rows = {}
+        for n in sizes:
+            per_set = 3 * n * n * 2
+            sets = int(max(1, min(8, (256 << 20) // per_set + 1)))
+            reps = 40 if n <= 4096 else (12 if n <= 16384 else 5)
+            g = torch.Generator(device=dev)
+            g.manual_seed(600 + n)
+            bufs = [(torch.empty((n, n), dtype=dt, device=dev).normal_(0, 1, generator=g),
+                     torch.empty((n, n), dtype=dt, device=dev).normal_(0, n ** -0.5, generator=g),
+                     torch.empty((n, n), dtype=dt, device=dev)) for _ in range(sets)]
+            for i in range(3):
+                A, B, C = bufs[i % sets]
+                tg.tile_gemm(A, B, C)
+            torch.cuda.synchronize()
+            ts = []
+            for i in range(reps):
+                A, B, C = bufs[i % sets]
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                tg.tile_gemm(A, B, C)
+                e1.record()
+                e1.synchronize()
+                ts.append(e0.elapsed_time(e1))
+            # back-to-back (launch latency hidden by the queue): what a pipeline of GEMMs sees
+            tdist.barrier()
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for i in range(reps):
+                A, B, C = bufs[i % sets]
+                tg.tile_gemm(A, B, C)
+            e1.record()
+            torch.cuda.synchronize()
+            b2b = e0.elapsed_time(e1) / reps
+            med = float(np.median(ts))
+            fl = 2.0 * n ** 3
+            rows[str(n)] = {"us_median": med * 1e3, "tflops_median": fl / (med * 1e-3) / 1e12,
+                            "us_back_to_back": b2b * 1e3, "tflops_back_to_back": fl / (b2b * 1e-3) / 1e12,
+                            "tile_config": tg.tile_gemm_query_config(n, n, n, tg.OUT_BF16)["config"],
+                            "operand_sets": sets}
+            del bufs
+            torch.cuda.empty_cache()
+        out[dt_name] = rows
+    return out
+
+
 def run_cuda(args):
     import torch
     from paper_2606_15991_b200 import binding as tg
@@ -398,6 +466,22 @@ def run_cuda(args):
                          "peak_source": f"{peaks['source']} copy bandwidth (MEASURED_PEAKS.json)",
                          "frac_of_8000": gbs / 8000.0, "kernel": "gemv_split_kernel<256,64,3,2>"},
         }
+        # element-wise add (Listing 1) at n = 2^28
+        n_add = 1 << 28
+        ms = bench_add(tg, torch, n_add, max(10, args.steps // 4), 3, tdist)
+        gbs = 12.0 * n_add / (ms * 1e-3) / 1e9
+        line["add"] = {
+            "metric": "elementwise_add_f32_hbm_gbs", "value": gbs * world, "unit": "GB/s", "n": n_add,
+            "us_per_launch": ms * 1e3, "paper_b200_gbs": 6970.0,
+            "roofline": {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                         "frac": gbs / peaks["hbm_gbs"], "traffic": ncu_traffic("add_2p28_dram_bytes"),
+                         "peak_source": f"{peaks['source']} copy bandwidth (MEASURED_PEAKS.json)",
+                         "frac_of_8000": gbs / 8000.0, "kernel": "add_f32_vec_kernel<1,4,true>",
+                         "algorithmic_bytes_per_launch": 12 * n_add},
+        }
+        # the paper's size sweep in f16 and bf16
+        if not args.no_sweep:
+            line["sweep"] = bench_sweep(tg, torch, [1024, 2048, 4096, 8192, 16384, 32768], tdist)
     if rank == 0:
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = cpu_baseline_leg()
@@ -417,6 +501,7 @@ def main():
     ap.add_argument("--decode-layers", type=int, default=64)
     ap.add_argument("--headline-only", action="store_true", help="skip the prefill and decode legs")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the f16/bf16 size sweep (SURVEY 8(f)1)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--gemm-config", type=int, default=0, help="force a GEMM tile config (tile_gemm_set_tuning key 0)")
     ap.add_argument("--group-m", type=int, default=0, help="force the raster group height (tuning key 1)")

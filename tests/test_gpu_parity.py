@@ -397,7 +397,7 @@ def test_precondition_failures_enqueue_nothing():
     assert tg.tile_gemm_raw(*p, 8, 8, 8, 7, 8, 8, 0) == tg.E_LDA
     assert tg.tile_gemm_raw(*p, 8, 8, 8, 8, 7, 8, 0) == tg.E_LDB
     assert tg.tile_gemm_raw(*p, 8, 8, 8, 8, 8, 7, 0) == tg.E_LDC
-    assert tg.tile_gemm_raw(*p, 8, 8, 8, 8, 8, 8, 2) == tg.E_DTYPE
+    assert tg.tile_gemm_raw(*p, 8, 8, 8, 8, 8, 8, 3) == tg.E_DTYPE   # 2 is TILE_GEMM_OUT_F16 since the 8(f)1 rows
     assert tg.tile_gemm_raw(A.data_ptr(), B.data_ptr(), A.data_ptr(), 8, 8, 8, 8, 8, 8, 1) == tg.E_ALIAS
     assert tg.tile_gemm_raw(0, B.data_ptr(), C.data_ptr(), 8, 8, 8, 8, 8, 8, 0) == tg.E_NULL
     assert tg.tile_gemm_raw(*p, 8, 8, 8, 8, 8, 8, 0, 0, tg.PATH_GEMV) == tg.E_PATH
