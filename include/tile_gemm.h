@@ -203,7 +203,8 @@ int tile_gemm_query_config(int64_t M, int64_t N, int64_t K, int out_dtype, int32
  * split-K with ticketed fix-up), 5 = ring shape of kernel 4 (0 auto; 1..8 =
  * {columns per CTA, rows per stage, stages, CTAs per SM}, table kGemvShapes in
  * csrc/tile_gemm.cu), 6 = bit 0 disables programmatic dependent launch, bit 1 makes
- * kernel 4 read x with global loads instead of through its TMA ring; key 3 also
+ * kernel 4 read x with global loads instead of through its TMA ring; bit 2 forces the GEMM's
+ * lockstep producers on, bit 3 off, bits 8-15 their window in k-tiles (0 = 32); key 3 also
  * overrides kernel 4's split, 7 = tile_add_f32 launch shape
  * (bits 0-3 vectors per thread in {1,2,4,8}, bits 4-11 CTAs per SM with 255 = one tile per
  * CTA, bits 12-15 access mode: 1/2 = 128-bit with/without streaming hints, 3/4 = 256-bit

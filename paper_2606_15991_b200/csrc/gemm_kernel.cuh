@@ -46,7 +46,22 @@ struct GemmParams {
     int32_t owner_mode;         // debug: write (tile << 8 | cta) instead of values
     void* C;
     int64_t ldc;                // elements
+    // lockstep (large problems): the producers of all clusters advance through the schedule in
+    // windows of `sync_window` k-tiles; a producer may run at most one window ahead of the slowest
+    // cluster.  Co-running tiles then read the same k-slices of their shared A/B panels within a
+    // window the L2 holds, instead of drifting apart over a long launch.  sync == nullptr: off.
+    uint32_t* sync;             // [windows] arrival counters, zero at launch
+    int32_t sync_window;
 };
+
+__device__ __forceinline__ uint32_t ld_relaxed_gpu_u32(const uint32_t* p) {
+    uint32_t v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void red_add_relaxed_gpu_u32(uint32_t* p, uint32_t v) {
+    asm volatile("red.relaxed.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
 
 // Tile index -> tile coordinates.  Grouped raster: tiles are numbered down the rows of a
 // group of `group_m` tile rows, then across columns, so that concurrently running tiles share
@@ -140,12 +155,29 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
         // ===== TMA producer (one lane) =====
         if (elect_one()) {
             uint32_t stage = 0, phase = 0;
+            // lockstep bookkeeping (leader CTA of each cluster only; its partner is held back by the
+            // shared pipeline): `pos` counts the k-tiles this cluster has issued over all its tiles
+            const bool lockstep = p.sync != nullptr && rank == 0;
+            const int tiles_max = (total_tiles + tile_stride - 1) / tile_stride;           // tiles of the busiest cluster
+            const int clusters_full = total_tiles - (tiles_max - 1) * tile_stride;         // clusters that own tiles_max tiles
+            uint32_t pos = 0, next_sync = 0;
             for (int t = first_tile; t < total_tiles; t += tile_stride) {
                 int tm, tn;
                 tile_coords(t, p.tiles_m, p.tiles_n, p.group_m, tm, tn);
                 const int m0 = (tm * CG + (int)rank) * GEMM_BM;
                 const int n0 = tn * TILE_N + (int)rank * (int)L::B_COLS;
-                for (int kt = 0; kt < p.num_k_tiles; ++kt) {
+                for (int kt = 0; kt < p.num_k_tiles; ++kt, ++pos) {
+                    if (lockstep && pos == next_sync) {
+                        const uint32_t w = pos / (uint32_t)p.sync_window;
+                        red_add_relaxed_gpu_u32(p.sync + w, 1u);
+                        if (w >= 1) {   // everyone who owns window w-1 must have entered it
+                            const bool all_own = (uint64_t)(w - 1) * (uint32_t)p.sync_window <
+                                                 (uint64_t)(tiles_max - 1) * (uint32_t)p.num_k_tiles;
+                            const uint32_t expect = all_own ? (uint32_t)tile_stride : (uint32_t)clusters_full;
+                            while (ld_relaxed_gpu_u32(p.sync + (w - 1)) < expect) __nanosleep(64);
+                        }
+                        next_sync += (uint32_t)p.sync_window;
+                    }
                     mbar_wait(empty_bar(stage), phase ^ 1u);
                     const uint32_t sa = smem_base + stage * L::STAGE_BYTES;
                     const uint32_t sb = sa + L::A_BYTES;

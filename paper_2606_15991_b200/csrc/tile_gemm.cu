@@ -268,6 +268,25 @@ int workspace_for(int dev, cudaStream_t s, size_t need, void** out) {
     return TILE_GEMM_OK;
 }
 
+// GEMM lockstep counters per (device, stream), zeroed before each launch that uses them
+std::unordered_map<uint64_t, Buf> g_sync_ws;
+
+int sync_workspace_for(int dev, cudaStream_t s, size_t bytes, uint32_t** out) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    Buf& b = g_sync_ws[((uint64_t)dev << 56) ^ (uint64_t)(uintptr_t)s];
+    if (b.n < bytes) {
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(s, &cs) == cudaSuccess && cs != cudaStreamCaptureStatusNone)
+            return fail(TILE_GEMM_E_CUDA,
+                        "the GEMM lockstep workspace of this stream must grow during stream capture; run the shape "
+                        "once on the stream before capturing");
+        int rc = grow(b, bytes);
+        if (rc) return rc;
+    }
+    *out = (uint32_t*)b.p;
+    return TILE_GEMM_OK;
+}
+
 // GEMV split-K workspace per (device, stream): fp32 partials [col_blocks][split][256] and one ticket per column
 // block (zero between launches: the CTA that draws the last ticket re-arms it).
 struct GemvWs {
@@ -326,6 +345,9 @@ GemmConfig choose_config(int64_t M, int64_t N, int sms) {
     if (t2 * 4 >= (int64_t)sms * 3) return kConfigs[2];
     return kConfigs[1];
 }
+
+// lockstep defaults: on from kLockstepMinTiles tiles per cluster and kLockstepMinKTiles k-tiles
+constexpr int kLockstepMinTiles = 3, kLockstepMinKTiles = 64, kLockstepWindow = 32;
 
 struct GemmLaunch {
     GemmConfig cfg;
@@ -452,6 +474,28 @@ int run_gemm(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_
         if (rc) return rc;
     } else {
         tc = ta;   // never dereferenced by the clipped st.global epilogue; must still be a valid map
+    }
+    // lockstep producers: only where a launch is long enough for clusters to drift (several tiles
+    // per cluster, long K loops); tuning key 6: bit 2 forces it on, bit 3 off, bits 8-15 = window
+    {
+        const int tune = g_tune[6].load();
+        const int clusters = gl.ctas / gl.cfg.cg;
+        const int64_t tiles = (int64_t)gl.p.tiles_m * gl.p.tiles_n;
+        const int64_t tiles_max = (tiles + clusters - 1) / clusters;
+        bool on = tiles_max >= kLockstepMinTiles && gl.p.num_k_tiles >= kLockstepMinKTiles;
+        if (tune & 4) on = tiles_max >= 1 && gl.p.num_k_tiles >= 1;
+        if (tune & 8) on = false;
+        if (on) {
+            int window = (tune >> 8) & 255;
+            if (window <= 0) window = kLockstepWindow;
+            const int64_t windows = (tiles_max * gl.p.num_k_tiles + window - 1) / window + 1;
+            uint32_t* sync = nullptr;
+            rc = sync_workspace_for(dev, s, (size_t)windows * 4, &sync);
+            if (rc) return rc;
+            CUDA_TRY(cudaMemsetAsync(sync, 0, (size_t)windows * 4, s));
+            gl.p.sync = sync;
+            gl.p.sync_window = window;
+        }
     }
     return launch_gemm(gl, ta, tb, tc, s, dev);
 }
@@ -875,6 +919,9 @@ int tile_gemm_shutdown(void) {
     for (auto& kv : g_ws)
         if (kv.second.p) cudaFree(kv.second.p);
     g_ws.clear();
+    for (auto& kv : g_sync_ws)
+        if (kv.second.p) cudaFree(kv.second.p);
+    g_sync_ws.clear();
     for (auto& kv : g_gemv_ws) {
         if (kv.second.partials.p) cudaFree(kv.second.partials.p);
         if (kv.second.tickets.p) cudaFree(kv.second.tickets.p);
