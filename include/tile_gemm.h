@@ -152,6 +152,33 @@ int tile_gemm_typed(const void* A, const void* B, void* C,
 int tile_add_f32(const float* x, const float* y, float* z, int64_t n, void* stream);
 
 /*
+ * Recorded steps (the paper's graph mode, PAPER.md:290, 322-326:
+ * "Graph captures the pipeline and replays all N kernels with one driver call",
+ * and Grout's recorded decode step).  Between record_begin and
+ * record_end every library call on `stream` (tile_gemm*, tile_add_f32) is
+ * recorded instead of executed, in call order; record_end returns an opaque
+ * step that tile_gemm_replay enqueues on any stream of the same device with ONE
+ * driver call.  Recorded nodes keep the operand ADDRESSES: the caller keeps
+ * those buffers alive and at the same place, and may rewrite their contents
+ * between replays ("replayed nodes do not depend on addresses that change across
+ * replays").  Nothing may allocate while recording: run every
+ * shape once on `stream` beforehand so that the library's workspaces exist
+ * (a call that would have to grow one fails with TILE_GEMM_E_CUDA and says so).
+ * The M == 1 kernels keep their programmatic-dependent-launch edges inside the
+ * step.  `stream` must not be NULL (the legacy default stream cannot be
+ * captured).  A failed call while recording leaves the capture open; still call
+ * record_end (it reports the invalidated capture).  tile_gemm_recorded_nodes
+ * returns the number of graph nodes (kernels and workspace memsets) in a step,
+ * -1 for anything that is not a live step; tile_gemm_launch_count grows by that
+ * number per replay.  tile_gemm_record_free destroys a step (NULL is a no-op).
+ */
+int tile_gemm_record_begin(void* stream);
+int tile_gemm_record_end(void* stream, void** step_out);
+int tile_gemm_replay(void* step, void* stream);
+int64_t tile_gemm_recorded_nodes(void* step);
+int tile_gemm_record_free(void* step);
+
+/*
  * Launch preconditions + shape selector as a pure host function (PAPER.md:200:
  * "runs once per launch before any work is queued"; tile shapes
  * chosen per size).  Never dereferences A/B/C and makes no CUDA call.

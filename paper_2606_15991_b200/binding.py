@@ -30,7 +30,8 @@ PATH_NAMES = {PATH_AUTO: "auto", PATH_GEMM_TMA: "gemm_tma", PATH_GEMM_REPACK: "g
 TUNE_GEMM_CONFIG, TUNE_GEMM_GROUP_M, TUNE_GEMM_MAX_CTAS, TUNE_GEMV_SPLIT, TUNE_GEMV_VARIANT, TUNE_GEMV_SHAPE, TUNE_FLAGS, TUNE_ADD_SHAPE = range(8)
 
 EXPORTS = ("tile_gemm", "tile_gemm_ex", "tile_gemm_static_b", "tile_gemm_typed", "tile_add_f32",
-           "tile_gemm_select", "tile_gemm_host",
+           "tile_gemm_record_begin", "tile_gemm_record_end", "tile_gemm_replay", "tile_gemm_recorded_nodes",
+           "tile_gemm_record_free", "tile_gemm_select", "tile_gemm_host",
            "tile_gemm_debug_owner_map", "tile_gemm_query_config", "tile_gemm_set_tuning",
            "tile_gemm_launch_count", "tile_gemm_status_string", "tile_gemm_last_error",
            "tile_gemm_shutdown")
@@ -78,6 +79,16 @@ def load_library():
     lib.tile_gemm_typed.restype = _int
     lib.tile_add_f32.argtypes = [_vp, _vp, _vp, _i64, _vp]
     lib.tile_add_f32.restype = _int
+    lib.tile_gemm_record_begin.argtypes = [_vp]
+    lib.tile_gemm_record_begin.restype = _int
+    lib.tile_gemm_record_end.argtypes = [_vp, ctypes.POINTER(_vp)]
+    lib.tile_gemm_record_end.restype = _int
+    lib.tile_gemm_replay.argtypes = [_vp, _vp]
+    lib.tile_gemm_replay.restype = _int
+    lib.tile_gemm_recorded_nodes.argtypes = [_vp]
+    lib.tile_gemm_recorded_nodes.restype = _i64
+    lib.tile_gemm_record_free.argtypes = [_vp]
+    lib.tile_gemm_record_free.restype = _int
     lib.tile_gemm_select.argtypes = [_i64] * 6 + [_vp, _vp, _vp, _int]
     lib.tile_gemm_select.restype = _int
     lib.tile_gemm_host.argtypes = g
@@ -212,6 +223,35 @@ def tile_add_f32(x: torch.Tensor, y: torch.Tensor, z: torch.Tensor | None = None
     _check(load_library().tile_add_f32(_vp(x.data_ptr()), _vp(y.data_ptr()), _vp(z.data_ptr()), x.numel(),
                                        _vp(_stream_handle(stream))))
     return z
+
+
+class RecordedStep:
+    """A recorded sequence of library calls (tile_gemm_record_begin/_end), replayed with one driver call."""
+
+    def __init__(self, handle: int):
+        self.handle = handle
+
+    @property
+    def nodes(self) -> int:
+        return int(load_library().tile_gemm_recorded_nodes(_vp(self.handle)))
+
+    def replay(self, stream=None) -> None:
+        _check(load_library().tile_gemm_replay(_vp(self.handle), _vp(_stream_handle(stream))))
+
+    def free(self) -> None:
+        if self.handle:
+            _check(load_library().tile_gemm_record_free(_vp(self.handle)))
+            self.handle = 0
+
+
+def tile_gemm_record_begin(stream) -> None:
+    _check(load_library().tile_gemm_record_begin(_vp(_stream_handle(stream))))
+
+
+def tile_gemm_record_end(stream) -> RecordedStep:
+    out = _vp()
+    _check(load_library().tile_gemm_record_end(_vp(_stream_handle(stream)), ctypes.byref(out)))
+    return RecordedStep(int(out.value))
 
 
 def tile_gemm_host(A_bits, B_bits, C_out, lda=None, ldb=None, ldc=None):

@@ -822,6 +822,70 @@ int tile_add_f32(const float* x, const float* y, float* z, int64_t n, void* stre
     return TILE_GEMM_OK;
 }
 
+// ---------------------------------------------------------------- recorded steps
+namespace {
+struct Recorded {
+    uint32_t magic;
+    cudaGraph_t graph;
+    cudaGraphExec_t exec;
+    int64_t nodes;
+};
+constexpr uint32_t kRecordedMagic = 0x7167656d;
+}  // namespace
+
+int tile_gemm_record_begin(void* stream) {
+    int dev = 0, sms = 0;
+    int rc = current_device(&dev, &sms);
+    if (rc) return rc;
+    if (stream == nullptr)
+        return fail(TILE_GEMM_E_PATH, "recording needs an explicit stream: the legacy default stream cannot be captured");
+    CUDA_TRY(cudaStreamBeginCapture((cudaStream_t)stream, cudaStreamCaptureModeThreadLocal));
+    return TILE_GEMM_OK;
+}
+
+int tile_gemm_record_end(void* stream, void** step_out) {
+    if (!step_out) return fail(TILE_GEMM_E_NULL, "step_out is NULL");
+    *step_out = nullptr;
+    cudaGraph_t graph = nullptr;
+    CUDA_TRY(cudaStreamEndCapture((cudaStream_t)stream, &graph));
+    if (!graph) return fail(TILE_GEMM_E_CUDA, "the capture on this stream was invalidated");
+    cudaGraphExec_t exec = nullptr;
+    cudaError_t e = cudaGraphInstantiate(&exec, graph, 0);
+    if (e != cudaSuccess) {
+        cudaGraphDestroy(graph);
+        return fail(TILE_GEMM_E_CUDA, "cudaGraphInstantiate failed: %s (%d)", cudaGetErrorString(e), (int)e);
+    }
+    size_t n = 0;
+    cudaGraphGetNodes(graph, nullptr, &n);
+    Recorded* r = new Recorded{kRecordedMagic, graph, exec, (int64_t)n};
+    *step_out = r;
+    return TILE_GEMM_OK;
+}
+
+int tile_gemm_replay(void* step, void* stream) {
+    Recorded* r = (Recorded*)step;
+    if (!r || r->magic != kRecordedMagic) return fail(TILE_GEMM_E_NULL, "not a recorded step: %p", step);
+    CUDA_TRY(cudaGraphLaunch(r->exec, (cudaStream_t)stream));
+    g_launches.fetch_add(r->nodes);
+    return TILE_GEMM_OK;
+}
+
+int64_t tile_gemm_recorded_nodes(void* step) {
+    Recorded* r = (Recorded*)step;
+    return (r && r->magic == kRecordedMagic) ? r->nodes : -1;
+}
+
+int tile_gemm_record_free(void* step) {
+    Recorded* r = (Recorded*)step;
+    if (!r) return TILE_GEMM_OK;
+    if (r->magic != kRecordedMagic) return fail(TILE_GEMM_E_NULL, "not a recorded step: %p", step);
+    cudaGraphExecDestroy(r->exec);
+    cudaGraphDestroy(r->graph);
+    r->magic = 0;
+    delete r;
+    return TILE_GEMM_OK;
+}
+
 int tile_gemm_host(const void* A_host, const void* B_host, void* C_host, int64_t M, int64_t N, int64_t K,
                    int64_t lda, int64_t ldb, int64_t ldc, int out_dtype) {
     Plan plan;

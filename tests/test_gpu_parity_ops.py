@@ -221,3 +221,77 @@ def test_typed_preconditions():
     assert tg.tile_gemm_typed_raw(x.data_ptr(), x.data_ptr(), c.data_ptr(), 8, 8, 8, 8, 8, 8, tg.IN_F16, 3) == tg.E_DTYPE
     torch.cuda.synchronize()
     assert torch.all(c == 5.0)
+
+
+# ------------------------------------------------------------------ recorded steps
+def test_recorded_step_replays_bit_identically_and_follows_new_inputs():
+    """A decode-like chain (4 GEMVs on the Qwen3 shapes scaled down, a GEMM and an add) recorded once
+    and replayed: same bits as the direct calls, and a replay after rewriting the inputs in place
+    matches the oracle on the new data (nodes keep addresses, not contents)."""
+    s = torch.cuda.Stream()
+    shapes = [(640, 1280), (640, 1024), (640, 6400), (3200, 640)]
+    xs = [torch.empty((1, K), dtype=torch.bfloat16, device=DEV) for K, N in shapes]
+    Ws = [torch.empty((K, N), dtype=torch.bfloat16, device=DEV) for K, N in shapes]
+    ys = [torch.empty((1, N), dtype=torch.float32, device=DEV) for K, N in shapes]
+    A = torch.empty((300, 640), dtype=torch.bfloat16, device=DEV)
+    C = torch.empty((300, 1280), dtype=torch.float32, device=DEV)
+    u = torch.empty(5000, dtype=torch.float32, device=DEV)
+    v = torch.empty(5000, dtype=torch.float32, device=DEV)
+    w = torch.empty(5000, dtype=torch.float32, device=DEV)
+
+    def fill(seed):
+        host = []
+        for i, (K, N) in enumerate(shapes):
+            a, b = wl.make_inputs_custom(1, N, K, sigma_b=0.05, seed=seed * 10 + i)
+            xs[i].copy_(wl.bits_to_torch(a, DEV))
+            Ws[i].copy_(wl.bits_to_torch(b, DEV))
+            host.append((a, b))
+        a, _ = wl.make_inputs_custom(300, 8, 640, seed=seed * 10 + 9)
+        A.copy_(wl.bits_to_torch(a, DEV))
+        hu, hv = wl.make_add_inputs(5000, seed=seed)
+        u.copy_(torch.from_numpy(hu))
+        v.copy_(torch.from_numpy(hv))
+        return host, a, hu, hv
+
+    def chain(stream):
+        for i in range(4):
+            tg.tile_gemm(xs[i], Ws[i], ys[i], stream=stream, static_b=True)
+        tg.tile_gemm(A, Ws[0], C, stream=stream)
+        tg.tile_add_f32(u, v, w, stream=stream)
+
+    fill(1)
+    chain(s)                                    # warm-up on the stream: workspaces exist before recording
+    s.synchronize()
+    direct = [y.clone() for y in ys] + [C.clone(), w.clone()]
+    before = tg.tile_gemm_launch_count()
+    tg.tile_gemm_record_begin(s)
+    chain(s)
+    step = tg.tile_gemm_record_end(s)
+    s.synchronize()
+    assert tg.tile_gemm_launch_count() - before == 6, "recording counts the recorded kernels once"
+    assert step.nodes >= 6
+    for t in ys + [C, w]:
+        t.fill_(float("nan"))                   # recording executed nothing
+    step.replay(s)
+    s.synchronize()
+    for got, want in zip(ys + [C, w], direct):
+        assert torch.equal(got, want)
+    host, a_host, hu, hv = fill(2)              # new contents, same addresses
+    step.replay(s)
+    step.replay(s)
+    s.synchronize()
+    for i, (K, N) in enumerate(shapes):
+        ref, S = oracle.gemm(*host[i])
+        check_close(ys[i].cpu().numpy().astype(np.float64), ref, S, K, "f32", f"replayed gemv {i}")
+    ref, S = oracle.gemm(a_host, host[0][1])
+    check_close(C.cpu().numpy().astype(np.float64), ref, S, 640, "f32", "replayed gemm")
+    assert np.array_equal(w.cpu().numpy().view(np.uint32), oracle.add_f32(hu, hv).view(np.uint32))
+    step.free()
+    assert step.nodes == -1
+
+
+def test_record_preconditions():
+    lib = tg.load_library()
+    assert lib.tile_gemm_record_begin(None) == tg.E_PATH
+    assert lib.tile_gemm_replay(None, None) == tg.E_NULL
+    assert lib.tile_gemm_record_free(None) == tg.E_OK
