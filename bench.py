@@ -291,29 +291,31 @@ def bench_decode(tg, wl, torch, passes, warmup, layers, tdist, static_b=True):
         torch.cuda.synchronize()
         t = e0.elapsed_time(e1) / len(sel)
         per_shape[f"K{K}_N{N}"] = {"us": t * 1e3, "gbs": (2 * K * N + 2 * K + 2 * N) / (t * 1e-3) / 1e9}
-    # CUDA-graph replay of the same pass (decode engines replay a recorded step)
+    # replay of the same pass as one recorded step of the library's own C ABI (tile_gemm_record_*:
+    # decode engines replay a recorded step)
     graph_ms = None
     try:
-        graph = torch.cuda.CUDAGraph()
         s = torch.cuda.Stream()
-        with torch.cuda.stream(s):
-            one_pass(0)
-            s.synchronize()
-            with torch.cuda.graph(graph, stream=s):
-                one_pass(0)
-        torch.cuda.synchronize()
-        graph.replay()
-        torch.cuda.synchronize()
+        for x, W, y in items:
+            tg.tile_gemm(x, W, y, static_b=static_b, stream=s)     # workspaces of this stream exist before recording
+        s.synchronize()
+        tg.tile_gemm_record_begin(s)
+        for x, W, y in items:
+            tg.tile_gemm(x, W, y, static_b=static_b, stream=s)
+        step = tg.tile_gemm_record_end(s)
+        step.replay(s)
+        s.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
+        e0.record(s)
         for _ in range(passes):
-            graph.replay()
-        e1.record()
-        torch.cuda.synchronize()
+            step.replay(s)
+        e1.record(s)
+        s.synchronize()
         graph_ms = e0.elapsed_time(e1) / passes
+        step.free()
     except Exception as exc:  # reported, never silently substituted for the headline
         graph_ms = None
-        sys.stderr.write(f"[bench] graph replay variant unavailable: {exc}\n")
+        sys.stderr.write(f"[bench] recorded-step variant unavailable: {exc}\n")
     return ms, alg_bytes, launches, per_shape, graph_ms, len(items), plain_ms
 
 
@@ -332,15 +334,58 @@ def bench_add(tg, torch, n, steps, warmup, tdist):
     return tdist.max_over_ranks(ms) / steps
 
 
+def bench_launch_overhead(tg, torch, n_ops=1000, elems=2048):
+    """PAPER.md:322-326 (Figure 8a): host cost per operation of a pipeline of N tiny element-wise
+    kernels, launched one by one with a single wait at the end ("sync" mode) versus recorded once
+    and replayed with one driver call ("graph" mode; the paper's floor is ~0.8 us/op on its GPU).
+    The op is tile_add_f32 on `elems` floats (the paper uses a length-2048 tile), z_{i+1} = z_i + y."""
+    dev = torch.device("cuda", torch.cuda.current_device())
+    s = torch.cuda.Stream()
+    y = torch.ones(elems, dtype=torch.float32, device=dev)
+    za = torch.zeros(elems, dtype=torch.float32, device=dev)
+    zb = torch.zeros(elems, dtype=torch.float32, device=dev)
+
+    def chain():
+        for i in range(n_ops):
+            src, dst = (za, zb) if i % 2 == 0 else (zb, za)
+            tg.tile_add_f32(src, y, dst, stream=s)
+
+    chain()
+    s.synchronize()
+    out = {}
+    best = 1e30
+    for _ in range(5):
+        t0 = time.perf_counter()
+        chain()
+        s.synchronize()
+        best = min(best, time.perf_counter() - t0)
+    out["stream_launch_us_per_op"] = best / n_ops * 1e6
+    tg.tile_gemm_record_begin(s)
+    chain()
+    step = tg.tile_gemm_record_end(s)
+    step.replay(s)
+    s.synchronize()
+    best = 1e30
+    for _ in range(5):
+        t0 = time.perf_counter()
+        step.replay(s)
+        s.synchronize()
+        best = min(best, time.perf_counter() - t0)
+    out["recorded_replay_us_per_op"] = best / n_ops * 1e6
+    out["ops"], out["elems_per_op"], out["nodes"] = n_ops, elems, step.nodes
+    step.free()
+    return out
+
+
 def bench_sweep(tg, torch, sizes, tdist):
     """the paper's Figure 6b sweep, M=N=K powers of two, f16 (the
     paper's precision) and bf16, 16-bit output.  Per size: median of `reps` single-launch timings
     (paper: medians) on rotating operand sets whose total exceeds L2 where the problem allows."""
     dev = torch.device("cuda", torch.cuda.current_device())
-    out = {}
-    for dt_name, dt in (("f16", torch.float16), ("bf16", torch.bfloat16)):
-        rows = {}
-        for n in sizes:
+    out = {"f16": {}, "bf16": {}}
+    for n in sizes:   # sizes outer, types inner: both types of a size see the same power state
+        for dt_name, dt in (("f16", torch.float16), ("bf16", torch.bfloat16)):
+            rows = out[dt_name]
             per_set = 3 * n * n * 2
             sets = int(max(1, min(8, (256 << 20) // per_set + 1)))
             reps = 40 if n <= 4096 else (12 if n <= 16384 else 5)
@@ -381,7 +426,6 @@ def bench_sweep(tg, torch, sizes, tdist):
                             "operand_sets": sets}
             del bufs
             torch.cuda.empty_cache()
-        out[dt_name] = rows
     return out
 
 
@@ -459,7 +503,7 @@ def run_cuda(args):
             "api": "tile_gemm_static_b (weights immutable: tiles are prefetched ahead of the PDL wait)",
             "plain_tile_gemm": {"ms_per_pass": plain_ms, "gbs": alg_bytes / (plain_ms * 1e-3) / 1e9},
             "per_shape": per_shape,
-            "graph_replay": None if graph_ms is None else {"ms_per_pass": graph_ms,
+            "recorded_step_replay": None if graph_ms is None else {"ms_per_pass": graph_ms,
                                                            "gbs": alg_bytes / (graph_ms * 1e-3) / 1e9},
             "roofline": {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                          "frac": gbs / peaks["hbm_gbs"], "traffic": ncu_traffic("gemv_gate_up_dram_bytes"),
@@ -479,6 +523,10 @@ def run_cuda(args):
                          "frac_of_8000": gbs / 8000.0, "kernel": "add_f32_vec_kernel<1,4,true>",
                          "algorithmic_bytes_per_launch": 12 * n_add},
         }
+        # per-op host cost, stream launches vs one recorded step
+        if rank == 0:
+            line["replay"] = bench_launch_overhead(tg, torch)
+        tdist.barrier()
         # the paper's size sweep in f16 and bf16
         if not args.no_sweep:
             line["sweep"] = bench_sweep(tg, torch, [1024, 2048, 4096, 8192, 16384, 32768], tdist)
