@@ -52,7 +52,44 @@ struct GemmParams {
     // window the L2 holds, instead of drifting apart over a long launch.  sync == nullptr: off.
     uint32_t* sync;             // [windows] arrival counters, zero at launch
     int32_t sync_window;
+    int32_t sync_rounds;        // lockstep covers the first sync_rounds units of every cluster (all whole tiles)
+    // Split-K for the last, partial wave (and for problems smaller than one wave): work units
+    // [0, full_units) are whole tiles; the remaining tiles are cut into `split` slices of `kps`
+    // k-tiles each, one unit per slice.  A slice's fp32 accumulators go to `partials`; the CTA that
+    // draws the last of a tile's `split` tickets adds the slices in slice order (fixed order:
+    // bitwise reproducible) and stores C.  split == 0: every unit is a whole tile.
+    int32_t full_units, split, kps, total_units;
+    float* partials;            // [split tiles][split][CG][8 warps][units][8 chunks][32 lanes][4 floats]
+    uint32_t* tickets;          // [split tiles][CG], zero between launches
 };
+
+// Work unit -> (tile, k-tile range, slice); slice < 0: a whole tile.  Pure function, all roles
+// evaluate it identically.
+struct GemmUnit {
+    int t, k0, k1, slice;
+};
+template <bool SPLIT>
+__device__ __forceinline__ GemmUnit gemm_unit(const GemmParams& p, int u) {
+    GemmUnit r;
+    if (!SPLIT || u < p.full_units) {
+        r.t = u; r.k0 = 0; r.k1 = p.num_k_tiles; r.slice = -1;
+    } else {
+        const int v = u - p.full_units;
+        r.t = p.full_units + v / p.split;
+        r.slice = v - (v / p.split) * p.split;
+        r.k0 = r.slice * p.kps;
+        r.k1 = min(p.num_k_tiles, r.k0 + p.kps);
+    }
+    return r;
+}
+__device__ __forceinline__ float4 ld_cg_f4(const float* p) {
+    float4 v;
+    asm volatile("ld.global.cg.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_cg_f4(float* p, float a, float b, float c, float d) {
+    asm volatile("st.global.cg.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+}
 
 __device__ __forceinline__ uint32_t ld_relaxed_gpu_u32(const uint32_t* p) {
     uint32_t v;
@@ -91,10 +128,13 @@ struct GemmSmem {
     static constexpr uint32_t BAR_OFF = EPI_OFF + EPI_BYTES;
     static constexpr uint32_t NUM_BARS = 2 * STAGES + 4;
     static constexpr uint32_t TMEM_PTR_OFF = BAR_OFF + NUM_BARS * 8;
+    static constexpr uint32_t LAST_FLAG_OFF = TMEM_PTR_OFF + 8;   // split-K: "this CTA drew the last ticket"
     static constexpr uint32_t TOTAL = TMEM_PTR_OFF + 16 + 1024;   // + slack for 1024 B alignment
 };
 
-template <int CG, int BN, int STAGES, int NACC>
+// SPLIT = false: every unit is a whole tile (the split-K epilogue is not even compiled in: it costs
+// the hot epilogue registers); SPLIT = true: launches whose last wave is cut into K slices.
+template <int CG, int BN, int STAGES, int NACC, bool SPLIT>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b,
                     const __grid_constant__ CUtensorMap tmap_c, const GemmParams p) {
@@ -114,7 +154,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
     const uint32_t rank = (CG == 2) ? cluster_ctarank() : 0u;
     const int first_tile = (CG == 2) ? (int)cluster_id_x() : (int)blockIdx.x;
     const int tile_stride = (CG == 2) ? (int)num_clusters_x() : (int)gridDim.x;
-    const int total_tiles = p.tiles_m * p.tiles_n;
+    const int total_units = p.total_units;
 
     const uint32_t bar_base = smem_base + L::BAR_OFF;
     auto full_bar = [&](uint32_t s) { return bar_base + s * 8u; };
@@ -158,24 +198,22 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
             // lockstep bookkeeping (leader CTA of each cluster only; its partner is held back by the
             // shared pipeline): `pos` counts the k-tiles this cluster has issued over all its tiles
             const bool lockstep = p.sync != nullptr && rank == 0;
-            const int tiles_max = (total_tiles + tile_stride - 1) / tile_stride;           // tiles of the busiest cluster
-            const int clusters_full = total_tiles - (tiles_max - 1) * tile_stride;         // clusters that own tiles_max tiles
+            // the first sync_rounds units of every cluster are whole tiles: positions below sync_limit
+            // exist in every cluster's schedule, so every window counter there reaches the cluster count
+            const uint32_t sync_limit = (uint32_t)p.sync_rounds * (uint32_t)p.num_k_tiles;
             uint32_t pos = 0, next_sync = 0;
-            for (int t = first_tile; t < total_tiles; t += tile_stride) {
+            for (int u = first_tile; u < total_units; u += tile_stride) {
+                const GemmUnit un = gemm_unit<SPLIT>(p, u);
                 int tm, tn;
-                tile_coords(t, p.tiles_m, p.tiles_n, p.group_m, tm, tn);
+                tile_coords(un.t, p.tiles_m, p.tiles_n, p.group_m, tm, tn);
                 const int m0 = (tm * CG + (int)rank) * GEMM_BM;
                 const int n0 = tn * TILE_N + (int)rank * (int)L::B_COLS;
-                for (int kt = 0; kt < p.num_k_tiles; ++kt, ++pos) {
-                    if (lockstep && pos == next_sync) {
+                for (int kt = un.k0; kt < un.k1; ++kt, ++pos) {
+                    if (lockstep && pos == next_sync && pos < sync_limit) {
                         const uint32_t w = pos / (uint32_t)p.sync_window;
                         red_add_relaxed_gpu_u32(p.sync + w, 1u);
-                        if (w >= 1) {   // everyone who owns window w-1 must have entered it
-                            const bool all_own = (uint64_t)(w - 1) * (uint32_t)p.sync_window <
-                                                 (uint64_t)(tiles_max - 1) * (uint32_t)p.num_k_tiles;
-                            const uint32_t expect = all_own ? (uint32_t)tile_stride : (uint32_t)clusters_full;
-                            while (ld_relaxed_gpu_u32(p.sync + (w - 1)) < expect) __nanosleep(64);
-                        }
+                        if (w >= 1)   // every cluster must have entered window w-1
+                            while (ld_relaxed_gpu_u32(p.sync + (w - 1)) < (uint32_t)tile_stride) __nanosleep(64);
                         next_sync += (uint32_t)p.sync_window;
                     }
                     mbar_wait(empty_bar(stage), phase ^ 1u);
@@ -226,10 +264,11 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
             // slot use: NACC == 1 -> slot = tile iteration & 1 (phase flips every 2nd tile);
             //           NACC == 2 -> both slots every tile (phase flips every tile)
             uint32_t stage = 0, phase = 0, it = 0;
-            for (int t = first_tile; t < total_tiles; t += tile_stride, ++it) {
+            for (int u = first_tile; u < total_units; u += tile_stride, ++it) {
+                const GemmUnit un = gemm_unit<SPLIT>(p, u);
                 const uint32_t slot0 = (NACC == 2) ? 0u : (it & 1u);
                 const uint32_t acc_phase = (NACC == 2) ? (it & 1u) : ((it >> 1) & 1u);
-                for (int kt = 0; kt < p.num_k_tiles; ++kt) {
+                for (int kt = un.k0; kt < un.k1; ++kt) {
                     mbar_wait(full_bar(stage), phase);
                     tc_fence_after();
                     const uint32_t sa = smem_base + stage * L::STAGE_BYTES;
@@ -237,7 +276,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
                     const uint64_t a_desc = a_desc_base | (uint64_t)((sa & 0x3FFFFu) >> 4);
 #pragma unroll
                     for (uint32_t j = 0; j < (uint32_t)NACC; ++j) {
-                        if (kt == 0) {   // the epilogue must have drained this slot
+                        if (kt == un.k0) {   // the epilogue must have drained this slot
                             mbar_wait(tmem_empty_bar(slot0 + j), acc_phase ^ 1u);
                             tc_fence_after();
                         }
@@ -249,10 +288,10 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
                             // A: +16 elements along K = +32 B inside the swizzled row;
                             // B: +16 k-rows of 128 B = +2048 B
                             umma_bf16<CG>(d_tmem, a_desc + (uint64_t)(k * 2), b_desc + (uint64_t)(k * 128), idesc,
-                                          (uint32_t)((kt | k) != 0));
+                                          (uint32_t)((kt != un.k0) | (k != 0)));
                         }
                         // accumulator slot ready for the epilogue after the last k-tile
-                        if (kt == p.num_k_tiles - 1) umma_commit<CG>(tmem_full_bar(slot0 + j));
+                        if (kt == un.k1 - 1) umma_commit<CG>(tmem_full_bar(slot0 + j));
                     }
                     umma_commit<CG>(empty_bar(stage));   // smem stage reusable once these MMAs retire
                     if (++stage == STAGES) { stage = 0; phase ^= 1u; }
@@ -292,7 +331,10 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
         // st.global path so that C[i][N..] is never written.
         const bool ragged_n = (p.N % (out_16 ? 8 : 4)) != 0;
         uint32_t it = 0, buf = 0;
-        for (int t = first_tile; t < total_tiles; t += tile_stride, ++it) {
+        volatile uint32_t* last_flag = reinterpret_cast<volatile uint32_t*>(smem_gen + L::LAST_FLAG_OFF);
+        for (int u_idx = first_tile; u_idx < total_units; u_idx += tile_stride, ++it) {
+            const GemmUnit un = gemm_unit<SPLIT>(p, u_idx);
+            const int t = un.t;
             int tm, tn;
             tile_coords(t, p.tiles_m, p.tiles_n, p.group_m, tm, tn);
             const int m0 = (tm * CG + (int)rank) * GEMM_BM + (int)q * 32;    // first row of this warp
@@ -399,6 +441,58 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
             };
 
             uint32_t va[32], vb[32];
+            if (SPLIT && un.slice >= 0) {
+                // ---- one K slice of a split tile: park the fp32 accumulators, take a ticket; the CTA
+                //      that draws the tile's last ticket adds all slices in slice order and stores C ----
+                constexpr size_t WARP_FLOATS = (size_t)UNITS * 32 * 32;
+                const int st = t - p.full_units;                      // index among the split tiles
+                auto slot_of = [&](int slice) -> float* {
+                    // per 32-column unit: [8 chunks][32 lanes][4 floats] -- a warp's st/ld.v4 covers 512 contiguous bytes
+                    return p.partials + ((((size_t)st * p.split + slice) * CG + rank) * 8 + ew) * WARP_FLOATS + lane * 4;
+                };
+                float* mine = slot_of(un.slice);
+                for (int uu = 0; uu < units; ++uu) {
+                    tmem_ld_32x32(t_acc + (uint32_t)(uu * 32), va);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int i = 0; i < 32; i += 4)
+                        st_cg_f4(mine + (size_t)uu * 1024 + i * 32, __uint_as_float(va[i]), __uint_as_float(va[i + 1]),
+                                 __uint_as_float(va[i + 2]), __uint_as_float(va[i + 3]));
+                }
+                release_tmem();
+                __threadfence();
+                asm volatile("bar.sync 1, 256;" ::: "memory");        // the eight epilogue warps
+                if (ew == 0 && lane == 0) {
+                    uint32_t* tk = p.tickets + (size_t)st * CG + rank;
+                    const uint32_t old = atomicAdd(tk, 1u);
+                    const bool last = (old == (uint32_t)(p.split - 1));
+                    if (last) *tk = 0u;                                 // every slice has arrived: re-arm
+                    *last_flag = last ? 1u : 0u;
+                }
+                asm volatile("bar.sync 1, 256;" ::: "memory");
+                const bool last = (*last_flag != 0u);
+                asm volatile("bar.sync 1, 256;" ::: "memory");        // flag is free for the next unit
+                if (last) {
+                    __threadfence();
+                    for (int uu = 0; uu < units; ++uu) {
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) va[i] = 0u;        // +0.0f
+                        for (int sl = 0; sl < p.split; ++sl) {          // fixed order
+                            const float* src = slot_of(sl) + (size_t)uu * 1024;
+#pragma unroll
+                            for (int i = 0; i < 32; i += 4) {
+                                const float4 f = ld_cg_f4(src + i * 32);
+                                va[i] = __float_as_uint(__uint_as_float(va[i]) + f.x);
+                                va[i + 1] = __float_as_uint(__uint_as_float(va[i + 1]) + f.y);
+                                va[i + 2] = __float_as_uint(__uint_as_float(va[i + 2]) + f.z);
+                                va[i + 3] = __float_as_uint(__uint_as_float(va[i + 3]) + f.w);
+                            }
+                        }
+                        stage_unit(va, uu);
+                    }
+                }
+                continue;
+            }
             if (units > 0) tmem_ld_32x32(t_acc, va);
 #pragma unroll 1
             for (int u = 0; u < units; u += 2) {

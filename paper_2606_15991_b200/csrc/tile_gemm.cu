@@ -347,7 +347,10 @@ GemmConfig choose_config(int64_t M, int64_t N, int sms) {
 }
 
 // lockstep defaults: on from kLockstepMinTiles tiles per cluster and kLockstepMinKTiles k-tiles
-constexpr int kLockstepMinTiles = 3, kLockstepMinKTiles = 64, kLockstepWindow = 32;
+constexpr int kLockstepMinTiles = 2, kLockstepMinKTiles = 128, kLockstepWindow = 32;
+
+// split-K of the last wave: at most kGemmMaxSplit slices of at least kGemmMinSliceKTiles k-tiles each
+constexpr int kGemmMaxSplit = 16, kGemmMinSliceKTiles = 4;
 
 struct GemmLaunch {
     GemmConfig cfg;
@@ -355,7 +358,8 @@ struct GemmLaunch {
     int ctas;
 };
 
-void plan_gemm(int64_t M, int64_t N, int64_t K, int in_dtype, int out_dtype, int sms, GemmLaunch* gl) {
+void plan_gemm(int64_t M, int64_t N, int64_t K, int in_dtype, int out_dtype, int sms, GemmLaunch* gl,
+               bool allow_split = false) {
     gl->cfg = choose_config(M, N, sms);
     const int tile_m = tg::GEMM_BM * gl->cfg.cg;
     tg::GemmParams& p = gl->p;
@@ -370,19 +374,58 @@ void plan_gemm(int64_t M, int64_t N, int64_t K, int in_dtype, int out_dtype, int
     p.out_16 = out_dtype != TILE_GEMM_OUT_F32;
     p.out_f16 = out_dtype == TILE_GEMM_OUT_F16;
     p.in_f16 = in_dtype == TILE_GEMM_IN_F16;
-    int64_t units = (int64_t)p.tiles_m * p.tiles_n;
+    const int64_t tiles = (int64_t)p.tiles_m * p.tiles_n;
     int max_units = sms / gl->cfg.cg;
     const int cap = g_tune[2].load();
     if (cap > 0 && cap / gl->cfg.cg >= 1 && cap / gl->cfg.cg < max_units) max_units = cap / gl->cfg.cg;
+    // Split-K for the partial last wave: `rem` tiles are left after the whole waves;
+    // cut each into floor(clusters / rem) slices so that the last round is one short, full wave.
+    p.full_units = (int32_t)tiles;
+    p.total_units = (int32_t)tiles;
+    p.split = 0;
+    p.kps = p.num_k_tiles;
+    const int64_t rem = tiles % max_units;
+    const int split_tune = g_tune[3].load();   // key 3 also overrides the GEMM split: 1 = never, >= 2 = that many slices
+    if (allow_split && rem > 0 && split_tune != 1 && p.num_k_tiles >= 2 * kGemmMinSliceKTiles) {
+        // The last wave as ceil(rem * c / clusters) rounds of 1/c-tile units, in microseconds: a whole
+        // tile at the per-cluster share of ~1500 TFLOP/s, plus what a slice costs on top (its fp32
+        // accumulators go through L2 once as a store and once as a load of the fix-up, ~100 GB/s per
+        // cluster, and a ticket round trip) -- measured on B200: ~8 us for a 256x512 slice, ~3.5 us
+        // for 128x128.  Cutting pays for long K loops and for problems below one wave (skinny M).
+        int64_t sl_max = p.num_k_tiles / kGemmMinSliceKTiles;
+        if (sl_max > kGemmMaxSplit) sl_max = kGemmMaxSplit;
+        const double tile_flop = 2.0 * tile_m * gl->cfg.tile_n() * (double)p.num_k_tiles * tg::GEMM_BK;
+        const double tile_us = tile_flop / (1500e6 * gl->cfg.cg / (double)sms);
+        const double ovh_us = 3.0 + (double)tile_m * gl->cfg.tile_n() * 4.0 / 100e3;
+        int64_t sl = 1;
+        double best = tile_us;
+        for (int64_t c = 2; c <= sl_max; ++c) {
+            const double rounds = (double)((rem * c + max_units - 1) / max_units);
+            const double cost = rounds / (double)c * tile_us + (rounds + 0.5 * (double)c) * ovh_us;
+            if (cost < best * 0.97) { best = cost; sl = c; }
+        }
+        if (split_tune >= 2) sl = split_tune < sl_max ? split_tune : sl_max;
+        if (sl >= 2) {
+            const int64_t kps = (p.num_k_tiles + sl - 1) / sl;
+            sl = (p.num_k_tiles + kps - 1) / kps;              // no empty slice
+            if (sl >= 2) {
+                p.split = (int32_t)sl;
+                p.kps = (int32_t)kps;
+                p.full_units = (int32_t)(tiles - rem);
+                p.total_units = (int32_t)(tiles - rem + rem * sl);
+            }
+        }
+    }
+    int64_t units = p.total_units;
     if (units > max_units) units = max_units;
     gl->ctas = (int)units * gl->cfg.cg;
 }
 
-template <int CG, int BN, int STAGES, int NACC>
+template <int CG, int BN, int STAGES, int NACC, bool SPLIT>
 int launch_gemm_inst(const CUtensorMap& ta, const CUtensorMap& tb, const CUtensorMap& tc, const tg::GemmParams& p,
                      int ctas, cudaStream_t s, int dev) {
     using L = tg::GemmSmem<CG, BN, STAGES, NACC>;
-    auto kern = tg::gemm_tcgen05_kernel<CG, BN, STAGES, NACC>;
+    auto kern = tg::gemm_tcgen05_kernel<CG, BN, STAGES, NACC, SPLIT>;
     static bool configured[64] = {};
     if (!configured[dev]) {
         CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::TOTAL));
@@ -409,10 +452,15 @@ int launch_gemm_inst(const CUtensorMap& ta, const CUtensorMap& tb, const CUtenso
 int launch_gemm(const GemmLaunch& gl, const CUtensorMap& ta, const CUtensorMap& tb, const CUtensorMap& tc,
                 cudaStream_t s, int dev) {
     switch (gl.cfg.id) {
-        case 1: return launch_gemm_inst<1, 128, 6, 1>(ta, tb, tc, gl.p, gl.ctas, s, dev);
-        case 2: return launch_gemm_inst<1, 256, 4, 1>(ta, tb, tc, gl.p, gl.ctas, s, dev);
-        case 3: return launch_gemm_inst<2, 256, 6, 1>(ta, tb, tc, gl.p, gl.ctas, s, dev);
-        case 4: return launch_gemm_inst<2, 256, 4, 2>(ta, tb, tc, gl.p, gl.ctas, s, dev);
+#define TG_GEMM_CASE(id, CG, BN, ST, NA)                                                              \
+    case id:                                                                                         \
+        return gl.p.split > 0 ? launch_gemm_inst<CG, BN, ST, NA, true>(ta, tb, tc, gl.p, gl.ctas, s, dev) \
+                              : launch_gemm_inst<CG, BN, ST, NA, false>(ta, tb, tc, gl.p, gl.ctas, s, dev);
+        TG_GEMM_CASE(1, 1, 128, 6, 1)
+        TG_GEMM_CASE(2, 1, 256, 4, 1)
+        TG_GEMM_CASE(3, 2, 256, 6, 1)
+        TG_GEMM_CASE(4, 2, 256, 4, 2)
+#undef TG_GEMM_CASE
     }
     return fail(TILE_GEMM_E_INTERNAL, "unknown GEMM config %d", gl.cfg.id);
 }
@@ -460,7 +508,14 @@ int run_gemm(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_
         }
     }
     GemmLaunch gl;
-    plan_gemm(M, N, K, in_dtype, out_dtype, sms, &gl);
+    plan_gemm(M, N, K, in_dtype, out_dtype, sms, &gl, true);
+    if (gl.p.split > 0) {
+        const size_t split_tiles = (size_t)((int64_t)gl.p.tiles_m * gl.p.tiles_n - gl.p.full_units);
+        const size_t tile_floats = (size_t)tg::GEMM_BM * gl.cfg.cg * gl.cfg.tile_n();
+        int rc2 = gemv_workspace_for(dev, s, split_tiles * gl.p.split * tile_floats * 4, split_tiles * gl.cfg.cg * 4 + 1024,
+                                     &gl.p.partials, &gl.p.tickets);
+        if (rc2) return rc2;
+    }
     gl.p.tma_store = plan.c_tma ? 1 : 0;
     gl.p.C = C;
     gl.p.ldc = ldc;
@@ -480,15 +535,16 @@ int run_gemm(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_
     {
         const int tune = g_tune[6].load();
         const int clusters = gl.ctas / gl.cfg.cg;
-        const int64_t tiles = (int64_t)gl.p.tiles_m * gl.p.tiles_n;
-        const int64_t tiles_max = (tiles + clusters - 1) / clusters;
-        bool on = tiles_max >= kLockstepMinTiles && gl.p.num_k_tiles >= kLockstepMinKTiles;
-        if (tune & 4) on = tiles_max >= 1 && gl.p.num_k_tiles >= 1;
+        // rounds in which every cluster owns a whole tile: lockstep covers exactly these
+        const int64_t rounds = gl.p.full_units / clusters;
+        bool on = rounds >= kLockstepMinTiles && gl.p.num_k_tiles >= kLockstepMinKTiles;
+        if (tune & 4) on = rounds >= 1 && gl.p.num_k_tiles >= 1;
         if (tune & 8) on = false;
         if (on) {
             int window = (tune >> 8) & 255;
             if (window <= 0) window = kLockstepWindow;
-            const int64_t windows = (tiles_max * gl.p.num_k_tiles + window - 1) / window + 1;
+            const int64_t windows = (rounds * gl.p.num_k_tiles + window - 1) / window + 1;
+            gl.p.sync_rounds = (int32_t)rounds;
             uint32_t* sync = nullptr;
             rc = sync_workspace_for(dev, s, (size_t)windows * 4, &sync);
             if (rc) return rc;

@@ -419,3 +419,31 @@ def test_host_entry_matches_oracle():
     y = np.zeros((1, 2048), np.uint16)
     tg.tile_gemm_host(x, W, y)
     check_close(oracle.bf16_decode(y), ref, S, 1024, "bf16", "host entry gemv")
+
+
+# ------------------------------------------------------------------ split-K of the last wave
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4])
+@pytest.mark.parametrize("split", [2, 3, 5, 16])
+def test_gemm_split_k_integer_bit_exact_and_canary(cfg, split):
+    """Forced K slices (tuning key 3) on the ragged cfg2 shape and on a long-K shape: integer inputs
+    are exact whatever the slicing, nothing outside C is written, every element is written."""
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMM_CONFIG, cfg)
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMV_SPLIT, split)
+    for (M, N, K), pads in (((1023, 1537, 769), (0, 0, 0)), ((300, 700, 4100), (8, 8, 8)), ((130, 520, 1030), (0, 0, 3))):
+        a, b = wl.make_inputs_custom(M, N, K, dist="int4", seed=31 + split)
+        ref, _ = oracle.gemm(a, b)
+        got = run_case(a, b, "f32", pads=pads, what=f"split {split} cfg {cfg}")
+        check_bit_exact(got.astype(np.float32), ref, f"split-K ints cfg{cfg} split{split} {M}x{N}x{K}")
+
+
+@pytest.mark.parametrize("out", ["f32", "bf16"])
+def test_gemm_split_k_auto_normal_inputs_and_determinism(out):
+    """Shapes on which the selector itself slices K (a long-K last wave, skinny M): full oracle, and
+    two runs give identical bits (slices are added in slice order, not arrival order)."""
+    for (M, N, K) in ((8, 5120, 6400), (64, 1024, 8192), (2304, 2560, 6400)):
+        a, b = wl.make_inputs_custom(M, N, K, sigma_b=K ** -0.5, seed=41)
+        ref, S = oracle.gemm(a, b)
+        got1 = run_case(a, b, out, what="split auto")
+        got2 = run_case(a, b, out, what="split auto")
+        check_close(got1, ref, S, K, out, f"split-K auto {M}x{N}x{K} {out}")
+        assert np.array_equal(got1, got2), "split-K result depends on arrival order"
