@@ -377,6 +377,32 @@ def bench_launch_overhead(tg, torch, n_ops=1000, elems=2048):
     return out
 
 
+def bench_skinny(tg, wl, torch, ms_list, tdist, layers=8):
+    """skinny M (decode with a few tokens in flight) on the four Qwen3-32B weight shapes,
+    through the tensor-core GEMM with K slices filling the SMs.  HBM-bound: reported as GB/s of
+    algorithmic bytes (weights once + activations + outputs), `layers` distinct weight sets."""
+    dev = torch.device("cuda", torch.cuda.current_device())
+    g = torch.Generator(device=dev)
+    g.manual_seed(8)
+    Ws = [[torch.empty((K, N), dtype=torch.bfloat16, device=dev).normal_(0, 0.02, generator=g)
+           for (K, N) in wl.QWEN3_32B] for _ in range(layers)]
+    out = {}
+    for M in ms_list:
+        xs = [torch.empty((M, K), dtype=torch.bfloat16, device=dev).normal_(0, 1, generator=g) for (K, N) in wl.QWEN3_32B]
+        ys = [torch.empty((M, N), dtype=torch.bfloat16, device=dev) for (K, N) in wl.QWEN3_32B]
+
+        def one_pass(_):
+            for layer in range(layers):
+                for p in range(4):
+                    tg.tile_gemm(xs[p], Ws[layer][p], ys[p])
+
+        one_pass(0)
+        ms = tdist.max_over_ranks(time_region(one_pass, 3, torch.cuda.synchronize, tdist.barrier)) / 3
+        byt = sum(2 * K * N + 2 * M * K + 2 * M * N for (K, N) in wl.QWEN3_32B) * layers
+        out[str(M)] = {"ms_per_pass": ms, "gbs": byt / (ms * 1e-3) / 1e9, "launches_per_pass": 4 * layers}
+    return out
+
+
 def bench_sweep(tg, torch, sizes, tdist):
     """the paper's Figure 6b sweep, M=N=K powers of two, f16 (the
     paper's precision) and bf16, 16-bit output.  Per size: median of `reps` single-launch timings
@@ -466,7 +492,7 @@ def run_cuda(args):
                      "peak_source": f"{peaks['source']} cuBLAS bf16 burst (MEASURED_PEAKS.json)",
                      "frac_of_sustained": per_gpu / peaks["bf16_tflops_sustained"],
                      "frac_of_nominal_2250": per_gpu / 2250.0,
-                     "kernel": "gemm_tcgen05_kernel<2,256,4,2>", "algorithmic_flops_per_launch": flops},
+                     "kernel": "gemm_tcgen05_kernel<2,256,4,2,false>", "algorithmic_flops_per_launch": flops},
     }
     del bufs
     torch.cuda.empty_cache()
@@ -527,6 +553,8 @@ def run_cuda(args):
         if rank == 0:
             line["replay"] = bench_launch_overhead(tg, torch)
         tdist.barrier()
+        # skinny M through the GEMM's K slices
+        line["skinny_m"] = bench_skinny(tg, wl, torch, [2, 4, 8, 16, 32, 64], tdist)
         # the paper's size sweep in f16 and bf16
         if not args.no_sweep:
             line["sweep"] = bench_sweep(tg, torch, [1024, 2048, 4096, 8192, 16384, 32768], tdist)
