@@ -149,3 +149,42 @@ def test_gloo_world_size_two_bench_helpers():
                          env=env, capture_output=True, text=True, timeout=300)
     assert res.returncode == 0, res.stdout + res.stderr
     assert "GLOO_OK rank0" in res.stdout
+
+
+# ------------------------------------------------------------------ SURVEY 8(f) entries: launch preconditions on the host
+def test_add_preconditions_are_checked_before_any_device_call():
+    X, Y, Z = 0x10000, 0x7000_0000_0000, 0x7100_0000_0000
+    assert tg.tile_add_f32_raw(X, Y, Z, -1) == tg.E_EXTENT
+    assert tg.tile_add_f32_raw(X, Y, Z, 0) == tg.E_OK                      # empty: success, nothing to do
+    assert tg.tile_add_f32_raw(X, Y, Z, (1 << 40) + 1) == tg.E_OVERFLOW
+    assert tg.tile_add_f32_raw(0, Y, Z, 8) == tg.E_NULL
+    assert tg.tile_add_f32_raw(X, Y, 0, 8) == tg.E_NULL
+    assert tg.tile_add_f32_raw(X + 2, Y, Z, 8) == tg.E_ALIGN
+    assert tg.tile_add_f32_raw(X, Y, X + 16, 8) == tg.E_ALIAS             # z overlaps x: the output is exclusively owned
+    assert tg.tile_add_f32_raw(X, Y, Y - 16, 8) == tg.E_ALIAS
+    assert tg.tile_add_f32_raw(X, Y, Y + 32, 8) != tg.E_ALIAS             # adjacent, not overlapping
+    assert "z" in tg.tile_gemm_last_error() or not torch.cuda.is_available()
+    if not torch.cuda.is_available():                                        # no CPU fallback: the device check fails loudly
+        assert tg.tile_add_f32_raw(X, X, Z, 8) == tg.E_DEVICE
+
+
+def test_typed_entry_preconditions():
+    args = (A0, B0, C0, 8, 8, 8, 8, 8, 8)
+    assert tg.tile_gemm_typed_raw(*args, 2, tg.OUT_F32) == tg.E_IN_DTYPE
+    assert tg.tile_gemm_typed_raw(*args, -1, tg.OUT_F32) == tg.E_IN_DTYPE
+    assert tg.tile_gemm_typed_raw(*args, tg.IN_F16, 3) == tg.E_DTYPE
+    assert tg.tile_gemm_typed_raw(A0, B0, C0, 8, 8, 8, 7, 8, 8, tg.IN_F16, tg.OUT_F16) == tg.E_LDA
+    # a 16-bit C (bf16 or f16) must be 2-byte aligned, an fp32 C 4-byte aligned
+    assert tg.tile_gemm_typed_raw(A0, B0, C0 + 2, 8, 8, 8, 8, 8, 8, tg.IN_F16, tg.OUT_F16) != tg.E_ALIGN
+    assert tg.tile_gemm_typed_raw(A0, B0, C0 + 2, 8, 8, 8, 8, 8, 8, tg.IN_F16, tg.OUT_F32) == tg.E_ALIGN
+    if not torch.cuda.is_available():
+        assert tg.tile_gemm_typed_raw(*args, tg.IN_F16, tg.OUT_F16) == tg.E_DEVICE
+
+
+def test_record_entries_reject_bad_handles_without_a_device():
+    lib = tg.load_library()
+    assert lib.tile_gemm_replay(None, None) == tg.E_NULL
+    assert lib.tile_gemm_recorded_nodes(None) == -1
+    assert lib.tile_gemm_record_free(None) == tg.E_OK
+    if not torch.cuda.is_available():
+        assert lib.tile_gemm_record_begin(None) == tg.E_DEVICE
