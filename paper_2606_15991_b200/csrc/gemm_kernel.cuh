@@ -189,6 +189,10 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
     if constexpr (CG == 2) cluster_sync(); else __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_ptr_gen;
+    // programmatic dependent launch: this kernel's set-up above overlapped the previous kernel's
+    // tail; every role waits for that kernel before its first global access, and the next kernel may
+    // start its own set-up as our CTAs retire
+    griddep_launch_dependents();
 
     // ------------------------------------------------------------------ warp roles
     if (warp == 0) {
@@ -202,6 +206,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
             // exist in every cluster's schedule, so every window counter there reaches the cluster count
             const uint32_t sync_limit = (uint32_t)p.sync_rounds * (uint32_t)p.num_k_tiles;
             uint32_t pos = 0, next_sync = 0;
+            griddep_wait();   // A, B (and the lockstep counters) may be the previous kernel's output
             for (int u = first_tile; u < total_units; u += tile_stride) {
                 const GemmUnit un = gemm_unit<SPLIT>(p, u);
                 int tm, tn;
@@ -332,6 +337,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
         const bool ragged_n = (p.N % (out_16 ? 8 : 4)) != 0;
         uint32_t it = 0, buf = 0;
         volatile uint32_t* last_flag = reinterpret_cast<volatile uint32_t*>(smem_gen + L::LAST_FLAG_OFF);
+        griddep_wait();   // C, the partials and the tickets may still be in the previous kernel's use
         for (int u_idx = first_tile; u_idx < total_units; u_idx += tile_stride, ++it) {
             const GemmUnit un = gemm_unit<SPLIT>(p, u_idx);
             const int t = un.t;

@@ -437,13 +437,15 @@ int launch_gemm_inst(const CUtensorMap& ta, const CUtensorMap& tb, const CUtenso
     cfg.blockDim = dim3(tg::GEMM_THREADS, 1, 1);
     cfg.dynamicSmemBytes = L::TOTAL;
     cfg.stream = s;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = CG;
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
+    attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[1].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = 1;
+    cfg.numAttrs = (g_tune[6].load() & 1) ? 1 : 2;   // tuning key 6 bit 0: no programmatic dependent launch
     CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, ta, tb, tc, p));
     g_launches.fetch_add(1);
     return TILE_GEMM_OK;
