@@ -174,3 +174,27 @@ def add_f32(x, y):
     z = np.empty_like(x)
     _load().oracle_add_f32(x.ctypes.data_as(_f32p), y.ctypes.data_as(_f32p), z.ctypes.data_as(_f32p), x.size)
     return z
+
+
+def silu(g):
+    """silu(g) = g * sigmoid(g) = g / (1 + exp(-g)) in float64 (the SwiGLU gate activation of the
+    Qwen3 MLP; the paper names the fused kernels around the projections,
+    PAPER.md:343, without printing the formula -- DESIGN.md reading c21)."""
+    g = np.asarray(g, dtype=np.float64)
+    with np.errstate(over="ignore"):
+        return g / (1.0 + np.exp(-g))
+
+
+def swiglu_gemm(X, Wgu, threads: int | None = None):
+    """Fused gate/up projection with the SwiGLU epilogue, stated step by step in float64:
+        G = X @ Wgu[:, :I],  U = X @ Wgu[:, I:],  H = silu(G) * U,   I = Wgu.shape[1] // 2
+    X: (M,K), Wgu: (K,2I) uint16 bf16 bit patterns ([gate | up] concatenated along N).
+    Returns (H, G, U, Sg, Su): the result, both projections and their tolerance scales."""
+    X = _as_u16_2d(X, "X")
+    Wgu = _as_u16_2d(Wgu, "Wgu")
+    if Wgu.shape[1] % 2:
+        raise ValueError("the fused gate/up weight needs an even number of columns")
+    inter = Wgu.shape[1] // 2
+    G, Sg = gemm(X, Wgu[:, :inter], threads=threads)
+    U, Su = gemm(X, Wgu[:, inter:], threads=threads)
+    return silu(G) * U, G, U, Sg, Su

@@ -183,3 +183,54 @@ def test_same_bits_mean_different_values_per_dtype():
     Ch, _ = oracle.gemm(one, one, in_dtype=oracle.IN_F16)
     Cb, _ = oracle.gemm(one, one, in_dtype=oracle.IN_BF16)
     assert np.all(Ch == 2.0) and np.all(Cb == 2 * 0.0078125 ** 2)
+
+
+# ---------------------------------------------------------------- SwiGLU epilogue
+def test_silu_closed_forms_and_identities():
+    import math
+    assert oracle.silu(0.0) == 0.0
+    assert oracle.silu(1.0) == 1.0 / (1.0 + math.exp(-1.0))
+    assert abs(oracle.silu(math.log(3.0)) - math.log(3.0) * 0.75) < 1e-15        # sigmoid(ln 3) = 3/4
+    x = np.linspace(-30, 30, 2001)
+    assert np.allclose(oracle.silu(x) - oracle.silu(-x), x, rtol=0, atol=1e-13)  # x*s(x) + x*s(-x) = x
+    assert np.all(np.abs(oracle.silu(np.array([50.0, 700.0, 1e4])) - [50.0, 700.0, 1e4]) < 1e-12)
+    assert np.all(np.abs(oracle.silu(np.array([-50.0, -700.0, -1e4]))) < 1e-19)  # no overflow to NaN on the left tail
+    xm = -1.2784645427610738                                                    # argmin of silu: 1 + e^x (1 + x) = 0
+    assert abs(oracle.silu(xm) - (-0.2784645427610738)) < 1e-12
+    assert np.all(oracle.silu(x) >= -0.2784645427610739)
+
+
+def test_silu_against_torch_float64():
+    import torch
+    rng = np.random.default_rng(12)
+    x = rng.standard_normal(100_000) * 6
+    ref = torch.nn.functional.silu(torch.from_numpy(x)).numpy()
+    assert np.allclose(oracle.silu(x), ref, rtol=1e-14, atol=1e-300)
+
+
+def test_swiglu_gemm_special_cases():
+    from paper_2606_15991_b200 import workloads as wl
+    rng = np.random.default_rng(13)
+    M, K, inter = 9, 40, 24
+    x = wl.f32_to_bf16_bits(rng.integers(-3, 4, (M, K)).astype(np.float32))
+    wg = rng.integers(-2, 3, (K, inter)).astype(np.float32)
+    wu = rng.integers(-2, 3, (K, inter)).astype(np.float32)
+    W = wl.f32_to_bf16_bits(np.concatenate([wg, wu], axis=1))
+    H, G, U, Sg, Su = oracle.swiglu_gemm(x, W)
+    xd = oracle.bf16_decode(x)
+    assert np.array_equal(G, xd @ wg) and np.array_equal(U, xd @ wu)              # the halves are [gate | up], in this order
+    expect = np.where(G == 0, 0.0, G / (1 + np.exp(-G))) * U
+    assert np.allclose(H, expect, rtol=1e-15, atol=0)
+    # gate weights zero -> H = 0 exactly; up weights zero -> H = 0 exactly
+    W0 = wl.f32_to_bf16_bits(np.concatenate([np.zeros_like(wg), wu], axis=1))
+    assert np.all(oracle.swiglu_gemm(x, W0)[0] == 0)
+    W1 = wl.f32_to_bf16_bits(np.concatenate([wg, np.zeros_like(wu)], axis=1))
+    assert np.all(oracle.swiglu_gemm(x, W1)[0] == 0)
+    # swapping the halves swaps the roles: silu(U) * G
+    Ws = wl.f32_to_bf16_bits(np.concatenate([wu, wg], axis=1))
+    assert np.allclose(oracle.swiglu_gemm(x, Ws)[0], oracle.silu(U) * G, rtol=1e-15, atol=0)
+    # a large positive gate passes the up projection through: K ones times 64 = gate 2560 -> silu = identity to 1e-300
+    xo = wl.f32_to_bf16_bits(np.ones((2, K), np.float32))
+    Wb = wl.f32_to_bf16_bits(np.concatenate([np.full((K, 4), 64.0, np.float32), wu[:, :4]], axis=1))
+    Hb, Gb, Ub, _, _ = oracle.swiglu_gemm(xo, Wb)
+    assert np.array_equal(Hb, Gb * Ub)
