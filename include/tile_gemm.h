@@ -138,6 +138,29 @@ int tile_gemm_typed(const void* A, const void* B, void* C,
                     int in_dtype, int out_dtype, void* stream);
 
 /*
+ * Fused gate/up projection with the SwiGLU epilogue (the MLP of
+ * the Qwen3 engine the paper builds, PAPER.md:330-343 -- the paper names its fused
+ * kernels around the projections without printing the formula, DESIGN.md c21):
+ *     G = X * Wgu[:, 0..I),  U = X * Wgu[:, I..2I),
+ *     H[i*ldh + j] = round_out( silu(G_ij) * U_ij ),  silu(g) = g / (1 + e^-g)
+ * X: M x K bf16 (row stride ldx), Wgu: K x 2I bf16 (row stride ldw >= 2I), gate
+ * columns first, then up; H: M x I, out_dtype F32, BF16 or F16 (row stride ldh).
+ * Both projections accumulate in fp32 in tensor memory side by side; silu and the
+ * product are evaluated in fp32 on the accumulators (fast exp and divide: relative
+ * error about 2^-21) and rounded once; the 2I-wide intermediate never reaches
+ * memory.  X and Wgu must be TMA-addressable (16-byte aligned base, ldx and ldw
+ * multiples of 8) and I a multiple of 8 (the up half is fetched by TMA boxes that
+ * start at column I, which the hardware wants on a 16-byte boundary): there is no
+ * repack path here (TILE_GEMM_E_PATH otherwise).
+ * K == 0 writes zeros.  All other rules and errors are tile_gemm's, with I in the
+ * role of N for H and 2I for Wgu (E_LDB when ldw < 2I).
+ */
+int tile_gemm_swiglu(const void* X, const void* Wgu, void* H,
+                     int64_t M, int64_t I, int64_t K,
+                     int64_t ldx, int64_t ldw, int64_t ldh,
+                     int out_dtype, void* stream);
+
+/*
  * Element-wise add (Listing 1; measured at n = 2^28):
  *     z[i] = fl32(x[i] + y[i])   for i in [0, n)
  * one IEEE-754 binary32 addition per element (round to nearest even; NaN and

@@ -29,7 +29,7 @@ PATH_NAMES = {PATH_AUTO: "auto", PATH_GEMM_TMA: "gemm_tma", PATH_GEMM_REPACK: "g
 
 TUNE_GEMM_CONFIG, TUNE_GEMM_GROUP_M, TUNE_GEMM_MAX_CTAS, TUNE_GEMV_SPLIT, TUNE_GEMV_VARIANT, TUNE_GEMV_SHAPE, TUNE_FLAGS, TUNE_ADD_SHAPE = range(8)
 
-EXPORTS = ("tile_gemm", "tile_gemm_ex", "tile_gemm_static_b", "tile_gemm_typed", "tile_add_f32",
+EXPORTS = ("tile_gemm", "tile_gemm_ex", "tile_gemm_static_b", "tile_gemm_typed", "tile_gemm_swiglu", "tile_add_f32",
            "tile_gemm_record_begin", "tile_gemm_record_end", "tile_gemm_replay", "tile_gemm_recorded_nodes",
            "tile_gemm_record_free", "tile_gemm_select", "tile_gemm_host",
            "tile_gemm_debug_owner_map", "tile_gemm_query_config", "tile_gemm_set_tuning",
@@ -77,6 +77,8 @@ def load_library():
     lib.tile_gemm_static_b.restype = _int
     lib.tile_gemm_typed.argtypes = g[:-1] + [_int, _int, _vp]
     lib.tile_gemm_typed.restype = _int
+    lib.tile_gemm_swiglu.argtypes = g + [_vp]
+    lib.tile_gemm_swiglu.restype = _int
     lib.tile_add_f32.argtypes = [_vp, _vp, _vp, _i64, _vp]
     lib.tile_add_f32.restype = _int
     lib.tile_gemm_record_begin.argtypes = [_vp]
@@ -204,6 +206,32 @@ def tile_gemm_typed_raw(A: int, B: int, C: int, M, N, K, lda, ldb, ldc, in_dtype
     """Raw pointer form of tile_gemm_typed; returns the status code instead of raising."""
     return int(load_library().tile_gemm_typed(_vp(A), _vp(B), _vp(C), M, N, K, lda, ldb, ldc, int(in_dtype),
                                               int(out_dtype), _vp(stream)))
+
+
+def tile_gemm_swiglu_raw(X: int, W: int, H: int, M, I, K, ldx, ldw, ldh, out_dtype, stream: int = 0) -> int:
+    return int(load_library().tile_gemm_swiglu(_vp(X), _vp(W), _vp(H), M, I, K, ldx, ldw, ldh, int(out_dtype), _vp(stream)))
+
+
+def tile_gemm_swiglu(X: torch.Tensor, Wgu: torch.Tensor, H: torch.Tensor | None = None, out_dtype=None,
+                     stream=None) -> torch.Tensor:
+    """H = silu(X @ Wgu[:, :I]) * (X @ Wgu[:, I:]) with I = Wgu.shape[1] // 2; X, Wgu bf16; H fp32, bf16 or f16."""
+    if X.dtype != torch.bfloat16 or Wgu.dtype != torch.bfloat16:
+        raise TypeError("X and Wgu must be torch.bfloat16")
+    M, K = X.shape
+    K2, N2 = Wgu.shape
+    if K != K2 or N2 % 2:
+        raise ValueError("Wgu must be (K, 2*I)")
+    inter = N2 // 2
+    if H is None:
+        dt = (torch.float32 if out_dtype in (OUT_F32, torch.float32)
+              else torch.float16 if out_dtype in (OUT_F16, torch.float16) else torch.bfloat16)
+        H = torch.empty((M, inter), dtype=dt, device=X.device)
+    if tuple(H.shape) != (M, inter):
+        raise TypeError("H must be (M, I)")
+    od = {torch.float32: OUT_F32, torch.bfloat16: OUT_BF16, torch.float16: OUT_F16}[H.dtype]
+    _check(load_library().tile_gemm_swiglu(_vp(X.data_ptr()), _vp(Wgu.data_ptr()), _vp(H.data_ptr()), M, inter, K,
+                                           _ld(X), _ld(Wgu), _ld(H), od, _vp(_stream_handle(stream))))
+    return H
 
 
 def tile_add_f32_raw(x: int, y: int, z: int, n: int, stream: int = 0) -> int:

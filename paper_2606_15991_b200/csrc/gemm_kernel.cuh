@@ -59,6 +59,7 @@ struct GemmParams {
     // draws the last of a tile's `split` tickets adds the slices in slice order (fixed order:
     // bitwise reproducible) and stores C.  split == 0: every unit is a whole tile.
     int32_t full_units, split, kps, total_units;
+    int32_t up_offset;          // SwiGLU epilogue: column of B where the `up` half starts (= N, the width of C)
     float* partials;            // [split tiles][split][CG][8 warps][units][8 chunks][32 lanes][4 floats]
     uint32_t* tickets;          // [split tiles][CG], zero between launches
 };
@@ -134,7 +135,11 @@ struct GemmSmem {
 
 // SPLIT = false: every unit is a whole tile (the split-K epilogue is not even compiled in: it costs
 // the hot epilogue registers); SPLIT = true: launches whose last wave is cut into K slices.
-template <int CG, int BN, int STAGES, int NACC, bool SPLIT>
+// EPI = 1 (needs NACC == 2): the SwiGLU epilogue of a fused gate/up projection.  B is K x 2N,
+// [gate | up]; accumulator slot 0 takes the tile's gate columns, slot 1 the same columns of `up`
+// (p.up_offset further right in B); the epilogue stores round_out(silu(gate) * up): the tile is
+// BM*CG x BN, and the 2N-wide intermediate never reaches memory.
+template <int CG, int BN, int STAGES, int NACC, bool SPLIT, int EPI = 0>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b,
                     const __grid_constant__ CUtensorMap tmap_c, const GemmParams p) {
@@ -142,7 +147,9 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
     static_assert(CG == 1 || CG == 2, "cta_group is 1 or 2");
     static_assert(BN == 128 || BN == 256, "accumulator width");
     static_assert(NACC == 1 || NACC == 2, "a tile is one or two accumulator slots wide");
-    constexpr int TILE_N = BN * NACC;
+    constexpr bool SWIGLU = (EPI == 1);
+    static_assert(!SWIGLU || (NACC == 2 && !SPLIT), "the SwiGLU epilogue pairs the two accumulator slots of a whole tile");
+    constexpr int TILE_N = SWIGLU ? BN : BN * NACC;   // width of the OUTPUT tile
     static_assert(L::TOTAL <= 232448, "exceeds 227 KB of shared memory");
 
     extern __shared__ uint8_t smem_raw[];
@@ -177,7 +184,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
         for (uint32_t a = 0; a < 2; ++a) {
             mbar_init(tmem_full_bar(a), 1);           // one tcgen05.commit
             // lane 0 of every epilogue warp of the pair that drains this slot
-            mbar_init(tmem_empty_bar(a), (NACC == 2 ? 4 : 8) * CG);
+            mbar_init(tmem_empty_bar(a), ((NACC == 2 && !SWIGLU) ? 4 : 8) * CG);
         }
         fence_mbar_init();
     }
@@ -206,6 +213,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
             // exist in every cluster's schedule, so every window counter there reaches the cluster count
             const uint32_t sync_limit = (uint32_t)p.sync_rounds * (uint32_t)p.num_k_tiles;
             uint32_t pos = 0, next_sync = 0;
+            const int slot_stride = SWIGLU ? p.up_offset : BN;   // B column distance between the two accumulator slots
             griddep_wait();   // A, B (and the lockstep counters) may be the previous kernel's output
             for (int u = first_tile; u < total_units; u += tile_stride) {
                 const GemmUnit un = gemm_unit<SPLIT>(p, u);
@@ -233,7 +241,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
 #pragma unroll
                             for (uint32_t b = 0; b < L::B_BOXES; ++b)
                                 tma_load_2d(sb + j * L::B_ACC_BYTES + b * L::B_BOX_BYTES, &tmap_b, full_bar(stage),
-                                            n0 + (int)j * BN + (int)b * 64, k0);
+                                            n0 + (int)j * slot_stride + (int)b * 64, k0);
                     } else {
                         // both CTAs' bytes are counted on the leader's barrier
                         const uint32_t lead_bar = map_to_cta(full_bar(stage), 0);
@@ -244,7 +252,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
 #pragma unroll
                             for (uint32_t b = 0; b < L::B_BOXES; ++b)
                                 tma_load_2d_cg2(sb + j * L::B_ACC_BYTES + b * L::B_BOX_BYTES, &tmap_b, lead_bar,
-                                                n0 + (int)j * BN + (int)b * 64, k0);
+                                                n0 + (int)j * slot_stride + (int)b * 64, k0);
                     }
                     if (++stage == STAGES) { stage = 0; phase ^= 1u; }
                 }
@@ -348,15 +356,21 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
             const uint32_t owner_val = ((uint32_t)t << 8) | (uint32_t)blockIdx.x;
             const uint32_t acc = (NACC == 2) ? half : (it & 1u);
             const uint32_t acc_phase = (NACC == 2) ? (it & 1u) : ((it >> 1) & 1u);
-            const uint32_t t_acc =
-                tmem_base + ((q * 32u) << 16) + acc * BN + ((NACC == 2) ? 0u : half * (uint32_t)WARP_COLS);
+            const uint32_t t_acc = SWIGLU ? tmem_base + ((q * 32u) << 16) + half * (uint32_t)WARP_COLS   // gate; up is BN further
+                                          : tmem_base + ((q * 32u) << 16) + acc * BN +
+                                                ((NACC == 2) ? 0u : half * (uint32_t)WARP_COLS);
             // units of this warp that intersect C (warp-uniform); the rest is never loaded or stored
             int units = 0;
             if (m0 < p.M && n_base < p.N) {
                 units = (p.N - n_base + 31) >> 5;
                 if (units > UNITS) units = UNITS;
             }
-            mbar_wait_sleep(tmem_full_bar(acc), acc_phase);
+            if constexpr (SWIGLU) {   // this warp reads the same columns of both slots
+                mbar_wait_sleep(tmem_full_bar(0), acc_phase);
+                mbar_wait_sleep(tmem_full_bar(1), acc_phase);
+            } else {
+                mbar_wait_sleep(tmem_full_bar(acc), acc_phase);
+            }
             tc_fence_after();
 
             // stage 16 words (64 B) of this thread's row as columns [n0, n0 + sub_cols) and send them
@@ -441,8 +455,16 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) {
-                    if constexpr (CG == 1) mbar_arrive(tmem_empty_bar(acc));
-                    else mbar_arrive_cluster(map_to_cta(tmem_empty_bar(acc), 0));
+                    if constexpr (SWIGLU) {
+                        if constexpr (CG == 1) { mbar_arrive(tmem_empty_bar(0)); mbar_arrive(tmem_empty_bar(1)); }
+                        else {
+                            mbar_arrive_cluster(map_to_cta(tmem_empty_bar(0), 0));
+                            mbar_arrive_cluster(map_to_cta(tmem_empty_bar(1), 0));
+                        }
+                    } else {
+                        if constexpr (CG == 1) mbar_arrive(tmem_empty_bar(acc));
+                        else mbar_arrive_cluster(map_to_cta(tmem_empty_bar(acc), 0));
+                    }
                 }
             };
 
@@ -497,6 +519,24 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
                         stage_unit(va, uu);
                     }
                 }
+                continue;
+            }
+            if constexpr (SWIGLU) {
+                // h = silu(g) * u on the fp32 accumulators: g / (1 + e^-g) with ex2.approx and a fast
+                // divide (relative error ~2^-21, far below the bf16/f16 output rounding)
+                for (int uu = 0; uu < units; ++uu) {
+                    tmem_ld_32x32(t_acc + (uint32_t)(uu * 32), va);
+                    tmem_ld_32x32(t_acc + (uint32_t)(BN + uu * 32), vb);
+                    tmem_ld_wait();
+                    if (uu + 1 == units) release_tmem();
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) {
+                        const float g = __uint_as_float(va[i]);
+                        va[i] = __float_as_uint(__fdividef(g, 1.0f + __expf(-g)) * __uint_as_float(vb[i]));
+                    }
+                    stage_unit(va, uu);
+                }
+                if (units == 0) release_tmem();
                 continue;
             }
             if (units > 0) tmem_ld_32x32(t_acc, va);

@@ -421,11 +421,11 @@ void plan_gemm(int64_t M, int64_t N, int64_t K, int in_dtype, int out_dtype, int
     gl->ctas = (int)units * gl->cfg.cg;
 }
 
-template <int CG, int BN, int STAGES, int NACC, bool SPLIT>
+template <int CG, int BN, int STAGES, int NACC, bool SPLIT, int EPI = 0>
 int launch_gemm_inst(const CUtensorMap& ta, const CUtensorMap& tb, const CUtensorMap& tc, const tg::GemmParams& p,
                      int ctas, cudaStream_t s, int dev) {
     using L = tg::GemmSmem<CG, BN, STAGES, NACC>;
-    auto kern = tg::gemm_tcgen05_kernel<CG, BN, STAGES, NACC, SPLIT>;
+    auto kern = tg::gemm_tcgen05_kernel<CG, BN, STAGES, NACC, SPLIT, EPI>;
     static bool configured[64] = {};
     if (!configured[dev]) {
         CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::TOTAL));
@@ -465,6 +465,34 @@ int launch_gemm(const GemmLaunch& gl, const CUtensorMap& ta, const CUtensorMap& 
 #undef TG_GEMM_CASE
     }
     return fail(TILE_GEMM_E_INTERNAL, "unknown GEMM config %d", gl.cfg.id);
+}
+
+// Lockstep producers: only where a launch is long enough for clusters to drift (several whole
+// tiles per cluster, long K loops); tuning key 6: bit 2 forces it on, bit 3 off, bits 8-15 = window.
+int setup_lockstep(GemmLaunch& gl, int dev, cudaStream_t s) {
+    int rc = TILE_GEMM_OK;
+    {
+        const int tune = g_tune[6].load();
+        const int clusters = gl.ctas / gl.cfg.cg;
+        // rounds in which every cluster owns a whole tile: lockstep covers exactly these
+        const int64_t rounds = gl.p.full_units / clusters;
+        bool on = rounds >= kLockstepMinTiles && gl.p.num_k_tiles >= kLockstepMinKTiles;
+        if (tune & 4) on = rounds >= 1 && gl.p.num_k_tiles >= 1;
+        if (tune & 8) on = false;
+        if (on) {
+            int window = (tune >> 8) & 255;
+            if (window <= 0) window = kLockstepWindow;
+            const int64_t windows = (rounds * gl.p.num_k_tiles + window - 1) / window + 1;
+            gl.p.sync_rounds = (int32_t)rounds;
+            uint32_t* sync = nullptr;
+            rc = sync_workspace_for(dev, s, (size_t)windows * 4, &sync);
+            if (rc) return rc;
+            CUDA_TRY(cudaMemsetAsync(sync, 0, (size_t)windows * 4, s));
+            gl.p.sync = sync;
+            gl.p.sync_window = window;
+        }
+    }
+    return rc;
 }
 
 int c_tensor_map(CUtensorMap* tc, void* C, int64_t M, int64_t N, int64_t ldc, int out_16) {
@@ -532,29 +560,8 @@ int run_gemm(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_
     } else {
         tc = ta;   // never dereferenced by the clipped st.global epilogue; must still be a valid map
     }
-    // lockstep producers: only where a launch is long enough for clusters to drift (several tiles
-    // per cluster, long K loops); tuning key 6: bit 2 forces it on, bit 3 off, bits 8-15 = window
-    {
-        const int tune = g_tune[6].load();
-        const int clusters = gl.ctas / gl.cfg.cg;
-        // rounds in which every cluster owns a whole tile: lockstep covers exactly these
-        const int64_t rounds = gl.p.full_units / clusters;
-        bool on = rounds >= kLockstepMinTiles && gl.p.num_k_tiles >= kLockstepMinKTiles;
-        if (tune & 4) on = rounds >= 1 && gl.p.num_k_tiles >= 1;
-        if (tune & 8) on = false;
-        if (on) {
-            int window = (tune >> 8) & 255;
-            if (window <= 0) window = kLockstepWindow;
-            const int64_t windows = (rounds * gl.p.num_k_tiles + window - 1) / window + 1;
-            gl.p.sync_rounds = (int32_t)rounds;
-            uint32_t* sync = nullptr;
-            rc = sync_workspace_for(dev, s, (size_t)windows * 4, &sync);
-            if (rc) return rc;
-            CUDA_TRY(cudaMemsetAsync(sync, 0, (size_t)windows * 4, s));
-            gl.p.sync = sync;
-            gl.p.sync_window = window;
-        }
-    }
+    rc = setup_lockstep(gl, dev, s);
+    if (rc) return rc;
     return launch_gemm(gl, ta, tb, tc, s, dev);
 }
 
@@ -821,6 +828,69 @@ int tile_gemm_typed(const void* A, const void* B, void* C, int64_t M, int64_t N,
 
 // tile_add_f32 launch shape (measured on B200 at n = 2^28)
 constexpr int kAddDefaultPerSm = 255, kAddDefaultUnroll = 1, kAddDefaultMode = 1;
+
+int tile_gemm_swiglu(const void* X, const void* Wgu, void* H, int64_t M, int64_t I, int64_t K, int64_t ldx,
+                     int64_t ldw, int64_t ldh, int out_dtype, void* stream) {
+    // the preconditions of tile_gemm on (X, Wgu[:, :I], H), then the ones the second half adds
+    Plan plan;
+    int rc = check_and_select(X, Wgu, H, M, I, K, ldx, ldw, ldh, TILE_GEMM_IN_BF16, out_dtype, &plan);
+    if (rc) return rc;
+    if (I > ((int64_t)INT32_MAX - 1024) / 2)
+        return fail(TILE_GEMM_E_OVERFLOW, "2*I = %lld columns of the fused weight overflow int32", (long long)(2 * I));
+    if (ldw < 2 * I) return fail(TILE_GEMM_E_LDB, "ldw=%lld < 2*I=%lld", (long long)ldw, (long long)(2 * I));
+    int64_t w_bytes = 0;
+    if (!span_bytes(K, 2 * I, ldw, 2, &w_bytes)) return fail(TILE_GEMM_E_OVERFLOW, "operand byte span overflows int64");
+    if (overlaps(H, plan.c_bytes, Wgu, w_bytes))
+        return fail(TILE_GEMM_E_ALIAS, "H [%p,+%lld) overlaps Wgu [%p,+%lld): the output must be exclusively owned", H,
+                    (long long)plan.c_bytes, Wgu, (long long)w_bytes);
+    if (plan.path == TILE_GEMM_PATH_NOOP) return TILE_GEMM_OK;
+    if (K > 0 && !(plan.a_tma && plan.b_tma))
+        return fail(TILE_GEMM_E_PATH,
+                    "tile_gemm_swiglu needs 16-byte aligned X and Wgu with ldx and ldw multiples of 8 (no repack path)");
+    if (K > 0 && I % 8 != 0)   // the up half is read through TMA boxes that start at column I: 16-byte granularity (measured)
+        return fail(TILE_GEMM_E_PATH, "tile_gemm_swiglu needs I (%lld) to be a multiple of 8", (long long)I);
+    int dev = 0, sms = 0;
+    rc = current_device(&dev, &sms);
+    if (rc) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (K == 0) return run_zero(H, M, I, ldh, plan.esize, s);   // silu(0) * 0 = 0
+    GemmLaunch gl;
+    gl.cfg = kConfigs[4];
+    tg::GemmParams& p = gl.p;
+    memset(&p, 0, sizeof p);
+    p.M = (int32_t)M; p.N = (int32_t)I; p.K = (int32_t)K;
+    p.tiles_m = (int32_t)((M + 255) / 256);
+    p.tiles_n = (int32_t)((I + 255) / 256);            // the output tile is 256 x 256: gate and up slots side by side in TMEM
+    int gm = g_tune[1].load();
+    if (gm <= 0) gm = 8;
+    p.group_m = gm < p.tiles_m ? gm : p.tiles_m;
+    p.num_k_tiles = (int32_t)((K + tg::GEMM_BK - 1) / tg::GEMM_BK);
+    p.out_16 = out_dtype != TILE_GEMM_OUT_F32;
+    p.out_f16 = out_dtype == TILE_GEMM_OUT_F16;
+    p.up_offset = (int32_t)I;
+    const int64_t tiles = (int64_t)p.tiles_m * p.tiles_n;
+    p.full_units = p.total_units = (int32_t)tiles;
+    p.kps = p.num_k_tiles;
+    const int64_t clusters = tiles < sms / 2 ? tiles : sms / 2;
+    gl.ctas = (int)clusters * 2;
+    p.tma_store = plan.c_tma ? 1 : 0;
+    p.C = H;
+    p.ldc = ldh;
+    CUtensorMap ta, tb, tc;
+    rc = get_tensor_map(&ta, X, 2, false, (uint64_t)K, (uint64_t)M, (uint64_t)ldx * 2, 64u, 128u, 128);
+    if (rc) return rc;
+    rc = get_tensor_map(&tb, Wgu, 2, false, (uint64_t)(2 * I), (uint64_t)K, (uint64_t)ldw * 2, 64u, 64u, 128);
+    if (rc) return rc;
+    if (plan.c_tma) {
+        rc = c_tensor_map(&tc, H, M, I, ldh, p.out_16);
+        if (rc) return rc;
+    } else {
+        tc = ta;
+    }
+    rc = setup_lockstep(gl, dev, s);
+    if (rc) return rc;
+    return launch_gemm_inst<2, 256, 4, 2, false, 1>(ta, tb, tc, p, gl.ctas, s, dev);
+}
 
 int tile_add_f32(const float* x, const float* y, float* z, int64_t n, void* stream) {
     if (n < 0) return fail(TILE_GEMM_E_EXTENT, "negative extent: n=%lld", (long long)n);

@@ -295,3 +295,118 @@ def test_record_preconditions():
     assert lib.tile_gemm_record_begin(None) == tg.E_PATH
     assert lib.tile_gemm_replay(None, None) == tg.E_NULL
     assert lib.tile_gemm_record_free(None) == tg.E_OK
+
+
+# ------------------------------------------------------------------ SwiGLU epilogue
+def swiglu_gate(got, H, G, U, Sg, Su, K, out, what):
+    """|err| <= output rounding + the two accumulation errors pushed through h = silu(g) * u
+    (|silu'| <= 1.1) + 2^-18 |H| for the fast exp / divide."""
+    eg = 2.0 * K * 2.0 ** -24 * Sg
+    eu = 2.0 * K * 2.0 ** -24 * Su
+    rnd = {"f32": 2.0 ** -23 * np.abs(H), "bf16": 2.0 ** -8 * np.abs(H), "f16": 2.0 ** -11 * np.abs(H) + 2.0 ** -24}[out]
+    tol = rnd + 1.1 * np.abs(U) * eg + np.abs(oracle.silu(G)) * eu + 2.0 ** -18 * np.abs(H) + 1e-30
+    err = np.abs(got - H)
+    assert not np.isnan(got).any(), f"{what}: NaN"
+    bad = err > tol
+    assert not bad.any(), f"{what}: {int(bad.sum())} elements out of tolerance, first {np.argwhere(bad)[:4].tolist()}, max ratio {np.max(err / tol):.3g}"
+
+
+def run_swiglu(x_bits, w_bits, out, pad=0):
+    M, K = x_bits.shape
+    inter = w_bits.shape[1] // 2
+    ldw = (2 * inter + 7) // 8 * 8 + pad
+    ldx = (K + 7) // 8 * 8
+    X = torch.zeros((M, ldx), dtype=torch.bfloat16, device=DEV)[:, :K]
+    W = torch.full((K, ldw), float("nan"), dtype=torch.bfloat16, device=DEV)[:, :2 * inter]
+    X.copy_(wl.bits_to_torch(x_bits, DEV))
+    W.copy_(wl.bits_to_torch(w_bits, DEV))
+    odt = {"f32": torch.float32, "bf16": torch.bfloat16, "f16": torch.float16}[out]
+    Hfull = torch.full((M + 2, inter + 8 + pad), float("nan"), dtype=odt, device=DEV)
+    H = Hfull[1:M + 1, :inter]
+    tg.tile_gemm_swiglu(X, W, H)
+    torch.cuda.synchronize()
+    host = Hfull.cpu()
+    assert torch.isnan(host[0]).all() and torch.isnan(host[-1]).all() and torch.isnan(host[:, inter:]).all(), "written outside H"
+    h = host[1:M + 1, :inter].contiguous()
+    if out == "f32":
+        return h.numpy().astype(np.float64)
+    bits = h.view(torch.int16).numpy().view(np.uint16)
+    return oracle.f16_decode(bits) if out == "f16" else oracle.bf16_decode(bits)
+
+
+@pytest.mark.parametrize("out", ["f32", "bf16", "f16"])
+@pytest.mark.parametrize("shape", [(1023, 1544, 769), (300, 256, 64), (8, 1000, 4100), (513, 520, 1030)])
+def test_swiglu_full_oracle_ragged(out, shape):
+    M, inter, K = shape
+    x, w = wl.make_inputs_custom(M, 2 * inter, K, sigma_b=2.0 * K ** -0.5, seed=51)
+    H, G, U, Sg, Su = oracle.swiglu_gemm(x, w)
+    got = run_swiglu(x, w, out, pad=8 if M == 513 else 0)
+    swiglu_gate(got, H, G, U, Sg, Su, K, out, f"swiglu {shape} {out}")
+
+
+def test_swiglu_integer_inputs_and_special_halves():
+    M, inter, K = 260, 296, 200
+    x, w = wl.make_inputs_custom(M, 2 * inter, K, dist="int4", seed=52)
+    H, G, U, Sg, Su = oracle.swiglu_gemm(x, w)                       # G, U exact integers up to 3200
+    got = run_swiglu(x, w, "f32")
+    assert np.all(np.abs(got - H) <= 2.0 ** -18 * np.abs(H) + 1e-30)
+    assert np.all(got[(G == 0) | (U == 0)] == 0)                      # silu(0) * u = 0 and g * 0 = 0, exactly
+    assert np.all(got[G < -110] == 0) and not np.isnan(got).any()     # e^110 overflows fp32: the left tail is a clean zero
+    wz = w.copy()
+    wz[:, :inter] = 0                                                 # gate weights zero -> H = 0 everywhere
+    assert np.all(run_swiglu(x, wz, "bf16") == 0)
+    ws = np.concatenate([w[:, inter:], w[:, :inter]], axis=1)         # swapped halves: silu(U) * G, not silu(G) * U
+    Hs = oracle.swiglu_gemm(x, ws)[0]
+    gots = run_swiglu(x, ws, "f32")
+    assert np.all(np.abs(gots - Hs) <= 2.0 ** -18 * np.abs(Hs) + 1e-30)
+    assert not np.allclose(Hs, H)
+
+
+def test_swiglu_matches_two_gemms_of_the_same_library():
+    """The fused kernel's accumulators are the ones tile_gemm produces for the two halves: H must
+    equal silu(G32) * U32 evaluated on those fp32 results to fast-math accuracy."""
+    M, inter, K = 512, 768, 2048
+    x, w = wl.make_inputs_custom(M, 2 * inter, K, sigma_b=2.0 * K ** -0.5, seed=53)
+    X, W = wl.bits_to_torch(x, DEV), wl.bits_to_torch(w, DEV)
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMM_CONFIG, 4)
+    G32 = tg.tile_gemm(X, W[:, :inter], out_dtype=tg.OUT_F32).double()
+    U32 = tg.tile_gemm(X, W[:, inter:], out_dtype=tg.OUT_F32).double()
+    H = tg.tile_gemm_swiglu(X, W, out_dtype=tg.OUT_F32).double()
+    ref = G32 / (1 + torch.exp(-G32)) * U32
+    assert torch.all((H - ref).abs() <= 2.0 ** -18 * ref.abs() + 1e-30)
+
+
+def test_swiglu_gate_up_shape_sampled():
+    """BASELINE.json's fused gate/up projection (M=4096, K=5120, 2I=51200), sampled against the oracle."""
+    M, K, inter = 4096, 5120, 25600
+    g = torch.Generator(device=DEV)
+    g.manual_seed(54)
+    X = torch.empty((M, K), dtype=torch.bfloat16, device=DEV).normal_(0, 1, generator=g)
+    W = torch.empty((K, 2 * inter), dtype=torch.bfloat16, device=DEV).normal_(0, 0.02, generator=g)
+    H = tg.tile_gemm_swiglu(X, W, out_dtype=tg.OUT_BF16)
+    rows, cols = wl.uniform_samples(M, inter, 2048, seed=54)
+    xb, wb = wl.torch_to_bits(X), wl.torch_to_bits(W)
+    Gs, Sg = oracle.gemm_sampled(xb, wb, rows, cols)
+    Us, Su = oracle.gemm_sampled(xb, wb, rows, cols + inter)
+    got = oracle.bf16_decode(wl.torch_to_bits(H)[rows, cols])
+    swiglu_gate(got, oracle.silu(Gs) * Us, Gs, Us, Sg, Su, K, "bf16", "swiglu gate_up sampled")
+    assert torch.isfinite(H.float()).all()
+
+
+def test_swiglu_preconditions():
+    X = torch.zeros((8, 64), dtype=torch.bfloat16, device=DEV)
+    W = torch.zeros((64, 32), dtype=torch.bfloat16, device=DEV)
+    H = torch.full((8, 16), 3.0, dtype=torch.float32, device=DEV)
+    a = (X.data_ptr(), W.data_ptr(), H.data_ptr())
+    assert tg.tile_gemm_swiglu_raw(*a, 8, 16, 64, 64, 31, 16, tg.OUT_F32) == tg.E_LDB         # ldw < 2I
+    assert tg.tile_gemm_swiglu_raw(*a, 8, 16, 64, 63, 32, 16, tg.OUT_F32) == tg.E_LDA
+    assert tg.tile_gemm_swiglu_raw(*a, 8, 16, 64, 64, 32, 15, tg.OUT_F32) == tg.E_LDC
+    assert tg.tile_gemm_swiglu_raw(*a, 8, 16, 64, 64, 32, 16, 5) == tg.E_DTYPE
+    assert tg.tile_gemm_swiglu_raw(X.data_ptr() + 2, W.data_ptr(), H.data_ptr(), 8, 16, 56, 64, 32, 16, tg.OUT_F32) == tg.E_PATH
+    assert tg.tile_gemm_swiglu_raw(X.data_ptr(), W.data_ptr(), W.data_ptr() + 32, 8, 8, 64, 64, 32, 16, tg.OUT_BF16) == tg.E_ALIAS
+    assert tg.tile_gemm_swiglu_raw(*a, 8, 12, 64, 64, 32, 16, tg.OUT_F32) == tg.E_PATH        # I not a multiple of 8
+    torch.cuda.synchronize()
+    assert torch.all(H == 3.0)
+    assert tg.tile_gemm_swiglu_raw(*a, 8, 16, 0, 64, 32, 16, tg.OUT_F32) == tg.E_OK            # K == 0 -> zeros
+    torch.cuda.synchronize()
+    assert torch.all(H == 0.0)
