@@ -553,6 +553,29 @@ def run_cuda(args):
         if rank == 0:
             line["replay"] = bench_launch_overhead(tg, torch)
         tdist.barrier()
+        # fused gate/up + SwiGLU epilogue on the cfg4 gate_up shape vs the plain GEMM that writes [gate | up]
+        c = wl.CFG4[2]
+        dev = torch.device("cuda", torch.cuda.current_device())
+        gg = torch.Generator(device=dev)
+        gg.manual_seed(55)
+        Xs = [torch.empty((c.M, c.K), dtype=torch.bfloat16, device=dev).normal_(0, 1, generator=gg) for _ in range(2)]
+        Wsw = [torch.empty((c.K, c.N), dtype=torch.bfloat16, device=dev).normal_(0, 0.02, generator=gg) for _ in range(2)]
+        Hs = torch.empty((c.M, c.N // 2), dtype=torch.bfloat16, device=dev)
+        Cp = torch.empty((c.M, c.N), dtype=torch.bfloat16, device=dev)
+        reps = max(5, args.steps // 8)
+        for i in range(3):
+            tg.tile_gemm_swiglu(Xs[i % 2], Wsw[i % 2], Hs)
+            tg.tile_gemm(Xs[i % 2], Wsw[i % 2], Cp)
+        ms_f = tdist.max_over_ranks(time_region(lambda i: tg.tile_gemm_swiglu(Xs[i % 2], Wsw[i % 2], Hs), reps,
+                                                torch.cuda.synchronize, tdist.barrier)) / reps
+        ms_p = tdist.max_over_ranks(time_region(lambda i: tg.tile_gemm(Xs[i % 2], Wsw[i % 2], Cp), reps,
+                                                torch.cuda.synchronize, tdist.barrier)) / reps
+        fl = 2.0 * c.M * c.N * c.K
+        line["swiglu"] = {"shape": f"M={c.M} K={c.K} 2I={c.N}", "fused_ms": ms_f, "fused_tflops": fl / (ms_f * 1e-3) / 1e12,
+                          "plain_gate_up_gemm_ms": ms_p, "plain_tflops": fl / (ms_p * 1e-3) / 1e12,
+                          "c_bytes_fused": c.M * c.N, "c_bytes_plain": 2 * c.M * c.N}
+        del Xs, Wsw, Hs, Cp
+        torch.cuda.empty_cache()
         # skinny M through the GEMM's K slices
         line["skinny_m"] = bench_skinny(tg, wl, torch, [2, 4, 8, 16, 32, 64], tdist)
         # the paper's size sweep in f16 and bf16

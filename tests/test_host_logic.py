@@ -188,3 +188,17 @@ def test_record_entries_reject_bad_handles_without_a_device():
     assert lib.tile_gemm_record_free(None) == tg.E_OK
     if not torch.cuda.is_available():
         assert lib.tile_gemm_record_begin(None) == tg.E_DEVICE
+
+
+def test_swiglu_preconditions_on_the_host():
+    a = (A0, B0, C0)
+    assert tg.tile_gemm_swiglu_raw(*a, 8, 16, 64, 64, 31, 16, tg.OUT_F32) == tg.E_LDB          # ldw < 2I
+    assert tg.tile_gemm_swiglu_raw(*a, 8, 16, 64, 63, 32, 16, tg.OUT_F32) == tg.E_LDA
+    assert tg.tile_gemm_swiglu_raw(*a, 8, 16, 64, 64, 32, 15, tg.OUT_F32) == tg.E_LDC
+    assert tg.tile_gemm_swiglu_raw(*a, 8, 16, 64, 64, 32, 16, 9) == tg.E_DTYPE
+    assert tg.tile_gemm_swiglu_raw(*a, 8, 12, 64, 64, 32, 16, tg.OUT_F32) == tg.E_PATH         # I % 8 != 0
+    assert tg.tile_gemm_swiglu_raw(A0 + 2, B0, C0, 8, 16, 64, 64, 32, 16, tg.OUT_F32) == tg.E_PATH   # X not TMA-addressable
+    assert tg.tile_gemm_swiglu_raw(A0, B0, B0 + 64 * 2 * 16 + 32, 8, 16, 64, 64, 64, 16, tg.OUT_BF16) == tg.E_ALIAS  # H inside the up half
+    assert tg.tile_gemm_swiglu_raw(*a, 0, 16, 64, 64, 32, 16, tg.OUT_F32) == tg.E_OK           # M == 0: no-op
+    if not torch.cuda.is_available():
+        assert tg.tile_gemm_swiglu_raw(*a, 8, 16, 64, 64, 32, 16, tg.OUT_F32) == tg.E_DEVICE
