@@ -347,7 +347,7 @@ GemmConfig choose_config(int64_t M, int64_t N, int sms) {
 }
 
 // lockstep defaults: on from kLockstepMinTiles tiles per cluster and kLockstepMinKTiles k-tiles
-constexpr int kLockstepMinTiles = 2, kLockstepMinKTiles = 128, kLockstepWindow = 32;
+constexpr int kLockstepMinTiles = 2, kLockstepMinKTiles = 256, kLockstepWindow = 32;
 
 // split-K of the last wave: at most kGemmMaxSplit slices of at least kGemmMinSliceKTiles k-tiles each
 constexpr int kGemmMaxSplit = 16, kGemmMinSliceKTiles = 4;
