@@ -59,6 +59,8 @@ struct GemmParams {
     // draws the last of a tile's `split` tickets adds the slices in slice order (fixed order:
     // bitwise reproducible) and stores C.  split == 0: every unit is a whole tile.
     int32_t full_units, split, kps, total_units;
+    int32_t a_rows;             // rows of the A box (16, 32, 64 or 128): for M <= 64 the rows past it are never loaded; the
+                                // MMA reads whatever the stage holds there and those output rows are clipped
     int32_t up_offset;          // SwiGLU epilogue: column of B where the `up` half starts (= N, the width of C)
     float* partials;            // [split tiles][split][CG][8 warps][units][8 chunks][32 lanes][4 floats]
     uint32_t* tickets;          // [split tiles][CG], zero between launches
@@ -213,6 +215,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
             // exist in every cluster's schedule, so every window counter there reaches the cluster count
             const uint32_t sync_limit = (uint32_t)p.sync_rounds * (uint32_t)p.num_k_tiles;
             uint32_t pos = 0, next_sync = 0;
+            const uint32_t stage_tx = (uint32_t)p.a_rows * (GEMM_BK * 2) + L::B_BYTES;   // bytes one CTA's boxes deliver per stage
             const int slot_stride = SWIGLU ? p.up_offset : BN;   // B column distance between the two accumulator slots
             griddep_wait();   // A, B (and the lockstep counters) may be the previous kernel's output
             for (int u = first_tile; u < total_units; u += tile_stride) {
@@ -234,7 +237,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
                     const uint32_t sb = sa + L::A_BYTES;
                     const int k0 = kt * GEMM_BK;
                     if constexpr (CG == 1) {
-                        mbar_arrive_expect_tx(full_bar(stage), L::STAGE_BYTES);
+                        mbar_arrive_expect_tx(full_bar(stage), stage_tx);
                         tma_load_2d(sa, &tmap_a, full_bar(stage), k0, m0);
 #pragma unroll
                         for (uint32_t j = 0; j < (uint32_t)NACC; ++j)
@@ -245,7 +248,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
                     } else {
                         // both CTAs' bytes are counted on the leader's barrier
                         const uint32_t lead_bar = map_to_cta(full_bar(stage), 0);
-                        if (rank == 0) mbar_arrive_expect_tx(full_bar(stage), 2 * L::STAGE_BYTES);
+                        if (rank == 0) mbar_arrive_expect_tx(full_bar(stage), 2 * stage_tx);
                         tma_load_2d_cg2(sa, &tmap_a, lead_bar, k0, m0);
 #pragma unroll
                         for (uint32_t j = 0; j < (uint32_t)NACC; ++j)

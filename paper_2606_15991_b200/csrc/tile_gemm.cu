@@ -550,7 +550,11 @@ int run_gemm(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_
     gl.p.C = C;
     gl.p.ldc = ldc;
     CUtensorMap ta, tb, tc;
-    int rc = get_tensor_map(&ta, Ap, 2, false, (uint64_t)K, (uint64_t)M, (uint64_t)lda * 2, 64u, 128u, 128);
+    // skinny M: an A box only as tall as M needs (measured: 13 us of 36 at M <= 12, K = 5120, where the
+    // 128-row box is almost all zero fill)
+    gl.p.a_rows = M <= 16 ? 16 : M <= 32 ? 32 : M <= 64 ? 64 : 128;
+    if (g_tune[6].load() & 32) gl.p.a_rows = 128;   // tuning key 6 bit 5: always the full box
+    int rc = get_tensor_map(&ta, Ap, 2, false, (uint64_t)K, (uint64_t)M, (uint64_t)lda * 2, 64u, (uint32_t)gl.p.a_rows, 128);
     if (rc) return rc;
     rc = get_tensor_map(&tb, Bp, 2, false, (uint64_t)N, (uint64_t)K, (uint64_t)ldb * 2, 64u, 64u, 128);
     if (rc) return rc;
@@ -877,6 +881,7 @@ int tile_gemm_swiglu(const void* X, const void* Wgu, void* H, int64_t M, int64_t
     p.C = H;
     p.ldc = ldh;
     CUtensorMap ta, tb, tc;
+    p.a_rows = 128;
     rc = get_tensor_map(&ta, X, 2, false, (uint64_t)K, (uint64_t)M, (uint64_t)ldx * 2, 64u, 128u, 128);
     if (rc) return rc;
     rc = get_tensor_map(&tb, Wgu, 2, false, (uint64_t)(2 * I), (uint64_t)K, (uint64_t)ldw * 2, 64u, 64u, 128);
