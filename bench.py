@@ -360,6 +360,20 @@ def bench_launch_overhead(tg, torch, n_ops=1000, elems=2048):
         s.synchronize()
         best = min(best, time.perf_counter() - t0)
     out["stream_launch_us_per_op"] = best / n_ops * 1e6
+    # the same chain through the bare C entry (arguments marshalled once): what a C caller pays
+    import ctypes
+    lib = tg.load_library()
+    vp = ctypes.c_void_p
+    pre = [(vp(za.data_ptr()), vp(y.data_ptr()), vp(zb.data_ptr()), elems, vp(s.cuda_stream)),
+           (vp(zb.data_ptr()), vp(y.data_ptr()), vp(za.data_ptr()), elems, vp(s.cuda_stream))]
+    best = 1e30
+    for _ in range(5):
+        t0 = time.perf_counter()
+        for i in range(n_ops):
+            lib.tile_add_f32(*pre[i & 1])
+        s.synchronize()
+        best = min(best, time.perf_counter() - t0)
+    out["stream_launch_us_per_op_c_abi"] = best / n_ops * 1e6
     tg.tile_gemm_record_begin(s)
     chain()
     step = tg.tile_gemm_record_end(s)
@@ -444,10 +458,30 @@ def bench_sweep(tg, torch, sizes, tdist):
             e1.record()
             torch.cuda.synchronize()
             b2b = e0.elapsed_time(e1) / reps
+            # the same launches as ONE recorded step: no host in the loop (a Python launch costs ~9 us,
+            # the C entry ~5 us, a 1024^3 GEMM ~6 us of GPU time -- the loop above is host-bound there)
+            rs = torch.cuda.Stream()
+            for i in range(min(reps, sets)):
+                tg.tile_gemm(*bufs[i % sets], stream=rs)
+            rs.synchronize()
+            tg.tile_gemm_record_begin(rs)
+            for i in range(reps):
+                tg.tile_gemm(*bufs[i % sets], stream=rs)
+            step = tg.tile_gemm_record_end(rs)
+            step.replay(rs)
+            rs.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(rs)
+            step.replay(rs)
+            e1.record(rs)
+            rs.synchronize()
+            rep_ms = e0.elapsed_time(e1) / reps
+            step.free()
             med = float(np.median(ts))
             fl = 2.0 * n ** 3
             rows[str(n)] = {"us_median": med * 1e3, "tflops_median": fl / (med * 1e-3) / 1e12,
                             "us_back_to_back": b2b * 1e3, "tflops_back_to_back": fl / (b2b * 1e-3) / 1e12,
+                            "us_recorded_replay": rep_ms * 1e3, "tflops_recorded_replay": fl / (rep_ms * 1e-3) / 1e12,
                             "tile_config": tg.tile_gemm_query_config(n, n, n, tg.OUT_BF16)["config"],
                             "operand_sets": sets}
             del bufs
