@@ -526,7 +526,7 @@ def run_cuda(args):
                      "peak_source": f"{peaks['source']} cuBLAS bf16 burst (MEASURED_PEAKS.json)",
                      "frac_of_sustained": per_gpu / peaks["bf16_tflops_sustained"],
                      "frac_of_nominal_2250": per_gpu / 2250.0,
-                     "kernel": "gemm_tcgen05_kernel<2,256,4,2,false>", "algorithmic_flops_per_launch": flops},
+                     "kernel": "gemm_tcgen05_kernel<2,256,4,2,false,0>", "algorithmic_flops_per_launch": flops},
     }
     del bufs
     torch.cuda.empty_cache()

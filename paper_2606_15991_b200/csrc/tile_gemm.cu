@@ -438,14 +438,21 @@ int launch_gemm_inst(const CUtensorMap& ta, const CUtensorMap& tb, const CUtenso
     cfg.dynamicSmemBytes = L::TOTAL;
     cfg.stream = s;
     cudaLaunchAttribute attr[2];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = CG;
-    attr[0].val.clusterDim.y = 1;
-    attr[0].val.clusterDim.z = 1;
-    attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[1].val.programmaticStreamSerializationAllowed = 1;
+    int na = 0;
+    if (CG == 2) {   // a 1-CTA "cluster" attribute would still take the driver's cluster launch path
+        attr[na].id = cudaLaunchAttributeClusterDimension;
+        attr[na].val.clusterDim.x = CG;
+        attr[na].val.clusterDim.y = 1;
+        attr[na].val.clusterDim.z = 1;
+        ++na;
+    }
+    if ((g_tune[6].load() & 1) == 0) {   // tuning key 6 bit 0: no programmatic dependent launch
+        attr[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[na].val.programmaticStreamSerializationAllowed = 1;
+        ++na;
+    }
     cfg.attrs = attr;
-    cfg.numAttrs = (g_tune[6].load() & 1) ? 1 : 2;   // tuning key 6 bit 0: no programmatic dependent launch
+    cfg.numAttrs = na;
     CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, ta, tb, tc, p));
     g_launches.fetch_add(1);
     return TILE_GEMM_OK;
