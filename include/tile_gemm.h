@@ -216,7 +216,12 @@ int tile_gemm_select(int64_t M, int64_t N, int64_t K,
  * End-to-end convenience entry on HOST buffers (pageable or pinned): copies A
  * and B to the device, runs tile_gemm, copies C[0..M) x [0..N) back (row pitch
  * ldc) and synchronises before returning.  Device staging buffers are grow-only
- * and owned by the library.  This is the call bench.py's `e2e` figure times.
+ * and owned by the library.  For M >= 2048 the rows of A go up in 1024-row chunks
+ * on one stream, each chunk's GEMM runs on a second stream as soon as its rows and
+ * all of B have landed, and its rows of C return on a third while the next chunk
+ * is still coming in (PCIe is full duplex); results are bit-identical to the
+ * one-shot order.  Pinned host memory is needed for the copies to overlap.  This
+ * is the call bench.py's `e2e` figure times.
  */
 int tile_gemm_host(const void* A_host, const void* B_host, void* C_host,
                    int64_t M, int64_t N, int64_t K,
@@ -254,7 +259,8 @@ int tile_gemm_query_config(int64_t M, int64_t N, int64_t K, int out_dtype, int32
  * {columns per CTA, rows per stage, stages, CTAs per SM}, table kGemvShapes in
  * csrc/tile_gemm.cu), 6 = bit 0 disables programmatic dependent launch, bit 1 makes
  * kernel 4 read x with global loads instead of through its TMA ring; bit 2 forces the GEMM's
- * lockstep producers on, bit 3 off, bits 8-15 their window in k-tiles (0 = 32); key 3 also
+ * lockstep producers on, bit 3 off, bits 8-15 their window in k-tiles (0 = 32), bit 5 = full 128-row A
+ * box even for skinny M, bit 6 = tile_gemm_host in one shot instead of pipelined chunks; key 3 also
  * overrides kernel 4's split, 7 = tile_add_f32 launch shape
  * (bits 0-3 vectors per thread in {1,2,4,8}, bits 4-11 CTAs per SM with 255 = one tile per
  * CTA, bits 12-15 access mode: 1/2 = 128-bit with/without streaming hints, 3/4 = 256-bit

@@ -16,6 +16,7 @@
 #include <cstring>
 #include <mutex>
 #include <unordered_map>
+#include <vector>
 
 #include "add_kernel.cuh"
 #include "aux_kernels.cuh"
@@ -246,7 +247,10 @@ struct Buf {
 };
 std::unordered_map<uint64_t, Buf> g_ws;   // (device, stream) -> repack workspace
 Buf g_stage[3];                            // tile_gemm_host staging (A, B, C)
-cudaStream_t g_host_stream = nullptr;
+cudaStream_t g_host_stream = nullptr;       // tile_gemm_host: copy-in (and everything, when not pipelined)
+cudaStream_t g_host_compute = nullptr;      // pipelined tile_gemm_host: the GEMMs
+cudaStream_t g_host_out = nullptr;          // pipelined tile_gemm_host: copy-out
+std::vector<cudaEvent_t> g_host_events;
 
 int grow(Buf& b, size_t need) {
     if (b.n >= need) return TILE_GEMM_OK;
@@ -1026,6 +1030,8 @@ int tile_gemm_record_free(void* step) {
     return TILE_GEMM_OK;
 }
 
+constexpr int64_t kHostChunkRows = 1024;
+
 int tile_gemm_host(const void* A_host, const void* B_host, void* C_host, int64_t M, int64_t N, int64_t K,
                    int64_t lda, int64_t ldb, int64_t ldc, int out_dtype) {
     Plan plan;
@@ -1043,6 +1049,47 @@ int tile_gemm_host(const void* A_host, const void* B_host, void* C_host, int64_t
         if ((rc = grow(g_stage[2], (size_t)plan.c_bytes + 16))) return rc;
     }
     cudaStream_t s = g_host_stream;
+    // Large M: rows of A go up in chunks, each chunk's GEMM starts as soon as its rows (and all of B)
+    // have landed, and its rows of C go back while the next chunk is still coming in.  PCIe is full
+    // duplex, so the call costs about max(H2D, D2H) instead of H2D + GEMM + D2H.  The per-element
+    // arithmetic is the same as in one call (same tiles along N and K; no K slicing at these sizes).
+    const int64_t chunk = kHostChunkRows;
+    if (K > 0 && M >= 2 * chunk && (g_tune[6].load() & 64) == 0) {   // tuning key 6 bit 6: one shot
+        const int64_t nchunks = (M + chunk - 1) / chunk;
+        {
+            std::lock_guard<std::mutex> lk(g_mu);
+            if (!g_host_compute) CUDA_TRY(cudaStreamCreateWithFlags(&g_host_compute, cudaStreamNonBlocking));
+            if (!g_host_out) CUDA_TRY(cudaStreamCreateWithFlags(&g_host_out, cudaStreamNonBlocking));
+            while ((int64_t)g_host_events.size() < 2 * nchunks + 1) {
+                cudaEvent_t e;
+                CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+                g_host_events.push_back(e);
+            }
+        }
+        const char* Ah = (const char*)A_host;
+        char* Ch = (char*)C_host;
+        char* Ad = (char*)g_stage[0].p;
+        char* Cd = (char*)g_stage[2].p;
+        CUDA_TRY(cudaMemcpyAsync(g_stage[1].p, B_host, (size_t)plan.b_bytes, cudaMemcpyHostToDevice, s));
+        for (int64_t i = 0; i < nchunks; ++i) {
+            const int64_t r0 = i * chunk, rows = (M - r0) < chunk ? (M - r0) : chunk;
+            const size_t a_off = (size_t)r0 * lda * 2, a_len = ((size_t)(rows - 1) * lda + K) * 2;
+            CUDA_TRY(cudaMemcpyAsync(Ad + a_off, Ah + a_off, a_len, cudaMemcpyHostToDevice, s));
+            CUDA_TRY(cudaEventRecord(g_host_events[2 * i], s));
+            CUDA_TRY(cudaStreamWaitEvent(g_host_compute, g_host_events[2 * i], 0));
+            rc = tile_gemm(Ad + a_off, g_stage[1].p, Cd + (size_t)r0 * ldc * plan.esize, rows, N, K, lda, ldb, ldc, out_dtype,
+                           (void*)g_host_compute);
+            if (rc) { cudaDeviceSynchronize(); return rc; }
+            CUDA_TRY(cudaEventRecord(g_host_events[2 * i + 1], g_host_compute));
+            CUDA_TRY(cudaStreamWaitEvent(g_host_out, g_host_events[2 * i + 1], 0));
+            CUDA_TRY(cudaMemcpy2DAsync(Ch + (size_t)r0 * ldc * plan.esize, (size_t)ldc * plan.esize,
+                                       Cd + (size_t)r0 * ldc * plan.esize, (size_t)ldc * plan.esize,
+                                       (size_t)N * plan.esize, (size_t)rows, cudaMemcpyDeviceToHost, g_host_out));
+        }
+        CUDA_TRY(cudaStreamSynchronize(g_host_out));
+        CUDA_TRY(cudaStreamSynchronize(s));
+        return TILE_GEMM_OK;
+    }
     if (plan.a_bytes) CUDA_TRY(cudaMemcpyAsync(g_stage[0].p, A_host, (size_t)plan.a_bytes, cudaMemcpyHostToDevice, s));
     if (plan.b_bytes) CUDA_TRY(cudaMemcpyAsync(g_stage[1].p, B_host, (size_t)plan.b_bytes, cudaMemcpyHostToDevice, s));
     rc = tile_gemm(g_stage[0].p, g_stage[1].p, g_stage[2].p, M, N, K, lda, ldb, ldc, out_dtype, (void*)s);
@@ -1136,6 +1183,10 @@ int tile_gemm_shutdown(void) {
         b = Buf();
     }
     if (g_host_stream) { cudaStreamDestroy(g_host_stream); g_host_stream = nullptr; }
+    if (g_host_compute) { cudaStreamDestroy(g_host_compute); g_host_compute = nullptr; }
+    if (g_host_out) { cudaStreamDestroy(g_host_out); g_host_out = nullptr; }
+    for (cudaEvent_t e : g_host_events) cudaEventDestroy(e);
+    g_host_events.clear();
     g_maps.clear();
     return TILE_GEMM_OK;
 }

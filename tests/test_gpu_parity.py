@@ -421,6 +421,32 @@ def test_host_entry_matches_oracle():
     check_close(oracle.bf16_decode(y), ref, S, 1024, "bf16", "host entry gemv")
 
 
+@pytest.mark.parametrize("out", ["f32", "bf16"])
+def test_host_entry_pipelined_chunks(out):
+    """M >= 2048 goes up in 1024-row chunks with copy-in, GEMM and copy-out overlapped: same bits as one
+    device call (integers: exact against the oracle), padded lda / ldc honoured, host padding untouched."""
+    M, N, K = 2304 + 77, 520, 300                      # three chunks, the last one ragged
+    a, b = wl.make_inputs_custom(M, N, K, "int4", seed=14)
+    ref, _ = oracle.gemm(a, b)
+    apad = np.full((M, K + 4), 0x7FC0, np.uint16)       # NaN padding columns in A
+    apad[:, :K] = a
+    if out == "f32":
+        C = np.full((M, N + 8), np.float32(-77.0))
+        tg.tile_gemm_host(apad[:, :K], b, C[:, :N])
+        check_bit_exact(C[:, :N], ref, "pipelined host entry")
+        assert np.all(C[:, N:] == -77.0)
+    else:
+        C = np.full((M, N + 8), 0x7FD5, np.uint16)
+        tg.tile_gemm_host(apad[:, :K], b, C[:, :N])
+        assert np.array_equal(oracle.bf16_decode(C[:, :N]), oracle.bf16_decode(oracle.bf16_encode(ref.astype(np.float32))))
+        assert np.all(C[:, N:] == 0x7FD5)
+    # and the one-shot path gives the same bits
+    tg.tile_gemm_set_tuning(tg.TUNE_FLAGS, 64)
+    C2 = np.zeros_like(C)
+    tg.tile_gemm_host(apad[:, :K], b, C2[:, :N])
+    assert np.array_equal(C2[:, :N], C[:, :N])
+
+
 # ------------------------------------------------------------------ split-K of the last wave
 @pytest.mark.parametrize("cfg", [1, 2, 3, 4])
 @pytest.mark.parametrize("split", [2, 3, 5, 16])
