@@ -473,3 +473,42 @@ def test_gemm_split_k_auto_normal_inputs_and_determinism(out):
         got2 = run_case(a, b, out, what="split auto")
         check_close(got1, ref, S, K, out, f"split-K auto {M}x{N}x{K} {out}")
         assert np.array_equal(got1, got2), "split-K result depends on arrival order"
+
+
+# ------------------------------------------------------------------ lockstep producers (long launches)
+@pytest.mark.parametrize("window", [0, 1, 8, 200])
+@pytest.mark.parametrize("cfg", [1, 3, 4])
+def test_gemm_lockstep_forced_small_windows_bit_exact(cfg, window):
+    """Lockstep forced on (tuning key 6 bit 2) with few CTAs so that every cluster walks many rounds
+    and many windows: integer inputs stay exact, nothing hangs, nothing outside C is written."""
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMM_CONFIG, cfg)
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMM_MAX_CTAS, 12)
+    tg.tile_gemm_set_tuning(tg.TUNE_FLAGS, 4 | (window << 8))
+    a, b = wl.make_inputs_custom(1023, 1537, 769, dist="int4", seed=61)
+    ref, _ = oracle.gemm(a, b)
+    got = run_case(a, b, "f32", what=f"lockstep cfg{cfg} window{window}")
+    check_bit_exact(got.astype(np.float32), ref, f"lockstep cfg{cfg} window{window}")
+
+
+def test_gemm_long_k_auto_lockstep_and_split_sampled():
+    """K = 16384 with 160 tiles on 74 clusters: the selector turns on lockstep producers (two whole
+    rounds) AND slices the 12 left-over tiles along K.  Integer inputs: sampled elements exact; normal
+    inputs: sampled oracle + Freivalds on the fp32 result + bf16 == RNE(fp32) bit for bit."""
+    M, N, K = 4096, 5120, 16384
+    a, b = wl.make_inputs_custom(M, N, K, dist="int4", seed=62)
+    A, B = wl.bits_to_torch(a, DEV), wl.bits_to_torch(b, DEV)
+    C = tg.tile_gemm(A, B, out_dtype=tg.OUT_F32).cpu().numpy()
+    rows, cols = wl.uniform_samples(M, N, 4096, seed=62)
+    c, _ = oracle.gemm_sampled(a, b, rows, cols)
+    check_bit_exact(C[rows, cols], c, "long-K ints sampled")
+    a, b = wl.make_inputs_custom(M, N, K, sigma_b=K ** -0.5, seed=63)
+    A, B = wl.bits_to_torch(a, DEV), wl.bits_to_torch(b, DEV)
+    C32 = tg.tile_gemm(A, B, out_dtype=tg.OUT_F32)
+    C16 = tg.tile_gemm(A, B, out_dtype=tg.OUT_BF16)
+    c, s = oracle.gemm_sampled(a, b, rows, cols)
+    h32 = C32.cpu().numpy()
+    check_close(h32[rows, cols], c, s, K, "f32", "long-K sampled")
+    freivalds_rows(h32.astype(np.float64), oracle.bf16_decode(a), oracle.bf16_decode(b), seed=63)
+    assert torch.equal(C16, C32.to(torch.bfloat16)), "bf16 output is not RNE of the fp32 output"
+    C32b = tg.tile_gemm(A, B, out_dtype=tg.OUT_F32)
+    assert torch.equal(C32, C32b), "long-K result is not reproducible"
