@@ -249,6 +249,16 @@ int tile_gemm_debug_owner_map(int32_t* owner, int64_t M, int64_t N, int64_t K,
 int tile_gemm_query_config(int64_t M, int64_t N, int64_t K, int out_dtype, int32_t out[8]);
 
 /*
+ * What the selector does with a GEMM shape (M >= 2) beyond the tile configuration:
+ * out[0] = config id, out[1] = CTAs launched, out[2] = work units that are whole
+ * tiles, out[3] = K slices per tile of the last, partial wave (0 = not cut),
+ * out[4] = k-tiles (of 64) per slice, out[5] = rounds the lockstep producers cover
+ * (0 = off), out[6] = their window in k-tiles, out[7] = rows of the A box (16, 32,
+ * 64 or 128: skinny M loads only the rows it has).  Needs a CUDA device (SM count).
+ */
+int tile_gemm_query_plan(int64_t M, int64_t N, int64_t K, int32_t out[8]);
+
+/*
  * Tuning / test overrides, process-global, not thread-safe against concurrent
  * tile_gemm calls.  key: 0 = GEMM config (0 auto, 1 = 1-CTA 128x128, 2 = 1-CTA
  * 128x256, 3 = 2-CTA 256x256, 4 = 2-CTA 256x512), 1 = GEMM GROUP_M (0 auto), 2 = GEMM max CTAs

@@ -32,7 +32,7 @@ TUNE_GEMM_CONFIG, TUNE_GEMM_GROUP_M, TUNE_GEMM_MAX_CTAS, TUNE_GEMV_SPLIT, TUNE_G
 EXPORTS = ("tile_gemm", "tile_gemm_ex", "tile_gemm_static_b", "tile_gemm_typed", "tile_gemm_swiglu", "tile_add_f32",
            "tile_gemm_record_begin", "tile_gemm_record_end", "tile_gemm_replay", "tile_gemm_recorded_nodes",
            "tile_gemm_record_free", "tile_gemm_select", "tile_gemm_host",
-           "tile_gemm_debug_owner_map", "tile_gemm_query_config", "tile_gemm_set_tuning",
+           "tile_gemm_debug_owner_map", "tile_gemm_query_config", "tile_gemm_query_plan", "tile_gemm_set_tuning",
            "tile_gemm_launch_count", "tile_gemm_status_string", "tile_gemm_last_error",
            "tile_gemm_shutdown")
 
@@ -99,6 +99,8 @@ def load_library():
     lib.tile_gemm_debug_owner_map.restype = _int
     lib.tile_gemm_query_config.argtypes = [_i64, _i64, _i64, _int, ctypes.POINTER(ctypes.c_int32)]
     lib.tile_gemm_query_config.restype = _int
+    lib.tile_gemm_query_plan.argtypes = [_i64, _i64, _i64, ctypes.POINTER(ctypes.c_int32)]
+    lib.tile_gemm_query_plan.restype = _int
     lib.tile_gemm_set_tuning.argtypes = [_int, _int]
     lib.tile_gemm_set_tuning.restype = _int
     lib.tile_gemm_launch_count.argtypes = []
@@ -307,6 +309,13 @@ def tile_gemm_query_config(M, N, K, out_dtype=OUT_F32) -> dict:
     _check(load_library().tile_gemm_query_config(M, N, K, int(out_dtype), out))
     return {"BM": out[0], "BN": out[1], "cta_group": out[2], "ctas": out[3], "group_m": out[4],
             "stages": out[5], "BK": out[6], "config": out[7]}
+
+
+def tile_gemm_query_plan(M, N, K) -> dict:
+    out = (ctypes.c_int32 * 8)()
+    _check(load_library().tile_gemm_query_plan(M, N, K, out))
+    return {"config": out[0], "ctas": out[1], "full_units": out[2], "split": out[3], "k_tiles_per_slice": out[4],
+            "lockstep_rounds": out[5], "lockstep_window": out[6], "a_box_rows": out[7]}
 
 
 def tile_gemm_debug_owner_map(M, N, K, out_dtype=OUT_F32, ld_owner=None, stream=None, device="cuda"):

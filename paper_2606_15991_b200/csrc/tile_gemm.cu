@@ -329,21 +329,56 @@ struct GemmConfig {
 const GemmConfig kConfigs[5] = {{0, 0, 0, 0, 0}, {1, 1, 128, 6, 1}, {2, 1, 256, 4, 1}, {3, 2, 256, 6, 1},
                                 {4, 2, 256, 4, 2}};
 
-// ceil(tiles / slots) * slots / tiles: how much longer than perfectly divisible work the last
-// wave makes a persistent launch run
-double wave_waste(int64_t tiles, int64_t slots) {
-    const int64_t waves = (tiles + slots - 1) / slots;
-    return (double)(waves * slots) / (double)tiles;
+// split-K of the last wave: at most kGemmMaxSplit slices of at least kGemmMinSliceKTiles k-tiles each
+constexpr int kGemmMaxSplit = 16, kGemmMinSliceKTiles = 4;
+
+// The last, partial wave of `rem` tiles on `slots` clusters, in microseconds, and the slice count that
+// gets it: a whole tile at the per-cluster share of ~1500 TFLOP/s, or ceil(rem * c / slots) rounds of
+// 1/c-tile units plus what a slice costs on top (its fp32 accumulators go through L2 once as a store
+// and once as a load of the fix-up, ~100 GB/s per cluster, and a ticket round trip) -- measured on
+// B200: ~8 us for a 256x512 slice, ~3.5 us for 128x128.  Cutting pays for long K loops and for
+// problems below one wave (skinny M).
+double last_wave_us(int64_t rem, int64_t slots, int tile_m, int tile_n, int cg, int64_t k_tiles, int sms, int64_t* slices) {
+    const double tile_us = 2.0 * tile_m * tile_n * (double)k_tiles * tg::GEMM_BK / (1500e6 * cg / (double)sms);
+    const double ovh_us = 3.0 + (double)tile_m * tile_n * 4.0 / 100e3;
+    *slices = 1;
+    if (rem <= 0) return 0.0;
+    double best = tile_us;
+    int64_t sl_max = k_tiles / kGemmMinSliceKTiles;
+    if (sl_max > kGemmMaxSplit) sl_max = kGemmMaxSplit;
+    if (k_tiles < 2 * kGemmMinSliceKTiles || g_tune[3].load() == 1) return best;
+    for (int64_t c = 2; c <= sl_max; ++c) {
+        const double rounds = (double)((rem * c + slots - 1) / slots);
+        const double cost = rounds / (double)c * tile_us + (rounds + 0.5 * (double)c) * ovh_us;
+        if (cost < best * 0.97) { best = cost; *slices = c; }
+    }
+    return best;
 }
 
-GemmConfig choose_config(int64_t M, int64_t N, int sms) {
+// estimated time of the whole launch with tiles of tile_m x tile_n on `slots` clusters
+double launch_us(int64_t M, int64_t N, int64_t K, int tile_m, int tile_n, int cg, int sms) {
+    const int64_t slots = sms / cg, k_tiles = (K + tg::GEMM_BK - 1) / tg::GEMM_BK;
+    const int64_t tiles = ((M + tile_m - 1) / tile_m) * ((N + tile_n - 1) / tile_n);
+    const double tile_us = 2.0 * tile_m * tile_n * (double)k_tiles * tg::GEMM_BK / (1500e6 * cg / (double)sms);
+    int64_t sl;
+    return (double)(tiles / slots) * tile_us + last_wave_us(tiles % slots, slots, tile_m, tile_n, cg, k_tiles, sms, &sl);
+}
+
+GemmConfig choose_config(int64_t M, int64_t N, int64_t K, int sms) {
     const int forced = g_tune[0].load();
     if (forced >= 1 && forced <= 4) return kConfigs[forced];
     const int64_t t3 = ((M + 255) / 256) * ((N + 255) / 256);
     const int64_t t4 = ((M + 255) / 256) * ((N + 511) / 512);
     // the 256x512 tile moves a quarter less operand data per FLOP (the kernel is power bound,
-    // DESIGN.md "Power"); take it unless its coarser wave quantisation costs more than that buys
-    if (t4 >= sms / 2 && wave_waste(t4, sms / 2) <= wave_waste(t3, sms / 2) * 1.06) return kConfigs[4];
+    // DESIGN.md "Power"); take it unless its coarser wave quantisation -- after the last wave has
+    // been cut along K where that pays -- costs more than that buys
+    // a 256x512 tile occupies both accumulator slots, so ~2 us of each tile's epilogue are not hidden
+    // behind the next main loop (calibrated on steady-state A/Bs: K = 5120 prefers 256x256 by 1-7 %,
+    // K >= 8192 prefers 256x512 by 3-4 %)
+    const double exposed4 = 2.0 * (double)((t4 + sms / 2 - 1) / (sms / 2));
+    if (t4 >= sms / 2 &&
+        launch_us(M, N, K, 256, 512, 2, sms) + exposed4 <= launch_us(M, N, K, 256, 256, 2, sms) * 1.06)
+        return kConfigs[4];
     if (t3 >= sms / 2) return kConfigs[3];
     const int64_t t2 = ((M + 127) / 128) * ((N + 255) / 256);
     if (t2 * 4 >= (int64_t)sms * 3) return kConfigs[2];
@@ -353,9 +388,6 @@ GemmConfig choose_config(int64_t M, int64_t N, int sms) {
 // lockstep defaults: on from kLockstepMinTiles tiles per cluster and kLockstepMinKTiles k-tiles
 constexpr int kLockstepMinTiles = 2, kLockstepMinKTiles = 256, kLockstepWindow = 32;
 
-// split-K of the last wave: at most kGemmMaxSplit slices of at least kGemmMinSliceKTiles k-tiles each
-constexpr int kGemmMaxSplit = 16, kGemmMinSliceKTiles = 4;
-
 struct GemmLaunch {
     GemmConfig cfg;
     tg::GemmParams p;
@@ -364,7 +396,7 @@ struct GemmLaunch {
 
 void plan_gemm(int64_t M, int64_t N, int64_t K, int in_dtype, int out_dtype, int sms, GemmLaunch* gl,
                bool allow_split = false) {
-    gl->cfg = choose_config(M, N, sms);
+    gl->cfg = choose_config(M, N, K, sms);
     const int tile_m = tg::GEMM_BM * gl->cfg.cg;
     tg::GemmParams& p = gl->p;
     memset(&p, 0, sizeof p);
@@ -391,23 +423,10 @@ void plan_gemm(int64_t M, int64_t N, int64_t K, int in_dtype, int out_dtype, int
     const int64_t rem = tiles % max_units;
     const int split_tune = g_tune[3].load();   // key 3 also overrides the GEMM split: 1 = never, >= 2 = that many slices
     if (allow_split && rem > 0 && split_tune != 1 && p.num_k_tiles >= 2 * kGemmMinSliceKTiles) {
-        // The last wave as ceil(rem * c / clusters) rounds of 1/c-tile units, in microseconds: a whole
-        // tile at the per-cluster share of ~1500 TFLOP/s, plus what a slice costs on top (its fp32
-        // accumulators go through L2 once as a store and once as a load of the fix-up, ~100 GB/s per
-        // cluster, and a ticket round trip) -- measured on B200: ~8 us for a 256x512 slice, ~3.5 us
-        // for 128x128.  Cutting pays for long K loops and for problems below one wave (skinny M).
         int64_t sl_max = p.num_k_tiles / kGemmMinSliceKTiles;
         if (sl_max > kGemmMaxSplit) sl_max = kGemmMaxSplit;
-        const double tile_flop = 2.0 * tile_m * gl->cfg.tile_n() * (double)p.num_k_tiles * tg::GEMM_BK;
-        const double tile_us = tile_flop / (1500e6 * gl->cfg.cg / (double)sms);
-        const double ovh_us = 3.0 + (double)tile_m * gl->cfg.tile_n() * 4.0 / 100e3;
         int64_t sl = 1;
-        double best = tile_us;
-        for (int64_t c = 2; c <= sl_max; ++c) {
-            const double rounds = (double)((rem * c + max_units - 1) / max_units);
-            const double cost = rounds / (double)c * tile_us + (rounds + 0.5 * (double)c) * ovh_us;
-            if (cost < best * 0.97) { best = cost; sl = c; }
-        }
+        last_wave_us(rem, max_units, tile_m, gl->cfg.tile_n(), gl->cfg.cg, p.num_k_tiles, sms, &sl);
         if (split_tune >= 2) sl = split_tune < sl_max ? split_tune : sl_max;
         if (sl >= 2) {
             const int64_t kps = (p.num_k_tiles + sl - 1) / sl;
@@ -480,19 +499,28 @@ int launch_gemm(const GemmLaunch& gl, const CUtensorMap& ta, const CUtensorMap& 
 
 // Lockstep producers: only where a launch is long enough for clusters to drift (several whole
 // tiles per cluster, long K loops); tuning key 6: bit 2 forces it on, bit 3 off, bits 8-15 = window.
+// rounds the lockstep covers (0: off) and its window, from the plan alone
+void lockstep_plan(const GemmLaunch& gl, int64_t* rounds_out, int* window_out) {
+    const int tune = g_tune[6].load();
+    const int clusters = gl.ctas / gl.cfg.cg;
+    // rounds in which every cluster owns a whole tile: lockstep covers exactly these
+    const int64_t rounds = clusters > 0 ? gl.p.full_units / clusters : 0;
+    bool on = rounds >= kLockstepMinTiles && gl.p.num_k_tiles >= kLockstepMinKTiles;
+    if (tune & 4) on = rounds >= 1 && gl.p.num_k_tiles >= 1;
+    if (tune & 8) on = false;
+    int window = (tune >> 8) & 255;
+    if (window <= 0) window = kLockstepWindow;
+    *rounds_out = on ? rounds : 0;
+    *window_out = window;
+}
+
 int setup_lockstep(GemmLaunch& gl, int dev, cudaStream_t s) {
     int rc = TILE_GEMM_OK;
     {
-        const int tune = g_tune[6].load();
-        const int clusters = gl.ctas / gl.cfg.cg;
-        // rounds in which every cluster owns a whole tile: lockstep covers exactly these
-        const int64_t rounds = gl.p.full_units / clusters;
-        bool on = rounds >= kLockstepMinTiles && gl.p.num_k_tiles >= kLockstepMinKTiles;
-        if (tune & 4) on = rounds >= 1 && gl.p.num_k_tiles >= 1;
-        if (tune & 8) on = false;
-        if (on) {
-            int window = (tune >> 8) & 255;
-            if (window <= 0) window = kLockstepWindow;
+        int64_t rounds = 0;
+        int window = 0;
+        lockstep_plan(gl, &rounds, &window);
+        if (rounds > 0) {
             const int64_t windows = (rounds * gl.p.num_k_tiles + window - 1) / window + 1;
             gl.p.sync_rounds = (int32_t)rounds;
             uint32_t* sync = nullptr;
@@ -1115,6 +1143,27 @@ int tile_gemm_query_config(int64_t M, int64_t N, int64_t K, int out_dtype, int32
     out[5] = gl.cfg.stages;
     out[6] = tg::GEMM_BK;
     out[7] = gl.cfg.id;
+    return TILE_GEMM_OK;
+}
+
+int tile_gemm_query_plan(int64_t M, int64_t N, int64_t K, int32_t out[8]) {
+    if (M <= 1 || N <= 0 || K <= 0 || !out) return fail(TILE_GEMM_E_EXTENT, "the plan query needs M >= 2, N > 0, K > 0");
+    int dev = 0, sms = 0;
+    int rc = current_device(&dev, &sms);
+    if (rc) return rc;
+    GemmLaunch gl;
+    plan_gemm(M, N, K, TILE_GEMM_IN_BF16, TILE_GEMM_OUT_BF16, sms, &gl, true);
+    int64_t rounds = 0;
+    int window = 0;
+    lockstep_plan(gl, &rounds, &window);
+    out[0] = gl.cfg.id;
+    out[1] = gl.ctas;
+    out[2] = gl.p.full_units;
+    out[3] = gl.p.split;
+    out[4] = gl.p.kps;
+    out[5] = (int32_t)rounds;
+    out[6] = rounds > 0 ? window : 0;
+    out[7] = M <= 16 ? 16 : M <= 32 ? 32 : M <= 64 ? 64 : 128;
     return TILE_GEMM_OK;
 }
 

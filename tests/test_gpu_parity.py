@@ -512,3 +512,21 @@ def test_gemm_long_k_auto_lockstep_and_split_sampled():
     assert torch.equal(C16, C32.to(torch.bfloat16)), "bf16 output is not RNE of the fp32 output"
     C32b = tg.tile_gemm(A, B, out_dtype=tg.OUT_F32)
     assert torch.equal(C32, C32b), "long-K result is not reproducible"
+
+
+def test_selector_plans_for_the_benchmarked_shapes():
+    """a2, extended: what the selector decides beyond the tile shape, on a 148-SM B200."""
+    plan = tg.tile_gemm_query_plan
+    p = plan(8192, 8192, 8192)            # cfg 3: whole tiles only (68 of 74 left over: cutting does not pay), K too short for lockstep
+    assert p["config"] == 4 and p["split"] == 0 and p["full_units"] == 512 and p["lockstep_rounds"] == 0
+    p = plan(4096, 5120, 25600)           # cfg 4 down: 12 of 160 tiles left over -> 6 K slices each, two lockstep rounds
+    assert p["config"] == 4 and p["full_units"] == 148 and p["split"] == 6 and p["lockstep_rounds"] == 2
+    assert p["split"] * p["k_tiles_per_slice"] >= 400 > (p["split"] - 1) * p["k_tiles_per_slice"]
+    p = plan(32768, 32768, 32768)
+    assert p["lockstep_rounds"] >= 100 and p["lockstep_window"] == 32
+    p = plan(1024, 1024, 1024)            # below one wave but a short K loop: not cut
+    assert p["split"] == 0 and p["a_box_rows"] == 128
+    for M in (2, 8, 16):                  # skinny M: below one wave, long K -> cut; A box only as tall as M needs
+        p = plan(M, 5120, 25600)
+        assert p["full_units"] == 0 and p["split"] >= 2 and p["a_box_rows"] == 16 and p["ctas"] >= 100
+    assert plan(40, 10240, 5120)["a_box_rows"] == 64
