@@ -86,7 +86,8 @@ extern "C" {
 #define TILE_GEMM_PATH_AUTO 0         /* force_path only                                      */
 #define TILE_GEMM_PATH_GEMM_TMA 1     /* tcgen05 GEMM, A and B read in place through TMA      */
 #define TILE_GEMM_PATH_GEMM_REPACK 2  /* same kernel after copying A and/or B to aligned rows */
-#define TILE_GEMM_PATH_GEMV 3         /* M == 1 HBM-bound weight-streaming kernel             */
+#define TILE_GEMM_PATH_GEMV 3         /* M == 1 (any alignment) or M <= 4 with 16-byte addressable A and B:
+                                         HBM-bound weight-streaming kernels                   */
 #define TILE_GEMM_PATH_ZERO 4         /* K == 0: C <- 0                                       */
 #define TILE_GEMM_PATH_NOOP 5         /* M == 0 or N == 0                                     */
 
@@ -102,7 +103,8 @@ int tile_gemm(const void* A, const void* B, void* C,
 /*
  * Same, with the path forced (tests / measurements): TILE_GEMM_PATH_AUTO,
  * _GEMM_TMA (fails with E_PATH when A or B is not TMA-addressable), _GEMM_REPACK
- * (always legal for K > 0) or _GEMV (requires M == 1).
+ * (always legal for K > 0) or _GEMV (requires M == 1, or M <= 4 with A and B
+ * 16-byte addressable: base aligned to 16 bytes, lda and ldb multiples of 8).
  */
 int tile_gemm_ex(const void* A, const void* B, void* C,
                  int64_t M, int64_t N, int64_t K,

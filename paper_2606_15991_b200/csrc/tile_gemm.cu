@@ -22,6 +22,7 @@
 #include "aux_kernels.cuh"
 #include "gemm_kernel.cuh"
 #include "gemv_kernel.cuh"
+#include "gemv_rows_kernel.cuh"
 
 namespace {
 
@@ -81,6 +82,8 @@ bool overlaps(const void* p, int64_t pn, const void* q, int64_t qn) {
     return a < b + (uintptr_t)qn && b < a + (uintptr_t)pn;
 }
 
+constexpr int64_t kGemvMaxRows = 4;   // M = 2..4 with TMA-addressable A and B take the multi-row GEMV (gemv_rows_kernel.cuh)
+
 int check_and_select(const void* A, const void* B, const void* C, int64_t M, int64_t N, int64_t K, int64_t lda,
                      int64_t ldb, int64_t ldc, int in_dtype, int out_dtype, Plan* plan) {
     if (M < 0 || N < 0 || K < 0)
@@ -128,6 +131,7 @@ int check_and_select(const void* A, const void* B, const void* C, int64_t M, int
     plan->c_tma = (((uintptr_t)C & 15) == 0) && ((ldc * plan->esize) % 16 == 0);
     if (K == 0) plan->path = TILE_GEMM_PATH_ZERO;
     else if (M == 1) plan->path = TILE_GEMM_PATH_GEMV;
+    else if (M <= kGemvMaxRows && plan->a_tma && plan->b_tma) plan->path = TILE_GEMM_PATH_GEMV;   // a few rows: still weight streaming
     else plan->path = (plan->a_tma && plan->b_tma) ? TILE_GEMM_PATH_GEMM_TMA : TILE_GEMM_PATH_GEMM_REPACK;
     return TILE_GEMM_OK;
 }
@@ -723,6 +727,87 @@ int run_gemv_split(const void* x, const void* B, void* y, int64_t N, int64_t K, 
     return fail(TILE_GEMM_E_INTERNAL, "unknown GEMV ring shape %d", shape);
 }
 
+// M = 2..4: the multi-row GEMV (gemv_rows_kernel.cuh); same (column block, slice) grid as the M = 1 kernel
+template <int MR, bool F16>
+int launch_gemv_rows(const CUtensorMap& tb, const CUtensorMap& tx, const tg::GemvRowsParams& p, int gx, int split, bool pdl,
+                     cudaStream_t s, int dev) {
+    using L = tg::GemvRowsSmem<MR, 3>;
+    auto kern = tg::gemv_rows_kernel<MR, F16>;
+    static bool configured[64] = {};
+    if (!configured[dev]) {
+        CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::TOTAL));
+        configured[dev] = true;
+    }
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof cfg);
+    cfg.gridDim = dim3((unsigned)gx, (unsigned)split, 1);
+    cfg.blockDim = dim3(tg::GEMV_TMA_THREADS, 1, 1);
+    cfg.dynamicSmemBytes = L::TOTAL;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = pdl ? 1 : 0;
+    CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, tb, tx, p));
+    g_launches.fetch_add(1);
+    return TILE_GEMM_OK;
+}
+
+int run_gemv_rows(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_t K, int64_t lda, int64_t ldb,
+                  int64_t ldc, int in_dtype, int out_dtype, cudaStream_t s, int dev, int sms, unsigned flags) {
+    const int64_t col_blocks = (N + tg::GEMV_COLS - 1) / tg::GEMV_COLS;
+    const int64_t k_tiles = (K + tg::GEMV_TILE_K - 1) / tg::GEMV_TILE_K;
+    int64_t budget = (int64_t)sms * 2;   // all CTAs co-resident, two per SM
+    const int cap = g_tune[2].load();
+    if (cap > 0 && cap < budget) budget = cap;
+    const int64_t gx = col_blocks < budget ? col_blocks : budget;
+    int64_t split = g_tune[3].load();
+    if (split <= 0) {
+        split = budget / gx;
+        if (split == 1 && col_blocks <= budget && col_blocks * 2 > budget) {   // see run_gemv_split
+            double best = (double)col_blocks / (double)budget;
+            for (int64_t c = 2; c <= 8 && k_tiles / c >= 16; ++c) {
+                const double waves = (double)(col_blocks * c) / (double)budget;
+                const double eff = waves / (double)(int64_t)(waves + 0.999999);
+                if (eff > best + 0.05) { best = eff; split = c; }
+            }
+        }
+    }
+    if (split > k_tiles) split = k_tiles;
+    if (split > 65535) split = 65535;
+    if (split < 1) split = 1;
+    tg::GemvRowsParams p;
+    memset(&p, 0, sizeof p);
+    p.y = C;
+    p.ldy = ldc;
+    p.N = (int32_t)N; p.K = (int32_t)K; p.k_tiles = (int32_t)k_tiles; p.col_blocks = (int32_t)col_blocks;
+    p.out_kind = out_dtype;
+    p.flags = (flags & TILE_GEMM_FLAG_B_IMMUTABLE) ? tg::GEMV_FLAG_B_IMMUTABLE : 0;
+    if (split > 1) {
+        int rc = gemv_workspace_for(dev, s, (size_t)col_blocks * split * M * tg::GEMV_COLS * 4, (size_t)col_blocks * 4,
+                                    &p.partials, &p.tickets);
+        if (rc) return rc;
+    }
+    CUtensorMap tb, tx;
+    int rc = get_tensor_map(&tb, B, 2, false, (uint64_t)N, (uint64_t)K, (uint64_t)ldb * 2, (uint32_t)tg::GEMV_COLS,
+                            (uint32_t)tg::GEMV_TILE_K, 0);
+    if (rc) return rc;
+    rc = get_tensor_map(&tx, A, 2, false, (uint64_t)K, (uint64_t)M, (uint64_t)lda * 2, (uint32_t)tg::GEMV_TILE_K, (uint32_t)M, 0);
+    if (rc) return rc;
+    const bool pdl = (g_tune[6].load() & 1) == 0;
+    const bool f16 = in_dtype == TILE_GEMM_IN_F16;
+    switch (M) {
+        case 2: return f16 ? launch_gemv_rows<2, true>(tb, tx, p, (int)gx, (int)split, pdl, s, dev)
+                           : launch_gemv_rows<2, false>(tb, tx, p, (int)gx, (int)split, pdl, s, dev);
+        case 3: return f16 ? launch_gemv_rows<3, true>(tb, tx, p, (int)gx, (int)split, pdl, s, dev)
+                           : launch_gemv_rows<3, false>(tb, tx, p, (int)gx, (int)split, pdl, s, dev);
+        case 4: return f16 ? launch_gemv_rows<4, true>(tb, tx, p, (int)gx, (int)split, pdl, s, dev)
+                           : launch_gemv_rows<4, false>(tb, tx, p, (int)gx, (int)split, pdl, s, dev);
+    }
+    return fail(TILE_GEMM_E_INTERNAL, "the multi-row GEMV handles M = 2..4 (M=%lld)", (long long)M);
+}
+
 int run_gemv(const void* x, const void* B, void* y, int64_t N, int64_t K, int64_t ldb, int in_dtype, int out_dtype,
              cudaStream_t s, const Plan& plan, int dev, int sms, unsigned flags) {
     const bool f16 = in_dtype == TILE_GEMM_IN_F16;
@@ -823,8 +908,9 @@ int gemm_entry(const void* A, const void* B, void* C, int64_t M, int64_t N, int6
     if (plan.path == TILE_GEMM_PATH_NOOP) return TILE_GEMM_OK;
     int path = plan.path;
     if (force_path != TILE_GEMM_PATH_AUTO && path != TILE_GEMM_PATH_ZERO) {
-        if (force_path == TILE_GEMM_PATH_GEMV && M != 1)
-            return fail(TILE_GEMM_E_PATH, "the GEMV path needs M == 1 (M=%lld)", (long long)M);
+        if (force_path == TILE_GEMM_PATH_GEMV && !(M == 1 || (M <= kGemvMaxRows && plan.a_tma && plan.b_tma)))
+            return fail(TILE_GEMM_E_PATH, "the GEMV path needs M == 1, or M <= 4 with 16-byte addressable A and B (M=%lld)",
+                        (long long)M);
         if (force_path == TILE_GEMM_PATH_GEMM_TMA && !(plan.a_tma && plan.b_tma))
             return fail(TILE_GEMM_E_PATH, "GEMM_TMA needs 16-byte aligned A/B with lda, ldb multiples of 8");
         path = force_path;
@@ -835,7 +921,9 @@ int gemm_entry(const void* A, const void* B, void* C, int64_t M, int64_t N, int6
     cudaStream_t s = (cudaStream_t)stream;
     switch (path) {
         case TILE_GEMM_PATH_ZERO: return run_zero(C, M, N, ldc, plan.esize, s);
-        case TILE_GEMM_PATH_GEMV: return run_gemv(A, B, C, N, K, ldb, in_dtype, out_dtype, s, plan, dev, sms, flags);
+        case TILE_GEMM_PATH_GEMV:
+            if (M > 1) return run_gemv_rows(A, B, C, M, N, K, lda, ldb, ldc, in_dtype, out_dtype, s, dev, sms, flags);
+            return run_gemv(A, B, C, N, K, ldb, in_dtype, out_dtype, s, plan, dev, sms, flags);
         case TILE_GEMM_PATH_GEMM_TMA:
             return run_gemm(A, B, C, M, N, K, lda, ldb, ldc, in_dtype, out_dtype, s, plan, false, dev, sms);
         case TILE_GEMM_PATH_GEMM_REPACK:   // forced: repack both operands; auto: only what TMA cannot address

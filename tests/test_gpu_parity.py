@@ -530,3 +530,47 @@ def test_selector_plans_for_the_benchmarked_shapes():
         p = plan(M, 5120, 25600)
         assert p["full_units"] == 0 and p["split"] >= 2 and p["a_box_rows"] == 16 and p["ctas"] >= 100
     assert plan(40, 10240, 5120)["a_box_rows"] == 64
+
+
+# ------------------------------------------------------------------ M = 2..4: the multi-row GEMV
+@pytest.mark.parametrize("M", [2, 3, 4])
+@pytest.mark.parametrize("split", [0, 1, 3, 8])
+def test_gemv_rows_integer_bit_exact_and_canary(M, split):
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMV_SPLIT, split)
+    for (K, N), pads in (((776, 1537), (0, 7, 3)), ((5120, 10240), (0, 0, 0)), ((64, 8), (8, 8, 0)), ((4104, 520), (8, 0, 8))):
+        a, b = wl.make_inputs_custom(M, N, K, dist="int4", seed=71 + M)
+        ref, _ = oracle.gemm(a, b)
+        pads_ok = (pads[0], pads[1] + (-(N + pads[1])) % 8, pads[2])          # ldb stays a multiple of 8: the GEMV path is taken
+        A = device_operand(a, pads_ok[0])
+        B = device_operand(b, pads_ok[1])
+        assert tg.tile_gemm_select(M, N, K, A.stride(0), B.stride(0), N + pads_ok[2], A.data_ptr(), B.data_ptr(), 1 << 41) \
+            == tg.PATH_GEMV
+        got = run_case(a, b, "f32", pads=pads_ok, what=f"gemv rows M={M}")
+        check_bit_exact(got.astype(np.float32), ref, f"gemv rows M={M} K={K} N={N} split={split}")
+
+
+@pytest.mark.parametrize("M", [2, 4])
+@pytest.mark.parametrize("out", ["f32", "bf16"])
+def test_gemv_rows_normal_inputs_and_agreement_with_the_gemm_path(M, out):
+    K, N = 5120, 8192
+    a, b = wl.make_inputs_custom(M, N, K, sigma_b=0.02, seed=73)
+    ref, S = oracle.gemm(a, b)
+    got = run_case(a, b, out, what="gemv rows")
+    check_close(got, ref, S, K, out, f"gemv rows M={M} {out}")
+    again = run_case(a, b, out, what="gemv rows")
+    assert np.array_equal(got, again), "multi-row GEMV is not reproducible"
+    via_gemm = run_case(a, b, out, force=tg.PATH_GEMM_TMA, what="gemm path")
+    check_close(via_gemm, ref, S, K, out, f"gemm path M={M} {out}")
+
+
+def test_gemv_rows_f16_and_unaligned_falls_back_to_the_gemm():
+    a, b = wl.make_inputs_f16(3, 2048, 1024, sigma_b=0.05, seed=74)
+    ref, S = oracle.gemm(a, b, in_dtype=oracle.IN_F16)
+    A, B = wl.bits_to_torch(a, DEV, torch.float16), wl.bits_to_torch(b, DEV, torch.float16)
+    C = tg.tile_gemm(A, B, out_dtype=tg.OUT_F16)
+    check_close(oracle.f16_decode(C.cpu().view(torch.int16).numpy().view(np.uint16)), ref, S, 1024, "f16", "gemv rows f16")
+    # lda not a multiple of 8: A is not TMA-addressable, the selector goes to the (repacking) GEMM
+    assert tg.tile_gemm_select(3, 2048, 1023, 1023, 2048, 2048) == tg.PATH_GEMM_REPACK
+    ai, bi = wl.make_inputs_custom(3, 2048, 1023, dist="int4", seed=75)
+    refi, _ = oracle.gemm(ai, bi)
+    check_bit_exact(run_case(ai, bi, "f32").astype(np.float32), refi, "M=3 unaligned")

@@ -202,3 +202,12 @@ def test_swiglu_preconditions_on_the_host():
     assert tg.tile_gemm_swiglu_raw(*a, 0, 16, 64, 64, 32, 16, tg.OUT_F32) == tg.E_OK           # M == 0: no-op
     if not torch.cuda.is_available():
         assert tg.tile_gemm_swiglu_raw(*a, 8, 16, 64, 64, 32, 16, tg.OUT_F32) == tg.E_DEVICE
+
+
+def test_selector_routes_a_few_rows_to_the_weight_streaming_path():
+    # M = 2..4 with 16-byte addressable A and B: GEMV family; otherwise, and from M = 5 on: tensor cores
+    for M in (2, 3, 4):
+        assert sel(M, 10240, 5120) == tg.PATH_GEMV
+        assert sel(M, 10240, 5120, lda=5121) == tg.PATH_GEMM_REPACK
+        assert sel(M, 10240, 5120, A=A0 + 2) == tg.PATH_GEMM_REPACK
+    assert sel(5, 10240, 5120) == tg.PATH_GEMM_TMA
