@@ -172,7 +172,9 @@ int tile_gemm_swiglu(const void* X, const void* Wgu, void* H,
  * (TILE_GEMM_E_ALIAS) while x and y may be the same buffer (shared
  * reads).  Only z[0..n) is written.  n == 0 is a successful no-op.  Errors:
  * E_EXTENT (n < 0), E_OVERFLOW (n > 2^40), E_NULL, E_ALIGN, E_ALIAS, E_DEVICE,
- * E_CUDA; nothing is enqueued on error.  Asynchronous on `stream`.
+ * E_CUDA; nothing is enqueued on error.  Asynchronous on `stream`.  Launched with
+ * programmatic dependent launch like every kernel of the library: a chain of
+ * small adds overlaps each launch with its predecessor's execution.
  */
 int tile_add_f32(const float* x, const float* y, float* z, int64_t n, void* stream);
 

@@ -17,6 +17,8 @@
 #pragma once
 #include <stdint.h>
 
+#include "ptx.cuh"
+
 namespace tg {
 
 constexpr int ADD_THREADS = 256;
@@ -78,6 +80,10 @@ template <int UNROLL, int VW, bool HINT>
 __global__ void __launch_bounds__(ADD_THREADS)
 add_f32_vec_kernel(const float* __restrict__ x, const float* __restrict__ y, float* __restrict__ z, int64_t n) {
     constexpr int64_t TILE_VECS = (int64_t)ADD_THREADS * UNROLL;
+    // programmatic dependent launch: the next kernel of the stream may be scheduled now; x and y may be
+    // the previous kernel's output, so nothing is read before the wait (a no-op without the attribute)
+    griddep_launch_dependents();
+    griddep_wait();
     const int64_t nvec = n / VW;
     const int64_t full_tiles = nvec / TILE_VECS;
     for (int64_t t = blockIdx.x; t < full_tiles; t += gridDim.x) {
@@ -111,6 +117,8 @@ add_f32_vec_kernel(const float* __restrict__ x, const float* __restrict__ y, flo
 // Any 4-byte alignment: element-wise, still coalesced (a warp touches 128 contiguous bytes).
 __global__ void __launch_bounds__(ADD_THREADS)
 add_f32_scalar_kernel(const float* __restrict__ x, const float* __restrict__ y, float* __restrict__ z, int64_t n) {
+    griddep_launch_dependents();
+    griddep_wait();
     for (int64_t i = (int64_t)blockIdx.x * ADD_THREADS + threadIdx.x; i < n; i += (int64_t)gridDim.x * ADD_THREADS)
         z[i] = __fadd_rn(__ldg(x + i), __ldg(y + i));
 }

@@ -1056,7 +1056,17 @@ int tile_add_f32(const float* x, const float* y, float* z, int64_t n, void* stre
         if (grid > tiles) grid = tiles;
         if (grid > 0x7fffffff) grid = 0x7fffffff;
         if (grid < 1) grid = 1;
-#define TG_ADD_CASE(U, VW, H) tg::add_f32_vec_kernel<U, VW, H><<<(unsigned)grid, tg::ADD_THREADS, 0, s>>>(x, y, z, n)
+        cudaLaunchConfig_t cfg;
+        memset(&cfg, 0, sizeof cfg);
+        cfg.gridDim = dim3((unsigned)grid, 1, 1);
+        cfg.blockDim = dim3(tg::ADD_THREADS, 1, 1);
+        cfg.stream = s;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = (g_tune[6].load() & 1) ? 0 : 1;   // tuning key 6 bit 0: no programmatic dependent launch
+#define TG_ADD_CASE(U, VW, H) CUDA_TRY(cudaLaunchKernelEx(&cfg, tg::add_f32_vec_kernel<U, VW, H>, x, y, z, n))
 #define TG_ADD_MODE(U)                                      \
     switch (mode) {                                         \
         case 1: TG_ADD_CASE(U, 4, true); break;             \
