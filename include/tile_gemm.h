@@ -198,6 +198,8 @@ int tile_add_f32(const float* x, const float* y, float* z, int64_t n, void* stre
  * returns the number of graph nodes (kernels and workspace memsets) in a step,
  * -1 for anything that is not a live step; tile_gemm_launch_count grows by that
  * number per replay.  tile_gemm_record_free destroys a step (NULL is a no-op).
+ * Steps reference the library's per-stream workspaces: free them (or stop
+ * replaying them) before tile_gemm_shutdown.
  */
 int tile_gemm_record_begin(void* stream);
 int tile_gemm_record_end(void* stream, void** step_out);

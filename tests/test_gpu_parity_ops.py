@@ -410,3 +410,30 @@ def test_swiglu_preconditions():
     assert tg.tile_gemm_swiglu_raw(*a, 8, 16, 0, 64, 32, 16, tg.OUT_F32) == tg.E_OK            # K == 0 -> zeros
     torch.cuda.synchronize()
     assert torch.all(H == 0.0)
+
+
+def test_recorded_step_with_lockstep_and_split_gemm():
+    """A long-K GEMM (lockstep counters zeroed by a memset node, K-cut last wave with workspace and
+    tickets) inside a recorded step: two replays give the bits of the direct call."""
+    M, N, K = 2048, 5120, 16384
+    a, b = wl.make_inputs_custom(M, N, K, sigma_b=K ** -0.5, seed=81)
+    A, B = wl.bits_to_torch(a, DEV), wl.bits_to_torch(b, DEV)
+    s = torch.cuda.Stream()
+    tg.tile_gemm_set_tuning(tg.TUNE_FLAGS, 4)            # lockstep on even with one whole round
+    C = torch.empty((M, N), dtype=torch.bfloat16, device=DEV)
+    tg.tile_gemm(A, B, C, stream=s)
+    s.synchronize()
+    want = C.clone()
+    tg.tile_gemm_record_begin(s)
+    tg.tile_gemm(A, B, C, stream=s)
+    step = tg.tile_gemm_record_end(s)
+    assert step.nodes >= 2                               # the kernel and its memset
+    for _ in range(2):
+        C.zero_()
+        step.replay(s)
+        s.synchronize()
+        assert torch.equal(C, want)
+    step.free()
+    rows, cols = wl.uniform_samples(M, N, 1024, seed=81)
+    c, sc = oracle.gemm_sampled(a, b, rows, cols)
+    check_close(oracle.bf16_decode(wl.torch_to_bits(want)[rows, cols]), c, sc, K, "bf16", "recorded long-K GEMM")
