@@ -570,6 +570,20 @@ def run_cuda(args):
                          "peak_source": f"{peaks['source']} copy bandwidth (MEASURED_PEAKS.json)",
                          "frac_of_8000": gbs / 8000.0, "kernel": "gemv_split_kernel<256,64,3,2>"},
         }
+        # what a pure streaming read achieves on this box (4 GiB, every word once)
+        dev0 = torch.device("cuda", torch.cuda.current_device())
+        pbuf = torch.empty(1 << 30, dtype=torch.int32, device=dev0).random_(0, 1 << 30)
+        pout = torch.zeros(1, dtype=torch.int64, device=dev0)
+        for _ in range(2):
+            tg.tile_read_probe_u32(pbuf, pout)
+        preps = 10
+        pms = tdist.max_over_ranks(time_region(lambda i: tg.tile_read_probe_u32(pbuf, pout), preps,
+                                               torch.cuda.synchronize, tdist.barrier)) / preps
+        probe_gbs = pbuf.numel() * 4 / (pms * 1e-3) / 1e9
+        del pbuf
+        torch.cuda.empty_cache()
+        line["read_probe"] = {"gbs": probe_gbs, "bytes": 4 << 30, "kernel": "read_probe_kernel (tile_read_probe_u32)"}
+        line["gemv"]["roofline"]["frac_of_read_probe"] = line["gemv"]["roofline"]["achieved"] / probe_gbs
         # element-wise add (Listing 1) at n = 2^28
         n_add = 1 << 28
         ms = bench_add(tg, torch, n_add, max(10, args.steps // 4), 3, tdist)

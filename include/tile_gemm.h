@@ -208,6 +208,18 @@ int64_t tile_gemm_recorded_nodes(void* step);
 int tile_gemm_record_free(void* step);
 
 /*
+ * Read-bandwidth probe of the measurement harness: adds the sum of
+ * the n 32-bit words of `buf` (device, 16-byte aligned), taken as a 64-bit integer
+ * modulo 2^64, to *out_sum (device, 8-byte aligned, not inside buf; the caller
+ * zeroes it).  Integer arithmetic: exact and independent of the order.  Every word
+ * is read exactly once with streaming 128-bit loads, one 32 KB tile per CTA: the
+ * rate of this kernel on a buffer much larger than L2 is what a pure read of HBM
+ * achieves on the box, the figure bench.py reports next to the GEMV's.
+ * Errors: E_EXTENT, E_NULL, E_ALIGN, E_OVERFLOW (n > 2^40), E_ALIAS, E_DEVICE, E_CUDA.
+ */
+int tile_read_probe_u32(const uint32_t* buf, int64_t n, unsigned long long* out_sum, void* stream);
+
+/*
  * Launch preconditions + shape selector as a pure host function (PAPER.md:200:
  * "runs once per launch before any work is queued"; tile shapes
  * chosen per size).  Never dereferences A/B/C and makes no CUDA call.

@@ -198,3 +198,10 @@ def swiglu_gemm(X, Wgu, threads: int | None = None):
     G, Sg = gemm(X, Wgu[:, :inter], threads=threads)
     U, Su = gemm(X, Wgu[:, inter:], threads=threads)
     return silu(G) * U, G, U, Sg, Su
+
+
+def word_sum_u32(buf) -> int:
+    """Sum of a buffer's 32-bit words as an integer modulo 2^64 (what the read-bandwidth probe of
+    the harness returns): the definition, through numpy's uint64 accumulation."""
+    w = np.ascontiguousarray(buf).view(np.uint32).ravel()
+    return int(np.sum(w, dtype=np.uint64))

@@ -29,7 +29,7 @@ PATH_NAMES = {PATH_AUTO: "auto", PATH_GEMM_TMA: "gemm_tma", PATH_GEMM_REPACK: "g
 
 TUNE_GEMM_CONFIG, TUNE_GEMM_GROUP_M, TUNE_GEMM_MAX_CTAS, TUNE_GEMV_SPLIT, TUNE_GEMV_VARIANT, TUNE_GEMV_SHAPE, TUNE_FLAGS, TUNE_ADD_SHAPE = range(8)
 
-EXPORTS = ("tile_gemm", "tile_gemm_ex", "tile_gemm_static_b", "tile_gemm_typed", "tile_gemm_swiglu", "tile_add_f32",
+EXPORTS = ("tile_gemm", "tile_gemm_ex", "tile_gemm_static_b", "tile_gemm_typed", "tile_gemm_swiglu", "tile_add_f32", "tile_read_probe_u32",
            "tile_gemm_record_begin", "tile_gemm_record_end", "tile_gemm_replay", "tile_gemm_recorded_nodes",
            "tile_gemm_record_free", "tile_gemm_select", "tile_gemm_host",
            "tile_gemm_debug_owner_map", "tile_gemm_query_config", "tile_gemm_query_plan", "tile_gemm_set_tuning",
@@ -79,6 +79,8 @@ def load_library():
     lib.tile_gemm_typed.restype = _int
     lib.tile_gemm_swiglu.argtypes = g + [_vp]
     lib.tile_gemm_swiglu.restype = _int
+    lib.tile_read_probe_u32.argtypes = [_vp, _i64, _vp, _vp]
+    lib.tile_read_probe_u32.restype = _int
     lib.tile_add_f32.argtypes = [_vp, _vp, _vp, _i64, _vp]
     lib.tile_add_f32.restype = _int
     lib.tile_gemm_record_begin.argtypes = [_vp]
@@ -234,6 +236,17 @@ def tile_gemm_swiglu(X: torch.Tensor, Wgu: torch.Tensor, H: torch.Tensor | None 
     _check(load_library().tile_gemm_swiglu(_vp(X.data_ptr()), _vp(Wgu.data_ptr()), _vp(H.data_ptr()), M, inter, K,
                                            _ld(X), _ld(Wgu), _ld(H), od, _vp(_stream_handle(stream))))
     return H
+
+
+def tile_read_probe_u32(buf: torch.Tensor, out_sum: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+    """Adds the sum of buf's 32-bit words (mod 2^64) to out_sum (a 1-element int64 tensor, created zeroed if None)."""
+    if buf.element_size() * buf.numel() % 4 or not buf.is_contiguous():
+        raise ValueError("buf must be contiguous and a whole number of 32-bit words")
+    if out_sum is None:
+        out_sum = torch.zeros(1, dtype=torch.int64, device=buf.device)
+    _check(load_library().tile_read_probe_u32(_vp(buf.data_ptr()), buf.element_size() * buf.numel() // 4,
+                                              _vp(out_sum.data_ptr()), _vp(_stream_handle(stream))))
+    return out_sum
 
 
 def tile_add_f32_raw(x: int, y: int, z: int, n: int, stream: int = 0) -> int:

@@ -41,4 +41,44 @@ zero_fill_kernel(void* C, int64_t M, int64_t N, int64_t ldc, int esize) {
     }
 }
 
+// Read-bandwidth probe ("a read-only streaming probe kernel ... to establish this
+// box's achievable read bandwidth"): *out += sum of n 32-bit words as a 64-bit integer (exact, order
+// independent).  One 32 KB tile per CTA, eight 16-byte loads in flight per thread (the shape of the
+// fastest stand-alone probe: 7.5 TB/s on B200), one atomic per CTA; the words past the last full
+// vector are added by the last CTA.
+constexpr int PROBE_THREADS = 256, PROBE_UNROLL = 8;
+__global__ void __launch_bounds__(PROBE_THREADS)
+read_probe_kernel(const uint32_t* __restrict__ buf, int64_t n, unsigned long long* out) {
+    __shared__ unsigned long long warp_sums[PROBE_THREADS / 32];
+    const int64_t nvec = n >> 2;
+    const uint4* v4 = reinterpret_cast<const uint4*>(buf);
+    const int64_t base = (int64_t)blockIdx.x * (PROBE_THREADS * PROBE_UNROLL) + threadIdx.x;
+    uint4 a[PROBE_UNROLL];
+#pragma unroll
+    for (int u = 0; u < PROBE_UNROLL; ++u) {
+        a[u] = make_uint4(0, 0, 0, 0);
+        if (base + u * PROBE_THREADS < nvec)
+            asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
+                         : "=r"(a[u].x), "=r"(a[u].y), "=r"(a[u].z), "=r"(a[u].w)
+                         : "l"(v4 + base + u * PROBE_THREADS));
+    }
+    unsigned long long s = 0;
+#pragma unroll
+    for (int u = 0; u < PROBE_UNROLL; ++u) s += (unsigned long long)a[u].x + a[u].y + a[u].z + a[u].w;
+    if (blockIdx.x == gridDim.x - 1) {
+        const int64_t e = (nvec << 2) + threadIdx.x;
+        if (e < n) s += __ldg(buf + e);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) warp_sums[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned long long t = 0;
+#pragma unroll
+        for (int w = 0; w < PROBE_THREADS / 32; ++w) t += warp_sums[w];
+        if (t) atomicAdd(out, t);
+    }
+}
+
 }  // namespace tg

@@ -1024,6 +1024,26 @@ int tile_gemm_swiglu(const void* X, const void* Wgu, void* H, int64_t M, int64_t
     return launch_gemm_inst<2, 256, 4, 2, false, 1>(ta, tb, tc, p, gl.ctas, s, dev);
 }
 
+int tile_read_probe_u32(const uint32_t* buf, int64_t n, unsigned long long* out_sum, void* stream) {
+    if (n < 0) return fail(TILE_GEMM_E_EXTENT, "negative extent: n=%lld", (long long)n);
+    if (!out_sum) return fail(TILE_GEMM_E_NULL, "out_sum is NULL");
+    if (n > 0 && !buf) return fail(TILE_GEMM_E_NULL, "buf is NULL but n > 0");
+    if (((uintptr_t)buf & 15) || ((uintptr_t)out_sum & 7))
+        return fail(TILE_GEMM_E_ALIGN, "buf (%p) must be 16-byte and out_sum (%p) 8-byte aligned", (const void*)buf, (void*)out_sum);
+    if (n > (int64_t(1) << 40)) return fail(TILE_GEMM_E_OVERFLOW, "n=%lld above 2^40 words", (long long)n);
+    if (overlaps(out_sum, 8, buf, n * 4)) return fail(TILE_GEMM_E_ALIAS, "out_sum lies inside buf");
+    int dev = 0, sms = 0;
+    int rc = current_device(&dev, &sms);
+    if (rc) return rc;
+    if (n == 0) return TILE_GEMM_OK;
+    const int64_t tile = (int64_t)tg::PROBE_THREADS * tg::PROBE_UNROLL;
+    const int64_t grid = ((n >> 2) + tile - 1) / tile + ((n >> 2) % tile == 0 ? 1 : 0);   // the last CTA also owns the < 4-word tail
+    tg::read_probe_kernel<<<(unsigned)grid, tg::PROBE_THREADS, 0, (cudaStream_t)stream>>>(buf, n, out_sum);
+    CUDA_TRY(cudaGetLastError());
+    g_launches.fetch_add(1);
+    return TILE_GEMM_OK;
+}
+
 int tile_add_f32(const float* x, const float* y, float* z, int64_t n, void* stream) {
     if (n < 0) return fail(TILE_GEMM_E_EXTENT, "negative extent: n=%lld", (long long)n);
     if (n == 0) return TILE_GEMM_OK;

@@ -437,3 +437,31 @@ def test_recorded_step_with_lockstep_and_split_gemm():
     rows, cols = wl.uniform_samples(M, N, 1024, seed=81)
     c, sc = oracle.gemm_sampled(a, b, rows, cols)
     check_close(oracle.bf16_decode(wl.torch_to_bits(want)[rows, cols]), c, sc, K, "bf16", "recorded long-K GEMM")
+
+
+# ------------------------------------------------------------------ read-bandwidth probe
+@pytest.mark.parametrize("n", [0, 1, 3, 4, 1023, 1024, 1025, 1027, 100_003, (1 << 24) + 5])
+def test_read_probe_is_the_word_sum(n):
+    g = torch.Generator(device=DEV)
+    g.manual_seed(90 + n % 97)
+    buf = torch.randint(-2 ** 31, 2 ** 31 - 1, (n + 4,), dtype=torch.int32, device=DEV, generator=g)[:n]
+    out = torch.full((1,), 5, dtype=torch.int64, device=DEV)          # accumulates on top of what is there
+    lib = tg.load_library()
+    import ctypes
+    rc = lib.tile_read_probe_u32(ctypes.c_void_p(buf.data_ptr()), n, ctypes.c_void_p(out.data_ptr()), None)
+    assert rc == tg.E_OK
+    torch.cuda.synchronize()
+    want = (oracle.word_sum_u32(buf.cpu().numpy()) + 5) % 2 ** 64
+    assert int(out.item()) % 2 ** 64 == want
+
+
+def test_read_probe_preconditions():
+    import ctypes
+    lib = tg.load_library()
+    buf = torch.zeros(64, dtype=torch.int32, device=DEV)
+    out = torch.zeros(1, dtype=torch.int64, device=DEV)
+    vp = ctypes.c_void_p
+    assert lib.tile_read_probe_u32(vp(buf.data_ptr()), -1, vp(out.data_ptr()), None) == tg.E_EXTENT
+    assert lib.tile_read_probe_u32(vp(buf.data_ptr() + 4), 8, vp(out.data_ptr()), None) == tg.E_ALIGN
+    assert lib.tile_read_probe_u32(vp(buf.data_ptr()), 8, None, None) == tg.E_NULL
+    assert lib.tile_read_probe_u32(vp(buf.data_ptr()), 64, vp(buf.data_ptr() + 8), None) == tg.E_ALIAS

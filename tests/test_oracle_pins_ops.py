@@ -234,3 +234,11 @@ def test_swiglu_gemm_special_cases():
     Wb = wl.f32_to_bf16_bits(np.concatenate([np.full((K, 4), 64.0, np.float32), wu[:, :4]], axis=1))
     Hb, Gb, Ub, _, _ = oracle.swiglu_gemm(xo, Wb)
     assert np.array_equal(Hb, Gb * Ub)
+
+
+def test_word_sum_against_python_integers():
+    rng = np.random.default_rng(14)
+    w = rng.integers(0, 2 ** 32, 5000, dtype=np.uint64).astype(np.uint32)
+    assert oracle.word_sum_u32(w) == sum(int(v) for v in w) % 2 ** 64
+    assert oracle.word_sum_u32(np.full(3, 0xFFFFFFFF, np.uint32)) == 3 * 0xFFFFFFFF
+    assert oracle.word_sum_u32(np.zeros(0, np.uint32)) == 0
