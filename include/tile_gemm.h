@@ -278,22 +278,25 @@ int tile_gemm_query_plan(int64_t M, int64_t N, int64_t K, int32_t out[8]);
 
 /*
  * Tuning / test overrides, process-global, not thread-safe against concurrent
- * tile_gemm calls.  key: 0 = GEMM config (0 auto, 1 = 1-CTA 128x128, 2 = 1-CTA
- * 128x256, 3 = 2-CTA 256x256, 4 = 2-CTA 256x512), 1 = GEMM GROUP_M (0 auto), 2 = GEMM max CTAs
- * (0 = all SMs; also caps the GEMV grid), 3 = split-K of the cluster GEMV
- * (0 auto), 4 = GEMV kernel (0 auto = 4 when B is TMA-addressable, 1 = TMA ring +
- * cluster split-K, 2 = 16-byte LDG, 3 = scalar LDG, 4 = TMA ring + interleaved
- * split-K with ticketed fix-up), 5 = ring shape of kernel 4 (0 auto; 1..8 =
- * {columns per CTA, rows per stage, stages, CTAs per SM}, table kGemvShapes in
- * csrc/tile_gemm.cu), 6 = bit 0 disables programmatic dependent launch, bit 1 makes
- * kernel 4 read x with global loads instead of through its TMA ring; bit 2 forces the GEMM's
- * lockstep producers on, bit 3 off, bits 8-15 their window in k-tiles (0 = 32), bit 5 = full 128-row A
- * box even for skinny M, bit 6 = tile_gemm_host in one shot instead of pipelined chunks; key 3 also
- * overrides kernel 4's split, 7 = tile_add_f32 launch shape
- * (bits 0-3 vectors per thread in {1,2,4,8}, bits 4-11 CTAs per SM with 255 = one tile per
- * CTA, bits 12-15 access mode: 1/2 = 128-bit with/without streaming hints, 3/4 = 256-bit
- * with/without; 0 in a field = its default).  Returns 0 or
- * E_PATH for an unknown key.
+ * library calls; 0 always means "automatic".  Returns 0, or E_PATH for an unknown key.
+ *   key 0  GEMM tile configuration: 1 = 1-CTA 128x128, 2 = 1-CTA 128x256, 3 = CTA pair
+ *          256x256, 4 = CTA pair 256x512.
+ *   key 1  GEMM GROUP_M: tile rows per raster group.
+ *   key 2  maximum number of CTAs of a GEMM launch; also caps the GEMV grids.
+ *   key 3  K slices: of the M = 1 / M <= 4 kernels' column blocks, and (1 = never, >= 2 = that
+ *          many) of the GEMM's partial last wave.
+ *   key 4  M = 1 kernel: 1 = TMA ring + cluster split-K, 2 = 16-byte LDG, 3 = scalar LDG,
+ *          4 = TMA ring + interleaved split-K with ticketed fix-up (the automatic choice when B
+ *          is TMA-addressable).
+ *   key 5  ring shape of kernel 4, 1..8 = {columns per CTA, rows per stage, stages, CTAs per SM}
+ *          (table kGemvShapes in csrc/tile_gemm.cu).
+ *   key 6  flag bits: 0 = no programmatic dependent launch; 1 = kernel 4 reads x with global loads
+ *          instead of through its TMA ring; 2 / 3 = GEMM lockstep producers forced on / off, bits
+ *          8-15 = their window in k-tiles; 5 = full 128-row A box even for skinny M; 6 =
+ *          tile_gemm_host in one shot instead of pipelined chunks.
+ *   key 7  tile_add_f32 launch shape: bits 0-3 vectors per thread in {1,2,4,8}, bits 4-11 CTAs
+ *          per SM (255 = one tile per CTA), bits 12-15 access mode (1 / 2 = 128-bit with / without
+ *          streaming hints, 3 / 4 = 256-bit with / without).
  */
 int tile_gemm_set_tuning(int key, int value);
 
