@@ -7,6 +7,7 @@ raises, and on a machine without an sm_100 device every compute entry returns
 """
 from __future__ import annotations
 
+import contextlib
 import ctypes
 import os
 
@@ -37,6 +38,7 @@ EXPORTS = ("tile_gemm", "tile_gemm_ex", "tile_gemm_static_b", "tile_gemm_typed",
            "tile_gemm_shutdown")
 
 _lib = None
+_NULL_CTX = contextlib.nullcontext()
 _i64 = ctypes.c_int64
 _vp = ctypes.c_void_p
 _int = ctypes.c_int
@@ -54,19 +56,21 @@ def library_path() -> str:
 
 
 def load_library():
-    """Loads (building first if the in-tree .so is missing or stale and nvcc exists)."""
+    """Loads csrc/libtilegemm.so, building it first when it is missing or older than its sources.
+    A rebuild that is needed and fails raises: a stale library is never loaded silently
+    (TILEGEMM_NO_REBUILD=1 skips the staleness check for a deployed, prebuilt library)."""
     global _lib
     if _lib is not None:
         return _lib
     path = _build.LIB
-    if not os.path.exists(path) or _build.needs_build():
+    stale_check = os.environ.get("TILEGEMM_NO_REBUILD", "0") != "1"
+    if not os.path.exists(path) or (stale_check and _build.needs_build()):
+        why = "is missing" if not os.path.exists(path) else "is older than its sources"
         try:
             _build.build()
-        except Exception as exc:  # no nvcc here and no prebuilt library: fail loudly
-            if not os.path.exists(path):
-                raise RuntimeError(
-                    f"libtilegemm.so is missing and could not be built ({exc}); "
-                    "the CUDA path has no fallback") from exc
+        except Exception as exc:
+            raise RuntimeError(f"libtilegemm.so {why} and could not be built ({exc}); "
+                               "the CUDA path has no fallback") from exc
     lib = ctypes.CDLL(path)
     g = [_vp, _vp, _vp, _i64, _i64, _i64, _i64, _i64, _i64, _int]
     lib.tile_gemm.argtypes = g + [_vp]
@@ -128,6 +132,20 @@ def _stream_handle(stream) -> int:
     return int(stream.cuda_stream) if hasattr(stream, "cuda_stream") else int(stream)
 
 
+def _on_device(*tensors):
+    """All tensors must live on one CUDA device; the call then runs with that device current
+    (the library launches on the current device and dereferences raw pointers)."""
+    dev = tensors[0].device
+    for t in tensors:
+        if not t.is_cuda:
+            raise TypeError("expected CUDA tensors (tile_gemm_host takes host buffers)")
+        if t.device != dev:
+            raise ValueError(f"operands live on different devices: {dev} and {t.device}")
+    if dev.index is None or dev.index == torch.cuda.current_device():
+        return _NULL_CTX
+    return torch.cuda.device(dev)
+
+
 def _ld(t: torch.Tensor) -> int:
     if t.dim() != 2 or (t.shape[1] > 1 and t.stride(1) != 1):
         raise ValueError("expected a 2-D row-major tensor (unit column stride)")
@@ -187,6 +205,13 @@ def tile_gemm(A: torch.Tensor, B: torch.Tensor, C: torch.Tensor | None = None, o
     if C.dtype not in (torch.float32, torch.bfloat16, torch.float16) or tuple(C.shape) != (M, N):
         raise TypeError("C must be an (M,N) float32, bfloat16 or float16 tensor")
     od = {torch.float32: OUT_F32, torch.bfloat16: OUT_BF16, torch.float16: OUT_F16}[C.dtype]
+    with _on_device(A, B, C):
+        st = _tile_gemm_call(A, B, C, M, N, K, od, stream, force_path, static_b)
+    _check(st)
+    return C
+
+
+def _tile_gemm_call(A, B, C, M, N, K, od, stream, force_path, static_b) -> int:
     if A.dtype == torch.float16 or od == OUT_F16:
         if static_b or force_path != PATH_AUTO:
             raise ValueError("static_b / force_path apply to the bf16 entries only")
@@ -202,8 +227,7 @@ def tile_gemm(A: torch.Tensor, B: torch.Tensor, C: torch.Tensor | None = None, o
         st = load_library().tile_gemm_ex(_vp(A.data_ptr()), _vp(B.data_ptr()), _vp(C.data_ptr()), M, N, K,
                                          _ld(A), _ld(B), _ld(C), od, _vp(_stream_handle(stream)),
                                          int(force_path))
-    _check(st)
-    return C
+    return int(st)
 
 
 def tile_gemm_typed_raw(A: int, B: int, C: int, M, N, K, lda, ldb, ldc, in_dtype, out_dtype, stream: int = 0) -> int:
@@ -232,9 +256,13 @@ def tile_gemm_swiglu(X: torch.Tensor, Wgu: torch.Tensor, H: torch.Tensor | None 
         H = torch.empty((M, inter), dtype=dt, device=X.device)
     if tuple(H.shape) != (M, inter):
         raise TypeError("H must be (M, I)")
+    if H.dtype not in (torch.float32, torch.bfloat16, torch.float16):
+        raise TypeError("H must be float32, bfloat16 or float16")
     od = {torch.float32: OUT_F32, torch.bfloat16: OUT_BF16, torch.float16: OUT_F16}[H.dtype]
-    _check(load_library().tile_gemm_swiglu(_vp(X.data_ptr()), _vp(Wgu.data_ptr()), _vp(H.data_ptr()), M, inter, K,
-                                           _ld(X), _ld(Wgu), _ld(H), od, _vp(_stream_handle(stream))))
+    with _on_device(X, Wgu, H):
+        st = load_library().tile_gemm_swiglu(_vp(X.data_ptr()), _vp(Wgu.data_ptr()), _vp(H.data_ptr()), M, inter, K,
+                                             _ld(X), _ld(Wgu), _ld(H), od, _vp(_stream_handle(stream)))
+    _check(st)
     return H
 
 
@@ -244,8 +272,10 @@ def tile_read_probe_u32(buf: torch.Tensor, out_sum: torch.Tensor | None = None, 
         raise ValueError("buf must be contiguous and a whole number of 32-bit words")
     if out_sum is None:
         out_sum = torch.zeros(1, dtype=torch.int64, device=buf.device)
-    _check(load_library().tile_read_probe_u32(_vp(buf.data_ptr()), buf.element_size() * buf.numel() // 4,
-                                              _vp(out_sum.data_ptr()), _vp(_stream_handle(stream))))
+    with _on_device(buf, out_sum):
+        st = load_library().tile_read_probe_u32(_vp(buf.data_ptr()), buf.element_size() * buf.numel() // 4,
+                                                _vp(out_sum.data_ptr()), _vp(_stream_handle(stream)))
+    _check(st)
     return out_sum
 
 
@@ -263,8 +293,10 @@ def tile_add_f32(x: torch.Tensor, y: torch.Tensor, z: torch.Tensor | None = None
         z = torch.empty_like(x)
     if z.dtype != torch.float32 or z.numel() != x.numel() or not z.is_contiguous():
         raise TypeError("z must be a contiguous float32 tensor of the same length")
-    _check(load_library().tile_add_f32(_vp(x.data_ptr()), _vp(y.data_ptr()), _vp(z.data_ptr()), x.numel(),
-                                       _vp(_stream_handle(stream))))
+    with _on_device(x, y, z):
+        st = load_library().tile_add_f32(_vp(x.data_ptr()), _vp(y.data_ptr()), _vp(z.data_ptr()), x.numel(),
+                                         _vp(_stream_handle(stream)))
+    _check(st)
     return z
 
 
@@ -301,8 +333,17 @@ def tile_gemm_host(A_bits, B_bits, C_out, lda=None, ldb=None, ldc=None):
     """End-to-end on HOST numpy arrays: A_bits (M,K) uint16, B_bits (K,N) uint16 bf16 patterns,
     C_out (M,N) float32 or uint16 (bf16 patterns), all C-contiguous rows."""
     import numpy as np
+    if A_bits.dtype != np.uint16 or B_bits.dtype != np.uint16:
+        raise TypeError("A_bits and B_bits must be uint16 arrays of bf16 bit patterns")
+    if C_out.dtype not in (np.float32, np.uint16):
+        raise TypeError("C_out must be float32 or uint16 (bf16 bit patterns)")
+    for arr in (A_bits, B_bits, C_out):
+        if arr.ndim != 2 or (arr.shape[1] > 1 and arr.strides[1] != arr.itemsize):
+            raise ValueError("expected 2-D arrays with contiguous rows")
     M, K = A_bits.shape
-    _, N = B_bits.shape
+    K2, N = B_bits.shape
+    if K2 != K or C_out.shape != (M, N):
+        raise ValueError("shapes do not form C (M,N) = A (M,K) @ B (K,N)")
     od = OUT_F32 if C_out.dtype == np.float32 else OUT_BF16
     lda = lda or max(A_bits.strides[0] // 2, K, 1)
     ldb = ldb or max(B_bits.strides[0] // 2, N, 1)
@@ -337,27 +378,3 @@ def tile_gemm_debug_owner_map(M, N, K, out_dtype=OUT_F32, ld_owner=None, stream=
     _check(load_library().tile_gemm_debug_owner_map(_vp(owner.data_ptr()), M, N, K, ld, int(out_dtype),
                                                     _vp(_stream_handle(stream))))
     return owner
-
-
-def expected_owner_map(M, N, cfg: dict):
-    """Host restatement of the kernel's tile -> owner function (csrc/gemm_kernel.cuh,
-    tile_coords + round-robin over clusters) for the owner-map test."""
-    import numpy as np
-    tile_m = cfg["BM"] * cfg["cta_group"]
-    tiles_m = -(-M // tile_m)
-    tiles_n = -(-N // cfg["BN"])
-    clusters = cfg["ctas"] // cfg["cta_group"]
-    own = np.full((M, N), -1, dtype=np.int64)
-    for t in range(tiles_m * tiles_n):
-        per_group = cfg["group_m"] * tiles_n
-        g = t // per_group
-        first_m = g * cfg["group_m"]
-        rows = min(cfg["group_m"], tiles_m - first_m)
-        r = t - g * per_group
-        tm, tn = first_m + r % rows, r // rows
-        cluster = t % clusters
-        for rank in range(cfg["cta_group"]):
-            cta = cluster * cfg["cta_group"] + rank
-            r0 = (tm * cfg["cta_group"] + rank) * cfg["BM"]
-            own[r0:r0 + cfg["BM"], tn * cfg["BN"]:(tn + 1) * cfg["BN"]] = (t << 8) | cta
-    return own

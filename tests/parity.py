@@ -75,3 +75,26 @@ def freivalds_rows(C_gpu_f64, a64, b64, seed=0):
     tol = rel * np.linalg.norm(C_gpu_f64, axis=0) + 1e-30
     bad = np.abs(lhs - rhs) > tol
     assert not bad.any(), f"Freivalds column test failed for columns {np.where(bad)[0][:8].tolist()}"
+
+
+def expected_owner_map(M, N, cfg: dict):
+    """Host restatement of the kernel's tile -> owner function (csrc/gemm_kernel.cuh,
+    tile_coords + round-robin over clusters) for the owner-map test."""
+    tile_m = cfg["BM"] * cfg["cta_group"]
+    tiles_m = -(-M // tile_m)
+    tiles_n = -(-N // cfg["BN"])
+    clusters = cfg["ctas"] // cfg["cta_group"]
+    own = np.full((M, N), -1, dtype=np.int64)
+    for t in range(tiles_m * tiles_n):
+        per_group = cfg["group_m"] * tiles_n
+        g = t // per_group
+        first_m = g * cfg["group_m"]
+        rows = min(cfg["group_m"], tiles_m - first_m)
+        r = t - g * per_group
+        tm, tn = first_m + r % rows, r // rows
+        cluster = t % clusters
+        for rank in range(cfg["cta_group"]):
+            cta = cluster * cfg["cta_group"] + rank
+            r0 = (tm * cfg["cta_group"] + rank) * cfg["BM"]
+            own[r0:r0 + cfg["BM"], tn * cfg["BN"]:(tn + 1) * cfg["BN"]] = (t << 8) | cta
+    return own

@@ -14,6 +14,7 @@ import torch
 import oracle
 from paper_2606_15991_b200 import binding as tg
 from paper_2606_15991_b200 import workloads as wl
+import parity
 from parity import check_bit_exact, check_close, freivalds_rows
 
 pytestmark = pytest.mark.gpu
@@ -366,7 +367,7 @@ def test_owner_map_is_the_documented_function(cfg, shape):
         torch.cuda.synchronize()
         host = owner.cpu().numpy()
         assert np.all(host[:, N:] == -1), "padding columns were written"
-        want = tg.expected_owner_map(M, N, conf)
+        want = parity.expected_owner_map(M, N, conf)
         assert np.array_equal(host[:, :N].astype(np.int64), want)
         ctas = np.unique(host[:, :N] & 0xFF)
         assert ctas.max() < conf["ctas"]

@@ -11,6 +11,7 @@ import numpy as np
 import pytest
 import torch
 
+import parity
 from paper_2606_15991_b200 import binding as tg
 from paper_2606_15991_b200 import workloads as wl
 
@@ -112,7 +113,7 @@ def test_schedule_function_covers_every_element_once(cfg, shape):
     """The tile -> owner map restated on the host is a function onto [0,M) x [0,N): every
     element has exactly one owning tile and CTA ids stay below the launched count."""
     M, N = shape
-    own = tg.expected_owner_map(M, N, cfg)
+    own = parity.expected_owner_map(M, N, cfg)
     assert own.min() >= 0
     tile_m = cfg["BM"] * cfg["cta_group"]
     tiles = -(-M // tile_m) * -(-N // cfg["BN"])
