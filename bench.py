@@ -290,7 +290,7 @@ def bench_decode(tg, wl, torch, passes, warmup, layers, tdist, static_b=True):
         e1.record()
         torch.cuda.synchronize()
         t = e0.elapsed_time(e1) / len(sel)
-        per_shape[f"K{K}_N{N}"] = {"us": t * 1e3, "gbs": (2 * K * N + 2 * K + 2 * N) / (t * 1e-3) / 1e9}
+        per_shape[f"K{K}_N{N}"] = {"us": round(t * 1e3, 2), "gbs": round((2 * K * N + 2 * K + 2 * N) / (t * 1e-3) / 1e9, 1)}
     # replay of the same pass as one recorded step of the library's own C ABI (tile_gemm_record_*:
     # decode engines replay a recorded step)
     graph_ms = None
@@ -413,19 +413,27 @@ def bench_skinny(tg, wl, torch, ms_list, tdist, layers=8):
         one_pass(0)
         ms = tdist.max_over_ranks(time_region(one_pass, 3, torch.cuda.synchronize, tdist.barrier)) / 3
         byt = sum(2 * K * N + 2 * M * K + 2 * M * N for (K, N) in wl.QWEN3_32B) * layers
-        out[str(M)] = {"ms_per_pass": ms, "gbs": byt / (ms * 1e-3) / 1e9, "launches_per_pass": 4 * layers}
+        out[str(M)] = {"ms_per_pass": round(ms, 4), "gbs": round(byt / (ms * 1e-3) / 1e9, 1), "launches_per_pass": 4 * layers}
     return out
 
 
-def bench_sweep(tg, torch, sizes, tdist):
+SWEEP_COLUMNS = ["us_median_single", "us_back_to_back", "us_recorded_replay", "tflops_recorded_replay", "tile_config"]
+
+
+def bench_sweep(tg, torch, sizes, tdist, warm_s=0.35):
     """the paper's Figure 6b sweep, M=N=K powers of two, f16 (the
-    paper's precision) and bf16, 16-bit output.  Per size: median of `reps` single-launch timings
-    (paper: medians) on rotating operand sets whose total exceeds L2 where the problem allows."""
+    paper's precision) and bf16, 16-bit output, on rotating operand sets whose total exceeds L2 where
+    the problem allows.  Steady-state protocol: every timing of a (size, type) is taken
+    directly after `warm_s` seconds of back-to-back launches of that same problem, so that all three
+    see the chip in the power state a pipeline of such GEMMs runs in; the type order alternates from
+    size to size.  Per size: median of per-launch event timings inside a back-to-back stream (paper:
+    medians), the back-to-back average without inner events (programmatic dependent launch intact),
+    and the same launches as ONE recorded step (no host in the loop).  Rows follow SWEEP_COLUMNS."""
     dev = torch.device("cuda", torch.cuda.current_device())
-    out = {"f16": {}, "bf16": {}}
-    for n in sizes:   # sizes outer, types inner: both types of a size see the same power state
-        for dt_name, dt in (("f16", torch.float16), ("bf16", torch.bfloat16)):
-            rows = out[dt_name]
+    out = {"columns": SWEEP_COLUMNS, "f16": {}, "bf16": {}}
+    types = (("f16", torch.float16), ("bf16", torch.bfloat16))
+    for si, n in enumerate(sizes):
+        for dt_name, dt in (types if si % 2 == 0 else types[::-1]):
             per_set = 3 * n * n * 2
             sets = int(max(1, min(8, (256 << 20) // per_set + 1)))
             reps = 40 if n <= 4096 else (12 if n <= 16384 else 5)
@@ -434,42 +442,45 @@ def bench_sweep(tg, torch, sizes, tdist):
             bufs = [(torch.empty((n, n), dtype=dt, device=dev).normal_(0, 1, generator=g),
                      torch.empty((n, n), dtype=dt, device=dev).normal_(0, n ** -0.5, generator=g),
                      torch.empty((n, n), dtype=dt, device=dev)) for _ in range(sets)]
-            for i in range(3):
-                A, B, C = bufs[i % sets]
-                tg.tile_gemm(A, B, C)
-            torch.cuda.synchronize()
-            ts = []
+
+            def warm(seconds):
+                t_end = time.perf_counter() + seconds
+                i = 0
+                while time.perf_counter() < t_end:
+                    for _ in range(8):
+                        tg.tile_gemm(*bufs[i % sets])
+                        i += 1
+                    if n >= 8192:
+                        torch.cuda.synchronize()   # keep the launch queue short: the warm-up must end on time
+
+            warm(warm_s)
+            # (a) per-launch events inside a back-to-back stream
+            evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
             for i in range(reps):
-                A, B, C = bufs[i % sets]
-                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                e0.record()
-                tg.tile_gemm(A, B, C)
-                e1.record()
-                e1.synchronize()
-                ts.append(e0.elapsed_time(e1))
-            # back-to-back (launch latency hidden by the queue): what a pipeline of GEMMs sees
-            tdist.barrier()
+                evs[i][0].record()
+                tg.tile_gemm(*bufs[i % sets])
+                evs[i][1].record()
             torch.cuda.synchronize()
+            med = float(np.median([a.elapsed_time(b) for a, b in evs]))
+            # (b) back to back, no inner events
+            warm(warm_s / 3)
+            tdist.barrier()
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record()
             for i in range(reps):
-                A, B, C = bufs[i % sets]
-                tg.tile_gemm(A, B, C)
+                tg.tile_gemm(*bufs[i % sets])
             e1.record()
             torch.cuda.synchronize()
             b2b = e0.elapsed_time(e1) / reps
-            # the same launches as ONE recorded step: no host in the loop (a Python launch costs ~9 us,
-            # the C entry ~5 us, a 1024^3 GEMM ~6 us of GPU time -- the loop above is host-bound there)
+            # (c) the same launches as one recorded step
             rs = torch.cuda.Stream()
-            for i in range(min(reps, sets)):
-                tg.tile_gemm(*bufs[i % sets], stream=rs)
-            rs.synchronize()
             tg.tile_gemm_record_begin(rs)
             for i in range(reps):
                 tg.tile_gemm(*bufs[i % sets], stream=rs)
             step = tg.tile_gemm_record_end(rs)
+            warm(warm_s / 3)
+            torch.cuda.synchronize()
             step.replay(rs)
-            rs.synchronize()
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record(rs)
             step.replay(rs)
@@ -477,16 +488,46 @@ def bench_sweep(tg, torch, sizes, tdist):
             rs.synchronize()
             rep_ms = e0.elapsed_time(e1) / reps
             step.free()
-            med = float(np.median(ts))
             fl = 2.0 * n ** 3
-            rows[str(n)] = {"us_median": med * 1e3, "tflops_median": fl / (med * 1e-3) / 1e12,
-                            "us_back_to_back": b2b * 1e3, "tflops_back_to_back": fl / (b2b * 1e-3) / 1e12,
-                            "us_recorded_replay": rep_ms * 1e3, "tflops_recorded_replay": fl / (rep_ms * 1e-3) / 1e12,
-                            "tile_config": tg.tile_gemm_query_config(n, n, n, tg.OUT_BF16)["config"],
-                            "operand_sets": sets}
+            out[dt_name][str(n)] = [round(med * 1e3, 1), round(b2b * 1e3, 1), round(rep_ms * 1e3, 1),
+                                    round(fl / (rep_ms * 1e-3) / 1e12, 1),
+                                    tg.tile_gemm_query_config(n, n, n, tg.OUT_BF16)["config"]]
             del bufs
             torch.cuda.empty_cache()
     return out
+
+
+def bench_sustained(tg, torch, case, seconds, local_rank, tdist):
+    """cfg3 back to back for >= `seconds`: the figure to hold against MEASURED_PEAKS.json's sustained
+    cuBLAS number (a seconds-long loop under the power cap), with its own clock record."""
+    dev = torch.device("cuda", torch.cuda.current_device())
+    g = torch.Generator(device=dev)
+    g.manual_seed(1000 + case.seed[0])
+    sets = 4
+    bufs = [(torch.empty((case.M, case.K), dtype=torch.bfloat16, device=dev).normal_(0, case.sigma_a, generator=g),
+             torch.empty((case.K, case.N), dtype=torch.bfloat16, device=dev).normal_(0, case.sigma_b, generator=g),
+             torch.empty((case.M, case.N), dtype=torch.bfloat16, device=dev)) for _ in range(sets)]
+    for i in range(8):
+        tg.tile_gemm(*bufs[i % sets])
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local_rank)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    tdist.barrier()
+    steps = 0
+    with sampler:
+        t_end = time.perf_counter() + seconds
+        e0.record()
+        while time.perf_counter() < t_end:
+            for _ in range(64):
+                tg.tile_gemm(*bufs[steps % sets])
+                steps += 1
+            torch.cuda.synchronize()      # bounded queue: the loop ends when the clock says so
+        e1.record()
+        torch.cuda.synchronize()
+    ms = tdist.max_over_ranks(e0.elapsed_time(e1))
+    del bufs
+    torch.cuda.empty_cache()
+    return ms / steps, steps, ms, sampler.summary()
 
 
 def run_cuda(args):
@@ -523,13 +564,20 @@ def run_cuda(args):
         "gpu_launches": int(launches * world),
         "roofline": {"bound": "tensor", "achieved": per_gpu, "peak": peaks["bf16_tflops"], "unit": "TFLOP/s",
                      "frac": per_gpu / peaks["bf16_tflops"], "traffic": ncu_traffic("gemm_8192_dram_bytes"),
-                     "peak_source": f"{peaks['source']} cuBLAS bf16 burst (MEASURED_PEAKS.json)",
-                     "frac_of_sustained": per_gpu / peaks["bf16_tflops_sustained"],
+                     "peak_source": f"{peaks['source']} cuBLAS bf16 burst (MEASURED_PEAKS.json): the --steps leg is a burst",
                      "frac_of_nominal_2250": per_gpu / 2250.0,
                      "kernel": "gemm_tcgen05_kernel<2,256,4,2,false,0>", "algorithmic_flops_per_launch": flops},
     }
     del bufs
     torch.cuda.empty_cache()
+    if not args.no_sustained:
+        # the same step back to back for seconds: what MEASURED_PEAKS.json's sustained cuBLAS figure is measured like
+        s_ms, s_steps, s_total, s_clocks = bench_sustained(tg, torch, case, args.sustained_seconds, local_rank, tdist)
+        s_tf = flops / (s_ms * 1e-3) / 1e12
+        line["roofline"]["sustained"] = {
+            "achieved": s_tf, "peak": peaks["bf16_tflops_sustained"], "frac": s_tf / peaks["bf16_tflops_sustained"],
+            "unit": "TFLOP/s", "ms_per_step": s_ms, "steps": s_steps, "seconds": s_total * 1e-3, "clocks": s_clocks,
+            "peak_source": f"{peaks['source']} cuBLAS bf16 back to back for seconds (MEASURED_PEAKS.json)"}
 
     if rank == 0 and not args.no_e2e:
         dt, h2d, d2h, _ = bench_e2e(tg, wl, torch, case, max(2, min(args.steps, 5)))
@@ -538,6 +586,7 @@ def run_cuda(args):
                        "api": "tile_gemm_host (pinned host A,B,C; H2D + GEMM + D2H per step)"}
     tdist.barrier()
 
+    gemv_rec = probe_rec = None
     if not args.headline_only:
         # config[3]: prefill projections
         pre = {}
@@ -547,7 +596,7 @@ def run_cuda(args):
             del b
             torch.cuda.empty_cache()
             fl = 2.0 * c.M * c.N * c.K
-            pre[c.name] = {"ms": ms, "tflops": fl / (ms * 1e-3) / 1e12}
+            pre[c.name] = {"ms": round(ms, 4), "tflops": round(fl / (ms * 1e-3) / 1e12, 1)}
             tot_ms += ms
             tot_fl += fl
         pre["aggregate_tflops"] = tot_fl / (tot_ms * 1e-3) / 1e12
@@ -557,10 +606,10 @@ def run_cuda(args):
         ms, alg_bytes, gl, per_shape, graph_ms, n, plain_ms = bench_decode(tg, wl, torch, args.decode_passes, 2,
                                                                            args.decode_layers, tdist)
         gbs = alg_bytes / (ms * 1e-3) / 1e9
-        line["gemv"] = {
+        gemv_rec = {
             "metric": "decode_gemv_hbm_gbs", "value": gbs * world, "unit": "GB/s", "ms_per_pass": ms,
             "launches_per_pass": n, "layers": args.decode_layers, "algorithmic_bytes_per_pass": alg_bytes,
-            "api": "tile_gemm_static_b (weights immutable: tiles are prefetched ahead of the PDL wait)",
+            "api": "tile_gemm_static_b, plain stream launches (weights immutable: tiles are prefetched ahead of the PDL wait)",
             "plain_tile_gemm": {"ms_per_pass": plain_ms, "gbs": alg_bytes / (plain_ms * 1e-3) / 1e9},
             "per_shape": per_shape,
             "recorded_step_replay": None if graph_ms is None else {"ms_per_pass": graph_ms,
@@ -582,8 +631,11 @@ def run_cuda(args):
         probe_gbs = pbuf.numel() * 4 / (pms * 1e-3) / 1e9
         del pbuf
         torch.cuda.empty_cache()
-        line["read_probe"] = {"gbs": probe_gbs, "bytes": 4 << 30, "kernel": "read_probe_kernel (tile_read_probe_u32)"}
-        line["gemv"]["roofline"]["frac_of_read_probe"] = line["gemv"]["roofline"]["achieved"] / probe_gbs
+        probe_rec = {"gbs": probe_gbs, "bytes": 4 << 30, "kernel": "read_probe_kernel (tile_read_probe_u32)"}
+        gemv_rec["roofline"]["frac_of_read_probe"] = gemv_rec["roofline"]["achieved"] / probe_gbs
+        # the GEMV half of BASELINE.json's metric, also inside the top-level roofline record
+        line["roofline"]["gemv"] = {k: gemv_rec["roofline"][k] for k in
+                                    ("bound", "achieved", "peak", "unit", "frac", "frac_of_8000", "frac_of_read_probe", "kernel")}
         # element-wise add (Listing 1) at n = 2^28
         n_add = 1 << 28
         ms = bench_add(tg, torch, n_add, max(10, args.steps // 4), 3, tdist)
@@ -599,7 +651,7 @@ def run_cuda(args):
         }
         # per-op host cost, stream launches vs one recorded step
         if rank == 0:
-            line["replay"] = bench_launch_overhead(tg, torch)
+            line["replay"] = {k: (round(v, 3) if isinstance(v, float) else v) for k, v in bench_launch_overhead(tg, torch).items()}
         tdist.barrier()
         # fused gate/up + SwiGLU epilogue on the cfg4 gate_up shape vs the plain GEMM that writes [gate | up]
         c = wl.CFG4[2]
@@ -619,16 +671,21 @@ def run_cuda(args):
         ms_p = tdist.max_over_ranks(time_region(lambda i: tg.tile_gemm(Xs[i % 2], Wsw[i % 2], Cp), reps,
                                                 torch.cuda.synchronize, tdist.barrier)) / reps
         fl = 2.0 * c.M * c.N * c.K
-        line["swiglu"] = {"shape": f"M={c.M} K={c.K} 2I={c.N}", "fused_ms": ms_f, "fused_tflops": fl / (ms_f * 1e-3) / 1e12,
-                          "plain_gate_up_gemm_ms": ms_p, "plain_tflops": fl / (ms_p * 1e-3) / 1e12,
+        line["swiglu"] = {"shape": f"M={c.M} K={c.K} 2I={c.N}", "fused_ms": round(ms_f, 4), "fused_tflops": round(fl / (ms_f * 1e-3) / 1e12, 1),
+                          "plain_gate_up_gemm_ms": round(ms_p, 4), "plain_tflops": round(fl / (ms_p * 1e-3) / 1e12, 1),
                           "c_bytes_fused": c.M * c.N, "c_bytes_plain": 2 * c.M * c.N}
         del Xs, Wsw, Hs, Cp
         torch.cuda.empty_cache()
-        # skinny M through the GEMM's K slices
+        # skinny M
         line["skinny_m"] = bench_skinny(tg, wl, torch, [2, 4, 8, 16, 32, 64], tdist)
         # the paper's size sweep in f16 and bf16
         if not args.no_sweep:
             line["sweep"] = bench_sweep(tg, torch, [1024, 2048, 4096, 8192, 16384, 32768], tdist)
+    # the GEMV half of the metric goes LAST (before the short cpu_baseline record), so that it is in the
+    # final kilobytes of the line whatever the other legs print
+    if gemv_rec is not None:
+        line["read_probe"] = probe_rec
+        line["gemv"] = gemv_rec
     if rank == 0:
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = cpu_baseline_leg()
@@ -650,6 +707,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-sweep", action="store_true", help="skip the f16/bf16 size sweep (SURVEY 8(f)1)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-sustained", action="store_true", help="skip the seconds-long back-to-back cfg3 leg")
+    ap.add_argument("--sustained-seconds", type=float, default=2.5)
     ap.add_argument("--gemm-config", type=int, default=0, help="force a GEMM tile config (tile_gemm_set_tuning key 0)")
     ap.add_argument("--group-m", type=int, default=0, help="force the raster group height (tuning key 1)")
     args = ap.parse_args()

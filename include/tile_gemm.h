@@ -188,18 +188,28 @@ int tile_add_f32(const float* x, const float* y, float* z, int64_t n, void* stre
  * driver call.  Recorded nodes keep the operand ADDRESSES: the caller keeps
  * those buffers alive and at the same place, and may rewrite their contents
  * between replays ("replayed nodes do not depend on addresses that change across
- * replays").  Nothing may allocate while recording: run every
- * shape once on `stream` beforehand so that the library's workspaces exist
- * (a call that would have to grow one fails with TILE_GEMM_E_CUDA and says so).
+ * replays").  The same holds for the library's own memory: a step
+ * OWNS the workspaces its nodes use (split-K partial sums and tickets, lockstep
+ * counters, repacked operands).  They are allocated while recording, belong to no
+ * other step and to no direct call, and live until tile_gemm_record_free -- so a
+ * step stays valid whatever runs on any stream afterwards (larger shapes
+ * included), it may be replayed on any stream of the same device, and replays of
+ * different steps may overlap.  One step must not run concurrently with itself.
  * The M == 1 kernels keep their programmatic-dependent-launch edges inside the
- * step.  `stream` must not be NULL (the legacy default stream cannot be
- * captured).  A failed call while recording leaves the capture open; still call
- * record_end (it reports the invalidated capture).  tile_gemm_recorded_nodes
- * returns the number of graph nodes (kernels and workspace memsets) in a step,
- * -1 for anything that is not a live step; tile_gemm_launch_count grows by that
- * number per replay.  tile_gemm_record_free destroys a step (NULL is a no-op).
- * Steps reference the library's per-stream workspaces: free them (or stop
- * replaying them) before tile_gemm_shutdown.
+ * step.  `stream` must not be NULL (the legacy default stream cannot be captured)
+ * and must not already be recording (E_PATH); record_end on a stream that is not
+ * recording fails with E_PATH.  The capture uses cudaStreamCaptureModeRelaxed.
+ * A failed call while recording leaves the capture open; still call record_end
+ * (it reports the invalidated capture and releases what the recording held).
+ * Library calls on a stream the CALLER captures itself (cudaStreamBeginCapture)
+ * work too, with the stream's ordinary workspaces: those must exist beforehand
+ * (a call that would have to grow one fails with TILE_GEMM_E_CUDA and says so)
+ * and are then kept until tile_gemm_shutdown.
+ * tile_gemm_recorded_nodes returns the number of graph nodes (kernels and
+ * workspace memsets) in a step, -1 for anything that is not a live step;
+ * tile_gemm_launch_count grows by that number per replay.  tile_gemm_record_free
+ * destroys a step and its workspaces (NULL is a no-op; it waits for replays still
+ * in flight).
  */
 int tile_gemm_record_begin(void* stream);
 int tile_gemm_record_end(void* stream, void** step_out);
@@ -237,9 +247,14 @@ int tile_gemm_select(int64_t M, int64_t N, int64_t K,
  * and owned by the library.  For M >= 2048 the rows of A go up in 1024-row chunks
  * on one stream, each chunk's GEMM runs on a second stream as soon as its rows and
  * all of B have landed, and its rows of C return on a third while the next chunk
- * is still coming in (PCIe is full duplex); results are bit-identical to the
- * one-shot order.  Pinned host memory is needed for the copies to overlap.  This
- * is the call bench.py's `e2e` figure times.
+ * is still coming in (PCIe is full duplex).  Every chunk is an ordinary tile_gemm
+ * call that plans itself, so fp32 results may differ from the one-shot order in
+ * the last bits (same tolerance; identical for integer-valued inputs).  Pinned
+ * host memory is needed for the copies to overlap.  This is the call bench.py's
+ * `e2e` figure times.
+ * Thread safety: the staging buffers, streams and events are kept per device and
+ * the whole call runs under one process-wide lock -- concurrent callers are
+ * serialised (they would share the PCIe link anyway), never mixed.
  */
 int tile_gemm_host(const void* A_host, const void* B_host, void* C_host,
                    int64_t M, int64_t N, int64_t K,
@@ -275,6 +290,28 @@ int tile_gemm_query_config(int64_t M, int64_t N, int64_t K, int out_dtype, int32
  * 64 or 128: skinny M loads only the rows it has).  Needs a CUDA device (SM count).
  */
 int tile_gemm_query_plan(int64_t M, int64_t N, int64_t K, int32_t out[8]);
+
+/*
+ * Test helper: `ctas` CTAs that each hold one SM (they ask for most of its shared memory) for `ns`
+ * nanoseconds (<= 2e9) on `stream`, waiting for nothing but the clock.  Used to check that a
+ * persistent GEMM whose CTAs cannot all be resident still completes (the lockstep producers give
+ * up waiting for clusters that have not started).  Errors: E_EXTENT, E_OVERFLOW, E_DEVICE, E_CUDA.
+ */
+int tile_gemm_debug_occupy(int ctas, int64_t ns, void* stream);
+
+/*
+ * Timeline trace of the M = 1 kernel (gemv_split_kernel), for profiles/ (where a
+ * bandwidth-bound launch loses time).  While `records` (DEVICE memory, 8-byte aligned, `capacity`
+ * records of 8 x 64-bit words, owned by the caller) is set, CTA (bx, by) of every following launch
+ * writes record by * gridDim.x + bx, when below capacity:
+ *   [0] smid | bx << 16 | by << 32, then %globaltimer in ns at [1] kernel entry, [2] release of the
+ *   dependency wait, [3] first tile in shared memory, [4] last tile consumed, [5] CTA done;
+ *   [6] tiles consumed; [7] unused.
+ * Later launches overwrite earlier ones: point it at a fresh buffer per launch.  records == NULL
+ * or capacity == 0 switches tracing off (one untaken branch per event).  Process-global like the
+ * tuning keys.  Returns 0, E_EXTENT or E_ALIGN.
+ */
+int tile_gemm_debug_trace(unsigned long long* records, int64_t capacity);
 
 /*
  * Tuning / test overrides, process-global, not thread-safe against concurrent

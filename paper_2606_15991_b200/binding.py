@@ -28,12 +28,14 @@ PATH_NAMES = {PATH_AUTO: "auto", PATH_GEMM_TMA: "gemm_tma", PATH_GEMM_REPACK: "g
 (E_OK, E_NULL, E_EXTENT, E_LDA, E_LDB, E_LDC, E_DTYPE, E_ALIGN, E_ALIAS, E_OVERFLOW, E_DEVICE,
  E_CUDA, E_PATH, E_INTERNAL, E_IN_DTYPE) = range(15)
 
-TUNE_GEMM_CONFIG, TUNE_GEMM_GROUP_M, TUNE_GEMM_MAX_CTAS, TUNE_GEMV_SPLIT, TUNE_GEMV_VARIANT, TUNE_GEMV_SHAPE, TUNE_FLAGS, TUNE_ADD_SHAPE = range(8)
+(TUNE_GEMM_CONFIG, TUNE_GEMM_GROUP_M, TUNE_GEMM_MAX_CTAS, TUNE_GEMV_SPLIT, TUNE_GEMV_VARIANT, TUNE_GEMV_SHAPE, TUNE_FLAGS,
+ TUNE_ADD_SHAPE, TUNE_GEMV_L2_PREFETCH, TUNE_GEMV_EVICT_FIRST) = range(10)
+NUM_TUNE_KEYS = 16
 
 EXPORTS = ("tile_gemm", "tile_gemm_ex", "tile_gemm_static_b", "tile_gemm_typed", "tile_gemm_swiglu", "tile_add_f32", "tile_read_probe_u32",
            "tile_gemm_record_begin", "tile_gemm_record_end", "tile_gemm_replay", "tile_gemm_recorded_nodes",
            "tile_gemm_record_free", "tile_gemm_select", "tile_gemm_host",
-           "tile_gemm_debug_owner_map", "tile_gemm_query_config", "tile_gemm_query_plan", "tile_gemm_set_tuning",
+           "tile_gemm_debug_owner_map", "tile_gemm_debug_trace", "tile_gemm_debug_occupy", "tile_gemm_query_config", "tile_gemm_query_plan", "tile_gemm_set_tuning",
            "tile_gemm_launch_count", "tile_gemm_status_string", "tile_gemm_last_error",
            "tile_gemm_shutdown")
 
@@ -103,6 +105,10 @@ def load_library():
     lib.tile_gemm_host.restype = _int
     lib.tile_gemm_debug_owner_map.argtypes = [_vp, _i64, _i64, _i64, _i64, _int, _vp]
     lib.tile_gemm_debug_owner_map.restype = _int
+    lib.tile_gemm_debug_occupy.argtypes = [_int, _i64, _vp]
+    lib.tile_gemm_debug_occupy.restype = _int
+    lib.tile_gemm_debug_trace.argtypes = [_vp, _i64]
+    lib.tile_gemm_debug_trace.restype = _int
     lib.tile_gemm_query_config.argtypes = [_i64, _i64, _i64, _int, ctypes.POINTER(ctypes.c_int32)]
     lib.tile_gemm_query_config.restype = _int
     lib.tile_gemm_query_plan.argtypes = [_i64, _i64, _i64, ctypes.POINTER(ctypes.c_int32)]
@@ -370,6 +376,21 @@ def tile_gemm_query_plan(M, N, K) -> dict:
     _check(load_library().tile_gemm_query_plan(M, N, K, out))
     return {"config": out[0], "ctas": out[1], "full_units": out[2], "split": out[3], "k_tiles_per_slice": out[4],
             "lockstep_rounds": out[5], "lockstep_window": out[6], "a_box_rows": out[7]}
+
+
+def tile_gemm_debug_occupy(ctas: int, ns: int, stream=None) -> None:
+    """`ctas` CTAs holding one SM each for `ns` nanoseconds on `stream` (test helper)."""
+    _check(load_library().tile_gemm_debug_occupy(int(ctas), int(ns), _vp(_stream_handle(stream))))
+
+
+def tile_gemm_debug_trace(records: torch.Tensor | None) -> None:
+    """records: int64 CUDA tensor of shape (capacity, 8) that the following M = 1 launches fill, or None to stop."""
+    if records is None:
+        _check(load_library().tile_gemm_debug_trace(_vp(0), 0))
+        return
+    if records.dtype != torch.int64 or records.dim() != 2 or records.shape[1] != 8 or not records.is_contiguous():
+        raise TypeError("records must be a contiguous int64 tensor of shape (capacity, 8)")
+    _check(load_library().tile_gemm_debug_trace(_vp(records.data_ptr()), records.shape[0]))
 
 
 def tile_gemm_debug_owner_map(M, N, K, out_dtype=OUT_F32, ld_owner=None, stream=None, device="cuda"):

@@ -81,4 +81,12 @@ read_probe_kernel(const uint32_t* __restrict__ buf, int64_t n, unsigned long lon
     }
 }
 
+// tile_gemm_debug_occupy: each CTA holds one SM (the launch asks for most of its shared memory) until
+// `ns` nanoseconds have passed.  It waits for nothing but the clock.
+__global__ void __launch_bounds__(128)
+occupy_kernel(unsigned long long ns) {
+    const unsigned long long t0 = global_timer_ns();
+    while (global_timer_ns() - t0 < ns) __nanosleep(1000);
+}
+
 }  // namespace tg

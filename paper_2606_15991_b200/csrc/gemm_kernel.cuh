@@ -33,6 +33,7 @@ constexpr int GEMM_UMMA_K = 16;   // K per tcgen05.mma for 16-bit inputs
 constexpr int GEMM_THREADS = 384;     // 4 control warps + 8 epilogue warps
 constexpr int GEMM_EPI_WARP0 = 4;
 constexpr uint32_t GEMM_EPI_BUF_BYTES = 2 * 32 * 64;   // per epilogue warp: two buffers of 32 rows x 64 B
+constexpr uint64_t GEMM_LOCKSTEP_PATIENCE_NS = 500000;  // a lockstep producer waits this long for the others (a window is ~30 us), then runs free
 
 struct GemmParams {
     int32_t M, N, K;
@@ -211,6 +212,11 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
             // lockstep bookkeeping (leader CTA of each cluster only; its partner is held back by the
             // shared pipeline): `pos` counts the k-tiles this cluster has issued over all its tiles
             const bool lockstep = p.sync != nullptr && rank == 0;
+            // Lockstep is a locality hint, never a correctness condition: if the clusters this one
+            // waits for do not show up in time (not co-resident: another kernel holds SMs, a MIG
+            // slice, ...) it stops waiting for the rest of the launch and only keeps counting itself
+            // in, so that nobody else waits for it.  The MMA order per tile does not change.
+            bool lock_wait = lockstep;
             // the first sync_rounds units of every cluster are whole tiles: positions below sync_limit
             // exist in every cluster's schedule, so every window counter there reaches the cluster count
             const uint32_t sync_limit = (uint32_t)p.sync_rounds * (uint32_t)p.num_k_tiles;
@@ -228,8 +234,17 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
                     if (lockstep && pos == next_sync && pos < sync_limit) {
                         const uint32_t w = pos / (uint32_t)p.sync_window;
                         red_add_relaxed_gpu_u32(p.sync + w, 1u);
-                        if (w >= 1)   // every cluster must have entered window w-1
-                            while (ld_relaxed_gpu_u32(p.sync + (w - 1)) < (uint32_t)tile_stride) __nanosleep(64);
+                        if (w >= 1 && lock_wait) {   // every cluster must have entered window w-1
+                            const uint64_t t0 = global_timer_ns();
+                            uint32_t spins = 0;
+                            while (ld_relaxed_gpu_u32(p.sync + (w - 1)) < (uint32_t)tile_stride) {
+                                __nanosleep(64);
+                                if ((++spins & 31u) == 0 && global_timer_ns() - t0 > GEMM_LOCKSTEP_PATIENCE_NS) {
+                                    lock_wait = false;
+                                    break;
+                                }
+                            }
+                        }
                         next_sync += (uint32_t)p.sync_window;
                     }
                     mbar_wait(empty_bar(stage), phase ^ 1u);

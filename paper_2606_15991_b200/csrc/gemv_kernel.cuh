@@ -211,18 +211,37 @@ gemv_tma_kernel(const __grid_constant__ CUtensorMap tmap_b, const GemvParams p) 
 // across kernel boundaries.
 constexpr int GEMV_FLAG_B_IMMUTABLE = 1;
 constexpr int GEMV_FLAG_X_TMA = 2;   // x is 16-byte aligned: its TILE_K-element slices ride the ring with the weight tiles
+constexpr int GEMV_FLAG_EVICT_FIRST = 4;   // weight tiles carry an L2 evict-first policy (read exactly once)
+constexpr int GEMV_FLAG_PACKED = 8;        // split-K fix-up through tagged 64-bit slots and a designated combiner (below)
+constexpr int GEMV_FLAG_X_PREFETCH = 16;   // bring this CTA's slices of x into L2 ahead of the dependency wait
 
 struct GemvSplitParams {
     const uint16_t* x;
     void* y;
     float* partials;      // [col_blocks][split][COLS]
     uint32_t* tickets;    // [col_blocks], zero between launches
+    unsigned long long* packed;   // GEMV_FLAG_PACKED: [col_blocks][split][COLS] slots {fp32 partial, tag}, all zero between launches
     int32_t N, K;
     int32_t k_tiles;      // ceil(K / TILE_K), >= split
     int32_t col_blocks;
     int32_t out_kind;     // 0: fp32 y, 1: bf16 y, 2: f16 y
     int32_t flags;
+    int32_t l2_prefetch;  // B_IMMUTABLE: units brought into L2 beyond the ring while waiting for the previous kernel
+    int32_t l2_post;      // units brought into L2 right after the dependency wait (while the first activations travel)
+    int32_t l2_steady;    // keep prefetching one unit into L2 per unit issued (stay l2_post units ahead of the ring)
+    // tile_gemm_debug_trace: CTA (bx, by) writes its record of GEMV_TRACE_WORDS 64-bit words at
+    // trace + (by * gridDim.x + bx) * GEMV_TRACE_WORDS when that index is below trace_cap
+    unsigned long long* trace;
+    int32_t trace_cap;
 };
+// trace record: [0] smid | bx << 16 | by << 32, then %globaltimer (ns) at [1] kernel entry, [2] release of
+// griddepcontrol.wait, [3] first tile in shared memory, [4] last tile consumed, [5] CTA done; [6] tiles consumed
+constexpr int GEMV_TRACE_WORDS = 8;
+__device__ __forceinline__ uint32_t sm_id() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%smid;" : "=r"(r));
+    return r;
+}
 
 __device__ __forceinline__ void consumer_bar_sync() {
     asm volatile("bar.sync 1, %0;" ::"n"(GEMV_CONSUMER_WARPS * 32) : "memory");
@@ -234,6 +253,45 @@ __device__ __forceinline__ float ld_cg_f32(const float* p) {
 }
 __device__ __forceinline__ void st_cg_f32(float* p, float v) {
     asm volatile("st.global.cg.f32 [%0], %1;" ::"l"(p), "f"(v) : "memory");
+}
+// one naturally aligned 64-bit access: the fp32 partial and its tag become visible together
+__device__ __forceinline__ void st_relaxed_gpu_u64(unsigned long long* p, unsigned long long v) {
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ unsigned long long ld_relaxed_gpu_u64(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void prefetch_l2(const void* p) {
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(p) : "memory");
+}
+// Tagged-slot split-K fix-up (GEMV_FLAG_PACKED; every CTA of the launch must be resident at once).
+// A slice's thread writes {partial, 1} as ONE 64-bit store and is done: no fence, no ticket, nothing
+// to wait for.  The CTA of the LAST slice is the designated combiner: its thread for column c polls
+// the S-1 other slots of that column until their tags show, adds the values in slice order (its own
+// last: the same order as the ticketed fix-up, so the two protocols give identical bits), and
+// writes the slots back to zero for the next launch.  One global round trip on the critical path
+// instead of three (store+fence, ticket, partial loads).
+__device__ __forceinline__ float gemv_poll_slot(const unsigned long long* slot) {
+    unsigned long long v = ld_relaxed_gpu_u64(slot);
+#if TILEGEMM_WATCHDOG
+    if ((uint32_t)(v >> 32) == 0u) {
+        const uint64_t t0 = global_timer_ns();
+        uint32_t spins = 0;
+        while ((uint32_t)((v = ld_relaxed_gpu_u64(slot)) >> 32) == 0u) {
+            __nanosleep(32);
+            if ((++spins & 0xfffu) == 0 && global_timer_ns() - t0 > 4000000000ull) {
+                printf("tilegemm watchdog: split-K slot wait timed out (block %d,%d thread %d)\n", (int)blockIdx.x,
+                       (int)blockIdx.y, (int)threadIdx.x);
+                __trap();
+            }
+        }
+    }
+#else
+    while ((uint32_t)(v >> 32) == 0u) v = ld_relaxed_gpu_u64(slot);
+#endif
+    return __uint_as_float((uint32_t)v);
 }
 
 template <int COLS, int TILE_K, int STAGES>
@@ -272,7 +330,14 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_const
     const int KT = p.k_tiles;
 
     const bool x_tma = (p.flags & GEMV_FLAG_X_TMA) != 0;
+    unsigned long long* trace = nullptr;   // thread 0 only
     if (threadIdx.x == 0) {
+        const int idx = (int)(blockIdx.y * gridDim.x + blockIdx.x);
+        if (p.trace != nullptr && idx < p.trace_cap) {
+            trace = p.trace + (size_t)idx * GEMV_TRACE_WORDS;
+            trace[0] = (unsigned long long)sm_id() | ((unsigned long long)blockIdx.x << 16) | ((unsigned long long)blockIdx.y << 32);
+            trace[1] = global_timer_ns();
+        }
         prefetch_tmap(&tmap_b);
         if (x_tma) prefetch_tmap(&tmap_x);
         for (uint32_t s = 0; s < STAGES; ++s) {
@@ -290,12 +355,19 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_const
         //       never wait on a global load of x =====
         if (elect_one()) {
             const uint32_t tx_bytes = L::TILE_BYTES + (x_tma ? (uint32_t)TILE_K * 2u : 0u);   // full boxes, even when clipped
+            const bool evict_first = (p.flags & GEMV_FLAG_EVICT_FIRST) != 0;
+            const uint64_t policy = evict_first ? l2_policy_evict_first() : 0ull;
             auto issue_b = [&](uint32_t stage, int cb, int kt) {
                 mbar_arrive_expect_tx(full_bar(stage), tx_bytes);
 #pragma unroll
-                for (int v = 0; v < NV; ++v)
-                    tma_load_2d(smem_base + stage * L::TILE_BYTES + v * L::BOX_BYTES, &tmap_b, full_bar(stage),
-                                cb * COLS + v * GEMV_COLS, kt * TILE_K);
+                for (int v = 0; v < NV; ++v) {
+                    if (evict_first)
+                        tma_load_2d_hint(smem_base + stage * L::TILE_BYTES + v * L::BOX_BYTES, &tmap_b, full_bar(stage),
+                                         cb * COLS + v * GEMV_COLS, kt * TILE_K, policy);
+                    else
+                        tma_load_2d(smem_base + stage * L::TILE_BYTES + v * L::BOX_BYTES, &tmap_b, full_bar(stage),
+                                    cb * COLS + v * GEMV_COLS, kt * TILE_K);
+                }
             };
             auto issue_x = [&](uint32_t stage, int kt) {
                 if (x_tma) tma_load_2d(smem_base + L::X_OFF + stage * 128u, &tmap_x, full_bar(stage), kt * TILE_K, 0);
@@ -305,6 +377,7 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_const
                 if (kt >= KT) { kt = slice; cb += (int)gridDim.x; }
             };
             int cb = (int)blockIdx.x, kt = slice;
+            int cbp = (int)gridDim.x * 0 + p.col_blocks, ktp = 0;   // L2 prefetch cursor (past the end: off)
             uint32_t stage = 0, phase = 0;
             const bool have_work = cb < p.col_blocks && kt < KT;
             if ((p.flags & GEMV_FLAG_B_IMMUTABLE) && have_work) {
@@ -316,6 +389,13 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_const
                     issue_b(n_pre, cb2, kt2);
                     next_unit(cb2, kt2);
                 }
+                // ... and the units after the ring go as far as L2: the previous kernel's last CTAs and the
+                // latency of x after the wait would otherwise leave HBM idle behind a full ring
+                for (int i = 0; i < p.l2_prefetch && cb2 < p.col_blocks; ++i) {
+#pragma unroll
+                    for (int v = 0; v < NV; ++v) tma_prefetch_l2_2d(&tmap_b, cb2 * COLS + v * GEMV_COLS, kt2 * TILE_K);
+                    next_unit(cb2, kt2);
+                }
                 griddep_wait();
                 for (uint32_t i = 0; i < n_pre; ++i) {
                     issue_x(i, kt);
@@ -323,6 +403,14 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_const
                 }
                 stage = n_pre % STAGES;
                 phase = n_pre / STAGES;
+                // the ring is full and its activations are on their way: meanwhile the next units go as far as L2
+                cb2 = cb; kt2 = kt;
+                for (int i = 0; i < p.l2_post && cb2 < p.col_blocks; ++i) {
+#pragma unroll
+                    for (int v = 0; v < NV; ++v) tma_prefetch_l2_2d(&tmap_b, cb2 * COLS + v * GEMV_COLS, kt2 * TILE_K);
+                    next_unit(cb2, kt2);
+                }
+                if (p.l2_steady) { cbp = cb2; ktp = kt2; }
             } else {
                 griddep_wait();
             }
@@ -330,6 +418,11 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_const
                 mbar_wait(empty_bar(stage), phase ^ 1u);
                 issue_b(stage, cb, kt);
                 issue_x(stage, kt);
+                if (cbp < p.col_blocks) {   // keep the L2 prefetch l2_post units ahead of the ring
+#pragma unroll
+                    for (int v = 0; v < NV; ++v) tma_prefetch_l2_2d(&tmap_b, cbp * COLS + v * GEMV_COLS, ktp * TILE_K);
+                    next_unit(cbp, ktp);
+                }
                 if (++stage == STAGES) { stage = 0; phase ^= 1u; }
             }
         }
@@ -339,7 +432,18 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_const
 
     // ===== consumers: warp w owns rows RPW*w .. RPW*w+RPW-1 of every tile; lane l owns columns
     //       256 v + 8 l .. + 7 of every box v =====
+    if (p.flags & GEMV_FLAG_X_PREFETCH) {
+        // an L2 prefetch has no semantics: whatever the previous kernel still writes to x lands in the
+        // same L2, so the loads behind the wait see it -- they just do not go to DRAM any more
+        const int my_tiles = (KT - slice + S - 1) / S;
+        if ((int)threadIdx.x < my_tiles) {
+            const int k = (slice + (int)threadIdx.x * S) * TILE_K;
+            if (k < p.K) prefetch_l2(p.x + k);
+        }
+    }
     griddep_wait();   // x may be the previous kernel's output; y and the workspace may still be in its use
+    if (trace) trace[2] = global_timer_ns();
+    int traced_tiles = 0;
     const uint32_t tid = threadIdx.x;   // 0..255
     auto load_x = [&](int kt_) -> float {   // only when x is not TMA-addressable
         const int k = kt_ * TILE_K + (int)warp * RPW + (int)(lane & (RPW - 1));
@@ -357,6 +461,7 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_const
             const float xv = xv_next;
             xv_next = load_x(kt + S);
             mbar_wait(full_bar(stage), phase);
+            if (trace && traced_tiles++ == 0) trace[3] = global_timer_ns();
             const uint8_t* tile = smem_gen + stage * L::TILE_BYTES + warp * RPW * (GEMV_COLS * 2) + lane * 16u;
             uint4 w[NV][RPW];
 #pragma unroll
@@ -383,6 +488,7 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_const
             if (++stage == STAGES) { stage = 0; phase ^= 1u; }
         }
         // ---- column block done for this slice: warps -> CTA -> (S > 1) slices ----
+        if (trace) { trace[4] = global_timer_ns(); trace[6] = (unsigned long long)traced_tiles; }
 #pragma unroll
         for (int v = 0; v < NV; ++v) {
             float4* r4 = reinterpret_cast<float4*>(red + warp * COLS + v * GEMV_COLS + lane * 8);
@@ -398,7 +504,36 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_const
             for (int w8 = 0; w8 < GEMV_CONSUMER_WARPS; ++w8) s[v] += red[w8 * COLS + v * GEMV_COLS + tid];   // fixed order
         }
         bool store = (S == 1);
-        if (!store) {
+        if (!store && (p.flags & GEMV_FLAG_PACKED)) {
+            unsigned long long* slots = p.packed + (size_t)cb * S * COLS + tid;
+            if (slice != S - 1) {
+#pragma unroll
+                for (int v = 0; v < NV; ++v)
+                    st_relaxed_gpu_u64(slots + (size_t)slice * COLS + v * GEMV_COLS,
+                                       (1ull << 32) | (unsigned long long)__float_as_uint(s[v]));
+            } else {
+#pragma unroll
+                for (int v = 0; v < NV; ++v) {
+                    const float own = s[v];
+                    s[v] = 0.f;
+                    for (int q0 = 0; q0 < S - 1; q0 += 8) {   // eight independent loads in flight, added in slice order
+                        unsigned long long got[8];
+#pragma unroll
+                        for (int j = 0; j < 8; ++j)
+                            if (q0 + j < S - 1) got[j] = ld_relaxed_gpu_u64(slots + (size_t)(q0 + j) * COLS + v * GEMV_COLS);
+#pragma unroll
+                        for (int j = 0; j < 8; ++j)
+                            if (q0 + j < S - 1) {
+                                unsigned long long* slot = slots + (size_t)(q0 + j) * COLS + v * GEMV_COLS;
+                                s[v] += ((uint32_t)(got[j] >> 32) != 0u) ? __uint_as_float((uint32_t)got[j]) : gemv_poll_slot(slot);
+                                st_relaxed_gpu_u64(slot, 0ull);   // re-arm for the next launch
+                            }
+                    }
+                    s[v] += own;
+                }
+                store = true;
+            }
+        } else if (!store) {
             float* part = p.partials + (size_t)cb * S * COLS + tid;
 #pragma unroll
             for (int v = 0; v < NV; ++v) st_cg_f32(part + (size_t)slice * COLS + v * GEMV_COLS, s[v]);
@@ -416,7 +551,15 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_const
 #pragma unroll
                 for (int v = 0; v < NV; ++v) {
                     s[v] = 0.f;
-                    for (int q = 0; q < S; ++q) s[v] += ld_cg_f32(part + (size_t)q * COLS + v * GEMV_COLS);   // fixed order
+                    for (int q0 = 0; q0 < S; q0 += 8) {   // eight independent loads in flight, added in slice order
+                        float got[8];
+#pragma unroll
+                        for (int j = 0; j < 8; ++j)
+                            if (q0 + j < S) got[j] = ld_cg_f32(part + (size_t)(q0 + j) * COLS + v * GEMV_COLS);
+#pragma unroll
+                        for (int j = 0; j < 8; ++j)
+                            if (q0 + j < S) s[v] += got[j];
+                    }
                 }
                 store = true;
             }
@@ -430,6 +573,7 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_const
         }
         consumer_bar_sync();   // red and s_last are free for the next column block
     }
+    if (trace) trace[5] = global_timer_ns();
 }
 
 // Generic fallback: no alignment requirement on B when VEC == false.

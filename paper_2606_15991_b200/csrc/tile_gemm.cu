@@ -56,7 +56,10 @@ const char* const kStatusNames[TILE_GEMM_NUM_STATUS] = {
 };
 
 std::atomic<int64_t> g_launches{0};
-std::atomic<int> g_tune[8];
+std::atomic<unsigned long long*> g_trace{nullptr};   // tile_gemm_debug_trace
+std::atomic<int64_t> g_trace_cap{0};
+constexpr int kNumTune = 16;
+std::atomic<int> g_tune[kNumTune];
 
 // ------------------------------------------------------------------ preconditions + selector
 struct Plan {
@@ -82,6 +85,7 @@ bool overlaps(const void* p, int64_t pn, const void* q, int64_t qn) {
     return a < b + (uintptr_t)qn && b < a + (uintptr_t)pn;
 }
 
+constexpr int kAuxCtasPerSm = 16;      // grid cap of the grid-stride helper kernels (repack, zero fill), per SM
 constexpr int64_t kGemvMaxRows = 4;   // M = 2..4 with TMA-addressable A and B take the multi-row GEMV (gemv_rows_kernel.cuh)
 
 int check_and_select(const void* A, const void* B, const void* C, int64_t M, int64_t N, int64_t K, int64_t lda,
@@ -245,16 +249,46 @@ int get_tensor_map(CUtensorMap* out, const void* base, int dtype_bytes, bool is_
 }
 
 // ------------------------------------------------------------------ workspaces
+// Library-owned device memory.  Lifetime rules (a replayed node must not depend on
+// an address that changes across replays):
+//   * direct calls use one WorkspaceSet per (device, stream), grown by free + allocate (cudaFree
+//     synchronises, so no in-flight kernel loses its buffer);
+//   * a recorded step (tile_gemm_record_begin .. _end) owns a PRIVATE WorkspaceSet: the addresses
+//     baked into its nodes belong to the step, live until tile_gemm_record_free and are shared with
+//     no direct call and no other step, whichever stream it is replayed on.  A buffer that must grow
+//     while the step is still being recorded is retired (kept for the nodes already captured), not freed;
+//   * a stream that the CALLER is capturing (its own cudaStreamBeginCapture) gets the per-stream set,
+//     which is then pinned: it is never freed before tile_gemm_shutdown, and growing it under that
+//     capture is refused (cudaMalloc is not allowed in a foreign capture).
 struct Buf {
     void* p = nullptr;
     size_t n = 0;
 };
-std::unordered_map<uint64_t, Buf> g_ws;   // (device, stream) -> repack workspace
-Buf g_stage[3];                            // tile_gemm_host staging (A, B, C)
-cudaStream_t g_host_stream = nullptr;       // tile_gemm_host: copy-in (and everything, when not pipelined)
-cudaStream_t g_host_compute = nullptr;      // pipelined tile_gemm_host: the GEMMs
-cudaStream_t g_host_out = nullptr;          // pipelined tile_gemm_host: copy-out
-std::vector<cudaEvent_t> g_host_events;
+struct WorkspaceSet {
+    Buf repack;     // 16-byte pitched copies of operands TMA cannot address
+    Buf sync;       // GEMM lockstep window counters, zeroed before each launch that uses them
+    Buf partials;   // split-K fp32 partial sums (GEMV: [col_blocks][split][cols]; GEMM: per split tile)
+    Buf tickets;    // split-K arrival tickets, zero between launches (the last arrival re-arms them)
+    Buf packed;     // M = 1 tagged split-K slots {fp32, tag}, all zero between launches (the combiner re-arms them)
+    bool pinned = false;           // baked into a graph this library does not own
+    std::vector<void*> retired;    // outgrown buffers that captured nodes may still reference
+};
+struct Recording {
+    int dev = 0;
+    WorkspaceSet ws;
+};
+std::unordered_map<uint64_t, WorkspaceSet> g_wsets;            // (device, stream) -> direct-call workspaces
+std::unordered_map<uintptr_t, Recording*> g_recording;         // streams between record_begin and record_end
+std::vector<void*> g_retired;                                   // retired buffers of pinned per-stream sets
+
+// tile_gemm_host: one staging set per device, used under g_host_mu for the whole call
+struct HostStage {
+    Buf a, b, c;
+    cudaStream_t in = nullptr, compute = nullptr, out = nullptr;   // copy-in, GEMMs, copy-out
+    std::vector<cudaEvent_t> events;
+};
+HostStage g_host[64];
+std::mutex g_host_mu;
 
 int grow(Buf& b, size_t need) {
     if (b.n >= need) return TILE_GEMM_OK;
@@ -267,61 +301,95 @@ int grow(Buf& b, size_t need) {
     return TILE_GEMM_OK;
 }
 
-int workspace_for(int dev, cudaStream_t s, size_t need, void** out) {
-    std::lock_guard<std::mutex> lk(g_mu);
-    Buf& b = g_ws[((uint64_t)dev << 56) ^ (uint64_t)(uintptr_t)s];
+// The workspace set a call on stream `s` uses, and whether its buffers may be (re)allocated now.
+struct WsRef {
+    WorkspaceSet* ws;
+    bool ours;       // a recording of this library
+    bool foreign;    // the caller's own capture
+};
+WsRef workspace_set(int dev, cudaStream_t s) {   // g_mu held
+    auto it = g_recording.find((uintptr_t)s);
+    if (it != g_recording.end()) return {&it->second->ws, true, false};
+    WorkspaceSet& w = g_wsets[((uint64_t)dev << 56) ^ (uint64_t)(uintptr_t)s];
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    const bool cap = cudaStreamIsCapturing(s, &cs) == cudaSuccess && cs != cudaStreamCaptureStatusNone;
+    if (cap) w.pinned = true;
+    return {&w, false, cap};
+}
+
+// make `b` at least `need` bytes under the rules above; *fresh is set when the buffer is new
+int ensure(const WsRef& r, Buf& b, size_t need, const char* what, bool* fresh = nullptr) {
+    if (fresh) *fresh = false;
+    if (b.n >= need) return TILE_GEMM_OK;
+    if (r.foreign)
+        return fail(TILE_GEMM_E_CUDA,
+                    "the %s workspace of this stream must grow during the caller's stream capture; run the shape "
+                    "once on the stream before capturing, or record with tile_gemm_record_begin", what);
+    if ((r.ours || r.ws->pinned) && b.p) {   // captured nodes may hold the old address
+        (r.ours ? r.ws->retired : g_retired).push_back(b.p);
+        b.p = nullptr;
+        b.n = 0;
+    }
     int rc = grow(b, need);
     if (rc) return rc;
-    *out = b.p;
+    if (fresh) *fresh = true;
     return TILE_GEMM_OK;
 }
 
-// GEMM lockstep counters per (device, stream), zeroed before each launch that uses them
-std::unordered_map<uint64_t, Buf> g_sync_ws;
+int workspace_for(int dev, cudaStream_t s, size_t need, void** out) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    const WsRef r = workspace_set(dev, s);
+    int rc = ensure(r, r.ws->repack, need, "operand repack");
+    if (rc) return rc;
+    *out = r.ws->repack.p;
+    return TILE_GEMM_OK;
+}
 
 int sync_workspace_for(int dev, cudaStream_t s, size_t bytes, uint32_t** out) {
     std::lock_guard<std::mutex> lk(g_mu);
-    Buf& b = g_sync_ws[((uint64_t)dev << 56) ^ (uint64_t)(uintptr_t)s];
-    if (b.n < bytes) {
-        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
-        if (cudaStreamIsCapturing(s, &cs) == cudaSuccess && cs != cudaStreamCaptureStatusNone)
-            return fail(TILE_GEMM_E_CUDA,
-                        "the GEMM lockstep workspace of this stream must grow during stream capture; run the shape "
-                        "once on the stream before capturing");
-        int rc = grow(b, bytes);
-        if (rc) return rc;
-    }
-    *out = (uint32_t*)b.p;
+    const WsRef r = workspace_set(dev, s);
+    int rc = ensure(r, r.ws->sync, bytes, "GEMM lockstep");
+    if (rc) return rc;
+    *out = (uint32_t*)r.ws->sync.p;
     return TILE_GEMM_OK;
 }
 
-// GEMV split-K workspace per (device, stream): fp32 partials [col_blocks][split][256] and one ticket per column
-// block (zero between launches: the CTA that draws the last ticket re-arms it).
-struct GemvWs {
-    Buf partials, tickets;
-};
-std::unordered_map<uint64_t, GemvWs> g_gemv_ws;
-
+// split-K workspace: fp32 partials and one ticket per (column block | tile, CTA rank)
 int gemv_workspace_for(int dev, cudaStream_t s, size_t partial_bytes, size_t ticket_bytes, float** partials,
                        uint32_t** tickets) {
     std::lock_guard<std::mutex> lk(g_mu);
-    GemvWs& w = g_gemv_ws[((uint64_t)dev << 56) ^ (uint64_t)(uintptr_t)s];
-    if (w.partials.n < partial_bytes || w.tickets.n < ticket_bytes) {
-        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
-        if (cudaStreamIsCapturing(s, &cs) == cudaSuccess && cs != cudaStreamCaptureStatusNone)
-            return fail(TILE_GEMM_E_CUDA,
-                        "the GEMV workspace of this stream must grow during stream capture; run the shape once on "
-                        "the stream before capturing");
-        int rc = grow(w.partials, partial_bytes);
-        if (rc) return rc;
-        const size_t before = w.tickets.n;
-        rc = grow(w.tickets, ticket_bytes);
-        if (rc) return rc;
-        if (w.tickets.n != before) CUDA_TRY(cudaMemsetAsync(w.tickets.p, 0, w.tickets.n, s));
-    }
-    *partials = (float*)w.partials.p;
-    *tickets = (uint32_t*)w.tickets.p;
+    const WsRef r = workspace_set(dev, s);
+    int rc = ensure(r, r.ws->partials, partial_bytes, "split-K partial sum");
+    if (rc) return rc;
+    bool fresh = false;
+    rc = ensure(r, r.ws->tickets, ticket_bytes, "split-K ticket", &fresh);
+    if (rc) return rc;
+    // a new ticket buffer starts at zero (in a recording this is a memset node: every replay re-zeroes it)
+    if (fresh) CUDA_TRY(cudaMemsetAsync(r.ws->tickets.p, 0, r.ws->tickets.n, s));
+    *partials = (float*)r.ws->partials.p;
+    *tickets = (uint32_t*)r.ws->tickets.p;
     return TILE_GEMM_OK;
+}
+
+// tagged split-K slots of the M = 1 kernel (gemv_kernel.cuh, GEMV_FLAG_PACKED)
+int packed_workspace_for(int dev, cudaStream_t s, size_t bytes, unsigned long long** out) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    const WsRef r = workspace_set(dev, s);
+    bool fresh = false;
+    int rc = ensure(r, r.ws->packed, bytes, "split-K slot", &fresh);
+    if (rc) return rc;
+    if (fresh) CUDA_TRY(cudaMemsetAsync(r.ws->packed.p, 0, r.ws->packed.n, s));
+    *out = (unsigned long long*)r.ws->packed.p;
+    return TILE_GEMM_OK;
+}
+
+void free_workspace_set(WorkspaceSet& w) {
+    for (Buf* b : {&w.repack, &w.sync, &w.partials, &w.tickets, &w.packed}) {
+        if (b->p) cudaFree(b->p);
+        *b = Buf();
+    }
+    for (void* q : w.retired) cudaFree(q);
+    w.retired.clear();
 }
 
 // ------------------------------------------------------------------ GEMM launch
@@ -342,9 +410,13 @@ constexpr int kGemmMaxSplit = 16, kGemmMinSliceKTiles = 4;
 // and once as a load of the fix-up, ~100 GB/s per cluster, and a ticket round trip) -- measured on
 // B200: ~8 us for a 256x512 slice, ~3.5 us for 128x128.  Cutting pays for long K loops and for
 // problems below one wave (skinny M).
+// cost-model constants (B200, measured): what the whole chip sustains on this kernel's main loop, in
+// FLOP per microsecond; a slice's fixed cost; the rate at which one cluster moves a slice's partials
+constexpr double kModelChipFlopPerUs = 1500e6, kModelSliceFixedUs = 3.0, kModelSliceBytesPerUs = 100e3;
+
 double last_wave_us(int64_t rem, int64_t slots, int tile_m, int tile_n, int cg, int64_t k_tiles, int sms, int64_t* slices) {
-    const double tile_us = 2.0 * tile_m * tile_n * (double)k_tiles * tg::GEMM_BK / (1500e6 * cg / (double)sms);
-    const double ovh_us = 3.0 + (double)tile_m * tile_n * 4.0 / 100e3;
+    const double tile_us = 2.0 * tile_m * tile_n * (double)k_tiles * tg::GEMM_BK / (kModelChipFlopPerUs * cg / (double)sms);
+    const double ovh_us = kModelSliceFixedUs + (double)tile_m * tile_n * 4.0 / kModelSliceBytesPerUs;
     *slices = 1;
     if (rem <= 0) return 0.0;
     double best = tile_us;
@@ -363,7 +435,7 @@ double last_wave_us(int64_t rem, int64_t slots, int tile_m, int tile_n, int cg, 
 double launch_us(int64_t M, int64_t N, int64_t K, int tile_m, int tile_n, int cg, int sms) {
     const int64_t slots = sms / cg, k_tiles = (K + tg::GEMM_BK - 1) / tg::GEMM_BK;
     const int64_t tiles = ((M + tile_m - 1) / tile_m) * ((N + tile_n - 1) / tile_n);
-    const double tile_us = 2.0 * tile_m * tile_n * (double)k_tiles * tg::GEMM_BK / (1500e6 * cg / (double)sms);
+    const double tile_us = 2.0 * tile_m * tile_n * (double)k_tiles * tg::GEMM_BK / (kModelChipFlopPerUs * cg / (double)sms);
     int64_t sl;
     return (double)(tiles / slots) * tile_us + last_wave_us(tiles % slots, slots, tile_m, tile_n, cg, k_tiles, sms, &sl);
 }
@@ -389,6 +461,54 @@ GemmConfig choose_config(int64_t M, int64_t N, int64_t K, int sms) {
     return kConfigs[1];
 }
 
+// How many work-unit owners (CTA pairs for cg = 2, CTAs for cg = 1) of a tile configuration the device
+// holds at once, from the occupancy calculator (GPC layout, shared memory, registers): the persistent
+// grid is never larger, so that every CTA of a launch is resident when nothing else runs on the device.
+template <int CG, int BN, int STAGES, int NACC>
+int query_resident_units(int sms) {
+    using L = tg::GemmSmem<CG, BN, STAGES, NACC>;
+    auto kern = tg::gemm_tcgen05_kernel<CG, BN, STAGES, NACC, false, 0>;
+    int n = 0;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::TOTAL) == cudaSuccess) {
+        if (CG == 2) {
+            cudaLaunchConfig_t cfg;
+            memset(&cfg, 0, sizeof cfg);
+            cfg.gridDim = dim3((unsigned)(sms & ~1), 1, 1);
+            cfg.blockDim = dim3(tg::GEMM_THREADS, 1, 1);
+            cfg.dynamicSmemBytes = L::TOTAL;
+            cudaLaunchAttribute attr[1];
+            attr[0].id = cudaLaunchAttributeClusterDimension;
+            attr[0].val.clusterDim.x = 2;
+            attr[0].val.clusterDim.y = 1;
+            attr[0].val.clusterDim.z = 1;
+            cfg.attrs = attr;
+            cfg.numAttrs = 1;
+            if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess) n = 0;
+        } else {
+            int per_sm = 0;
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, tg::GEMM_THREADS, L::TOTAL) == cudaSuccess)
+                n = per_sm * sms;
+        }
+    }
+    cudaGetLastError();   // a failed query is not an error of the call that asked
+    if (n <= 0 || n > sms / CG) n = sms / CG;   // one CTA per SM at most: a CTA allocates all of tensor memory
+    return n;
+}
+
+int resident_units(const GemmConfig& cfg, int dev, int sms) {
+    static std::atomic<int> cache[5][64];
+    int v = cache[cfg.id][dev].load();
+    if (v > 0) return v;
+    switch (cfg.id) {
+        case 1: v = query_resident_units<1, 128, 6, 1>(sms); break;
+        case 2: v = query_resident_units<1, 256, 4, 1>(sms); break;
+        case 3: v = query_resident_units<2, 256, 6, 1>(sms); break;
+        default: v = query_resident_units<2, 256, 4, 2>(sms); break;
+    }
+    cache[cfg.id][dev].store(v);
+    return v;
+}
+
 // lockstep defaults: on from kLockstepMinTiles tiles per cluster and kLockstepMinKTiles k-tiles
 constexpr int kLockstepMinTiles = 2, kLockstepMinKTiles = 256, kLockstepWindow = 32;
 
@@ -398,7 +518,7 @@ struct GemmLaunch {
     int ctas;
 };
 
-void plan_gemm(int64_t M, int64_t N, int64_t K, int in_dtype, int out_dtype, int sms, GemmLaunch* gl,
+void plan_gemm(int64_t M, int64_t N, int64_t K, int in_dtype, int out_dtype, int dev, int sms, GemmLaunch* gl,
                bool allow_split = false) {
     gl->cfg = choose_config(M, N, K, sms);
     const int tile_m = tg::GEMM_BM * gl->cfg.cg;
@@ -415,7 +535,7 @@ void plan_gemm(int64_t M, int64_t N, int64_t K, int in_dtype, int out_dtype, int
     p.out_f16 = out_dtype == TILE_GEMM_OUT_F16;
     p.in_f16 = in_dtype == TILE_GEMM_IN_F16;
     const int64_t tiles = (int64_t)p.tiles_m * p.tiles_n;
-    int max_units = sms / gl->cfg.cg;
+    int max_units = resident_units(gl->cfg, dev, sms);
     const int cap = g_tune[2].load();
     if (cap > 0 && cap / gl->cfg.cg >= 1 && cap / gl->cfg.cg < max_units) max_units = cap / gl->cfg.cg;
     // Split-K for the partial last wave: `rem` tiles are left after the whole waves;
@@ -562,7 +682,8 @@ int run_gemm(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_
         if (rc) return rc;
         if (rep_a) {
             const int64_t chunks = M * (lda2 >> 3);
-            const int blocks = (int)((chunks + 255) / 256 < 148 * 16 ? (chunks + 255) / 256 : 148 * 16);
+            const int64_t cap_blocks = (int64_t)sms * kAuxCtasPerSm;
+            const int blocks = (int)((chunks + 255) / 256 < cap_blocks ? (chunks + 255) / 256 : cap_blocks);
             tg::repack_rows_kernel<<<blocks, 256, 0, s>>>(Ap, lda, (uint16_t*)ws, lda2, M, K);
             CUDA_TRY(cudaGetLastError());
             g_launches.fetch_add(1);
@@ -572,7 +693,8 @@ int run_gemm(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_
         if (rep_b) {
             uint16_t* dst = (uint16_t*)((char*)ws + a_sz);
             const int64_t chunks = K * (ldb2 >> 3);
-            const int blocks = (int)((chunks + 255) / 256 < 148 * 16 ? (chunks + 255) / 256 : 148 * 16);
+            const int64_t cap_blocks = (int64_t)sms * kAuxCtasPerSm;
+            const int blocks = (int)((chunks + 255) / 256 < cap_blocks ? (chunks + 255) / 256 : cap_blocks);
             tg::repack_rows_kernel<<<blocks, 256, 0, s>>>(Bp, ldb, dst, ldb2, K, N);
             CUDA_TRY(cudaGetLastError());
             g_launches.fetch_add(1);
@@ -581,7 +703,7 @@ int run_gemm(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_
         }
     }
     GemmLaunch gl;
-    plan_gemm(M, N, K, in_dtype, out_dtype, sms, &gl, true);
+    plan_gemm(M, N, K, in_dtype, out_dtype, dev, sms, &gl, true);
     if (gl.p.split > 0) {
         const size_t split_tiles = (size_t)((int64_t)gl.p.tiles_m * gl.p.tiles_n - gl.p.full_units);
         const size_t tile_floats = (size_t)tg::GEMM_BM * gl.cfg.cg * gl.cfg.tile_n();
@@ -700,11 +822,27 @@ int run_gemv_split(const void* x, const void* B, void* y, int64_t N, int64_t K, 
     p.out_kind = out_dtype;
     p.flags = (flags & TILE_GEMM_FLAG_B_IMMUTABLE) ? tg::GEMV_FLAG_B_IMMUTABLE : 0;
     if ((((uintptr_t)x) & 15) == 0 && (g_tune[6].load() & 2) == 0) p.flags |= tg::GEMV_FLAG_X_TMA;
+    if (g_tune[9].load() == 1) p.flags |= tg::GEMV_FLAG_EVICT_FIRST;
+    p.l2_prefetch = g_tune[8].load() > 0 ? g_tune[8].load() : 0;
+    p.trace = g_trace.load();
+    p.trace_cap = (int32_t)g_trace_cap.load();
+    p.l2_post = g_tune[10].load() > 0 ? g_tune[10].load() : 0;
+    p.l2_steady = g_tune[12].load() > 0 ? 1 : 0;
+    if (g_tune[11].load() & 1) p.flags |= tg::GEMV_FLAG_X_PREFETCH;
     p.partials = nullptr;
     p.tickets = nullptr;
+    p.packed = nullptr;
     if (split > 1) {
-        int rc = gemv_workspace_for(dev, s, (size_t)col_blocks * split * gs.cols * 4, (size_t)col_blocks * 4,
+        // tagged slots + designated combiner need every CTA of the launch resident at once
+        const bool packed = (g_tune[11].load() & 2) && gx * split <= budget;
+        int rc;
+        if (packed) {
+            rc = packed_workspace_for(dev, s, (size_t)col_blocks * split * gs.cols * 8, &p.packed);
+            p.flags |= tg::GEMV_FLAG_PACKED;
+        } else {
+            rc = gemv_workspace_for(dev, s, (size_t)col_blocks * split * gs.cols * 4, (size_t)col_blocks * 4,
                                     &p.partials, &p.tickets);
+        }
         if (rc) return rc;
     }
     const bool pdl = (g_tune[6].load() & 1) == 0;
@@ -874,9 +1012,10 @@ int run_gemv(const void* x, const void* B, void* y, int64_t N, int64_t K, int64_
     return TILE_GEMM_OK;
 }
 
-int run_zero(void* C, int64_t M, int64_t N, int64_t ldc, int esize, cudaStream_t s) {
+int run_zero(void* C, int64_t M, int64_t N, int64_t ldc, int esize, cudaStream_t s, int sms) {
     const int64_t total = M * N;
-    const int blocks = (int)((total + 255) / 256 < 148 * 8 ? (total + 255) / 256 : 148 * 8);
+    const int64_t cap_blocks = (int64_t)sms * kAuxCtasPerSm / 2;
+    const int blocks = (int)((total + 255) / 256 < cap_blocks ? (total + 255) / 256 : cap_blocks);
     tg::zero_fill_kernel<<<blocks, 256, 0, s>>>(C, M, N, ldc, esize);
     CUDA_TRY(cudaGetLastError());
     g_launches.fetch_add(1);
@@ -920,7 +1059,7 @@ int gemm_entry(const void* A, const void* B, void* C, int64_t M, int64_t N, int6
     if (rc) return rc;
     cudaStream_t s = (cudaStream_t)stream;
     switch (path) {
-        case TILE_GEMM_PATH_ZERO: return run_zero(C, M, N, ldc, plan.esize, s);
+        case TILE_GEMM_PATH_ZERO: return run_zero(C, M, N, ldc, plan.esize, s, sms);
         case TILE_GEMM_PATH_GEMV:
             if (M > 1) return run_gemv_rows(A, B, C, M, N, K, lda, ldb, ldc, in_dtype, out_dtype, s, dev, sms, flags);
             return run_gemv(A, B, C, N, K, ldb, in_dtype, out_dtype, s, plan, dev, sms, flags);
@@ -984,7 +1123,7 @@ int tile_gemm_swiglu(const void* X, const void* Wgu, void* H, int64_t M, int64_t
     rc = current_device(&dev, &sms);
     if (rc) return rc;
     cudaStream_t s = (cudaStream_t)stream;
-    if (K == 0) return run_zero(H, M, I, ldh, plan.esize, s);   // silu(0) * 0 = 0
+    if (K == 0) return run_zero(H, M, I, ldh, plan.esize, s, sms);   // silu(0) * 0 = 0
     GemmLaunch gl;
     gl.cfg = kConfigs[4];
     tg::GemmParams& p = gl.p;
@@ -1002,7 +1141,8 @@ int tile_gemm_swiglu(const void* X, const void* Wgu, void* H, int64_t M, int64_t
     const int64_t tiles = (int64_t)p.tiles_m * p.tiles_n;
     p.full_units = p.total_units = (int32_t)tiles;
     p.kps = p.num_k_tiles;
-    const int64_t clusters = tiles < sms / 2 ? tiles : sms / 2;
+    const int64_t slots = resident_units(gl.cfg, dev, sms);
+    const int64_t clusters = tiles < slots ? tiles : slots;
     gl.ctas = (int)clusters * 2;
     p.tma_store = plan.c_tma ? 1 : 0;
     p.C = H;
@@ -1119,6 +1259,7 @@ struct Recorded {
     cudaGraph_t graph;
     cudaGraphExec_t exec;
     int64_t nodes;
+    Recording* rec;   // the step's private workspaces: every address its nodes hold lives as long as the step
 };
 constexpr uint32_t kRecordedMagic = 0x7167656d;
 }  // namespace
@@ -1129,25 +1270,52 @@ int tile_gemm_record_begin(void* stream) {
     if (rc) return rc;
     if (stream == nullptr)
         return fail(TILE_GEMM_E_PATH, "recording needs an explicit stream: the legacy default stream cannot be captured");
-    CUDA_TRY(cudaStreamBeginCapture((cudaStream_t)stream, cudaStreamCaptureModeThreadLocal));
+    {
+        std::lock_guard<std::mutex> lk(g_mu);
+        if (g_recording.count((uintptr_t)stream))
+            return fail(TILE_GEMM_E_PATH, "stream %p is already recording a step", stream);
+    }
+    // relaxed mode: the step's private workspaces are allocated (cudaMalloc) while the stream captures
+    CUDA_TRY(cudaStreamBeginCapture((cudaStream_t)stream, cudaStreamCaptureModeRelaxed));
+    Recording* rec = new Recording();
+    rec->dev = dev;
+    std::lock_guard<std::mutex> lk(g_mu);
+    g_recording[(uintptr_t)stream] = rec;
     return TILE_GEMM_OK;
 }
 
 int tile_gemm_record_end(void* stream, void** step_out) {
     if (!step_out) return fail(TILE_GEMM_E_NULL, "step_out is NULL");
     *step_out = nullptr;
+    Recording* rec = nullptr;
+    {
+        std::lock_guard<std::mutex> lk(g_mu);
+        auto it = g_recording.find((uintptr_t)stream);
+        if (it == g_recording.end())
+            return fail(TILE_GEMM_E_PATH, "stream %p is not recording (tile_gemm_record_begin was not called on it)", stream);
+        rec = it->second;
+        g_recording.erase(it);
+    }
+    auto drop = [&]() {
+        free_workspace_set(rec->ws);
+        delete rec;
+    };
     cudaGraph_t graph = nullptr;
-    CUDA_TRY(cudaStreamEndCapture((cudaStream_t)stream, &graph));
-    if (!graph) return fail(TILE_GEMM_E_CUDA, "the capture on this stream was invalidated");
+    cudaError_t e = cudaStreamEndCapture((cudaStream_t)stream, &graph);
+    if (e != cudaSuccess || !graph) {
+        drop();
+        return fail(TILE_GEMM_E_CUDA, "the capture on this stream was invalidated: %s (%d)", cudaGetErrorString(e), (int)e);
+    }
     cudaGraphExec_t exec = nullptr;
-    cudaError_t e = cudaGraphInstantiate(&exec, graph, 0);
+    e = cudaGraphInstantiate(&exec, graph, 0);
     if (e != cudaSuccess) {
         cudaGraphDestroy(graph);
+        drop();
         return fail(TILE_GEMM_E_CUDA, "cudaGraphInstantiate failed: %s (%d)", cudaGetErrorString(e), (int)e);
     }
     size_t n = 0;
     cudaGraphGetNodes(graph, nullptr, &n);
-    Recorded* r = new Recorded{kRecordedMagic, graph, exec, (int64_t)n};
+    Recorded* r = new Recorded{kRecordedMagic, graph, exec, (int64_t)n, rec};
     *step_out = r;
     return TILE_GEMM_OK;
 }
@@ -1171,6 +1339,10 @@ int tile_gemm_record_free(void* step) {
     if (r->magic != kRecordedMagic) return fail(TILE_GEMM_E_NULL, "not a recorded step: %p", step);
     cudaGraphExecDestroy(r->exec);
     cudaGraphDestroy(r->graph);
+    if (r->rec) {
+        free_workspace_set(r->rec->ws);   // cudaFree synchronises with replays still in flight
+        delete r->rec;
+    }
     r->magic = 0;
     delete r;
     return TILE_GEMM_OK;
@@ -1187,60 +1359,61 @@ int tile_gemm_host(const void* A_host, const void* B_host, void* C_host, int64_t
     int dev = 0, sms = 0;
     rc = current_device(&dev, &sms);
     if (rc) return rc;
-    {
-        std::lock_guard<std::mutex> lk(g_mu);
-        if (!g_host_stream) CUDA_TRY(cudaStreamCreateWithFlags(&g_host_stream, cudaStreamNonBlocking));
-        if ((rc = grow(g_stage[0], (size_t)plan.a_bytes + 16))) return rc;
-        if ((rc = grow(g_stage[1], (size_t)plan.b_bytes + 16))) return rc;
-        if ((rc = grow(g_stage[2], (size_t)plan.c_bytes + 16))) return rc;
-    }
-    cudaStream_t s = g_host_stream;
+    // One host call at a time (per process): the staging buffers, the three streams and the events of
+    // the current device are used for the whole call, and concurrent callers would only share the
+    // PCIe link anyway.  Other threads block here; they never see each other's staging data.
+    std::lock_guard<std::mutex> host_lk(g_host_mu);
+    HostStage& hs = g_host[dev];
+    if (!hs.in) CUDA_TRY(cudaStreamCreateWithFlags(&hs.in, cudaStreamNonBlocking));
+    if ((rc = grow(hs.a, (size_t)plan.a_bytes + 16))) return rc;
+    if ((rc = grow(hs.b, (size_t)plan.b_bytes + 16))) return rc;
+    if ((rc = grow(hs.c, (size_t)plan.c_bytes + 16))) return rc;
+    cudaStream_t s = hs.in;
     // Large M: rows of A go up in chunks, each chunk's GEMM starts as soon as its rows (and all of B)
     // have landed, and its rows of C go back while the next chunk is still coming in.  PCIe is full
-    // duplex, so the call costs about max(H2D, D2H) instead of H2D + GEMM + D2H.  The per-element
-    // arithmetic is the same as in one call (same tiles along N and K; no K slicing at these sizes).
+    // duplex, so the call costs about max(H2D, D2H) instead of H2D + GEMM + D2H.  Every chunk is an
+    // ordinary tile_gemm call that plans itself (tile configuration, K slices), so the fp32 bits may
+    // differ from one whole-problem call by a different summation order: same tolerance, and the
+    // same bits for integer-valued inputs.
     const int64_t chunk = kHostChunkRows;
     if (K > 0 && M >= 2 * chunk && (g_tune[6].load() & 64) == 0) {   // tuning key 6 bit 6: one shot
         const int64_t nchunks = (M + chunk - 1) / chunk;
-        {
-            std::lock_guard<std::mutex> lk(g_mu);
-            if (!g_host_compute) CUDA_TRY(cudaStreamCreateWithFlags(&g_host_compute, cudaStreamNonBlocking));
-            if (!g_host_out) CUDA_TRY(cudaStreamCreateWithFlags(&g_host_out, cudaStreamNonBlocking));
-            while ((int64_t)g_host_events.size() < 2 * nchunks + 1) {
-                cudaEvent_t e;
-                CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
-                g_host_events.push_back(e);
-            }
+        if (!hs.compute) CUDA_TRY(cudaStreamCreateWithFlags(&hs.compute, cudaStreamNonBlocking));
+        if (!hs.out) CUDA_TRY(cudaStreamCreateWithFlags(&hs.out, cudaStreamNonBlocking));
+        while ((int64_t)hs.events.size() < 2 * nchunks + 1) {
+            cudaEvent_t e;
+            CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+            hs.events.push_back(e);
         }
         const char* Ah = (const char*)A_host;
         char* Ch = (char*)C_host;
-        char* Ad = (char*)g_stage[0].p;
-        char* Cd = (char*)g_stage[2].p;
-        CUDA_TRY(cudaMemcpyAsync(g_stage[1].p, B_host, (size_t)plan.b_bytes, cudaMemcpyHostToDevice, s));
+        char* Ad = (char*)hs.a.p;
+        char* Cd = (char*)hs.c.p;
+        CUDA_TRY(cudaMemcpyAsync(hs.b.p, B_host, (size_t)plan.b_bytes, cudaMemcpyHostToDevice, s));
         for (int64_t i = 0; i < nchunks; ++i) {
             const int64_t r0 = i * chunk, rows = (M - r0) < chunk ? (M - r0) : chunk;
             const size_t a_off = (size_t)r0 * lda * 2, a_len = ((size_t)(rows - 1) * lda + K) * 2;
             CUDA_TRY(cudaMemcpyAsync(Ad + a_off, Ah + a_off, a_len, cudaMemcpyHostToDevice, s));
-            CUDA_TRY(cudaEventRecord(g_host_events[2 * i], s));
-            CUDA_TRY(cudaStreamWaitEvent(g_host_compute, g_host_events[2 * i], 0));
-            rc = tile_gemm(Ad + a_off, g_stage[1].p, Cd + (size_t)r0 * ldc * plan.esize, rows, N, K, lda, ldb, ldc, out_dtype,
-                           (void*)g_host_compute);
+            CUDA_TRY(cudaEventRecord(hs.events[2 * i], s));
+            CUDA_TRY(cudaStreamWaitEvent(hs.compute, hs.events[2 * i], 0));
+            rc = tile_gemm(Ad + a_off, hs.b.p, Cd + (size_t)r0 * ldc * plan.esize, rows, N, K, lda, ldb, ldc, out_dtype,
+                           (void*)hs.compute);
             if (rc) { cudaDeviceSynchronize(); return rc; }
-            CUDA_TRY(cudaEventRecord(g_host_events[2 * i + 1], g_host_compute));
-            CUDA_TRY(cudaStreamWaitEvent(g_host_out, g_host_events[2 * i + 1], 0));
+            CUDA_TRY(cudaEventRecord(hs.events[2 * i + 1], hs.compute));
+            CUDA_TRY(cudaStreamWaitEvent(hs.out, hs.events[2 * i + 1], 0));
             CUDA_TRY(cudaMemcpy2DAsync(Ch + (size_t)r0 * ldc * plan.esize, (size_t)ldc * plan.esize,
                                        Cd + (size_t)r0 * ldc * plan.esize, (size_t)ldc * plan.esize,
-                                       (size_t)N * plan.esize, (size_t)rows, cudaMemcpyDeviceToHost, g_host_out));
+                                       (size_t)N * plan.esize, (size_t)rows, cudaMemcpyDeviceToHost, hs.out));
         }
-        CUDA_TRY(cudaStreamSynchronize(g_host_out));
+        CUDA_TRY(cudaStreamSynchronize(hs.out));
         CUDA_TRY(cudaStreamSynchronize(s));
         return TILE_GEMM_OK;
     }
-    if (plan.a_bytes) CUDA_TRY(cudaMemcpyAsync(g_stage[0].p, A_host, (size_t)plan.a_bytes, cudaMemcpyHostToDevice, s));
-    if (plan.b_bytes) CUDA_TRY(cudaMemcpyAsync(g_stage[1].p, B_host, (size_t)plan.b_bytes, cudaMemcpyHostToDevice, s));
-    rc = tile_gemm(g_stage[0].p, g_stage[1].p, g_stage[2].p, M, N, K, lda, ldb, ldc, out_dtype, (void*)s);
+    if (plan.a_bytes) CUDA_TRY(cudaMemcpyAsync(hs.a.p, A_host, (size_t)plan.a_bytes, cudaMemcpyHostToDevice, s));
+    if (plan.b_bytes) CUDA_TRY(cudaMemcpyAsync(hs.b.p, B_host, (size_t)plan.b_bytes, cudaMemcpyHostToDevice, s));
+    rc = tile_gemm(hs.a.p, hs.b.p, hs.c.p, M, N, K, lda, ldb, ldc, out_dtype, (void*)s);
     if (rc) return rc;
-    CUDA_TRY(cudaMemcpy2DAsync(C_host, (size_t)ldc * plan.esize, g_stage[2].p, (size_t)ldc * plan.esize,
+    CUDA_TRY(cudaMemcpy2DAsync(C_host, (size_t)ldc * plan.esize, hs.c.p, (size_t)ldc * plan.esize,
                                (size_t)N * plan.esize, (size_t)M, cudaMemcpyDeviceToHost, s));
     CUDA_TRY(cudaStreamSynchronize(s));
     return TILE_GEMM_OK;
@@ -1252,7 +1425,7 @@ int tile_gemm_query_config(int64_t M, int64_t N, int64_t K, int out_dtype, int32
     int rc = current_device(&dev, &sms);
     if (rc) return rc;
     GemmLaunch gl;
-    plan_gemm(M, N, K, TILE_GEMM_IN_BF16, out_dtype, sms, &gl);
+    plan_gemm(M, N, K, TILE_GEMM_IN_BF16, out_dtype, dev, sms, &gl);
     out[0] = tg::GEMM_BM;
     out[1] = gl.cfg.tile_n();
     out[2] = gl.cfg.cg;
@@ -1270,7 +1443,7 @@ int tile_gemm_query_plan(int64_t M, int64_t N, int64_t K, int32_t out[8]) {
     int rc = current_device(&dev, &sms);
     if (rc) return rc;
     GemmLaunch gl;
-    plan_gemm(M, N, K, TILE_GEMM_IN_BF16, TILE_GEMM_OUT_BF16, sms, &gl, true);
+    plan_gemm(M, N, K, TILE_GEMM_IN_BF16, TILE_GEMM_OUT_BF16, dev, sms, &gl, true);
     int64_t rounds = 0;
     int window = 0;
     lockstep_plan(gl, &rounds, &window);
@@ -1295,7 +1468,7 @@ int tile_gemm_debug_owner_map(int32_t* owner, int64_t M, int64_t N, int64_t K, i
     int rc = current_device(&dev, &sms);
     if (rc) return rc;
     GemmLaunch gl;
-    plan_gemm(M, N, K, TILE_GEMM_IN_BF16, out_dtype, sms, &gl);
+    plan_gemm(M, N, K, TILE_GEMM_IN_BF16, out_dtype, dev, sms, &gl);
     gl.p.num_k_tiles = 0;   // same schedule and epilogue, no loads and no MMAs
     gl.p.out_16 = 0;        // the map itself is written through the 32-bit epilogue
     gl.p.out_f16 = 0;
@@ -1317,8 +1490,35 @@ int tile_gemm_debug_owner_map(int32_t* owner, int64_t M, int64_t N, int64_t K, i
     return launch_gemm(gl, tc, tc, tc, (cudaStream_t)stream, dev);
 }
 
+int tile_gemm_debug_occupy(int ctas, int64_t ns, void* stream) {
+    if (ctas < 0 || ns < 0) return fail(TILE_GEMM_E_EXTENT, "negative extent: ctas=%d ns=%lld", ctas, (long long)ns);
+    if (ns > 2000000000ll) return fail(TILE_GEMM_E_OVERFLOW, "ns=%lld above 2 s", (long long)ns);
+    int dev = 0, sms = 0;
+    int rc = current_device(&dev, &sms);
+    if (rc) return rc;
+    if (ctas == 0) return TILE_GEMM_OK;
+    constexpr int smem = 200 * 1024;   // more than half an SM: one CTA per SM
+    static bool configured[64] = {};
+    if (!configured[dev]) {
+        CUDA_TRY(cudaFuncSetAttribute(tg::occupy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        configured[dev] = true;
+    }
+    tg::occupy_kernel<<<(unsigned)ctas, 128, smem, (cudaStream_t)stream>>>((unsigned long long)ns);
+    CUDA_TRY(cudaGetLastError());
+    g_launches.fetch_add(1);
+    return TILE_GEMM_OK;
+}
+
+int tile_gemm_debug_trace(unsigned long long* records, int64_t capacity) {
+    if (capacity < 0 || capacity > INT32_MAX) return fail(TILE_GEMM_E_EXTENT, "trace capacity %lld out of range", (long long)capacity);
+    if (records && ((uintptr_t)records & 7)) return fail(TILE_GEMM_E_ALIGN, "trace buffer (%p) is not 8-byte aligned", (void*)records);
+    g_trace.store(capacity > 0 ? records : nullptr);
+    g_trace_cap.store(records ? capacity : 0);
+    return TILE_GEMM_OK;
+}
+
 int tile_gemm_set_tuning(int key, int value) {
-    if (key < 0 || key >= 8) return fail(TILE_GEMM_E_PATH, "unknown tuning key %d", key);
+    if (key < 0 || key >= kNumTune) return fail(TILE_GEMM_E_PATH, "unknown tuning key %d", key);
     g_tune[key].store(value);
     return TILE_GEMM_OK;
 }
@@ -1333,27 +1533,23 @@ const char* tile_gemm_status_string(int status) {
 const char* tile_gemm_last_error(void) { return g_err; }
 
 int tile_gemm_shutdown(void) {
+    std::lock_guard<std::mutex> host_lk(g_host_mu);
     std::lock_guard<std::mutex> lk(g_mu);
-    for (auto& kv : g_ws)
-        if (kv.second.p) cudaFree(kv.second.p);
-    g_ws.clear();
-    for (auto& kv : g_sync_ws)
-        if (kv.second.p) cudaFree(kv.second.p);
-    g_sync_ws.clear();
-    for (auto& kv : g_gemv_ws) {
-        if (kv.second.partials.p) cudaFree(kv.second.partials.p);
-        if (kv.second.tickets.p) cudaFree(kv.second.tickets.p);
+    for (auto& kv : g_wsets) free_workspace_set(kv.second);
+    g_wsets.clear();
+    for (void* q : g_retired) cudaFree(q);
+    g_retired.clear();
+    for (HostStage& hs : g_host) {
+        for (Buf* b : {&hs.a, &hs.b, &hs.c}) {
+            if (b->p) cudaFree(b->p);
+            *b = Buf();
+        }
+        if (hs.in) { cudaStreamDestroy(hs.in); hs.in = nullptr; }
+        if (hs.compute) { cudaStreamDestroy(hs.compute); hs.compute = nullptr; }
+        if (hs.out) { cudaStreamDestroy(hs.out); hs.out = nullptr; }
+        for (cudaEvent_t e : hs.events) cudaEventDestroy(e);
+        hs.events.clear();
     }
-    g_gemv_ws.clear();
-    for (Buf& b : g_stage) {
-        if (b.p) cudaFree(b.p);
-        b = Buf();
-    }
-    if (g_host_stream) { cudaStreamDestroy(g_host_stream); g_host_stream = nullptr; }
-    if (g_host_compute) { cudaStreamDestroy(g_host_compute); g_host_compute = nullptr; }
-    if (g_host_out) { cudaStreamDestroy(g_host_out); g_host_out = nullptr; }
-    for (cudaEvent_t e : g_host_events) cudaEventDestroy(e);
-    g_host_events.clear();
     g_maps.clear();
     return TILE_GEMM_OK;
 }

@@ -26,7 +26,7 @@ CANARY_BF16 = 0x7FD5
 @pytest.fixture(autouse=True)
 def _reset_tuning():
     yield
-    for key in range(8):
+    for key in range(tg.NUM_TUNE_KEYS):
         tg.tile_gemm_set_tuning(key, 0)
     torch.cuda.synchronize()
 

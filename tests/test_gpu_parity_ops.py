@@ -18,7 +18,7 @@ CANARY = 0x7FC0DEAD
 @pytest.fixture(autouse=True)
 def _reset_tuning():
     yield
-    for key in range(8):
+    for key in range(tg.NUM_TUNE_KEYS):
         tg.tile_gemm_set_tuning(key, 0)
     torch.cuda.synchronize()
 

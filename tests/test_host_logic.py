@@ -187,8 +187,25 @@ def test_record_entries_reject_bad_handles_without_a_device():
     assert lib.tile_gemm_replay(None, None) == tg.E_NULL
     assert lib.tile_gemm_recorded_nodes(None) == -1
     assert lib.tile_gemm_record_free(None) == tg.E_OK
+    import ctypes
+    out = ctypes.c_void_p(1)
+    assert lib.tile_gemm_record_end(ctypes.c_void_p(0x1000), ctypes.byref(out)) == tg.E_PATH   # that stream is not recording
+    assert out.value is None and "not recording" in tg.tile_gemm_last_error()
+    assert lib.tile_gemm_record_end(ctypes.c_void_p(0x1000), None) == tg.E_NULL
     if not torch.cuda.is_available():
         assert lib.tile_gemm_record_begin(None) == tg.E_DEVICE
+
+
+def test_debug_entries_check_their_arguments_on_the_host():
+    lib = tg.load_library()
+    import ctypes
+    assert lib.tile_gemm_debug_trace(ctypes.c_void_p(0x1004), 4) == tg.E_ALIGN
+    assert lib.tile_gemm_debug_trace(ctypes.c_void_p(0x1000), -1) == tg.E_EXTENT
+    assert lib.tile_gemm_debug_trace(None, 0) == tg.E_OK
+    assert lib.tile_gemm_debug_occupy(-1, 10, None) == tg.E_EXTENT
+    assert lib.tile_gemm_debug_occupy(1, 3_000_000_000, None) == tg.E_OVERFLOW
+    for key in range(tg.NUM_TUNE_KEYS):
+        tg.tile_gemm_set_tuning(key, 0)
 
 
 def test_swiglu_preconditions_on_the_host():
