@@ -306,7 +306,7 @@ int tile_gemm_debug_occupy(int ctas, int64_t ns, void* stream);
  * writes record by * gridDim.x + bx, when below capacity:
  *   [0] smid | bx << 16 | by << 32, then %globaltimer in ns at [1] kernel entry, [2] release of the
  *   dependency wait, [3] first tile in shared memory, [4] last tile consumed, [5] CTA done;
- *   [6] tiles consumed; [7] unused.
+ *   [6] tiles consumed; [7] %globaltimer when this CTA's partial sums were handed over (split-K only).
  * Later launches overwrite earlier ones: point it at a fresh buffer per launch.  records == NULL
  * or capacity == 0 switches tracing off (one untaken branch per event).  Process-global like the
  * tuning keys.  Returns 0, E_EXTENT or E_ALIGN.
@@ -331,6 +331,14 @@ int tile_gemm_debug_trace(unsigned long long* records, int64_t capacity);
  *          instead of through its TMA ring; 2 / 3 = GEMM lockstep producers forced on / off, bits
  *          8-15 = their window in k-tiles; 5 = full 128-row A box even for skinny M; 6 =
  *          tile_gemm_host in one shot instead of pipelined chunks.
+ *   key 8  split-K hand-over of the M = 1 kernel (csrc/gemv_kernel.cuh): 1 = tickets only, 2 = tagged
+ *          slots with a designated combiner where the launch fits the device, else tickets, 3 =
+ *          thread-block cluster + DSMEM where the slice count is <= 8, else tickets; automatic =
+ *          cluster, else tagged slots, else tickets.  All three add the partial sums in slice order.
+ *   key 9  weight tiles the M = 1 kernel sends as far as L2 right behind the dependency wait
+ *          (tile_gemm_static_b only): n >= 1 means n - 1 tiles; automatic = 2.
+ *   key 10 automatic cluster size of the M = 1 kernel: per cent of the occupancy calculator's
+ *          resident-cluster figure that the column blocks may fill; automatic = 88.
  *   key 7  tile_add_f32 launch shape: bits 0-3 vectors per thread in {1,2,4,8}, bits 4-11 CTAs
  *          per SM (255 = one tile per CTA), bits 12-15 access mode (1 / 2 = 128-bit with / without
  *          streaming hints, 3 / 4 = 256-bit with / without).

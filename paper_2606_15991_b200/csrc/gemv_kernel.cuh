@@ -199,43 +199,58 @@ gemv_tma_kernel(const __grid_constant__ CUtensorMap tmap_b, const GemvParams p) 
 // All CTAs are co-resident and HBM-bound CTAs progress at equal rates, so equal tile counts per
 // CTA (+-1) finish together whatever the SM count.
 //
-// Split-K fix-up without clusters or float atomics: a CTA with S > 1 writes its 256 fp32 partial
-// sums to the workspace, takes a ticket on the column block, and the CTA that draws the last
-// ticket adds the S partials in slice order (fixed order: bitwise reproducible) and stores y.
+// Split-K fix-up: a CTA with S > 1 hands its 256 fp32 partial sums to one CTA of its column block,
+// which adds the S partials in slice order (fixed order: bitwise reproducible, and the same bits
+// whichever of the three protocols carries them) and stores y.  The hand-over is what ends a launch:
+// it starts when the last tile has been consumed and nothing overlaps it, so its length in global
+// round trips is what the short decode launches pay (measured with tile_gemm_debug_trace on
+// K = 5120, N = 8192: 5 us of a 15 us launch with tickets, profiles/r02_gemv_trace.md).
+//   * GEMV_FLAG_CLUSTER (S <= 8, one column block per CTA): the S slices are one thread-block
+//     cluster.  Slice r > 0 pushes its partials into slice 0's shared memory with st.async, each
+//     store counting its bytes on slice 0's mbarrier; slice 0 waits on that barrier.  No global
+//     memory, no polling: ~1 us from last tile to y.
+//   * GEMV_FLAG_PACKED (every CTA of the launch resident at once): a slice's thread writes
+//     {partial, tag 1} as ONE 64-bit store into its slot and is done -- no fence, no ticket.  The CTA
+//     of the LAST slice polls the S-1 other slots of its column block, sixteen loads in flight per
+//     round, and writes them back to zero for the next launch.  One round trip + polling jitter.
+//   * tickets (any launch, any S): partials to the workspace, __threadfence, a ticket on the column
+//     block; the CTA that draws the last ticket re-reads all S partials.  Three dependent round trips.
 //
 // Programmatic dependent launch: every CTA signals launch_dependents at once, so the next kernel
-// of the stream is scheduled while this one runs (the launch leaves one CTA slot per SM free for
-// it); everything that touches x, y or the workspace sits behind griddepcontrol.wait.  With
-// GEMV_FLAG_B_IMMUTABLE (the caller promises that no work still in flight writes B: decode
-// weights) the producer fills its ring with weight tiles ahead of that wait, so HBM stays busy
-// across kernel boundaries.
+// of the stream is scheduled while this one runs; everything that touches x, y or the workspace
+// sits behind griddepcontrol.wait.  With GEMV_FLAG_B_IMMUTABLE (the caller promises that no work
+// still in flight writes B: decode weights) the producer fills its ring with weight tiles ahead of
+// that wait and, right after it, sends `l2_post` more units as far as L2 while the ring's
+// activations are still on their way, so HBM stays busy across the kernel boundary.  (Measured and
+// not kept: L2 prefetch ahead of the wait or all through the launch costs 1-15 %, it competes with
+// the loads that are on the critical path; an evict-first policy on the weight stream and an L2
+// prefetch of x change nothing.)
 constexpr int GEMV_FLAG_B_IMMUTABLE = 1;
-constexpr int GEMV_FLAG_X_TMA = 2;   // x is 16-byte aligned: its TILE_K-element slices ride the ring with the weight tiles
-constexpr int GEMV_FLAG_EVICT_FIRST = 4;   // weight tiles carry an L2 evict-first policy (read exactly once)
-constexpr int GEMV_FLAG_PACKED = 8;        // split-K fix-up through tagged 64-bit slots and a designated combiner (below)
-constexpr int GEMV_FLAG_X_PREFETCH = 16;   // bring this CTA's slices of x into L2 ahead of the dependency wait
+constexpr int GEMV_FLAG_X_TMA = 2;       // x is 16-byte aligned: its TILE_K-element slices ride the ring with the weight tiles
+constexpr int GEMV_FLAG_PACKED = 8;
+constexpr int GEMV_FLAG_CLUSTER = 32;
+constexpr int GEMV_MAX_CLUSTER = 8;      // portable cluster size
 
 struct GemvSplitParams {
     const uint16_t* x;
     void* y;
-    float* partials;      // [col_blocks][split][COLS]
-    uint32_t* tickets;    // [col_blocks], zero between launches
+    float* partials;      // tickets: [col_blocks][split][COLS]
+    uint32_t* tickets;    // tickets: [col_blocks], zero between launches
     unsigned long long* packed;   // GEMV_FLAG_PACKED: [col_blocks][split][COLS] slots {fp32 partial, tag}, all zero between launches
     int32_t N, K;
     int32_t k_tiles;      // ceil(K / TILE_K), >= split
     int32_t col_blocks;
     int32_t out_kind;     // 0: fp32 y, 1: bf16 y, 2: f16 y
     int32_t flags;
-    int32_t l2_prefetch;  // B_IMMUTABLE: units brought into L2 beyond the ring while waiting for the previous kernel
-    int32_t l2_post;      // units brought into L2 right after the dependency wait (while the first activations travel)
-    int32_t l2_steady;    // keep prefetching one unit into L2 per unit issued (stay l2_post units ahead of the ring)
+    int32_t l2_post;      // B_IMMUTABLE: units brought into L2 right after the dependency wait
     // tile_gemm_debug_trace: CTA (bx, by) writes its record of GEMV_TRACE_WORDS 64-bit words at
     // trace + (by * gridDim.x + bx) * GEMV_TRACE_WORDS when that index is below trace_cap
     unsigned long long* trace;
     int32_t trace_cap;
 };
 // trace record: [0] smid | bx << 16 | by << 32, then %globaltimer (ns) at [1] kernel entry, [2] release of
-// griddepcontrol.wait, [3] first tile in shared memory, [4] last tile consumed, [5] CTA done; [6] tiles consumed
+// griddepcontrol.wait, [3] first tile in shared memory, [4] last tile consumed, [5] CTA done; [6] tiles
+// consumed; [7] ns: partial sums handed over (S > 1)
 constexpr int GEMV_TRACE_WORDS = 8;
 __device__ __forceinline__ uint32_t sm_id() {
     uint32_t r;
@@ -263,46 +278,19 @@ __device__ __forceinline__ unsigned long long ld_relaxed_gpu_u64(const unsigned 
     asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
     return v;
 }
-__device__ __forceinline__ void prefetch_l2(const void* p) {
-    asm volatile("prefetch.global.L2 [%0];" ::"l"(p) : "memory");
-}
-// Tagged-slot split-K fix-up (GEMV_FLAG_PACKED; every CTA of the launch must be resident at once).
-// A slice's thread writes {partial, 1} as ONE 64-bit store and is done: no fence, no ticket, nothing
-// to wait for.  The CTA of the LAST slice is the designated combiner: its thread for column c polls
-// the S-1 other slots of that column until their tags show, adds the values in slice order (its own
-// last: the same order as the ticketed fix-up, so the two protocols give identical bits), and
-// writes the slots back to zero for the next launch.  One global round trip on the critical path
-// instead of three (store+fence, ticket, partial loads).
-__device__ __forceinline__ float gemv_poll_slot(const unsigned long long* slot) {
-    unsigned long long v = ld_relaxed_gpu_u64(slot);
-#if TILEGEMM_WATCHDOG
-    if ((uint32_t)(v >> 32) == 0u) {
-        const uint64_t t0 = global_timer_ns();
-        uint32_t spins = 0;
-        while ((uint32_t)((v = ld_relaxed_gpu_u64(slot)) >> 32) == 0u) {
-            __nanosleep(32);
-            if ((++spins & 0xfffu) == 0 && global_timer_ns() - t0 > 4000000000ull) {
-                printf("tilegemm watchdog: split-K slot wait timed out (block %d,%d thread %d)\n", (int)blockIdx.x,
-                       (int)blockIdx.y, (int)threadIdx.x);
-                __trap();
-            }
-        }
-    }
-#else
-    while ((uint32_t)(v >> 32) == 0u) v = ld_relaxed_gpu_u64(slot);
-#endif
-    return __uint_as_float((uint32_t)v);
-}
-
 template <int COLS, int TILE_K, int STAGES>
 struct GemvSplitSmem {
     static constexpr uint32_t BOX_BYTES = TILE_K * GEMV_COLS * 2;          // one TMA box: TILE_K rows x 256 columns
     static constexpr uint32_t TILE_BYTES = (COLS / GEMV_COLS) * BOX_BYTES;
     static constexpr uint32_t X_OFF = STAGES * TILE_BYTES;                 // per stage: TILE_K activations (128 B slots)
     static constexpr uint32_t RED_OFF = X_OFF + STAGES * 128;
-    static constexpr uint32_t FLAG_OFF = RED_OFF + GEMV_CONSUMER_WARPS * COLS * 4;
+    // cluster fix-up (default ring shape only: the other shapes have no shared memory to spare at their
+    // occupancy): the combiner receives the partial sums of the other <= 7 slices here
+    static constexpr uint32_t RECV_BYTES = (COLS == GEMV_COLS && TILE_K == 64 && STAGES == 3) ? (GEMV_MAX_CLUSTER - 1) * COLS * 4 : 0;
+    static constexpr uint32_t RECV_OFF = RED_OFF + GEMV_CONSUMER_WARPS * COLS * 4;
+    static constexpr uint32_t FLAG_OFF = RECV_OFF + RECV_BYTES;
     static constexpr uint32_t BAR_OFF = FLAG_OFF + 16;
-    static constexpr uint32_t TOTAL = BAR_OFF + 2 * STAGES * 8 + 128;   // + slack for 128 B alignment
+    static constexpr uint32_t TOTAL = BAR_OFF + (2 * STAGES + 1) * 8 + 128;   // + slack for 128 B alignment
 };
 
 // COLS columns per CTA (NV = COLS / 256 TMA boxes side by side: a row segment of COLS * 2
@@ -323,11 +311,14 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_const
     volatile uint32_t* s_last = reinterpret_cast<volatile uint32_t*>(smem_gen + L::FLAG_OFF);
     auto full_bar = [&](uint32_t s) { return smem_base + L::BAR_OFF + s * 8u; };
     auto empty_bar = [&](uint32_t s) { return smem_base + L::BAR_OFF + (STAGES + s) * 8u; };
+    const uint32_t recv_bar = smem_base + L::BAR_OFF + 2 * STAGES * 8u;
 
     const uint32_t warp = threadIdx.x >> 5;
     const uint32_t lane = threadIdx.x & 31;
     const int S = (int)gridDim.y, slice = (int)blockIdx.y;
     const int KT = p.k_tiles;
+    // cluster mode: gridDim.y == cluster size, so %cluster_ctarank == slice
+    const bool clus = L::RECV_BYTES > 0 && (p.flags & GEMV_FLAG_CLUSTER) != 0;
 
     const bool x_tma = (p.flags & GEMV_FLAG_X_TMA) != 0;
     unsigned long long* trace = nullptr;   // thread 0 only
@@ -344,9 +335,11 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_const
             mbar_init(full_bar(s), 1);
             mbar_init(empty_bar(s), GEMV_CONSUMER_WARPS);
         }
+        if (clus) mbar_init(recv_bar, 1);
         fence_mbar_init();
     }
     __syncthreads();
+    if (clus) cluster_arrive();   // "my barriers exist"; the matching wait sits in front of the first remote access, at the very end
     griddep_launch_dependents();
 
     if (warp == GEMV_CONSUMER_WARPS) {
@@ -355,19 +348,12 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_const
         //       never wait on a global load of x =====
         if (elect_one()) {
             const uint32_t tx_bytes = L::TILE_BYTES + (x_tma ? (uint32_t)TILE_K * 2u : 0u);   // full boxes, even when clipped
-            const bool evict_first = (p.flags & GEMV_FLAG_EVICT_FIRST) != 0;
-            const uint64_t policy = evict_first ? l2_policy_evict_first() : 0ull;
             auto issue_b = [&](uint32_t stage, int cb, int kt) {
                 mbar_arrive_expect_tx(full_bar(stage), tx_bytes);
 #pragma unroll
-                for (int v = 0; v < NV; ++v) {
-                    if (evict_first)
-                        tma_load_2d_hint(smem_base + stage * L::TILE_BYTES + v * L::BOX_BYTES, &tmap_b, full_bar(stage),
-                                         cb * COLS + v * GEMV_COLS, kt * TILE_K, policy);
-                    else
-                        tma_load_2d(smem_base + stage * L::TILE_BYTES + v * L::BOX_BYTES, &tmap_b, full_bar(stage),
-                                    cb * COLS + v * GEMV_COLS, kt * TILE_K);
-                }
+                for (int v = 0; v < NV; ++v)
+                    tma_load_2d(smem_base + stage * L::TILE_BYTES + v * L::BOX_BYTES, &tmap_b, full_bar(stage),
+                                cb * COLS + v * GEMV_COLS, kt * TILE_K);
             };
             auto issue_x = [&](uint32_t stage, int kt) {
                 if (x_tma) tma_load_2d(smem_base + L::X_OFF + stage * 128u, &tmap_x, full_bar(stage), kt * TILE_K, 0);
@@ -377,7 +363,6 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_const
                 if (kt >= KT) { kt = slice; cb += (int)gridDim.x; }
             };
             int cb = (int)blockIdx.x, kt = slice;
-            int cbp = (int)gridDim.x * 0 + p.col_blocks, ktp = 0;   // L2 prefetch cursor (past the end: off)
             uint32_t stage = 0, phase = 0;
             const bool have_work = cb < p.col_blocks && kt < KT;
             if ((p.flags & GEMV_FLAG_B_IMMUTABLE) && have_work) {
@@ -387,13 +372,6 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_const
                 uint32_t n_pre = 0;
                 for (; n_pre < (uint32_t)STAGES && cb2 < p.col_blocks; ++n_pre) {
                     issue_b(n_pre, cb2, kt2);
-                    next_unit(cb2, kt2);
-                }
-                // ... and the units after the ring go as far as L2: the previous kernel's last CTAs and the
-                // latency of x after the wait would otherwise leave HBM idle behind a full ring
-                for (int i = 0; i < p.l2_prefetch && cb2 < p.col_blocks; ++i) {
-#pragma unroll
-                    for (int v = 0; v < NV; ++v) tma_prefetch_l2_2d(&tmap_b, cb2 * COLS + v * GEMV_COLS, kt2 * TILE_K);
                     next_unit(cb2, kt2);
                 }
                 griddep_wait();
@@ -410,7 +388,6 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_const
                     for (int v = 0; v < NV; ++v) tma_prefetch_l2_2d(&tmap_b, cb2 * COLS + v * GEMV_COLS, kt2 * TILE_K);
                     next_unit(cb2, kt2);
                 }
-                if (p.l2_steady) { cbp = cb2; ktp = kt2; }
             } else {
                 griddep_wait();
             }
@@ -418,11 +395,6 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_const
                 mbar_wait(empty_bar(stage), phase ^ 1u);
                 issue_b(stage, cb, kt);
                 issue_x(stage, kt);
-                if (cbp < p.col_blocks) {   // keep the L2 prefetch l2_post units ahead of the ring
-#pragma unroll
-                    for (int v = 0; v < NV; ++v) tma_prefetch_l2_2d(&tmap_b, cbp * COLS + v * GEMV_COLS, ktp * TILE_K);
-                    next_unit(cbp, ktp);
-                }
                 if (++stage == STAGES) { stage = 0; phase ^= 1u; }
             }
         }
@@ -432,15 +404,6 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_const
 
     // ===== consumers: warp w owns rows RPW*w .. RPW*w+RPW-1 of every tile; lane l owns columns
     //       256 v + 8 l .. + 7 of every box v =====
-    if (p.flags & GEMV_FLAG_X_PREFETCH) {
-        // an L2 prefetch has no semantics: whatever the previous kernel still writes to x lands in the
-        // same L2, so the loads behind the wait see it -- they just do not go to DRAM any more
-        const int my_tiles = (KT - slice + S - 1) / S;
-        if ((int)threadIdx.x < my_tiles) {
-            const int k = (slice + (int)threadIdx.x * S) * TILE_K;
-            if (k < p.K) prefetch_l2(p.x + k);
-        }
-    }
     griddep_wait();   // x may be the previous kernel's output; y and the workspace may still be in its use
     if (trace) trace[2] = global_timer_ns();
     int traced_tiles = 0;
@@ -504,29 +467,76 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_const
             for (int w8 = 0; w8 < GEMV_CONSUMER_WARPS; ++w8) s[v] += red[w8 * COLS + v * GEMV_COLS + tid];   // fixed order
         }
         bool store = (S == 1);
-        if (!store && (p.flags & GEMV_FLAG_PACKED)) {
+        if (!store && clus) {
+            // DSMEM fix-up: slice r > 0 pushes its 256 partial sums into slice 0's shared memory with
+            // st.async (each store counts its bytes on slice 0's mbarrier) and is done; slice 0 waits on
+            // that barrier -- no global memory, no polling -- and adds own + slice 1 + ... in slice order
+            // (the order of the other two protocols: identical bits)
+            if constexpr (L::RECV_BYTES > 0) {
+                cluster_wait();
+                if (slice != 0) {
+                    const uint32_t rbar = map_to_cta(recv_bar, 0);
+                    const uint32_t dst = map_to_cta(smem_base + L::RECV_OFF + (uint32_t)((slice - 1) * COLS + (int)tid) * 4u, 0);
+                    st_async_f32(dst, s[0], rbar);
+                    if (trace) trace[7] = global_timer_ns();
+                } else {
+                    if (tid == 0) mbar_arrive_expect_tx(recv_bar, (uint32_t)(S - 1) * COLS * 4u);
+                    if (trace) trace[7] = global_timer_ns();
+                    mbar_wait(recv_bar, 0);
+                    const float* recv = reinterpret_cast<const float*>(smem_gen + L::RECV_OFF);
+                    for (int r = 1; r < S; ++r) s[0] += recv[(r - 1) * COLS + (int)tid];   // fixed order
+                    store = true;
+                }
+            }
+        } else if (!store && (p.flags & GEMV_FLAG_PACKED)) {
             unsigned long long* slots = p.packed + (size_t)cb * S * COLS + tid;
             if (slice != S - 1) {
 #pragma unroll
                 for (int v = 0; v < NV; ++v)
                     st_relaxed_gpu_u64(slots + (size_t)slice * COLS + v * GEMV_COLS,
                                        (1ull << 32) | (unsigned long long)__float_as_uint(s[v]));
+                if (trace) trace[7] = global_timer_ns();
             } else {
+                if (trace) trace[7] = global_timer_ns();
 #pragma unroll
                 for (int v = 0; v < NV; ++v) {
                     const float own = s[v];
                     s[v] = 0.f;
-                    for (int q0 = 0; q0 < S - 1; q0 += 8) {   // eight independent loads in flight, added in slice order
-                        unsigned long long got[8];
+                    // sixteen slots at a time: all loads of a round are in flight together, a round is repeated
+                    // until every tag of the chunk shows, then the chunk is added in slice order
+                    for (int q0 = 0; q0 < S - 1; q0 += 16) {
+                        unsigned long long got[16];
 #pragma unroll
-                        for (int j = 0; j < 8; ++j)
-                            if (q0 + j < S - 1) got[j] = ld_relaxed_gpu_u64(slots + (size_t)(q0 + j) * COLS + v * GEMV_COLS);
+                        for (int j = 0; j < 16; ++j) got[j] = 0ull;
+#if TILEGEMM_WATCHDOG
+                        uint64_t t0 = 0;
+                        uint32_t rounds = 0;
+#endif
+                        for (;;) {
+                            bool all = true;
 #pragma unroll
-                        for (int j = 0; j < 8; ++j)
+                            for (int j = 0; j < 16; ++j)
+                                if (q0 + j < S - 1 && (uint32_t)(got[j] >> 32) == 0u) {
+                                    got[j] = ld_relaxed_gpu_u64(slots + (size_t)(q0 + j) * COLS + v * GEMV_COLS);
+                                    all = all && (uint32_t)(got[j] >> 32) != 0u;
+                                }
+                            if (all) break;
+#if TILEGEMM_WATCHDOG
+                            if ((++rounds & 0xfffu) == 0) {
+                                if (t0 == 0) t0 = global_timer_ns();
+                                else if (global_timer_ns() - t0 > 4000000000ull) {
+                                    printf("tilegemm watchdog: split-K slot wait timed out (block %d,%d thread %d)\n",
+                                           (int)blockIdx.x, (int)blockIdx.y, (int)threadIdx.x);
+                                    __trap();
+                                }
+                            }
+#endif
+                        }
+#pragma unroll
+                        for (int j = 0; j < 16; ++j)
                             if (q0 + j < S - 1) {
-                                unsigned long long* slot = slots + (size_t)(q0 + j) * COLS + v * GEMV_COLS;
-                                s[v] += ((uint32_t)(got[j] >> 32) != 0u) ? __uint_as_float((uint32_t)got[j]) : gemv_poll_slot(slot);
-                                st_relaxed_gpu_u64(slot, 0ull);   // re-arm for the next launch
+                                s[v] += __uint_as_float((uint32_t)got[j]);
+                                st_relaxed_gpu_u64(slots + (size_t)(q0 + j) * COLS + v * GEMV_COLS, 0ull);   // re-arm
                             }
                     }
                     s[v] += own;
@@ -546,6 +556,7 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_const
                 *s_last = last ? 1u : 0u;
             }
             consumer_bar_sync();
+            if (trace) trace[7] = global_timer_ns();
             if (*s_last) {
                 __threadfence();
 #pragma unroll

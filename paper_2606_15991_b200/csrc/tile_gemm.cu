@@ -762,15 +762,59 @@ int launch_gemv_split(const void* B, int64_t N, int64_t K, int64_t ldb, tg::Gemv
     cfg.blockDim = dim3(tg::GEMV_TMA_THREADS, 1, 1);
     cfg.dynamicSmemBytes = L::TOTAL;
     cfg.stream = s;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchAttribute attr[2];
+    int na = 0;
+    if (pdl) {
+        attr[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[na].val.programmaticStreamSerializationAllowed = 1;
+        ++na;
+    }
+    if (p.flags & tg::GEMV_FLAG_CLUSTER) {   // the slices of a column block form one cluster along y
+        attr[na].id = cudaLaunchAttributeClusterDimension;
+        attr[na].val.clusterDim.x = 1;
+        attr[na].val.clusterDim.y = (unsigned)split;
+        attr[na].val.clusterDim.z = 1;
+        ++na;
+    }
     cfg.attrs = attr;
-    cfg.numAttrs = pdl ? 1 : 0;
+    cfg.numAttrs = na;
     CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, tb, tx, p));
     g_launches.fetch_add(1);
     return TILE_GEMM_OK;
 }
+
+// clusters of `cs` CTAs of the default M = 1 kernel the device holds at once (occupancy calculator, cached)
+int gemv_cluster_capacity(int cs, int dev, int sms) {
+    static std::atomic<int> cache[tg::GEMV_MAX_CLUSTER + 1][64];
+    if (cs < 1 || cs > tg::GEMV_MAX_CLUSTER) return 0;
+    int v = cache[cs][dev].load();
+    if (v > 0) return v;
+    using L = tg::GemvSplitSmem<256, 64, 3>;
+    auto kern = tg::gemv_split_kernel<256, 64, 3, 2, false>;
+    int n = 0;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::TOTAL) == cudaSuccess) {
+        cudaLaunchConfig_t cfg;
+        memset(&cfg, 0, sizeof cfg);
+        cfg.gridDim = dim3(64, (unsigned)cs, 1);
+        cfg.blockDim = dim3(tg::GEMV_TMA_THREADS, 1, 1);
+        cfg.dynamicSmemBytes = L::TOTAL;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 1;
+        attr[0].val.clusterDim.y = (unsigned)cs;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess) n = 0;
+    }
+    cudaGetLastError();
+    if (n <= 0) n = (sms * 2) / (cs + 1);   // conservative guess
+    cache[cs][dev].store(n);
+    return n;
+}
+
+// measured on B200: two units into L2 behind the dependency wait; clusters sized to 88 % of capacity
+constexpr int kGemvL2PostUnits = 2, kGemvClusterMarginPct = 88;
 
 // ring shapes of the split kernel: {columns per CTA, rows per stage, stages, CTAs per SM}
 struct GemvShape { int cols, tile_k, stages, occ; };
@@ -809,10 +853,27 @@ int run_gemv_split(const void* x, const void* B, void* y, int64_t N, int64_t K, 
             }
         }
     }
+    // Fix-up protocol (gemv_kernel.cuh; tuning key 8: 0 auto, 1 tickets, 2 tagged slots else tickets, 3 cluster
+    // else tickets).  Cluster: default ring shape, one column block per CTA, S <= 8 -- and when the automatic S is
+    // within reach (<= 10) it becomes the largest cluster size whose clusters all fit the device at once with
+    // slots to spare (key 10: per cent of the occupancy calculator's figure, default 88), because clusters of the
+    // next kernel can only start where a whole cluster's worth of slots is free.
+    const int fix_mode = g_tune[8].load();
+    const bool cluster_ok = (fix_mode == 0 || fix_mode == 3) && shape == 2 && gx == col_blocks;
+    if (cluster_ok && g_tune[3].load() <= 0 && split > 1 && split <= tg::GEMV_MAX_CLUSTER + 2) {
+        int margin = g_tune[10].load();
+        if (margin <= 0) margin = kGemvClusterMarginPct;
+        for (int64_t cs = tg::GEMV_MAX_CLUSTER; cs >= 2; --cs)
+            if (col_blocks * 100 <= (int64_t)gemv_cluster_capacity((int)cs, dev, sms) * margin && k_tiles / cs >= 4) {
+                if (cs <= split) split = cs;
+                break;
+            }
+    }
     if (split > k_tiles) split = k_tiles;
     if (split > 65535) split = 65535;
     if (split < 1) split = 1;
     tg::GemvSplitParams p;
+    memset(&p, 0, sizeof p);
     p.x = (const uint16_t*)x;
     p.y = y;
     p.N = (int32_t)N;
@@ -822,21 +883,16 @@ int run_gemv_split(const void* x, const void* B, void* y, int64_t N, int64_t K, 
     p.out_kind = out_dtype;
     p.flags = (flags & TILE_GEMM_FLAG_B_IMMUTABLE) ? tg::GEMV_FLAG_B_IMMUTABLE : 0;
     if ((((uintptr_t)x) & 15) == 0 && (g_tune[6].load() & 2) == 0) p.flags |= tg::GEMV_FLAG_X_TMA;
-    if (g_tune[9].load() == 1) p.flags |= tg::GEMV_FLAG_EVICT_FIRST;
-    p.l2_prefetch = g_tune[8].load() > 0 ? g_tune[8].load() : 0;
     p.trace = g_trace.load();
     p.trace_cap = (int32_t)g_trace_cap.load();
-    p.l2_post = g_tune[10].load() > 0 ? g_tune[10].load() : 0;
-    p.l2_steady = g_tune[12].load() > 0 ? 1 : 0;
-    if (g_tune[11].load() & 1) p.flags |= tg::GEMV_FLAG_X_PREFETCH;
-    p.partials = nullptr;
-    p.tickets = nullptr;
-    p.packed = nullptr;
+    const int post = g_tune[9].load();                       // tuning key 9: n >= 1 -> n - 1 units
+    p.l2_post = post > 0 ? post - 1 : kGemvL2PostUnits;
     if (split > 1) {
-        // tagged slots + designated combiner need every CTA of the launch resident at once
-        const bool packed = (g_tune[11].load() & 2) && gx * split <= budget;
-        int rc;
-        if (packed) {
+        int rc = TILE_GEMM_OK;
+        if (cluster_ok && split <= tg::GEMV_MAX_CLUSTER) {
+            p.flags |= tg::GEMV_FLAG_CLUSTER;
+        } else if ((fix_mode == 0 || fix_mode == 2) && gx * split <= budget) {
+            // tagged slots: the designated combiner polls, so every CTA of the launch must fit the device at once
             rc = packed_workspace_for(dev, s, (size_t)col_blocks * split * gs.cols * 8, &p.packed);
             p.flags |= tg::GEMV_FLAG_PACKED;
         } else {

@@ -215,12 +215,14 @@ def test_gemv_variants_integer_bit_exact(variant, split):
 @pytest.mark.parametrize("shape", [1, 2, 3, 4, 5, 6, 7, 8])
 @pytest.mark.parametrize("cap", [0, 1, 3, 7, 100])
 @pytest.mark.parametrize("nopdl", [0, 1])
-def test_gemv_split_decompositions_integer_bit_exact(shape, cap, nopdl):
+@pytest.mark.parametrize("fix", [0, 1])
+def test_gemv_split_decompositions_integer_bit_exact(shape, cap, nopdl, fix):
     """The interleaved split-K kernel under every decomposition: one CTA looping over all column
-    blocks (cap=1), fewer CTAs than column blocks (cap 3, 7), deep splits with the ticketed fix-up
-    (cap 100 and the full budget); K and N tails; every ring shape; with and without programmatic
-    dependent launch."""
+    blocks (cap=1), fewer CTAs than column blocks (cap 3, 7), deep splits (cap 100 and the full
+    budget); K and N tails; every ring shape; with and without programmatic dependent launch; with
+    the automatic choice of fix-up protocol (cluster / tagged slots / tickets) and with tickets only."""
     occ = shape
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMV_FIXUP, fix)
     tg.tile_gemm_set_tuning(tg.TUNE_GEMV_VARIANT, 4)
     tg.tile_gemm_set_tuning(tg.TUNE_GEMV_SHAPE, shape)
     tg.tile_gemm_set_tuning(tg.TUNE_GEMM_MAX_CTAS, cap)
@@ -233,11 +235,64 @@ def test_gemv_split_decompositions_integer_bit_exact(shape, cap, nopdl):
             check_bit_exact(got, ref, f"flat occ{occ} cap{cap} K={K} N={N} rep{rep}")
 
 
+@pytest.mark.parametrize("split", [0, 2, 3, 5, 8, 11, 24])
 @pytest.mark.parametrize("static_b", [False, True])
-def test_gemv_chain_is_stream_ordered_under_pdl(static_b):
+def test_gemv_fixup_protocols_give_the_same_bits(split, static_b):
+    """The three split-K hand-over protocols of the M = 1 kernel (thread-block cluster + DSMEM, tagged
+    slots with a designated combiner, tickets) add the S partial sums in the same slice order: on
+    normal inputs they must agree bit for bit, call after call (slots and tickets re-armed), and each
+    matches the oracle."""
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMV_SPLIT, split)
+    for (K, N) in ((5120, 2048), (2560, 8200), (1999, 1000)):
+        a, b = wl.make_inputs_custom(1, N, K, sigma_b=K ** -0.5, seed=K + N + split)
+        ref, S = oracle.gemm(a, b)
+        x, W = wl.bits_to_torch(a, DEV), wl.bits_to_torch(b, DEV)
+        outs = {}
+        for fix in (1, 2, 3, 0):
+            tg.tile_gemm_set_tuning(tg.TUNE_GEMV_FIXUP, fix)
+            for rep in range(3):
+                y = torch.full((1, N), float("nan"), dtype=torch.float32, device=DEV)
+                tg.tile_gemm(x, W, y, static_b=static_b)
+                torch.cuda.synchronize()
+                outs[(fix, rep)] = y.cpu().numpy()
+            check_close(outs[(fix, 0)].astype(np.float64), ref, S, K, "f32", f"fix-up {fix} K={K} N={N} S={split}")
+        # with the automatic slice count the cluster protocol may pick another S (a cluster size that fits the
+        # device), so only protocols that ran the same decomposition are comparable bit for bit
+        same_cut = (1, 2) if split == 0 else (1, 2, 3, 0)
+        first = outs[(1, 0)].view(np.uint32)
+        for (fix, rep), v in outs.items():
+            want = first if fix in same_cut else outs[(fix, 0)].view(np.uint32)
+            assert np.array_equal(v.view(np.uint32), want), f"fix-up {fix} rep {rep}: bits differ (K={K} N={N} S={split})"
+
+
+def test_gemv_completes_next_to_a_kernel_that_holds_sms():
+    """Tagged slots and clusters assume the launch fits the device; with 100 SMs held by another kernel
+    the CTAs arrive in waves instead.  The designated combiner is the LAST slice of its column block,
+    so everything it waits for was dispatched before it: the launch still completes, with the same bits."""
+    K, N = 5120, 8192
+    a, b = wl.make_inputs_custom(1, N, K, "int4", seed=77)
+    ref, _ = oracle.gemm(a, b)
+    x, W = wl.bits_to_torch(a, DEV), wl.bits_to_torch(b, DEV)
+    blocker, worker = torch.cuda.Stream(), torch.cuda.Stream()
+    for fix in (0, 2, 3):
+        tg.tile_gemm_set_tuning(tg.TUNE_GEMV_FIXUP, fix)
+        y = torch.full((1, N), float("nan"), dtype=torch.float32, device=DEV)
+        torch.cuda.synchronize()
+        tg.tile_gemm_debug_occupy(100, 20_000_000, stream=blocker)
+        for _ in range(3):
+            tg.tile_gemm(x, W, y, stream=worker, static_b=True)
+        worker.synchronize()
+        blocker.synchronize()
+        check_bit_exact(y.cpu().numpy(), ref, f"GEMV next to a blocker, fix-up {fix}")
+
+
+@pytest.mark.parametrize("fix", [0, 1, 2])
+@pytest.mark.parametrize("static_b", [False, True])
+def test_gemv_chain_is_stream_ordered_under_pdl(static_b, fix):
     """y of one GEMV is x of the next, launched back to back with programmatic dependent launch:
     the bits must equal those of the same chain run with a synchronise after every launch, and every
     link must match the oracle on the bits it was given."""
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMV_FIXUP, fix)
     K = N = 2048
     depth = 6
     rng = np.random.default_rng(31)
@@ -329,28 +384,119 @@ def test_cfg4_prefill_sampled(proj):
     assert np.all(np.abs(Cband @ r - a64 @ br) <= tol)
 
 
+# ------------------------------------------------------------------ the accumulator's arithmetic
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4])
+def test_tcgen05_accumulator_model_predicts_every_bit(cfg):
+    """DESIGN.md 7 / tests/parity.py widen the fp32 gates by (K/16) * 2^-24 because "the tensor core
+    adds each K = 16 step with truncation".  This pins that claim: parity.tcgen05_accumulate_model
+    (align 16 products + accumulator to the largest exponent, truncate each toward zero with two guard
+    bits, add exactly, truncate to fp32) predicts the kernel's fp32 output BIT FOR BIT -- on inputs
+    constructed so that round-to-nearest and truncation differ, and on random normal inputs -- for the
+    1-CTA and the 2-CTA tile configurations alike."""
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMM_CONFIG, cfg)
+    M = N = 256
+    for groups, exact, nearest, want in parity.TRUNCATION_CASES:
+        v = []
+        for g in groups:
+            v += list(g) + [0.0] * (16 - len(g))
+        K = max(64, len(v))
+        a32 = np.zeros((M, K), dtype=np.float32)
+        a32[:, :len(v)] = np.asarray(v, dtype=np.float32)
+        a = wl.f32_to_bf16_bits(a32)
+        a64 = oracle.bf16_decode(a)
+        assert np.array_equal(a64, a32.astype(np.float64)), "the constructed values must be exact in bf16"
+        b = wl.f32_to_bf16_bits(np.ones((K, N), dtype=np.float32))
+        ref, S = oracle.gemm(a, b)
+        assert ref[0, 0] == exact                                     # the oracle states the exact sum
+        got = run_case(a, b, "f32", what=f"constructed {groups}")
+        assert np.all(got == want), f"{groups}: kernel {got[0, 0]}, truncation model says {want}, round-to-nearest {nearest}"
+        model = parity.tcgen05_accumulate_model(a64, oracle.bf16_decode(b))
+        assert np.all(model == want), f"{groups}: the model itself gives {model[0, 0]}, expected {want}"
+        assert np.all(np.abs(got - ref) <= 2.0 * K * 2.0 ** -24 * S)    # and all of it is inside the tight gate
+    rng = np.random.default_rng([77, cfg])
+    for K in (16, 80, 256, 1024):
+        a = wl.f32_to_bf16_bits(rng.standard_normal((M, K), dtype=np.float32))
+        b = wl.f32_to_bf16_bits(rng.standard_normal((K, N), dtype=np.float32) * np.float32(K ** -0.5))
+        got = run_case(a, b, "f32", what=f"random K={K}")
+        model = parity.tcgen05_accumulate_model(oracle.bf16_decode(a), oracle.bf16_decode(b))
+        bad = got != model
+        assert not bad.any(), f"K={K}: {int(bad.sum())} of {bad.size} elements differ from the truncation model"
+        ref, S = oracle.gemm(a, b)
+        signed = (got - ref) * np.sign(ref)
+        assert signed.mean() < 0, "truncation toward zero must show as a bias toward zero against the exact sums"
+
+
 # ------------------------------------------------------------------ config 5 (decode GEMV)
 def _cfg5_layers():
-    if os.environ.get("TILEGEMM_FULL_CFG5") == "1":
+    """All 64 layers by default (BASELINE.json config 5: "full oracle comparison");
+    TILEGEMM_CFG5_LAYERS=n restricts a quick local run to layers {0, ..., n-2, 63}."""
+    n = int(os.environ.get("TILEGEMM_CFG5_LAYERS", wl.DECODE_LAYERS))
+    if n >= wl.DECODE_LAYERS:
         return list(range(wl.DECODE_LAYERS))
-    return [0, wl.DECODE_LAYERS - 1]
+    return sorted(set(list(range(max(n - 1, 1))) + [wl.DECODE_LAYERS - 1]))
 
 
 def test_cfg5_decode_full_oracle():
-    """Every output of every checked GEMV against the oracle, in the auto launch configuration.
-    Default: layers {0, 63} x 4 projections (8 GEMVs, 1.95 GB of weights); TILEGEMM_FULL_CFG5=1
-    checks all 64 layers (256 GEMVs, 62.4 GB)."""
-    for layer in _cfg5_layers():
-        for proj in range(4):
-            case = wl.cfg5_case(layer, proj)
-            x, W = wl.make_inputs_device(case, DEV)
-            y = torch.empty((1, case.N), dtype=torch.bfloat16, device=DEV)
-            assert tg.tile_gemm_select(1, case.N, case.K, case.K, case.N, case.N) == tg.PATH_GEMV
-            tg.tile_gemm(x, W, y)
-            torch.cuda.synchronize()
-            ref, S = oracle.gemm(wl.torch_to_bits(x), wl.torch_to_bits(W))
-            check_close(y.float().cpu().numpy(), ref, S, case.K, "bf16", case.name)
-            del W
+    """Every output of all 256 GEMVs of config 5 (64 layers x 4 projections, 62.4 GB of weights, each
+    generated in its own buffer) against the oracle, in the auto launch configuration; odd layers go
+    through tile_gemm_static_b (the entry bench.py times), even layers through tile_gemm.  The four
+    oracle calls of a layer (M = 1: one thread each) run side by side on the host."""
+    from concurrent.futures import ThreadPoolExecutor
+    checked = 0
+    with ThreadPoolExecutor(max_workers=4) as pool:
+        for layer in _cfg5_layers():
+            jobs = []
+            for proj in range(4):
+                case = wl.cfg5_case(layer, proj)
+                x, W = wl.make_inputs_device(case, DEV)
+                y = torch.empty((1, case.N), dtype=torch.bfloat16, device=DEV)
+                assert tg.tile_gemm_select(1, case.N, case.K, case.K, case.N, case.N) == tg.PATH_GEMV
+                tg.tile_gemm(x, W, y, static_b=(layer % 2 == 1))
+                torch.cuda.synchronize()
+                xb, Wb, got = wl.torch_to_bits(x), wl.torch_to_bits(W), y.float().cpu().numpy()
+                del W
+                jobs.append((case, got, pool.submit(oracle.gemm, xb, Wb)))
+            for case, got, fut in jobs:
+                ref, S = fut.result()
+                check_close(got, ref, S, case.K, "bf16", case.name)
+                checked += 1
+    assert checked == 4 * len(_cfg5_layers())
+
+
+# ------------------------------------------------------------------ column shards (SURVEY 8(e))
+@pytest.mark.parametrize("G", [2, 8])
+def test_column_shards_equal_the_unsharded_result(G):
+    """SURVEY 8(e) / DESIGN.md 9: a caller that shards N over G devices calls tile_gemm on
+    B[:, n_g] (ldb = N) and C[:, n_g] (ldc = N).  Every output element is the same K-ordered sum
+    whatever tile it falls in, so as long as neither launch cuts K the shards reproduce the
+    unsharded bits exactly (normal inputs); M = 1 shards change the K slicing, so there the check is
+    bit-exact on integer-valued inputs and within tolerance on normal ones."""
+    M, N, K = 384, 4096, 768
+    a, b = wl.make_inputs_custom(M, N, K, sigma_b=K ** -0.5, seed=90 + G)
+    A, B = wl.bits_to_torch(a, DEV), wl.bits_to_torch(b, DEV)
+    assert tg.tile_gemm_query_plan(M, N, K)["split"] == 0 and tg.tile_gemm_query_plan(M, N // G, K)["split"] == 0
+    for out_dt in (torch.float32, torch.bfloat16):
+        whole = torch.empty((M, N), dtype=out_dt, device=DEV)
+        tg.tile_gemm(A, B, whole)
+        shards = torch.full((M, N), float("nan"), dtype=out_dt, device=DEV)
+        w = N // G
+        for g in range(G):
+            tg.tile_gemm(A, B[:, g * w:(g + 1) * w], shards[:, g * w:(g + 1) * w])
+        torch.cuda.synchronize()
+        assert torch.equal(whole, shards), f"G={G} {out_dt}: column shards differ from the unsharded result"
+    ref, S = oracle.gemm(a, b)
+    check_close(whole.float().cpu().numpy(), ref, S, K, "bf16", f"unsharded G={G}")
+    # M = 1 (decode): integer-valued inputs, bit-exact against the oracle shard by shard
+    N1, K1 = 8192, 2560
+    x, Wt = wl.make_inputs_custom(1, N1, K1, "int4", seed=95 + G)
+    ref1, _ = oracle.gemm(x, Wt)
+    xd, Wd = wl.bits_to_torch(x, DEV), wl.bits_to_torch(Wt, DEV)
+    y = torch.full((1, N1), float("nan"), dtype=torch.float32, device=DEV)
+    w = N1 // G
+    for g in range(G):
+        tg.tile_gemm(xd, Wd[:, g * w:(g + 1) * w], y[:, g * w:(g + 1) * w], static_b=True)
+    torch.cuda.synchronize()
+    check_bit_exact(y.cpu().numpy(), ref1, f"M=1 column shards G={G}")
 
 
 # ------------------------------------------------------------------ ownership

@@ -229,3 +229,33 @@ def test_selector_routes_a_few_rows_to_the_weight_streaming_path():
         assert sel(M, 10240, 5120, lda=5121) == tg.PATH_GEMM_REPACK
         assert sel(M, 10240, 5120, A=A0 + 2) == tg.PATH_GEMM_REPACK
     assert sel(5, 10240, 5120) == tg.PATH_GEMM_TMA
+
+
+@pytest.mark.parametrize("G", [2, 8])
+def test_selector_on_column_shards(G):
+    """column shard g of a row-major B (K x N) is the pointer B + g*N/G with ldb = N.
+    For the Qwen3 shapes every shard stays TMA-addressable (16-byte aligned start, ldb % 8 == 0) and
+    disjoint from the other shards' C columns, so the selector takes the same paths as unsharded."""
+    for (K, N) in wl.QWEN3_32B:
+        w = N // G
+        for g in (0, G - 1):
+            Bg, Cg = B0 + 2 * g * w, C0 + 2 * g * w
+            assert tg.tile_gemm_select(4096, w, K, K, N, N, A0, Bg, Cg, tg.OUT_BF16) == tg.PATH_GEMM_TMA
+            assert tg.tile_gemm_select(1, w, K, K, N, N, A0, Bg, Cg, tg.OUT_BF16) == tg.PATH_GEMV
+    # a shard whose first column is not 16-byte aligned falls back to the repack path, still legal
+    assert tg.tile_gemm_select(64, 100, 256, 256, 1004, 1004, A0, B0 + 2 * 100, C0 + 4 * 100, tg.OUT_F32) == tg.PATH_GEMM_REPACK
+
+
+def test_truncation_model_on_the_hand_worked_cases():
+    """parity.tcgen05_accumulate_model (the statement of how the tensor core sums) gives
+    the hand-worked values of parity.TRUNCATION_CASES; the GPU test then holds the kernel to both."""
+    for groups, exact, nearest, want in parity.TRUNCATION_CASES:
+        v = []
+        for g in groups:
+            v += list(g) + [0.0] * (16 - len(g))
+        a = np.array([v])
+        assert a.sum() == exact
+        assert np.float64(np.float32(exact)) == nearest or abs(exact) % 1 == 0.5   # RNE of the exact sum (ties listed by hand)
+        got = parity.tcgen05_accumulate_model(a, np.ones((len(v), 1)))[0, 0]
+        assert got == want
+
