@@ -443,6 +443,11 @@ double launch_us(int64_t M, int64_t N, int64_t K, int tile_m, int tile_n, int cg
 GemmConfig choose_config(int64_t M, int64_t N, int64_t K, int sms) {
     const int forced = g_tune[0].load();
     if (forced >= 1 && forced <= 4) return kConfigs[forced];
+    // One row of 128-tall tiles covers M: a CTA pair's second CTA would own rows that do not exist, and the
+    // launch is a weight stream where many narrow tiles keep more SMs pulling (measured at M = 8 on the decode
+    // shapes: 128x128 tiles 4.4 / 3.9 / 6.3 / 5.0 TB/s, 128x256 3.5 / 3.2 / 5.8 / 4.5, the pair kernels 5.2 on
+    // K = 5120, N = 51200 where they used to be chosen).
+    if (M <= tg::GEMM_BM) return kConfigs[1];
     const int64_t t3 = ((M + 255) / 256) * ((N + 255) / 256);
     const int64_t t4 = ((M + 255) / 256) * ((N + 511) / 512);
     // the 256x512 tile moves a quarter less operand data per FLOP (the kernel is power bound,

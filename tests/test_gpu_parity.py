@@ -677,6 +677,10 @@ def test_selector_plans_for_the_benchmarked_shapes():
         p = plan(M, 5120, 25600)
         assert p["full_units"] == 0 and p["split"] >= 2 and p["a_box_rows"] == 16 and p["ctas"] >= 100
     assert plan(40, 10240, 5120)["a_box_rows"] == 64
+    for M in (8, 64, 128):                # one row of 128-tall tiles: never a CTA pair, 128x128 tiles on every SM
+        p = plan(M, 51200, 5120)
+        assert p["config"] == 1 and p["ctas"] == 148
+    assert plan(129, 51200, 5120)["config"] in (3, 4)
 
 
 # ------------------------------------------------------------------ M = 2..4: the multi-row GEMV
