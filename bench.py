@@ -453,41 +453,44 @@ def bench_sweep(tg, torch, sizes, tdist, warm_s=0.35):
                     if n >= 8192:
                         torch.cuda.synchronize()   # keep the launch queue short: the warm-up must end on time
 
-            warm(warm_s)
-            # (a) per-launch events inside a back-to-back stream
-            evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
-            for i in range(reps):
-                evs[i][0].record()
-                tg.tile_gemm(*bufs[i % sets])
-                evs[i][1].record()
-            torch.cuda.synchronize()
-            med = float(np.median([a.elapsed_time(b) for a, b in evs]))
-            # (b) back to back, no inner events
-            warm(warm_s / 3)
-            tdist.barrier()
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record()
-            for i in range(reps):
-                tg.tile_gemm(*bufs[i % sets])
-            e1.record()
-            torch.cuda.synchronize()
-            b2b = e0.elapsed_time(e1) / reps
-            # (c) the same launches as one recorded step
+            # the same launches as one recorded step (mode c)
             rs = torch.cuda.Stream()
             tg.tile_gemm_record_begin(rs)
             for i in range(reps):
                 tg.tile_gemm(*bufs[i % sets], stream=rs)
             step = tg.tile_gemm_record_end(rs)
-            warm(warm_s / 3)
-            torch.cuda.synchronize()
-            step.replay(rs)
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record(rs)
-            step.replay(rs)
-            e1.record(rs)
-            rs.synchronize()
-            rep_ms = e0.elapsed_time(e1) / reps
+            meds, b2bs, recs = [], [], []
+            for rnd in range(3):   # the three modes interleaved, three rounds, median of each: drift of the power state averages out
+                warm(warm_s if rnd == 0 else warm_s / 3)
+                # (a) per-launch events inside a back-to-back stream
+                evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+                for i in range(reps):
+                    evs[i][0].record()
+                    tg.tile_gemm(*bufs[i % sets])
+                    evs[i][1].record()
+                torch.cuda.synchronize()
+                meds.append(float(np.median([a.elapsed_time(b) for a, b in evs])))
+                # (b) back to back, no inner events
+                warm(warm_s / 3)
+                tdist.barrier()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                for i in range(reps):
+                    tg.tile_gemm(*bufs[i % sets])
+                e1.record()
+                torch.cuda.synchronize()
+                b2bs.append(e0.elapsed_time(e1) / reps)
+                # (c) one recorded step
+                warm(warm_s / 3)
+                torch.cuda.synchronize()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(rs)
+                step.replay(rs)
+                e1.record(rs)
+                rs.synchronize()
+                recs.append(e0.elapsed_time(e1) / reps)
             step.free()
+            med, b2b, rep_ms = float(np.median(meds)), float(np.median(b2bs)), float(np.median(recs))
             fl = 2.0 * n ** 3
             out[dt_name][str(n)] = [round(med * 1e3, 1), round(b2b * 1e3, 1), round(rep_ms * 1e3, 1),
                                     round(fl / (rep_ms * 1e-3) / 1e12, 1),

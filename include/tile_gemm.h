@@ -245,9 +245,10 @@ int tile_gemm_select(int64_t M, int64_t N, int64_t K,
  * and B to the device, runs tile_gemm, copies C[0..M) x [0..N) back (row pitch
  * ldc) and synchronises before returning.  Device staging buffers are grow-only
  * and owned by the library.  For M >= 2048 the rows of A go up in 1024-row chunks
- * on one stream, each chunk's GEMM runs on a second stream as soon as its rows and
- * all of B have landed, and its rows of C return on a third while the next chunk
- * is still coming in (PCIe is full duplex).  Every chunk is an ordinary tile_gemm
+ * (the last 1024 rows in halving chunks down to 128 rows, so that little is left to
+ * do after the last byte has arrived) on one stream, each chunk's GEMM runs on a
+ * second stream as soon as its rows and all of B have landed, and its rows of C
+ * return on a third while the next chunk is still coming in (PCIe is full duplex).  Every chunk is an ordinary tile_gemm
  * call that plans itself, so fp32 results may differ from the one-shot order in
  * the last bits (same tolerance; identical for integer-valued inputs).  Pinned
  * host memory is needed for the copies to overlap.  This is the call bench.py's

@@ -1409,7 +1409,7 @@ int tile_gemm_record_free(void* step) {
     return TILE_GEMM_OK;
 }
 
-constexpr int64_t kHostChunkRows = 1024;
+constexpr int64_t kHostChunkRows = 1024, kHostTailRows = 128;
 
 int tile_gemm_host(const void* A_host, const void* B_host, void* C_host, int64_t M, int64_t N, int64_t K,
                    int64_t lda, int64_t ldb, int64_t ldc, int out_dtype) {
@@ -1438,7 +1438,16 @@ int tile_gemm_host(const void* A_host, const void* B_host, void* C_host, int64_t
     // same bits for integer-valued inputs.
     const int64_t chunk = kHostChunkRows;
     if (K > 0 && M >= 2 * chunk && (g_tune[6].load() & 64) == 0) {   // tuning key 6 bit 6: one shot
-        const int64_t nchunks = (M + chunk - 1) / chunk;
+        // chunk heights: kHostChunkRows while more than that is left, then the rest halves down to
+        // kHostTailRows -- what follows the last uploaded byte (that chunk's GEMM and its copy-out) is the only
+        // part of the call nothing overlaps, so the last chunk is small
+        std::vector<int64_t> heights;
+        int64_t left = M;
+        while (left > chunk) { heights.push_back(chunk); left -= chunk; }
+        while (left > 2 * kHostTailRows) { heights.push_back(left / 2); left -= left / 2; }
+        if (left > kHostTailRows) { heights.push_back(left - kHostTailRows); left = kHostTailRows; }
+        heights.push_back(left);
+        const int64_t nchunks = (int64_t)heights.size();
         if (!hs.compute) CUDA_TRY(cudaStreamCreateWithFlags(&hs.compute, cudaStreamNonBlocking));
         if (!hs.out) CUDA_TRY(cudaStreamCreateWithFlags(&hs.out, cudaStreamNonBlocking));
         while ((int64_t)hs.events.size() < 2 * nchunks + 1) {
@@ -1451,8 +1460,9 @@ int tile_gemm_host(const void* A_host, const void* B_host, void* C_host, int64_t
         char* Ad = (char*)hs.a.p;
         char* Cd = (char*)hs.c.p;
         CUDA_TRY(cudaMemcpyAsync(hs.b.p, B_host, (size_t)plan.b_bytes, cudaMemcpyHostToDevice, s));
+        int64_t r0 = 0;
         for (int64_t i = 0; i < nchunks; ++i) {
-            const int64_t r0 = i * chunk, rows = (M - r0) < chunk ? (M - r0) : chunk;
+            const int64_t rows = heights[i];
             const size_t a_off = (size_t)r0 * lda * 2, a_len = ((size_t)(rows - 1) * lda + K) * 2;
             CUDA_TRY(cudaMemcpyAsync(Ad + a_off, Ah + a_off, a_len, cudaMemcpyHostToDevice, s));
             CUDA_TRY(cudaEventRecord(hs.events[2 * i], s));
@@ -1465,6 +1475,7 @@ int tile_gemm_host(const void* A_host, const void* B_host, void* C_host, int64_t
             CUDA_TRY(cudaMemcpy2DAsync(Ch + (size_t)r0 * ldc * plan.esize, (size_t)ldc * plan.esize,
                                        Cd + (size_t)r0 * ldc * plan.esize, (size_t)ldc * plan.esize,
                                        (size_t)N * plan.esize, (size_t)rows, cudaMemcpyDeviceToHost, hs.out));
+            r0 += rows;
         }
         CUDA_TRY(cudaStreamSynchronize(hs.out));
         CUDA_TRY(cudaStreamSynchronize(s));
