@@ -392,9 +392,11 @@ def bench_launch_overhead(tg, torch, n_ops=1000, elems=2048):
 
 
 def bench_skinny(tg, wl, torch, ms_list, tdist, layers=8):
-    """skinny M (decode with a few tokens in flight) on the four Qwen3-32B weight shapes,
-    through the tensor-core GEMM with K slices filling the SMs.  HBM-bound: reported as GB/s of
-    algorithmic bytes (weights once + activations + outputs), `layers` distinct weight sets."""
+    """skinny M (decode with a few tokens in flight) on the four Qwen3-32B weight shapes:
+    the weight-streaming tensor-core kernel for M <= 32, the tiled GEMM with K slices above.  Weights are
+    immutable (tile_gemm_static_b, as in the M = 1 leg).  HBM-bound: reported as GB/s of algorithmic bytes
+    (weights once + activations + outputs), `layers` distinct weight sets; `per_shape_gbs` times each of
+    the four shapes in a chain of its own (qkv, attn_out, gate_up, down)."""
     dev = torch.device("cuda", torch.cuda.current_device())
     g = torch.Generator(device=dev)
     g.manual_seed(8)
@@ -408,12 +410,22 @@ def bench_skinny(tg, wl, torch, ms_list, tdist, layers=8):
         def one_pass(_):
             for layer in range(layers):
                 for p in range(4):
-                    tg.tile_gemm(xs[p], Ws[layer][p], ys[p])
+                    tg.tile_gemm(xs[p], Ws[layer][p], ys[p], static_b=True)
 
         one_pass(0)
         ms = tdist.max_over_ranks(time_region(one_pass, 3, torch.cuda.synchronize, tdist.barrier)) / 3
         byt = sum(2 * K * N + 2 * M * K + 2 * M * N for (K, N) in wl.QWEN3_32B) * layers
-        out[str(M)] = {"ms_per_pass": round(ms, 4), "gbs": round(byt / (ms * 1e-3) / 1e9, 1), "launches_per_pass": 4 * layers}
+        per_shape = []
+        for p, (K, N) in enumerate(wl.QWEN3_32B):
+            def chain(_, p=p):
+                for layer in range(layers):
+                    tg.tile_gemm(xs[p], Ws[layer][p], ys[p], static_b=True)
+            chain(0)
+            ms_p = tdist.max_over_ranks(time_region(chain, 5, torch.cuda.synchronize, tdist.barrier)) / 5
+            per_shape.append(round((2 * K * N + 2 * M * K + 2 * M * N) * layers / (ms_p * 1e-3) / 1e9))
+        K0, N0 = wl.QWEN3_32B[0]
+        out[str(M)] = {"ms_per_pass": round(ms, 4), "gbs": round(byt / (ms * 1e-3) / 1e9, 1), "per_shape_gbs": per_shape,
+                       "config": tg.tile_gemm_query_plan(M, N0, K0)["config"] if M >= 2 else 0, "launches_per_pass": 4 * layers}
     return out
 
 

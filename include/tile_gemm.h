@@ -84,10 +84,12 @@ extern "C" {
 
 /* execution paths (what the selector returns / what force_path accepts) */
 #define TILE_GEMM_PATH_AUTO 0         /* force_path only                                      */
-#define TILE_GEMM_PATH_GEMM_TMA 1     /* tcgen05 GEMM, A and B read in place through TMA      */
+#define TILE_GEMM_PATH_GEMM_TMA 1     /* tcgen05 GEMM, A and B read in place through TMA: the tiled
+                                         persistent kernel, or for 2 <= M <= 32 the weight-streaming
+                                         one (csrc/skinny_kernel.cuh); tile_gemm_query_plan says which */
 #define TILE_GEMM_PATH_GEMM_REPACK 2  /* same kernel after copying A and/or B to aligned rows */
-#define TILE_GEMM_PATH_GEMV 3         /* M == 1 (any alignment) or M <= 4 with 16-byte addressable A and B:
-                                         HBM-bound weight-streaming kernels                   */
+#define TILE_GEMM_PATH_GEMV 3         /* M == 1 (any alignment): HBM-bound weight-streaming kernel on
+                                         the CUDA cores                                       */
 #define TILE_GEMM_PATH_ZERO 4         /* K == 0: C <- 0                                       */
 #define TILE_GEMM_PATH_NOOP 5         /* M == 0 or N == 0                                     */
 
@@ -103,8 +105,7 @@ int tile_gemm(const void* A, const void* B, void* C,
 /*
  * Same, with the path forced (tests / measurements): TILE_GEMM_PATH_AUTO,
  * _GEMM_TMA (fails with E_PATH when A or B is not TMA-addressable), _GEMM_REPACK
- * (always legal for K > 0) or _GEMV (requires M == 1, or M <= 4 with A and B
- * 16-byte addressable: base aligned to 16 bytes, lda and ldb multiples of 8).
+ * (always legal for K > 0) or _GEMV (requires M == 1).
  */
 int tile_gemm_ex(const void* A, const void* B, void* C,
                  int64_t M, int64_t N, int64_t K,
@@ -114,8 +115,9 @@ int tile_gemm_ex(const void* A, const void* B, void* C,
 /*
  * tile_gemm plus one promise from the caller: B holds weights -- no work that is
  * still in flight when this call's kernel starts (earlier in `stream` or on any
- * other stream) writes B.  The M == 1 path is launched with programmatic
- * dependent launch in either entry; with this promise it streams weight tiles
+ * other stream) writes B.  The weight-streaming kernels (M == 1, and 2 <= M <= 32
+ * with TMA-addressable operands) are launched with programmatic dependent launch
+ * in either entry; with this promise they stream weight tiles
  * ahead of the wait on the previous kernel of the stream, so back-to-back
  * decode projections (a recorded decode step) keep HBM
  * busy across kernel boundaries.  A, C and every other rule are as in tile_gemm.
@@ -283,12 +285,15 @@ int tile_gemm_debug_owner_map(int32_t* owner, int64_t M, int64_t N, int64_t K,
 int tile_gemm_query_config(int64_t M, int64_t N, int64_t K, int out_dtype, int32_t out[8]);
 
 /*
- * What the selector does with a GEMM shape (M >= 2) beyond the tile configuration:
- * out[0] = config id, out[1] = CTAs launched, out[2] = work units that are whole
- * tiles, out[3] = K slices per tile of the last, partial wave (0 = not cut),
- * out[4] = k-tiles (of 64) per slice, out[5] = rounds the lockstep producers cover
- * (0 = off), out[6] = their window in k-tiles, out[7] = rows of the A box (16, 32,
- * 64 or 128: skinny M loads only the rows it has).  Needs a CUDA device (SM count).
+ * What the selector does with a GEMM shape (M >= 2, operands assumed TMA-addressable)
+ * beyond the tile configuration:
+ * out[0] = config id (1..4: the tiled kernel's configurations; 5: the weight-streaming
+ * tensor-core kernel of 2 <= M <= 32, one CTA per 128 columns and K slice),
+ * out[1] = CTAs launched, out[2] = work units that are whole
+ * tiles, out[3] = K slices per tile of the last, partial wave (config 5: per column
+ * block; 0 = not cut), out[4] = k-tiles (of 64) per slice, out[5] = rounds the lockstep
+ * producers cover (0 = off), out[6] = their window in k-tiles, out[7] = rows of the A box
+ * (16, 32, 64 or 128: skinny M loads only the rows it has).  Needs a CUDA device (SM count).
  */
 int tile_gemm_query_plan(int64_t M, int64_t N, int64_t K, int32_t out[8]);
 
@@ -321,8 +326,8 @@ int tile_gemm_debug_trace(unsigned long long* records, int64_t capacity);
  *          256x256, 4 = CTA pair 256x512.
  *   key 1  GEMM GROUP_M: tile rows per raster group.
  *   key 2  maximum number of CTAs of a GEMM launch; also caps the GEMV grids.
- *   key 3  K slices: of the M = 1 / M <= 4 kernels' column blocks, and (1 = never, >= 2 = that
- *          many) of the GEMM's partial last wave.
+ *   key 3  K slices: of the M = 1 kernel's column blocks, and (1 = never, >= 2 = that
+ *          many) of the tiled GEMM's partial last wave.
  *   key 4  M = 1 kernel: 1 = TMA ring + cluster split-K, 2 = 16-byte LDG, 3 = scalar LDG,
  *          4 = TMA ring + interleaved split-K with ticketed fix-up (the automatic choice when B
  *          is TMA-addressable).
@@ -336,10 +341,14 @@ int tile_gemm_debug_trace(unsigned long long* records, int64_t capacity);
  *          slots with a designated combiner where the launch fits the device, else tickets, 3 =
  *          thread-block cluster + DSMEM where the slice count is <= 8, else tickets; automatic =
  *          cluster, else tagged slots, else tickets.  All three add the partial sums in slice order.
- *   key 9  weight tiles the M = 1 kernel sends as far as L2 right behind the dependency wait
- *          (tile_gemm_static_b only): n >= 1 means n - 1 tiles; automatic = 2.
- *   key 10 automatic cluster size of the M = 1 kernel: per cent of the occupancy calculator's
- *          resident-cluster figure that the column blocks may fill; automatic = 88.
+ *   key 9  weight tiles the weight-streaming kernels send as far as L2 right behind the dependency
+ *          wait (tile_gemm_static_b only): n >= 1 means n - 1 tiles; automatic = 2.
+ *   key 10 automatic cluster size of the weight-streaming kernels: per cent of the occupancy
+ *          calculator's resident-cluster figure that the column blocks may fill; automatic = 88
+ *          (M = 1) and 92 (2 <= M <= 32).
+ *   key 11 weight-streaming tensor-core kernel of 2 <= M <= 32: bits 0-3: 1 = never (the tiled
+ *          kernel takes every GEMM shape), 2 = wherever it can run; bits 8-15 = K slices per
+ *          column block (1..8); bits 16-23 = 32: a 32-row activation box even for M <= 16.
  *   key 7  tile_add_f32 launch shape: bits 0-3 vectors per thread in {1,2,4,8}, bits 4-11 CTAs
  *          per SM (255 = one tile per CTA), bits 12-15 access mode (1 / 2 = 128-bit with / without
  *          streaming hints, 3 / 4 = 256-bit with / without).

@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(CSRC, "libtilegemm.so")
 SOURCES = ["tile_gemm.cu"]
-HEADERS = ["ptx.cuh", "gemm_kernel.cuh", "gemv_kernel.cuh", "gemv_rows_kernel.cuh", "aux_kernels.cuh", "add_kernel.cuh",
+HEADERS = ["ptx.cuh", "gemm_kernel.cuh", "gemv_kernel.cuh", "skinny_kernel.cuh", "aux_kernels.cuh", "add_kernel.cuh",
            os.path.join("..", "..", "include", "tile_gemm.h")]
 
 NVCC_FLAGS = [

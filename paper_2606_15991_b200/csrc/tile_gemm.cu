@@ -22,7 +22,7 @@
 #include "aux_kernels.cuh"
 #include "gemm_kernel.cuh"
 #include "gemv_kernel.cuh"
-#include "gemv_rows_kernel.cuh"
+#include "skinny_kernel.cuh"
 
 namespace {
 
@@ -58,7 +58,7 @@ const char* const kStatusNames[TILE_GEMM_NUM_STATUS] = {
 std::atomic<int64_t> g_launches{0};
 std::atomic<unsigned long long*> g_trace{nullptr};   // tile_gemm_debug_trace
 std::atomic<int64_t> g_trace_cap{0};
-constexpr int kNumTune = 16;
+constexpr int kNumTune = 16;   // keys 0..11 are documented in include/tile_gemm.h
 std::atomic<int> g_tune[kNumTune];
 
 // ------------------------------------------------------------------ preconditions + selector
@@ -86,7 +86,6 @@ bool overlaps(const void* p, int64_t pn, const void* q, int64_t qn) {
 }
 
 constexpr int kAuxCtasPerSm = 16;      // grid cap of the grid-stride helper kernels (repack, zero fill), per SM
-constexpr int64_t kGemvMaxRows = 4;   // M = 2..4 with TMA-addressable A and B take the multi-row GEMV (gemv_rows_kernel.cuh)
 
 int check_and_select(const void* A, const void* B, const void* C, int64_t M, int64_t N, int64_t K, int64_t lda,
                      int64_t ldb, int64_t ldc, int in_dtype, int out_dtype, Plan* plan) {
@@ -135,7 +134,6 @@ int check_and_select(const void* A, const void* B, const void* C, int64_t M, int
     plan->c_tma = (((uintptr_t)C & 15) == 0) && ((ldc * plan->esize) % 16 == 0);
     if (K == 0) plan->path = TILE_GEMM_PATH_ZERO;
     else if (M == 1) plan->path = TILE_GEMM_PATH_GEMV;
-    else if (M <= kGemvMaxRows && plan->a_tma && plan->b_tma) plan->path = TILE_GEMM_PATH_GEMV;   // a few rows: still weight streaming
     else plan->path = (plan->a_tma && plan->b_tma) ? TILE_GEMM_PATH_GEMM_TMA : TILE_GEMM_PATH_GEMM_REPACK;
     return TILE_GEMM_OK;
 }
@@ -663,6 +661,127 @@ int setup_lockstep(GemmLaunch& gl, int dev, cudaStream_t s) {
     return rc;
 }
 
+// ------------------------------------------------------------------ skinny M: weight stream on the tensor cores
+// skinny_tc_kernel (skinny_kernel.cuh): 128 weight columns per CTA, a four-stage ring, two CTAs per SM.
+// Measured on B200 against the 256-column and the deeper-ring variants, and against the
+// tiled GEMM: it wins for M <= 32 on every decode shape; from M = 33 on the 128x128 tiles are level or ahead.
+constexpr int kSkinnyStages = 4;
+constexpr int kSkinnyClusterMarginPct = 92, kSkinnyMinKTilesPerSlice = 4, kSkinnyL2PostTiles = 2;
+using SkinnyL = tg::SkinnySmem<kSkinnyStages>;
+// Two CTAs per SM by shared memory (<= 109 KB each).  The occupancy calculator is no help here: for a
+// kernel that allocates tensor memory it answers one CTA per SM (it cannot know how many columns), while
+// the hardware co-schedules two (32 of 512 columns each; ncu: launch__occupancy_limit_shared_mem = 2).  How
+// many CLUSTERS fit is a property of the GPC layout at two CTAs per SM, which the M = 1 kernel -- same
+// occupancy, no tensor memory -- gets from the calculator: gemv_cluster_capacity.
+constexpr int kSkinnyCtasPerSm = 2;
+static_assert(2 * (SkinnyL::total(tg::SKINNY_MAX_ROWS, tg::SKINNY_MAX_CLUSTER, tg::SKINNY_MAX_ROWS) + 1024) <= 228 * 1024,
+              "two skinny CTAs (and their 1 KB reserve each) must fit one SM's shared memory");
+int gemv_cluster_capacity(int cs, int dev, int sms);
+
+struct SkinnyPlan {
+    bool ok = false;   // false: the tiled GEMM takes the shape
+    int split = 1, col_blocks = 0, a_rows = 16;
+};
+
+// K slices of a skinny launch (tuning key 11 bits 8-15 force them).  Column blocks that fill the CTA slots
+// (two per SM) run unsliced: the hardware scheduler and the next launch of the stream fill the slots as
+// CTAs retire.  Fewer column blocks are cut into the largest number of slices (= cluster size) whose
+// clusters all fit the device at once with slots to spare -- clusters of the next launch can only start
+// where a whole cluster's worth of slots is free (the M = 1 kernel's rule).
+SkinnyPlan plan_skinny(int64_t M, int64_t N, int64_t K, int dev, int sms) {
+    SkinnyPlan sp;
+    sp.a_rows = M <= 16 ? 16 : 32;
+    const int tune = g_tune[11].load();
+    const int want_split = (tune >> 8) & 255, want_rows = (tune >> 16) & 255;
+    if (want_rows == 32) sp.a_rows = 32;
+    const int64_t k_tiles = (K + tg::SKINNY_BK - 1) / tg::SKINNY_BK;
+    const int64_t cb = (N + tg::SKINNY_COLS - 1) / tg::SKINNY_COLS;
+    const int64_t slots1 = (int64_t)sms * kSkinnyCtasPerSm;
+    if (cb > 0x7fffffff) return sp;
+    sp.col_blocks = (int)cb;
+    sp.split = 1;
+    int margin = g_tune[10].load();
+    if (margin <= 0) margin = kSkinnyClusterMarginPct;
+    // 17..32 rows on weights wide enough to fill the CTA slots unsliced: the 128x128 tiles of the GEMM kernel re-read
+    // the activations less often and are ahead (measured on K = 5120, N = 51200: 6.45 vs 6.23 TB/s)
+    if (sp.a_rows == 32 && want_split == 0 && (tune & 15) != 2 && cb * 100 > slots1 * margin) return sp;
+    sp.ok = true;
+    if (want_split > 0) {
+        sp.split = (int)(want_split < k_tiles ? want_split : k_tiles);
+        if (sp.split > tg::SKINNY_MAX_CLUSTER) sp.split = tg::SKINNY_MAX_CLUSTER;
+        return sp;
+    }
+    for (int64_t cs = tg::SKINNY_MAX_CLUSTER; cs >= 2; --cs) {
+        if (cs > k_tiles || k_tiles / cs < kSkinnyMinKTilesPerSlice) continue;
+        if (cb * cs * 100 > slots1 * margin) continue;
+        if (cb * 100 > (int64_t)gemv_cluster_capacity((int)cs, dev, sms) * margin) continue;
+        sp.split = (int)cs;
+        break;
+    }
+    return sp;
+}
+
+int run_skinny(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_t K, int64_t lda, int64_t ldb,
+               int64_t ldc, int in_dtype, int out_dtype, cudaStream_t s, int dev, const SkinnyPlan& sp, unsigned flags) {
+    tg::SkinnyParams p;
+    memset(&p, 0, sizeof p);
+    p.C = C;
+    p.ldc = ldc;
+    p.M = (int32_t)M; p.N = (int32_t)N; p.K = (int32_t)K;
+    p.k_tiles = (int32_t)((K + tg::SKINNY_BK - 1) / tg::SKINNY_BK);
+    p.a_rows = sp.a_rows;
+    p.out_kind = out_dtype;
+    p.in_f16 = in_dtype == TILE_GEMM_IN_F16;
+    p.flags = (flags & TILE_GEMM_FLAG_B_IMMUTABLE) ? tg::GEMV_FLAG_B_IMMUTABLE : 0;
+    const int post = g_tune[9].load();                       // tuning key 9: n >= 1 -> n - 1 tiles
+    p.l2_post = post > 0 ? post - 1 : kSkinnyL2PostTiles;
+    CUtensorMap tw, tx;
+    int rc = get_tensor_map(&tw, B, 2, false, (uint64_t)N, (uint64_t)K, (uint64_t)ldb * 2, 64u, 64u, 128);
+    if (rc) return rc;
+    rc = get_tensor_map(&tx, A, 2, false, (uint64_t)K, (uint64_t)M, (uint64_t)lda * 2, 64u, (uint32_t)sp.a_rows, 128);
+    if (rc) return rc;
+    auto kern = tg::skinny_tc_kernel<kSkinnyStages>;
+    const int smem = (int)SkinnyL::total(sp.a_rows, sp.split, (int)((M + 3) & ~int64_t(3)));
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof cfg);
+    cfg.gridDim = dim3((unsigned)sp.col_blocks, (unsigned)sp.split, 1);
+    cfg.blockDim = dim3(tg::SKINNY_THREADS, 1, 1);
+    cfg.dynamicSmemBytes = (size_t)smem;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[2];
+    int na = 0;
+    if ((g_tune[6].load() & 1) == 0) {
+        attr[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[na].val.programmaticStreamSerializationAllowed = 1;
+        ++na;
+    }
+    if (sp.split > 1) {   // the slices of a column block form one cluster along y
+        attr[na].id = cudaLaunchAttributeClusterDimension;
+        attr[na].val.clusterDim.x = 1;
+        attr[na].val.clusterDim.y = (unsigned)sp.split;
+        attr[na].val.clusterDim.z = 1;
+        ++na;
+    }
+    cfg.attrs = attr;
+    cfg.numAttrs = na;
+    static bool configured[64] = {};
+    if (!configured[dev]) {
+        CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)SkinnyL::total(tg::SKINNY_MAX_ROWS, tg::SKINNY_MAX_CLUSTER, tg::SKINNY_MAX_ROWS)));
+        configured[dev] = true;
+    }
+    CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, tw, tx, p));
+    g_launches.fetch_add(1);
+    return TILE_GEMM_OK;
+}
+
+// does the weight-streaming tensor-core kernel take this GEMM shape?  (tuning key 11 bits 0-3: 1 = never, 2 = wherever it can run)
+bool skinny_applies(int64_t M, int64_t K, const Plan& plan, bool force_repack) {
+    if ((g_tune[11].load() & 15) == 1 || force_repack || !plan.a_tma || !plan.b_tma || K <= 0 || M > tg::SKINNY_MAX_ROWS) return false;
+    const int forced_cfg = g_tune[0].load();
+    return !(forced_cfg >= 1 && forced_cfg <= 4);   // a forced tile configuration means the tiled kernel
+}
+
 int c_tensor_map(CUtensorMap* tc, void* C, int64_t M, int64_t N, int64_t ldc, int out_16) {
     // one epilogue sub-chunk: 32 rows x 64 bytes, 64B-swizzled in shared memory (a 16-bit C is
     // described as bf16 whichever 16-bit format it holds: tiled TMA moves bits, it never converts)
@@ -672,8 +791,12 @@ int c_tensor_map(CUtensorMap* tc, void* C, int64_t M, int64_t N, int64_t ldc, in
 
 int run_gemm(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_t K, int64_t lda, int64_t ldb,
              int64_t ldc, int in_dtype, int out_dtype, cudaStream_t s, const Plan& plan, bool force_repack, int dev,
-             int sms) {
+             int sms, unsigned flags = 0u) {
     const int out_16 = out_dtype != TILE_GEMM_OUT_F32;
+    if (skinny_applies(M, K, plan, force_repack)) {
+        const SkinnyPlan sp = plan_skinny(M, N, K, dev, sms);
+        if (sp.ok) return run_skinny(A, B, C, M, N, K, lda, ldb, ldc, in_dtype, out_dtype, s, dev, sp, flags);
+    }
     const bool rep_a = force_repack || !plan.a_tma;
     const bool rep_b = force_repack || !plan.b_tma;
     const uint16_t* Ap = (const uint16_t*)A;
@@ -926,87 +1049,6 @@ int run_gemv_split(const void* x, const void* B, void* y, int64_t N, int64_t K, 
     return fail(TILE_GEMM_E_INTERNAL, "unknown GEMV ring shape %d", shape);
 }
 
-// M = 2..4: the multi-row GEMV (gemv_rows_kernel.cuh); same (column block, slice) grid as the M = 1 kernel
-template <int MR, bool F16>
-int launch_gemv_rows(const CUtensorMap& tb, const CUtensorMap& tx, const tg::GemvRowsParams& p, int gx, int split, bool pdl,
-                     cudaStream_t s, int dev) {
-    using L = tg::GemvRowsSmem<MR, 3>;
-    auto kern = tg::gemv_rows_kernel<MR, F16>;
-    static bool configured[64] = {};
-    if (!configured[dev]) {
-        CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::TOTAL));
-        configured[dev] = true;
-    }
-    cudaLaunchConfig_t cfg;
-    memset(&cfg, 0, sizeof cfg);
-    cfg.gridDim = dim3((unsigned)gx, (unsigned)split, 1);
-    cfg.blockDim = dim3(tg::GEMV_TMA_THREADS, 1, 1);
-    cfg.dynamicSmemBytes = L::TOTAL;
-    cfg.stream = s;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = pdl ? 1 : 0;
-    CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, tb, tx, p));
-    g_launches.fetch_add(1);
-    return TILE_GEMM_OK;
-}
-
-int run_gemv_rows(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_t K, int64_t lda, int64_t ldb,
-                  int64_t ldc, int in_dtype, int out_dtype, cudaStream_t s, int dev, int sms, unsigned flags) {
-    const int64_t col_blocks = (N + tg::GEMV_COLS - 1) / tg::GEMV_COLS;
-    const int64_t k_tiles = (K + tg::GEMV_TILE_K - 1) / tg::GEMV_TILE_K;
-    int64_t budget = (int64_t)sms * 2;   // all CTAs co-resident, two per SM
-    const int cap = g_tune[2].load();
-    if (cap > 0 && cap < budget) budget = cap;
-    const int64_t gx = col_blocks < budget ? col_blocks : budget;
-    int64_t split = g_tune[3].load();
-    if (split <= 0) {
-        split = budget / gx;
-        if (split == 1 && col_blocks <= budget && col_blocks * 2 > budget) {   // see run_gemv_split
-            double best = (double)col_blocks / (double)budget;
-            for (int64_t c = 2; c <= 8 && k_tiles / c >= 16; ++c) {
-                const double waves = (double)(col_blocks * c) / (double)budget;
-                const double eff = waves / (double)(int64_t)(waves + 0.999999);
-                if (eff > best + 0.05) { best = eff; split = c; }
-            }
-        }
-    }
-    if (split > k_tiles) split = k_tiles;
-    if (split > 65535) split = 65535;
-    if (split < 1) split = 1;
-    tg::GemvRowsParams p;
-    memset(&p, 0, sizeof p);
-    p.y = C;
-    p.ldy = ldc;
-    p.N = (int32_t)N; p.K = (int32_t)K; p.k_tiles = (int32_t)k_tiles; p.col_blocks = (int32_t)col_blocks;
-    p.out_kind = out_dtype;
-    p.flags = (flags & TILE_GEMM_FLAG_B_IMMUTABLE) ? tg::GEMV_FLAG_B_IMMUTABLE : 0;
-    if (split > 1) {
-        int rc = gemv_workspace_for(dev, s, (size_t)col_blocks * split * M * tg::GEMV_COLS * 4, (size_t)col_blocks * 4,
-                                    &p.partials, &p.tickets);
-        if (rc) return rc;
-    }
-    CUtensorMap tb, tx;
-    int rc = get_tensor_map(&tb, B, 2, false, (uint64_t)N, (uint64_t)K, (uint64_t)ldb * 2, (uint32_t)tg::GEMV_COLS,
-                            (uint32_t)tg::GEMV_TILE_K, 0);
-    if (rc) return rc;
-    rc = get_tensor_map(&tx, A, 2, false, (uint64_t)K, (uint64_t)M, (uint64_t)lda * 2, (uint32_t)tg::GEMV_TILE_K, (uint32_t)M, 0);
-    if (rc) return rc;
-    const bool pdl = (g_tune[6].load() & 1) == 0;
-    const bool f16 = in_dtype == TILE_GEMM_IN_F16;
-    switch (M) {
-        case 2: return f16 ? launch_gemv_rows<2, true>(tb, tx, p, (int)gx, (int)split, pdl, s, dev)
-                           : launch_gemv_rows<2, false>(tb, tx, p, (int)gx, (int)split, pdl, s, dev);
-        case 3: return f16 ? launch_gemv_rows<3, true>(tb, tx, p, (int)gx, (int)split, pdl, s, dev)
-                           : launch_gemv_rows<3, false>(tb, tx, p, (int)gx, (int)split, pdl, s, dev);
-        case 4: return f16 ? launch_gemv_rows<4, true>(tb, tx, p, (int)gx, (int)split, pdl, s, dev)
-                           : launch_gemv_rows<4, false>(tb, tx, p, (int)gx, (int)split, pdl, s, dev);
-    }
-    return fail(TILE_GEMM_E_INTERNAL, "the multi-row GEMV handles M = 2..4 (M=%lld)", (long long)M);
-}
-
 int run_gemv(const void* x, const void* B, void* y, int64_t N, int64_t K, int64_t ldb, int in_dtype, int out_dtype,
              cudaStream_t s, const Plan& plan, int dev, int sms, unsigned flags) {
     const bool f16 = in_dtype == TILE_GEMM_IN_F16;
@@ -1108,9 +1150,8 @@ int gemm_entry(const void* A, const void* B, void* C, int64_t M, int64_t N, int6
     if (plan.path == TILE_GEMM_PATH_NOOP) return TILE_GEMM_OK;
     int path = plan.path;
     if (force_path != TILE_GEMM_PATH_AUTO && path != TILE_GEMM_PATH_ZERO) {
-        if (force_path == TILE_GEMM_PATH_GEMV && !(M == 1 || (M <= kGemvMaxRows && plan.a_tma && plan.b_tma)))
-            return fail(TILE_GEMM_E_PATH, "the GEMV path needs M == 1, or M <= 4 with 16-byte addressable A and B (M=%lld)",
-                        (long long)M);
+        if (force_path == TILE_GEMM_PATH_GEMV && M != 1)
+            return fail(TILE_GEMM_E_PATH, "the GEMV path needs M == 1 (M=%lld)", (long long)M);
         if (force_path == TILE_GEMM_PATH_GEMM_TMA && !(plan.a_tma && plan.b_tma))
             return fail(TILE_GEMM_E_PATH, "GEMM_TMA needs 16-byte aligned A/B with lda, ldb multiples of 8");
         path = force_path;
@@ -1122,13 +1163,12 @@ int gemm_entry(const void* A, const void* B, void* C, int64_t M, int64_t N, int6
     switch (path) {
         case TILE_GEMM_PATH_ZERO: return run_zero(C, M, N, ldc, plan.esize, s, sms);
         case TILE_GEMM_PATH_GEMV:
-            if (M > 1) return run_gemv_rows(A, B, C, M, N, K, lda, ldb, ldc, in_dtype, out_dtype, s, dev, sms, flags);
             return run_gemv(A, B, C, N, K, ldb, in_dtype, out_dtype, s, plan, dev, sms, flags);
         case TILE_GEMM_PATH_GEMM_TMA:
-            return run_gemm(A, B, C, M, N, K, lda, ldb, ldc, in_dtype, out_dtype, s, plan, false, dev, sms);
+            return run_gemm(A, B, C, M, N, K, lda, ldb, ldc, in_dtype, out_dtype, s, plan, false, dev, sms, flags);
         case TILE_GEMM_PATH_GEMM_REPACK:   // forced: repack both operands; auto: only what TMA cannot address
             return run_gemm(A, B, C, M, N, K, lda, ldb, ldc, in_dtype, out_dtype, s, plan,
-                            force_path == TILE_GEMM_PATH_GEMM_REPACK, dev, sms);
+                            force_path == TILE_GEMM_PATH_GEMM_REPACK, dev, sms, flags);
     }
     return fail(TILE_GEMM_E_INTERNAL, "unhandled path %d", path);
 }
@@ -1514,6 +1554,25 @@ int tile_gemm_query_plan(int64_t M, int64_t N, int64_t K, int32_t out[8]) {
     int dev = 0, sms = 0;
     int rc = current_device(&dev, &sms);
     if (rc) return rc;
+    {   // skinny M with TMA-addressable operands (assumed here: the query sees no pointers): the weight-streaming kernel
+        Plan aligned;
+        aligned.a_tma = aligned.b_tma = true;
+        if (skinny_applies(M, K, aligned, false)) {
+            const SkinnyPlan sp = plan_skinny(M, N, K, dev, sms);
+            if (sp.ok) {
+                const int64_t k_tiles = (K + tg::SKINNY_BK - 1) / tg::SKINNY_BK;
+                out[0] = 5;
+                out[1] = sp.col_blocks * sp.split;
+                out[2] = 0;
+                out[3] = sp.split > 1 ? sp.split : 0;
+                out[4] = (int32_t)((k_tiles + sp.split - 1) / sp.split);
+                out[5] = 0;
+                out[6] = 0;
+                out[7] = sp.a_rows;
+                return TILE_GEMM_OK;
+            }
+        }
+    }
     GemmLaunch gl;
     plan_gemm(M, N, K, TILE_GEMM_IN_BF16, TILE_GEMM_OUT_BF16, dev, sms, &gl, true);
     int64_t rounds = 0;

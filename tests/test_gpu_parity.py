@@ -77,13 +77,13 @@ class CanaryC:
         return oracle.bf16_decode(np.ascontiguousarray(inside))
 
 
-def run_case(a_bits, b_bits, out="f32", pads=(0, 0, 0), force=tg.PATH_AUTO, misalign=(0, 0, 0), what=""):
+def run_case(a_bits, b_bits, out="f32", pads=(0, 0, 0), force=tg.PATH_AUTO, misalign=(0, 0, 0), what="", static_b=False):
     M, K = a_bits.shape
     N = b_bits.shape[1]
     A = device_operand(a_bits, pads[0], misalign[0])
     B = device_operand(b_bits, pads[1], misalign[1])
     cc = CanaryC(M, N, out, pads[2], misalign_elems=misalign[2])
-    tg.tile_gemm(A, B, cc.C, force_path=force)
+    tg.tile_gemm(A, B, cc.C, force_path=force, static_b=static_b)
     torch.cuda.synchronize()
     return cc.check(what)
 
@@ -673,54 +673,89 @@ def test_selector_plans_for_the_benchmarked_shapes():
     assert p["lockstep_rounds"] >= 100 and p["lockstep_window"] == 32
     p = plan(1024, 1024, 1024)            # below one wave but a short K loop: not cut
     assert p["split"] == 0 and p["a_box_rows"] == 128
-    for M in (2, 8, 16):                  # skinny M: below one wave, long K -> cut; A box only as tall as M needs
+    for M in (2, 8, 16):                  # skinny M: the weight-streaming kernel, K-sliced over clusters; A box only as tall as M needs
         p = plan(M, 5120, 25600)
-        assert p["full_units"] == 0 and p["split"] >= 2 and p["a_box_rows"] == 16 and p["ctas"] >= 100
-    assert plan(40, 10240, 5120)["a_box_rows"] == 64
-    for M in (8, 64, 128):                # one row of 128-tall tiles: never a CTA pair, 128x128 tiles on every SM
+        assert p["config"] == 5 and p["full_units"] == 0 and p["split"] >= 4 and p["a_box_rows"] == 16 and 148 <= p["ctas"] <= 296
+    p = plan(24, 10240, 5120)
+    assert p["config"] == 5 and p["a_box_rows"] == 32 and p["split"] >= 2
+    for M in (8, 16):                     # column blocks that fill the CTA slots run unsliced
+        p = plan(M, 51200, 5120)
+        assert p["config"] == 5 and p["split"] == 0 and p["ctas"] == 400
+    assert plan(32, 51200, 5120)["config"] == 1       # 17..32 rows on wide weights: the 128x128 tiles are ahead (measured)
+    for M in (40, 64):                    # from M = 33 on: the tiled kernel, K-sliced below one wave, A box as tall as M needs
+        p = plan(M, 5120, 25600)
+        assert p["config"] == 1 and p["full_units"] == 0 and p["split"] >= 2 and p["a_box_rows"] == 64 and p["ctas"] >= 100
+    for M in (64, 128):                   # one row of 128-tall tiles: never a CTA pair, 128x128 tiles on every SM
         p = plan(M, 51200, 5120)
         assert p["config"] == 1 and p["ctas"] == 148
     assert plan(129, 51200, 5120)["config"] in (3, 4)
 
 
-# ------------------------------------------------------------------ M = 2..4: the multi-row GEMV
-@pytest.mark.parametrize("M", [2, 3, 4])
-@pytest.mark.parametrize("split", [0, 1, 3, 8])
-def test_gemv_rows_integer_bit_exact_and_canary(M, split):
-    tg.tile_gemm_set_tuning(tg.TUNE_GEMV_SPLIT, split)
-    for (K, N), pads in (((776, 1537), (0, 7, 3)), ((5120, 10240), (0, 0, 0)), ((64, 8), (8, 8, 0)), ((4104, 520), (8, 0, 8))):
+# ------------------------------------------------------------------ 2 <= M <= 32: the weight-streaming tensor-core kernel
+SKINNY_SHAPES = (((776, 1537), (0, 7, 3)), ((5120, 10240), (0, 0, 0)), ((64, 8), (8, 8, 0)), ((4104, 520), (8, 0, 8)),
+                 ((1030, 130), (0, 6, 1)))
+
+
+def _skinny_tune(mode=0, split=0, rows=0):
+    tg.tile_gemm_set_tuning(tg.TUNE_SKINNY, mode | (split << 8) | (rows << 16))
+
+
+@pytest.mark.parametrize("M", [2, 3, 4, 5, 8, 13, 16, 17, 31, 32])
+@pytest.mark.parametrize("split", [0, 1, 2, 3, 5, 7, 8])
+def test_skinny_integer_bit_exact_and_canary(M, split):
+    """Every cluster size of the split-K reduce-scatter (1 = no cluster; 3, 5, 7: groups unevenly owned; 5..8: slices
+    that own nothing) on ragged N, K and padded strides: integer inputs are exact whatever the slicing, nothing
+    outside C is written, every element is written."""
+    _skinny_tune(2, split)
+    for (K, N), pads in SKINNY_SHAPES:
         a, b = wl.make_inputs_custom(M, N, K, dist="int4", seed=71 + M)
         ref, _ = oracle.gemm(a, b)
-        pads_ok = (pads[0], pads[1] + (-(N + pads[1])) % 8, pads[2])          # ldb stays a multiple of 8: the GEMV path is taken
-        A = device_operand(a, pads_ok[0])
-        B = device_operand(b, pads_ok[1])
-        assert tg.tile_gemm_select(M, N, K, A.stride(0), B.stride(0), N + pads_ok[2], A.data_ptr(), B.data_ptr(), 1 << 41) \
-            == tg.PATH_GEMV
-        got = run_case(a, b, "f32", pads=pads_ok, what=f"gemv rows M={M}")
-        check_bit_exact(got.astype(np.float32), ref, f"gemv rows M={M} K={K} N={N} split={split}")
+        pads_ok = (pads[0], pads[1] + (-(N + pads[1])) % 8, pads[2])          # ldb stays a multiple of 8: operands TMA-addressable
+        assert tg.tile_gemm_query_plan(M, N, K)["config"] == 5
+        got = run_case(a, b, "f32", pads=pads_ok, what=f"skinny M={M}")
+        check_bit_exact(got.astype(np.float32), ref, f"skinny M={M} K={K} N={N} split={split}")
 
 
-@pytest.mark.parametrize("M", [2, 4])
+@pytest.mark.parametrize("M", [2, 8, 24, 32])
 @pytest.mark.parametrize("out", ["f32", "bf16"])
-def test_gemv_rows_normal_inputs_and_agreement_with_the_gemm_path(M, out):
+def test_skinny_normal_inputs_reproducible_and_agrees_with_the_tiled_gemm(M, out):
     K, N = 5120, 8192
     a, b = wl.make_inputs_custom(M, N, K, sigma_b=0.02, seed=73)
     ref, S = oracle.gemm(a, b)
-    got = run_case(a, b, out, what="gemv rows")
-    check_close(got, ref, S, K, out, f"gemv rows M={M} {out}")
-    again = run_case(a, b, out, what="gemv rows")
-    assert np.array_equal(got, again), "multi-row GEMV is not reproducible"
-    via_gemm = run_case(a, b, out, force=tg.PATH_GEMM_TMA, what="gemm path")
-    check_close(via_gemm, ref, S, K, out, f"gemm path M={M} {out}")
+    assert tg.tile_gemm_query_plan(M, N, K)["config"] == 5 and tg.tile_gemm_query_plan(M, N, K)["split"] >= 2
+    got = run_case(a, b, out, what="skinny")
+    check_close(got, ref, S, K, out, f"skinny M={M} {out}")
+    again = run_case(a, b, out, what="skinny")
+    assert np.array_equal(got, again), "the skinny-M kernel is not reproducible"
+    static = run_case(a, b, out, what="skinny static_b", static_b=True)
+    assert np.array_equal(got, static), "weights prefetched ahead of the dependency wait change the result"
+    _skinny_tune(1)                                                         # the tiled kernel on the same problem
+    assert tg.tile_gemm_query_plan(M, N, K)["config"] == 1
+    tiled = run_case(a, b, out, what="tiled")
+    check_close(tiled, ref, S, K, out, f"tiled M={M} {out}")
 
 
-def test_gemv_rows_f16_and_unaligned_falls_back_to_the_gemm():
+def test_skinny_32_row_box_for_few_rows_gives_the_same_bits():
+    """The rows past M are TMA zero fill: a 32-row activation box (N = 32 of the MMA) on M = 8 changes nothing."""
+    a, b = wl.make_inputs_custom(8, 1537 + 7, 2048, sigma_b=0.02, seed=76)
+    got16 = run_case(a, b, "f32", what="skinny 16-row box")
+    _skinny_tune(0, 0, 32)
+    assert tg.tile_gemm_query_plan(8, 1544, 2048)["a_box_rows"] == 32
+    got32 = run_case(a, b, "f32", what="skinny 32-row box")
+    assert np.array_equal(got16, got32)
+
+
+def test_skinny_f16_and_unaligned_falls_back_to_the_tiled_gemm():
     a, b = wl.make_inputs_f16(3, 2048, 1024, sigma_b=0.05, seed=74)
     ref, S = oracle.gemm(a, b, in_dtype=oracle.IN_F16)
     A, B = wl.bits_to_torch(a, DEV, torch.float16), wl.bits_to_torch(b, DEV, torch.float16)
     C = tg.tile_gemm(A, B, out_dtype=tg.OUT_F16)
-    check_close(oracle.f16_decode(C.cpu().view(torch.int16).numpy().view(np.uint16)), ref, S, 1024, "f16", "gemv rows f16")
-    # lda not a multiple of 8: A is not TMA-addressable, the selector goes to the (repacking) GEMM
+    check_close(oracle.f16_decode(C.cpu().view(torch.int16).numpy().view(np.uint16)), ref, S, 1024, "f16", "skinny f16")
+    ai, bi = wl.make_inputs_f16(20, 1000, 520, dist="int4", seed=77)           # f16 integers through the f16 decode: exact
+    refi, _ = oracle.gemm(ai, bi, in_dtype=oracle.IN_F16)
+    Ci = tg.tile_gemm(wl.bits_to_torch(ai, DEV, torch.float16), wl.bits_to_torch(bi, DEV, torch.float16), out_dtype=tg.OUT_F32)
+    check_bit_exact(Ci.cpu().numpy(), refi, "skinny f16 ints")
+    # lda not a multiple of 8: A is not TMA-addressable, the selector goes to the (repacking) tiled GEMM
     assert tg.tile_gemm_select(3, 2048, 1023, 1023, 2048, 2048) == tg.PATH_GEMM_REPACK
     ai, bi = wl.make_inputs_custom(3, 2048, 1023, dist="int4", seed=75)
     refi, _ = oracle.gemm(ai, bi)

@@ -39,15 +39,15 @@ def _int_case(M, N, K, seed):
 
 
 def test_recorded_step_owns_its_workspaces():
-    """Record (with NO warm-up on the stream) a K-sliced GEMM, a split-K GEMV, a multi-row GEMV and a
-    GEMM whose B has an odd row stride (repack workspace); then run 4x larger split shapes directly on
+    """Record (with NO warm-up on the stream) a K-sliced GEMM, a split-K GEMV, a skinny-M weight-streaming
+    GEMM (cluster hand-over: no workspace at all) and a GEMM whose B has an odd row stride (repack workspace); then run 4x larger split shapes directly on
     the recording stream, which regrows that stream's workspaces; then replay -- on the recording
     stream, and on a second stream while direct split-K calls keep the first one busy."""
     tg.tile_gemm_set_tuning(tg.TUNE_GEMV_SPLIT, 5)        # K slices for the GEMV column blocks and the GEMM's last wave
     s, s2 = torch.cuda.Stream(), torch.cuda.Stream()
     A1, B1, ref1 = _int_case(130, 384, 2048, 301)         # GEMM, partial last wave cut into 5 slices
     x2, B2, ref2 = _int_case(1, 1536, 2560, 302)          # M = 1, 5 slices per column block
-    A3, B3, ref3 = _int_case(3, 1024, 1280, 303)          # M = 3, multi-row GEMV, 5 slices
+    A3, B3, ref3 = _int_case(3, 1024, 1280, 303)          # M = 3: the weight-streaming tensor-core kernel
     a4, b4 = wl.make_inputs_custom(140, 200, 264, "int4", seed=304)
     ref4, _ = oracle.gemm(a4, b4)
     A4 = wl.bits_to_torch(a4, DEV)

@@ -222,13 +222,16 @@ def test_swiglu_preconditions_on_the_host():
         assert tg.tile_gemm_swiglu_raw(*a, 8, 16, 64, 64, 32, 16, tg.OUT_F32) == tg.E_DEVICE
 
 
-def test_selector_routes_a_few_rows_to_the_weight_streaming_path():
-    # M = 2..4 with 16-byte addressable A and B: GEMV family; otherwise, and from M = 5 on: tensor cores
-    for M in (2, 3, 4):
-        assert sel(M, 10240, 5120) == tg.PATH_GEMV
+def test_selector_routes_a_few_rows_to_the_tensor_cores():
+    # only M = 1 is the CUDA-core GEMV; from M = 2 on the tensor-core path (in place through TMA where A and B
+    # are 16-byte addressable -- the weight-streaming kernel up to M = 32 -- else after a repack)
+    assert sel(1, 10240, 5120) == tg.PATH_GEMV
+    for M in (2, 3, 4, 5, 32, 33):
+        assert sel(M, 10240, 5120) == tg.PATH_GEMM_TMA
         assert sel(M, 10240, 5120, lda=5121) == tg.PATH_GEMM_REPACK
         assert sel(M, 10240, 5120, A=A0 + 2) == tg.PATH_GEMM_REPACK
-    assert sel(5, 10240, 5120) == tg.PATH_GEMM_TMA
+    st = tg.tile_gemm_raw(A0, B0, C0, 2, 64, 64, 64, 64, 64, tg.OUT_F32, force_path=tg.PATH_GEMV)
+    assert st == tg.E_PATH and "M == 1" in tg.tile_gemm_last_error()
 
 
 @pytest.mark.parametrize("G", [2, 8])
