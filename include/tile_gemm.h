@@ -279,7 +279,9 @@ int tile_gemm_debug_owner_map(int32_t* owner, int64_t M, int64_t N, int64_t K,
  * host program can rebuild the owner map: out[0]=BM (rows per CTA),
  * out[1]=BN (columns per tile), out[2]=cta_group (1 or 2: CTAs per tile, tile
  * rows = BM*cta_group), out[3]=number of CTAs launched, out[4]=GROUP_M (tile
- * rows per raster group), out[5]=pipeline stages, out[6]=BK, out[7]=config id.
+ * rows per raster group), out[5]=pipeline stages, out[6]=BK, out[7]=config id
+ * (1..4; 6 = config 4 with two CTA pairs per cluster, tuning key 12: a work unit is then
+ * two tile rows of one tile column, out[4] counts unit rows, and CTAs 4c..4c+3 own a unit).
  * Needs a CUDA device (SM count).  Returns a status code.
  */
 int tile_gemm_query_config(int64_t M, int64_t N, int64_t K, int out_dtype, int32_t out[8]);
@@ -349,6 +351,10 @@ int tile_gemm_debug_trace(unsigned long long* records, int64_t capacity);
  *   key 11 weight-streaming tensor-core kernel of 2 <= M <= 32: bits 0-3: 1 = never (the tiled
  *          kernel takes every GEMM shape), 2 = wherever it can run; bits 8-15 = K slices per
  *          column block (1..8); bits 16-23 = 32: a 32-row activation box even for M <= 16.
+ *   key 12 config 4 with clusters of two CTA pairs that share each B stage through TMA multicast
+ *          (csrc/gemm_kernel.cuh, MC = 1): 1 = never, 2 = whenever the shape has two tile rows and
+ *          runs on config 4; automatic = never (measured slower on this part: clusters of four
+ *          leave 16 of 148 SMs idle).  tile_gemm_query_config reports it as config 6.
  *   key 7  tile_add_f32 launch shape: bits 0-3 vectors per thread in {1,2,4,8}, bits 4-11 CTAs
  *          per SM (255 = one tile per CTA), bits 12-15 access mode (1 / 2 = 128-bit with / without
  *          streaming hints, 3 / 4 = 256-bit with / without).

@@ -29,7 +29,7 @@ PATH_NAMES = {PATH_AUTO: "auto", PATH_GEMM_TMA: "gemm_tma", PATH_GEMM_REPACK: "g
  E_CUDA, E_PATH, E_INTERNAL, E_IN_DTYPE) = range(15)
 
 (TUNE_GEMM_CONFIG, TUNE_GEMM_GROUP_M, TUNE_GEMM_MAX_CTAS, TUNE_GEMV_SPLIT, TUNE_GEMV_VARIANT, TUNE_GEMV_SHAPE, TUNE_FLAGS,
- TUNE_ADD_SHAPE, TUNE_GEMV_FIXUP, TUNE_GEMV_L2_POST, TUNE_GEMV_CLUSTER_MARGIN, TUNE_SKINNY) = range(12)
+ TUNE_ADD_SHAPE, TUNE_GEMV_FIXUP, TUNE_GEMV_L2_POST, TUNE_GEMV_CLUSTER_MARGIN, TUNE_SKINNY, TUNE_GEMM_MULTICAST) = range(13)
 NUM_TUNE_KEYS = 16
 
 EXPORTS = ("tile_gemm", "tile_gemm_ex", "tile_gemm_static_b", "tile_gemm_typed", "tile_gemm_swiglu", "tile_add_f32", "tile_read_probe_u32",

@@ -22,6 +22,11 @@
 //   cuts the L2 -> shared-memory fill traffic per FLOP by a quarter (the kernel is power bound on
 //   B200); each slot keeps its own full/empty barriers, so the next tile's
 //   main loop restarts on slot 0 while the epilogue still drains slot 1.
+//   MC = 1 (CTA pairs only): a cluster is TWO pairs, one tile row above the other, working on the same
+//   tile column in step.  They need the same B panel, so each CTA fetches only every other 64-column
+//   box of its B half and TMA multicasts it into its own shared memory and that of the CTA of the same
+//   rank in the other pair: a third less L2 -> SM traffic per FLOP (the kernel is power bound).  A stage
+//   is refilled only when BOTH pairs' MMAs have released it (every commit arrives at all four CTAs).
 #pragma once
 #include "ptx.cuh"
 
@@ -33,6 +38,7 @@ constexpr int GEMM_UMMA_K = 16;   // K per tcgen05.mma for 16-bit inputs
 constexpr int GEMM_THREADS = 384;     // 4 control warps + 8 epilogue warps
 constexpr int GEMM_EPI_WARP0 = 4;
 constexpr uint32_t GEMM_EPI_BUF_BYTES = 2 * 32 * 64;   // per epilogue warp: two buffers of 32 rows x 64 B
+constexpr uint32_t GEMM_PEER_BIT_MASK = 0xFEFFFFFFu;   // a shared-memory address with the bit that tells the two CTAs of a pair apart cleared
 constexpr uint64_t GEMM_LOCKSTEP_PATIENCE_NS = 500000;  // a lockstep producer waits this long for the others (a window is ~30 us), then runs free
 
 struct GemmParams {
@@ -142,7 +148,7 @@ struct GemmSmem {
 // [gate | up]; accumulator slot 0 takes the tile's gate columns, slot 1 the same columns of `up`
 // (p.up_offset further right in B); the epilogue stores round_out(silu(gate) * up): the tile is
 // BM*CG x BN, and the 2N-wide intermediate never reaches memory.
-template <int CG, int BN, int STAGES, int NACC, bool SPLIT, int EPI = 0>
+template <int CG, int BN, int STAGES, int NACC, bool SPLIT, int EPI = 0, int MC = 0>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b,
                     const __grid_constant__ CUtensorMap tmap_c, const GemmParams p) {
@@ -152,6 +158,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
     static_assert(NACC == 1 || NACC == 2, "a tile is one or two accumulator slots wide");
     constexpr bool SWIGLU = (EPI == 1);
     static_assert(!SWIGLU || (NACC == 2 && !SPLIT), "the SwiGLU epilogue pairs the two accumulator slots of a whole tile");
+    static_assert(MC == 0 || (CG == 2 && !SPLIT), "B multicast joins two CTA pairs working on whole tiles");
     constexpr int TILE_N = SWIGLU ? BN : BN * NACC;   // width of the OUTPUT tile
     static_assert(L::TOTAL <= 232448, "exceeds 227 KB of shared memory");
 
@@ -161,7 +168,10 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
 
     const uint32_t warp = threadIdx.x >> 5;
     const uint32_t lane = threadIdx.x & 31;
-    const uint32_t rank = (CG == 2) ? cluster_ctarank() : 0u;
+    const uint32_t crank = (CG == 2) ? cluster_ctarank() : 0u;    // rank in the cluster: 0..1, with MC 0..3
+    const uint32_t rank = crank & 1u;                             // rank in the CTA pair (the pair's leader is 0)
+    const uint32_t pair = MC ? (crank >> 1) : 0u;                 // MC: which of the cluster's two pairs = which of the unit's two tile rows
+    const uint32_t lead = pair * 2u;                              // cluster rank of this pair's leader
     const int first_tile = (CG == 2) ? (int)cluster_id_x() : (int)blockIdx.x;
     const int tile_stride = (CG == 2) ? (int)num_clusters_x() : (int)gridDim.x;
     const int total_units = p.total_units;
@@ -182,7 +192,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
     if (warp == 1 && elect_one()) {
         for (uint32_t s = 0; s < STAGES; ++s) {
             mbar_init(full_bar(s), 1);    // producer's arrive.expect_tx (+ TMA transaction bytes)
-            mbar_init(empty_bar(s), 1);   // one tcgen05.commit
+            mbar_init(empty_bar(s), MC ? 2 : 1);   // one tcgen05.commit per pair that reads the stage
         }
         for (uint32_t a = 0; a < 2; ++a) {
             mbar_init(tmem_full_bar(a), 1);           // one tcgen05.commit
@@ -211,7 +221,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
             uint32_t stage = 0, phase = 0;
             // lockstep bookkeeping (leader CTA of each cluster only; its partner is held back by the
             // shared pipeline): `pos` counts the k-tiles this cluster has issued over all its tiles
-            const bool lockstep = p.sync != nullptr && rank == 0;
+            const bool lockstep = p.sync != nullptr && crank == 0;
             // Lockstep is a locality hint, never a correctness condition: if the clusters this one
             // waits for do not show up in time (not co-resident: another kernel holds SMs, a MIG
             // slice, ...) it stops waiting for the rest of the launch and only keeps counting itself
@@ -228,6 +238,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
                 const GemmUnit un = gemm_unit<SPLIT>(p, u);
                 int tm, tn;
                 tile_coords(un.t, p.tiles_m, p.tiles_n, p.group_m, tm, tn);
+                if constexpr (MC != 0) tm = tm * 2 + (int)pair;   // a unit is two tile rows, one per pair (a row past M is all zero fill)
                 const int m0 = (tm * CG + (int)rank) * GEMM_BM;
                 const int n0 = tn * TILE_N + (int)rank * (int)L::B_COLS;
                 for (int kt = un.k0; kt < un.k1; ++kt, ++pos) {
@@ -261,16 +272,26 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
                                 tma_load_2d(sb + j * L::B_ACC_BYTES + b * L::B_BOX_BYTES, &tmap_b, full_bar(stage),
                                             n0 + (int)j * slot_stride + (int)b * 64, k0);
                     } else {
-                        // both CTAs' bytes are counted on the leader's barrier
-                        const uint32_t lead_bar = map_to_cta(full_bar(stage), 0);
+                        // both CTAs' bytes are counted on the pair leader's barrier: the address is this CTA's
+                        // own barrier with the pair-peer bit cleared, which cta_group::2 resolves in every
+                        // destination CTA to the even CTA of ITS pair
+                        const uint32_t lead_bar = full_bar(stage) & GEMM_PEER_BIT_MASK;
                         if (rank == 0) mbar_arrive_expect_tx(full_bar(stage), 2 * stage_tx);
                         tma_load_2d_cg2(sa, &tmap_a, lead_bar, k0, m0);
 #pragma unroll
                         for (uint32_t j = 0; j < (uint32_t)NACC; ++j)
 #pragma unroll
-                            for (uint32_t b = 0; b < L::B_BOXES; ++b)
-                                tma_load_2d_cg2(sb + j * L::B_ACC_BYTES + b * L::B_BOX_BYTES, &tmap_b, lead_bar,
-                                                n0 + (int)j * slot_stride + (int)b * 64, k0);
+                            for (uint32_t b = 0; b < L::B_BOXES; ++b) {
+                                const uint32_t dst = sb + j * L::B_ACC_BYTES + b * L::B_BOX_BYTES;
+                                const int c0 = n0 + (int)j * slot_stride + (int)b * 64;
+                                if constexpr (MC != 0) {
+                                    // every other box is this pair's to fetch, for both CTAs of rank `rank`
+                                    if (((j * L::B_BOXES + b) & 1u) == pair)
+                                        tma_load_2d_cg2_mc(dst, &tmap_b, lead_bar, c0, k0, (uint16_t)(0x5u << rank));
+                                } else {
+                                    tma_load_2d_cg2(dst, &tmap_b, lead_bar, c0, k0);
+                                }
+                            }
                     }
                     if (++stage == STAGES) { stage = 0; phase ^= 1u; }
                 }
@@ -322,16 +343,17 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
                                           (uint32_t)((kt != un.k0) | (k != 0)));
                         }
                         // accumulator slot ready for the epilogue after the last k-tile
-                        if (kt == un.k1 - 1) umma_commit<CG>(tmem_full_bar(slot0 + j));
+                        if (kt == un.k1 - 1) umma_commit<CG>(tmem_full_bar(slot0 + j), (uint16_t)(3u << lead));
                     }
-                    umma_commit<CG>(empty_bar(stage));   // smem stage reusable once these MMAs retire
+                    // smem stage reusable once these MMAs retire (MC: told to all four CTAs, the other pair multicasts into ours)
+                    umma_commit<CG>(empty_bar(stage), MC ? (uint16_t)0xF : (uint16_t)3);
                     if (++stage == STAGES) { stage = 0; phase ^= 1u; }
                 }
                 if (p.num_k_tiles == 0) {   // owner-map mode: no MMAs, hand the slots over directly
 #pragma unroll
                     for (uint32_t j = 0; j < (uint32_t)NACC; ++j) {
                         mbar_wait(tmem_empty_bar(slot0 + j), acc_phase ^ 1u);
-                        umma_commit<CG>(tmem_full_bar(slot0 + j));
+                        umma_commit<CG>(tmem_full_bar(slot0 + j), (uint16_t)(3u << lead));
                     }
                 }
             }
@@ -369,6 +391,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
             const int t = un.t;
             int tm, tn;
             tile_coords(t, p.tiles_m, p.tiles_n, p.group_m, tm, tn);
+            if constexpr (MC != 0) tm = tm * 2 + (int)pair;
             const int m0 = (tm * CG + (int)rank) * GEMM_BM + (int)q * 32;    // first row of this warp
             const int n_base = tn * TILE_N + (int)half * WARP_COLS;         // first column of this warp
             const uint32_t owner_val = ((uint32_t)t << 8) | (uint32_t)blockIdx.x;
@@ -476,12 +499,12 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
                     if constexpr (SWIGLU) {
                         if constexpr (CG == 1) { mbar_arrive(tmem_empty_bar(0)); mbar_arrive(tmem_empty_bar(1)); }
                         else {
-                            mbar_arrive_cluster(map_to_cta(tmem_empty_bar(0), 0));
-                            mbar_arrive_cluster(map_to_cta(tmem_empty_bar(1), 0));
+                            mbar_arrive_cluster(map_to_cta(tmem_empty_bar(0), lead));
+                            mbar_arrive_cluster(map_to_cta(tmem_empty_bar(1), lead));
                         }
                     } else {
                         if constexpr (CG == 1) mbar_arrive(tmem_empty_bar(acc));
-                        else mbar_arrive_cluster(map_to_cta(tmem_empty_bar(acc), 0));
+                        else mbar_arrive_cluster(map_to_cta(tmem_empty_bar(acc), lead));
                     }
                 }
             };

@@ -186,6 +186,16 @@ __device__ __forceinline__ void tma_load_2d_cg2(uint32_t dst, const CUtensorMap*
         ::"r"(dst), "l"(reinterpret_cast<uint64_t>(m)), "r"(cluster_bar), "r"(c0), "r"(c1)
         : "memory");
 }
+// the same, delivered to the same shared-memory offset of every CTA of the cluster named in `mask`
+// (bit i = cluster rank i); each destination's bytes are counted on the barrier of ITS pair
+__device__ __forceinline__ void tma_load_2d_cg2_mc(uint32_t dst, const CUtensorMap* m, uint32_t bar, int32_t c0,
+                                                   int32_t c1, uint16_t mask) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster"
+        " [%0], [%1, {%3, %4}], [%2], %5;"
+        ::"r"(dst), "l"(reinterpret_cast<uint64_t>(m)), "r"(bar), "r"(c0), "r"(c1), "h"(mask)
+        : "memory");
+}
 // bring a tile into L2 only (no shared-memory destination, nothing to wait for)
 __device__ __forceinline__ void tma_prefetch_l2_2d(const CUtensorMap* m, int32_t c0, int32_t c1) {
     asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global [%0, {%1, %2}];"
@@ -257,15 +267,16 @@ __device__ __forceinline__ void umma_bf16(uint32_t d_tmem, uint64_t a_desc, uint
 // All previously issued tcgen05.mma of this thread arrive on `bar` when they complete
 // (implies tcgen05.fence::before_thread_sync).  CG==2: the arrival is multicast to the
 // same barrier offset in both CTAs of the pair.
+// `mask` (CG == 2): the cluster ranks whose barrier at this offset gets the arrival; default = a cluster of one pair
 template <int CG>
-__device__ __forceinline__ void umma_commit(uint32_t bar) {
+__device__ __forceinline__ void umma_commit(uint32_t bar, uint16_t mask = 3) {
     if constexpr (CG == 1)
         asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar)
                      : "memory");
     else
         asm volatile(
             "tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
-            ::"r"(bar), "h"(static_cast<uint16_t>(3))
+            ::"r"(bar), "h"(mask)
             : "memory");
 }
 

@@ -467,21 +467,22 @@ GemmConfig choose_config(int64_t M, int64_t N, int64_t K, int sms) {
 // How many work-unit owners (CTA pairs for cg = 2, CTAs for cg = 1) of a tile configuration the device
 // holds at once, from the occupancy calculator (GPC layout, shared memory, registers): the persistent
 // grid is never larger, so that every CTA of a launch is resident when nothing else runs on the device.
-template <int CG, int BN, int STAGES, int NACC>
+template <int CG, int BN, int STAGES, int NACC, int MC = 0>
 int query_resident_units(int sms) {
     using L = tg::GemmSmem<CG, BN, STAGES, NACC>;
-    auto kern = tg::gemm_tcgen05_kernel<CG, BN, STAGES, NACC, false, 0>;
+    auto kern = tg::gemm_tcgen05_kernel<CG, BN, STAGES, NACC, false, 0, MC>;
+    constexpr int CL = CG * (MC ? 2 : 1);   // CTAs per cluster
     int n = 0;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::TOTAL) == cudaSuccess) {
         if (CG == 2) {
             cudaLaunchConfig_t cfg;
             memset(&cfg, 0, sizeof cfg);
-            cfg.gridDim = dim3((unsigned)(sms & ~1), 1, 1);
+            cfg.gridDim = dim3((unsigned)(sms / CL * CL), 1, 1);
             cfg.blockDim = dim3(tg::GEMM_THREADS, 1, 1);
             cfg.dynamicSmemBytes = L::TOTAL;
             cudaLaunchAttribute attr[1];
             attr[0].id = cudaLaunchAttributeClusterDimension;
-            attr[0].val.clusterDim.x = 2;
+            attr[0].val.clusterDim.x = CL;
             attr[0].val.clusterDim.y = 1;
             attr[0].val.clusterDim.z = 1;
             cfg.attrs = attr;
@@ -494,21 +495,23 @@ int query_resident_units(int sms) {
         }
     }
     cudaGetLastError();   // a failed query is not an error of the call that asked
-    if (n <= 0 || n > sms / CG) n = sms / CG;   // one CTA per SM at most: a CTA allocates all of tensor memory
+    if (n <= 0 || n > sms / CL) n = sms / CL;   // one CTA per SM at most: a CTA allocates all of tensor memory
     return n;
 }
 
-int resident_units(const GemmConfig& cfg, int dev, int sms) {
-    static std::atomic<int> cache[5][64];
-    int v = cache[cfg.id][dev].load();
+// config ids 1..4, and 5 = config 4 with two pairs per cluster (B multicast): resident clusters
+int resident_units(int id, int dev, int sms) {
+    static std::atomic<int> cache[6][64];
+    int v = cache[id][dev].load();
     if (v > 0) return v;
-    switch (cfg.id) {
+    switch (id) {
         case 1: v = query_resident_units<1, 128, 6, 1>(sms); break;
         case 2: v = query_resident_units<1, 256, 4, 1>(sms); break;
         case 3: v = query_resident_units<2, 256, 6, 1>(sms); break;
-        default: v = query_resident_units<2, 256, 4, 2>(sms); break;
+        case 4: v = query_resident_units<2, 256, 4, 2>(sms); break;
+        default: v = query_resident_units<2, 256, 4, 2, 1>(sms); break;
     }
-    cache[cfg.id][dev].store(v);
+    cache[id][dev].store(v);
     return v;
 }
 
@@ -519,10 +522,13 @@ struct GemmLaunch {
     GemmConfig cfg;
     tg::GemmParams p;
     int ctas;
+    bool mc = false;   // two CTA pairs per cluster, one tile row above the other, B multicast (gemm_kernel.cuh, MC = 1)
 };
 
+constexpr bool kGemmMulticastDefault = false;
+
 void plan_gemm(int64_t M, int64_t N, int64_t K, int in_dtype, int out_dtype, int dev, int sms, GemmLaunch* gl,
-               bool allow_split = false) {
+               bool allow_split = false, bool allow_mc = true) {
     gl->cfg = choose_config(M, N, K, sms);
     const int tile_m = tg::GEMM_BM * gl->cfg.cg;
     tg::GemmParams& p = gl->p;
@@ -537,10 +543,21 @@ void plan_gemm(int64_t M, int64_t N, int64_t K, int in_dtype, int out_dtype, int
     p.out_16 = out_dtype != TILE_GEMM_OUT_F32;
     p.out_f16 = out_dtype == TILE_GEMM_OUT_F16;
     p.in_f16 = in_dtype == TILE_GEMM_IN_F16;
-    const int64_t tiles = (int64_t)p.tiles_m * p.tiles_n;
-    int max_units = resident_units(gl->cfg, dev, sms);
+    int64_t tiles = (int64_t)p.tiles_m * p.tiles_n;
+    // B multicast across two pairs (tuning key 12: 1 = never, 2 = whenever the configuration has it): a work unit
+    // becomes two tile rows of the same tile column, and no unit is cut along K
+    const int mc_tune = g_tune[12].load();
+    gl->mc = gl->cfg.id == 4 && allow_mc && p.tiles_m >= 2 && mc_tune != 1 && (mc_tune == 2 || kGemmMulticastDefault);
+    if (gl->mc) {
+        p.tiles_m = (p.tiles_m + 1) / 2;
+        p.group_m = (p.group_m + 1) / 2;
+        tiles = (int64_t)p.tiles_m * p.tiles_n;
+        allow_split = false;
+    }
+    int max_units = resident_units(gl->mc ? 5 : gl->cfg.id, dev, sms);
     const int cap = g_tune[2].load();
-    if (cap > 0 && cap / gl->cfg.cg >= 1 && cap / gl->cfg.cg < max_units) max_units = cap / gl->cfg.cg;
+    const int cl = gl->cfg.cg * (gl->mc ? 2 : 1);   // CTAs per cluster
+    if (cap > 0 && cap / cl >= 1 && cap / cl < max_units) max_units = cap / cl;
     // Split-K for the partial last wave: `rem` tiles are left after the whole waves;
     // cut each into floor(clusters / rem) slices so that the last round is one short, full wave.
     p.full_units = (int32_t)tiles;
@@ -568,14 +585,14 @@ void plan_gemm(int64_t M, int64_t N, int64_t K, int in_dtype, int out_dtype, int
     }
     int64_t units = p.total_units;
     if (units > max_units) units = max_units;
-    gl->ctas = (int)units * gl->cfg.cg;
+    gl->ctas = (int)units * cl;
 }
 
-template <int CG, int BN, int STAGES, int NACC, bool SPLIT, int EPI = 0>
+template <int CG, int BN, int STAGES, int NACC, bool SPLIT, int EPI = 0, int MC = 0>
 int launch_gemm_inst(const CUtensorMap& ta, const CUtensorMap& tb, const CUtensorMap& tc, const tg::GemmParams& p,
                      int ctas, cudaStream_t s, int dev) {
     using L = tg::GemmSmem<CG, BN, STAGES, NACC>;
-    auto kern = tg::gemm_tcgen05_kernel<CG, BN, STAGES, NACC, SPLIT, EPI>;
+    auto kern = tg::gemm_tcgen05_kernel<CG, BN, STAGES, NACC, SPLIT, EPI, MC>;
     static bool configured[64] = {};
     if (!configured[dev]) {
         CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::TOTAL));
@@ -591,7 +608,7 @@ int launch_gemm_inst(const CUtensorMap& ta, const CUtensorMap& tb, const CUtenso
     int na = 0;
     if (CG == 2) {   // a 1-CTA "cluster" attribute would still take the driver's cluster launch path
         attr[na].id = cudaLaunchAttributeClusterDimension;
-        attr[na].val.clusterDim.x = CG;
+        attr[na].val.clusterDim.x = CG * (MC ? 2 : 1);
         attr[na].val.clusterDim.y = 1;
         attr[na].val.clusterDim.z = 1;
         ++na;
@@ -610,6 +627,7 @@ int launch_gemm_inst(const CUtensorMap& ta, const CUtensorMap& tb, const CUtenso
 
 int launch_gemm(const GemmLaunch& gl, const CUtensorMap& ta, const CUtensorMap& tb, const CUtensorMap& tc,
                 cudaStream_t s, int dev) {
+    if (gl.mc) return launch_gemm_inst<2, 256, 4, 2, false, 0, 1>(ta, tb, tc, gl.p, gl.ctas, s, dev);
     switch (gl.cfg.id) {
 #define TG_GEMM_CASE(id, CG, BN, ST, NA)                                                              \
     case id:                                                                                         \
@@ -629,7 +647,7 @@ int launch_gemm(const GemmLaunch& gl, const CUtensorMap& ta, const CUtensorMap& 
 // rounds the lockstep covers (0: off) and its window, from the plan alone
 void lockstep_plan(const GemmLaunch& gl, int64_t* rounds_out, int* window_out) {
     const int tune = g_tune[6].load();
-    const int clusters = gl.ctas / gl.cfg.cg;
+    const int clusters = gl.ctas / (gl.cfg.cg * (gl.mc ? 2 : 1));
     // rounds in which every cluster owns a whole tile: lockstep covers exactly these
     const int64_t rounds = clusters > 0 ? gl.p.full_units / clusters : 0;
     bool on = rounds >= kLockstepMinTiles && gl.p.num_k_tiles >= kLockstepMinKTiles;
@@ -1242,7 +1260,7 @@ int tile_gemm_swiglu(const void* X, const void* Wgu, void* H, int64_t M, int64_t
     const int64_t tiles = (int64_t)p.tiles_m * p.tiles_n;
     p.full_units = p.total_units = (int32_t)tiles;
     p.kps = p.num_k_tiles;
-    const int64_t slots = resident_units(gl.cfg, dev, sms);
+    const int64_t slots = resident_units(gl.cfg.id, dev, sms);
     const int64_t clusters = tiles < slots ? tiles : slots;
     gl.ctas = (int)clusters * 2;
     p.tma_store = plan.c_tma ? 1 : 0;
@@ -1545,7 +1563,7 @@ int tile_gemm_query_config(int64_t M, int64_t N, int64_t K, int out_dtype, int32
     out[4] = gl.p.group_m;
     out[5] = gl.cfg.stages;
     out[6] = tg::GEMM_BK;
-    out[7] = gl.cfg.id;
+    out[7] = gl.mc ? 6 : gl.cfg.id;
     return TILE_GEMM_OK;
 }
 

@@ -80,10 +80,11 @@ def freivalds_rows(C_gpu_f64, a64, b64, seed=0):
 def expected_owner_map(M, N, cfg: dict):
     """Host restatement of the kernel's tile -> owner function (csrc/gemm_kernel.cuh,
     tile_coords + round-robin over clusters) for the owner-map test."""
+    pairs = 2 if cfg["config"] == 6 else 1          # config 6: two CTA pairs per cluster (B multicast), a unit = two tile rows
     tile_m = cfg["BM"] * cfg["cta_group"]
-    tiles_m = -(-M // tile_m)
+    tiles_m = -(-M // (tile_m * pairs))             # unit rows
     tiles_n = -(-N // cfg["BN"])
-    clusters = cfg["ctas"] // cfg["cta_group"]
+    clusters = cfg["ctas"] // (cfg["cta_group"] * pairs)
     own = np.full((M, N), -1, dtype=np.int64)
     for t in range(tiles_m * tiles_n):
         per_group = cfg["group_m"] * tiles_n
@@ -93,10 +94,11 @@ def expected_owner_map(M, N, cfg: dict):
         r = t - g * per_group
         tm, tn = first_m + r % rows, r // rows
         cluster = t % clusters
-        for rank in range(cfg["cta_group"]):
-            cta = cluster * cfg["cta_group"] + rank
-            r0 = (tm * cfg["cta_group"] + rank) * cfg["BM"]
-            own[r0:r0 + cfg["BM"], tn * cfg["BN"]:(tn + 1) * cfg["BN"]] = (t << 8) | cta
+        for pair in range(pairs):
+            for rank in range(cfg["cta_group"]):
+                cta = (cluster * pairs + pair) * cfg["cta_group"] + rank
+                r0 = ((tm * pairs + pair) * cfg["cta_group"] + rank) * cfg["BM"]
+                own[r0:r0 + cfg["BM"], tn * cfg["BN"]:(tn + 1) * cfg["BN"]] = (t << 8) | cta
     return own
 
 

@@ -500,14 +500,17 @@ def test_column_shards_equal_the_unsharded_result(G):
 
 
 # ------------------------------------------------------------------ ownership
-@pytest.mark.parametrize("cfg", [1, 2, 3, 4])
-@pytest.mark.parametrize("shape", [(1023, 1537), (256, 256), (4096, 5120), (130, 70)])
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 6])
+@pytest.mark.parametrize("shape", [(1023, 1537), (256, 256), (4096, 5120), (130, 70), (1300, 520)])
 def test_owner_map_is_the_documented_function(cfg, shape):
     """Each output element is written by exactly one CTA, the one tile_coords assigns
-    (PAPER.md:163 'each sub-tensor has exactly one owner')."""
-    tg.tile_gemm_set_tuning(tg.TUNE_GEMM_CONFIG, cfg)
+    (PAPER.md:163 'each sub-tensor has exactly one owner').  cfg 6 = config 4 with two CTA pairs per
+    cluster (B multicast): a work unit is two tile rows, one per pair."""
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMM_CONFIG, min(cfg, 4))
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMM_MULTICAST, 2 if cfg == 6 else 1)
     M, N = shape
     conf = tg.tile_gemm_query_config(M, N, 64)
+    assert conf["config"] == (4 if cfg == 6 and M <= 256 else cfg)     # one tile row: nothing to pair up
     for ld in (N, N + 3):
         owner = tg.tile_gemm_debug_owner_map(M, N, 64, ld_owner=ld)
         torch.cuda.synchronize()
@@ -620,6 +623,49 @@ def test_gemm_split_k_auto_normal_inputs_and_determinism(out):
         got2 = run_case(a, b, out, what="split auto")
         check_close(got1, ref, S, K, out, f"split-K auto {M}x{N}x{K} {out}")
         assert np.array_equal(got1, got2), "split-K result depends on arrival order"
+
+
+# ------------------------------------------------------------------ B multicast across two CTA pairs (tuning key 12)
+@pytest.mark.parametrize("cap", [0, 8, 20])
+def test_gemm_multicast_pairs_integer_bit_exact_and_canary(cap):
+    """Config 4 with clusters of two CTA pairs that share every B stage through TMA multicast: ragged shapes, an odd
+    number of tile rows (one pair of the last unit owns rows past M), few clusters walking many units; integer inputs
+    are exact, nothing outside C is written, every element is written; lockstep producers on top stay exact."""
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMM_CONFIG, 4)
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMM_MULTICAST, 2)
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMM_MAX_CTAS, cap)
+    for (M, N, K), pads in (((1023, 1537, 769), (0, 0, 0)), ((300, 700, 4100), (8, 8, 8)), ((1300, 520, 1030), (0, 0, 3)),
+                            ((2304, 2560, 512), (0, 8, 0))):
+        assert tg.tile_gemm_query_config(M, N, K)["config"] == 6
+        a, b = wl.make_inputs_custom(M, N, K, dist="int4", seed=51 + cap)
+        ref, _ = oracle.gemm(a, b)
+        for out in ("f32", "bf16"):
+            got = run_case(a, b, out, pads=pads, what=f"multicast pairs cap {cap}")
+            if out == "f32":
+                check_bit_exact(got.astype(np.float32), ref, f"multicast pairs {M}x{N}x{K} cap {cap}")
+            else:
+                assert np.array_equal(got, rne_bf16(ref))
+    tg.tile_gemm_set_tuning(tg.TUNE_FLAGS, 4 | (2 << 8))                  # lockstep forced on, window 2
+    a, b = wl.make_inputs_custom(1023, 1537, 769, dist="int4", seed=59)
+    ref, _ = oracle.gemm(a, b)
+    check_bit_exact(run_case(a, b, "f32", what="multicast + lockstep").astype(np.float32), ref, "multicast + lockstep")
+
+
+def test_gemm_multicast_pairs_give_the_bits_of_the_plain_config():
+    """The MMA order per tile does not depend on how the operands reached shared memory."""
+    M, N, K = 2304, 2560, 2048
+    a, b = wl.make_inputs_custom(M, N, K, sigma_b=K ** -0.5, seed=58)
+    A, B = wl.bits_to_torch(a, DEV), wl.bits_to_torch(b, DEV)
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMM_CONFIG, 4)
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMM_MULTICAST, 1)
+    plain = tg.tile_gemm(A, B, out_dtype=tg.OUT_F32)
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMM_MULTICAST, 2)
+    mc = tg.tile_gemm(A, B, out_dtype=tg.OUT_F32)
+    torch.cuda.synchronize()
+    assert torch.equal(plain, mc)
+    rows, cols = wl.uniform_samples(M, N, 2048, seed=58)
+    c, s = oracle.gemm_sampled(a, b, rows, cols)
+    check_close(mc.cpu().numpy()[rows, cols], c, s, K, "f32", "multicast pairs sampled")
 
 
 # ------------------------------------------------------------------ lockstep producers (long launches)
