@@ -71,6 +71,11 @@ struct GemmParams {
     int32_t up_offset;          // SwiGLU epilogue: column of B where the `up` half starts (= N, the width of C)
     float* partials;            // [split tiles][split][CG][8 warps][units][8 chunks][32 lanes][4 floats]
     uint32_t* tickets;          // [split tiles][CG], zero between launches
+    // debug (tile_gemm_debug_trace): cluster c writes record c of 8 words -- clock cycles the MMA issuer [0] waited for
+    // operand stages, [1] waited for accumulator slots, [2] spent in its loop in total, [3] k-tiles it issued; [4] cycles one
+    // epilogue warp spent between "accumulator full" and "slot handed back" summed over its [5] tiles
+    unsigned long long* trace;
+    int32_t trace_cap;          // clusters that fit the trace buffer
 };
 
 // Work unit -> (tile, k-tile range, slice); slice < 0: a whole tile.  Pure function, all roles
@@ -316,12 +321,22 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
             // slot use: NACC == 1 -> slot = tile iteration & 1 (phase flips every 2nd tile);
             //           NACC == 2 -> both slots every tile (phase flips every tile)
             uint32_t stage = 0, phase = 0, it = 0;
+            const bool traced = p.trace != nullptr && first_tile < p.trace_cap;
+            long long t_full = 0, t_acc = 0, n_kt = 0;
+            const long long t_begin = clock64();
             for (int u = first_tile; u < total_units; u += tile_stride, ++it) {
                 const GemmUnit un = gemm_unit<SPLIT>(p, u);
                 const uint32_t slot0 = (NACC == 2) ? 0u : (it & 1u);
                 const uint32_t acc_phase = (NACC == 2) ? (it & 1u) : ((it >> 1) & 1u);
                 for (int kt = un.k0; kt < un.k1; ++kt) {
-                    mbar_wait(full_bar(stage), phase);
+                    if (traced) {
+                        const long long t0 = clock64();
+                        mbar_wait(full_bar(stage), phase);
+                        t_full += clock64() - t0;
+                        ++n_kt;
+                    } else {
+                        mbar_wait(full_bar(stage), phase);
+                    }
                     tc_fence_after();
                     const uint32_t sa = smem_base + stage * L::STAGE_BYTES;
                     const uint32_t sb = sa + L::A_BYTES;
@@ -329,7 +344,9 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
 #pragma unroll
                     for (uint32_t j = 0; j < (uint32_t)NACC; ++j) {
                         if (kt == un.k0) {   // the epilogue must have drained this slot
+                            const long long t0 = traced ? clock64() : 0;
                             mbar_wait(tmem_empty_bar(slot0 + j), acc_phase ^ 1u);
+                            if (traced) t_acc += clock64() - t0;
                             tc_fence_after();
                         }
                         const uint32_t d_tmem = tmem_base + (slot0 + j) * BN;
@@ -356,6 +373,13 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
                         umma_commit<CG>(tmem_full_bar(slot0 + j), (uint16_t)(3u << lead));
                     }
                 }
+            }
+            if (traced) {
+                unsigned long long* rec = p.trace + (size_t)first_tile * 8;
+                rec[0] = (unsigned long long)t_full;
+                rec[1] = (unsigned long long)t_acc;
+                rec[2] = (unsigned long long)(clock64() - t_begin);
+                rec[3] = (unsigned long long)n_kt;
             }
         }
         __syncwarp();
@@ -384,6 +408,8 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
         // st.global path so that C[i][N..] is never written.
         const bool ragged_n = (p.N % (out_16 ? 8 : 4)) != 0;
         uint32_t it = 0, buf = 0;
+        const bool dbg = p.trace != nullptr && first_tile < p.trace_cap && rank == 0 && ew == 4;   // tile_gemm_debug_trace: one warp per cluster
+        long long dbg_drain = 0;
         volatile uint32_t* last_flag = reinterpret_cast<volatile uint32_t*>(smem_gen + L::LAST_FLAG_OFF);
         griddep_wait();   // C, the partials and the tickets may still be in the previous kernel's use
         for (int u_idx = first_tile; u_idx < total_units; u_idx += tile_stride, ++it) {
@@ -413,6 +439,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
                 mbar_wait_sleep(tmem_full_bar(acc), acc_phase);
             }
             tc_fence_after();
+            const long long dbg_t0 = dbg ? clock64() : 0;
 
             // stage 16 words (64 B) of this thread's row as columns [n0, n0 + sub_cols) and send them
             auto emit = [&](uint32_t w0, uint32_t w1, uint32_t w2, uint32_t w3, uint32_t w4, uint32_t w5,
@@ -493,18 +520,19 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
             };
             // all TMEM reads of this accumulator slot are complete: hand it back to the MMA warp
             auto release_tmem = [&]() {
+                if (dbg) dbg_drain += clock64() - dbg_t0;
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) {
                     if constexpr (SWIGLU) {
                         if constexpr (CG == 1) { mbar_arrive(tmem_empty_bar(0)); mbar_arrive(tmem_empty_bar(1)); }
                         else {
-                            mbar_arrive_cluster(map_to_cta(tmem_empty_bar(0), lead));
-                            mbar_arrive_cluster(map_to_cta(tmem_empty_bar(1), lead));
+                            mbar_arrive_cluster_relaxed(map_to_cta(tmem_empty_bar(0), lead));
+                            mbar_arrive_cluster_relaxed(map_to_cta(tmem_empty_bar(1), lead));
                         }
                     } else {
                         if constexpr (CG == 1) mbar_arrive(tmem_empty_bar(acc));
-                        else mbar_arrive_cluster(map_to_cta(tmem_empty_bar(acc), lead));
+                        else mbar_arrive_cluster_relaxed(map_to_cta(tmem_empty_bar(acc), lead));
                     }
                 }
             };
@@ -595,6 +623,10 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
                 }
             }
             if (units == 0) release_tmem();
+        }
+        if (dbg && lane == 0) {
+            p.trace[(size_t)first_tile * 8 + 4] = (unsigned long long)dbg_drain;
+            p.trace[(size_t)first_tile * 8 + 5] = (unsigned long long)it;
         }
         if (lane == 0) tma_store_wait_all<0>();
         __syncwarp();

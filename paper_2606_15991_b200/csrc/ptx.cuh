@@ -104,6 +104,14 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_bar) {
     asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
 }
+// The same without release semantics: hands over something no generic-proxy memory operation of this thread
+// produced (a tensor-memory slot whose reads were completed by tcgen05.wait::ld and ordered by
+// tcgen05.fence::before_thread_sync).  The releasing form compiles to MEMBAR + ERRBAR, which waits for every store
+// this thread still has in flight -- in the GEMM epilogue that kept a drained accumulator slot from the MMA warp
+// until the warp's staged C stores had landed (ncu source view: a fifth of the drain).
+__device__ __forceinline__ void mbar_arrive_cluster_relaxed(uint32_t cluster_bar) {
+    asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
+}
 __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
     uint32_t ok;
     asm volatile(

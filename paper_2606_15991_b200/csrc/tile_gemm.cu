@@ -877,6 +877,8 @@ int run_gemm(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_
     }
     rc = setup_lockstep(gl, dev, s);
     if (rc) return rc;
+    gl.p.trace = g_trace.load();                                   // tile_gemm_debug_trace: 4 words per cluster
+    gl.p.trace_cap = (int32_t)g_trace_cap.load();
     return launch_gemm(gl, ta, tb, tc, s, dev);
 }
 

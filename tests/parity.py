@@ -80,7 +80,7 @@ def freivalds_rows(C_gpu_f64, a64, b64, seed=0):
 def expected_owner_map(M, N, cfg: dict):
     """Host restatement of the kernel's tile -> owner function (csrc/gemm_kernel.cuh,
     tile_coords + round-robin over clusters) for the owner-map test."""
-    pairs = 2 if cfg["config"] == 6 else 1          # config 6: two CTA pairs per cluster (B multicast), a unit = two tile rows
+    pairs = 2 if cfg.get("config") == 6 else 1          # config 6: two CTA pairs per cluster (B multicast), a unit = two tile rows
     tile_m = cfg["BM"] * cfg["cta_group"]
     tiles_m = -(-M // (tile_m * pairs))             # unit rows
     tiles_n = -(-N // cfg["BN"])

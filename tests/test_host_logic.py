@@ -107,6 +107,8 @@ def test_bad_force_path_and_tuning_key():
     dict(BM=128, BN=256, cta_group=1, ctas=56, group_m=16),
     dict(BM=128, BN=256, cta_group=2, ctas=148, group_m=8),
     dict(BM=128, BN=256, cta_group=2, ctas=8, group_m=3),
+    dict(BM=128, BN=512, cta_group=2, ctas=132, group_m=8, config=6),    # two CTA pairs per cluster: a unit is two tile rows
+    dict(BM=128, BN=512, cta_group=2, ctas=12, group_m=2, config=6),
 ])
 @pytest.mark.parametrize("shape", [(1023, 1537), (8192, 8192), (130, 70), (4096, 5120)])
 def test_schedule_function_covers_every_element_once(cfg, shape):
@@ -115,15 +117,18 @@ def test_schedule_function_covers_every_element_once(cfg, shape):
     M, N = shape
     own = parity.expected_owner_map(M, N, cfg)
     assert own.min() >= 0
-    tile_m = cfg["BM"] * cfg["cta_group"]
+    tile_m = cfg["BM"] * cfg["cta_group"] * (2 if cfg.get("config") == 6 else 1)      # rows of a work unit
     tiles = -(-M // tile_m) * -(-N // cfg["BN"])
     ids = np.unique(own >> 8)
     assert ids.size == tiles and ids.max() == tiles - 1
     assert (own & 0xFF).max() < cfg["ctas"]
-    # each tile id occupies one BM*cg x BN rectangle
+    # each unit id occupies one rectangle of unit rows x BN, every CTA of its cluster a BM-row band of it
     t = int(ids[len(ids) // 2])
     rr, cc = np.where((own >> 8) == t)
     assert rr.max() - rr.min() < tile_m and cc.max() - cc.min() < cfg["BN"]
+    for cta in np.unique(own[rr, cc] & 0xFF):
+        r2 = rr[(own[rr, cc] & 0xFF) == cta]
+        assert r2.max() - r2.min() < cfg["BM"]
 
 
 def test_workload_shapes_match_baseline_json():
