@@ -316,9 +316,10 @@ int tile_gemm_debug_occupy(int ctas, int64_t ns, void* stream);
  *   dependency wait, [3] first tile in shared memory, [4] last tile consumed, [5] CTA done;
  *   [6] tiles consumed; [7] %globaltimer when this CTA's partial sums were handed over (split-K only).
  * The tiled GEMM kernel fills the same buffer while it is set: cluster c writes record c (when below
- * capacity): clock cycles its MMA issuer [0] waited for operand stages, [1] waited for accumulator slots
- * to be drained, [2] spent in its loop in total, [3] k-tiles it issued; [4] cycles one epilogue warp
- * spent between "accumulator full" and "slot handed back", summed over its [5] tiles; [6], [7] unused.
+ * capacity): clock cycles its MMA issuer [1] waited for accumulator slots to be drained (taken once
+ * per tile: the K loop itself is not touched), [2] spent in its loop in total, [3] k-tiles it issued;
+ * [4] cycles one epilogue warp spent between "accumulator full" and "slot handed back", summed over
+ * its [5] tiles; [0], [6], [7] unused.
  * Later launches overwrite earlier ones: point it at a fresh buffer per launch.  records == NULL
  * or capacity == 0 switches tracing off (one untaken branch per event).  Process-global like the
  * tuning keys.  Returns 0, E_EXTENT or E_ALIGN.

@@ -71,8 +71,8 @@ struct GemmParams {
     int32_t up_offset;          // SwiGLU epilogue: column of B where the `up` half starts (= N, the width of C)
     float* partials;            // [split tiles][split][CG][8 warps][units][8 chunks][32 lanes][4 floats]
     uint32_t* tickets;          // [split tiles][CG], zero between launches
-    // debug (tile_gemm_debug_trace): cluster c writes record c of 8 words -- clock cycles the MMA issuer [0] waited for
-    // operand stages, [1] waited for accumulator slots, [2] spent in its loop in total, [3] k-tiles it issued; [4] cycles one
+    // debug (tile_gemm_debug_trace): cluster c writes record c of 8 words -- [0] unused, clock cycles the MMA issuer
+    // [1] waited for accumulator slots (once per tile), [2] spent in its loop in total, [3] k-tiles it issued; [4] cycles one
     // epilogue warp spent between "accumulator full" and "slot handed back" summed over its [5] tiles
     unsigned long long* trace;
     int32_t trace_cap;          // clusters that fit the trace buffer
@@ -322,21 +322,15 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
             //           NACC == 2 -> both slots every tile (phase flips every tile)
             uint32_t stage = 0, phase = 0, it = 0;
             const bool traced = p.trace != nullptr && first_tile < p.trace_cap;
-            long long t_full = 0, t_acc = 0, n_kt = 0;
+            long long t_acc = 0, n_kt = 0;   // the trace touches the tile boundary only: the K loop below stays as it is
             const long long t_begin = clock64();
             for (int u = first_tile; u < total_units; u += tile_stride, ++it) {
                 const GemmUnit un = gemm_unit<SPLIT>(p, u);
                 const uint32_t slot0 = (NACC == 2) ? 0u : (it & 1u);
                 const uint32_t acc_phase = (NACC == 2) ? (it & 1u) : ((it >> 1) & 1u);
+                n_kt += un.k1 - un.k0;
                 for (int kt = un.k0; kt < un.k1; ++kt) {
-                    if (traced) {
-                        const long long t0 = clock64();
-                        mbar_wait(full_bar(stage), phase);
-                        t_full += clock64() - t0;
-                        ++n_kt;
-                    } else {
-                        mbar_wait(full_bar(stage), phase);
-                    }
+                    mbar_wait(full_bar(stage), phase);
                     tc_fence_after();
                     const uint32_t sa = smem_base + stage * L::STAGE_BYTES;
                     const uint32_t sb = sa + L::A_BYTES;
@@ -376,7 +370,7 @@ gemm_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_con
             }
             if (traced) {
                 unsigned long long* rec = p.trace + (size_t)first_tile * 8;
-                rec[0] = (unsigned long long)t_full;
+                rec[0] = 0ull;
                 rec[1] = (unsigned long long)t_acc;
                 rec[2] = (unsigned long long)(clock64() - t_begin);
                 rec[3] = (unsigned long long)n_kt;

@@ -37,7 +37,7 @@ def trace_once(n: int, cfg: int, dev) -> str:
     tg.tile_gemm_set_tuning(tg.TUNE_GEMM_CONFIG, 0)
     r = rec.cpu().double()
     r = r[r[:, 2] > 0]
-    full, acc, tot, nk, drain, tiles = (r[:, i] for i in range(6))
+    _, acc, tot, nk, drain, tiles = (r[:, i] for i in range(6))
     us = e0.elapsed_time(e1) * 1e3
     return (f"| {n} | {cfg} | {us:.0f} | {len(r)} | {tot.mean():.0f} | {100 * (acc / tot).mean():.1f} % | {(acc / tiles).mean():.0f} | "
             f"{(drain / tiles).mean():.0f} | {(tot / nk).mean():.0f} | {tot.mean() / us / 1e3:.2f} |")
