@@ -512,6 +512,56 @@ def bench_sweep(tg, torch, sizes, tdist, warm_s=0.35):
     return out
 
 
+def bench_cublas_context(tg, torch, case, seconds=1.0, pause=2.5):
+    """CONTEXT, not product path: torch.matmul (cuBLAS) and tile_gemm on cfg3 under ONE protocol in this very run, so that
+    the roofline fraction (whose denominator MEASURED_PEAKS.json was taken on another day, possibly another box: the pool's
+    B200s differ by +-5 % under the power cap) can be read next to a same-box, same-minute ratio.  Burst = 20 launches after
+    `pause` seconds of idle and 5 warm-up launches; sustained = back to back for `seconds` right after 0.35 s of the same."""
+    dev = torch.device("cuda", torch.cuda.current_device())
+    g = torch.Generator(device=dev)
+    g.manual_seed(1000 + case.seed[0])
+    sets = 4
+    bufs = [(torch.empty((case.M, case.K), dtype=torch.bfloat16, device=dev).normal_(0, case.sigma_a, generator=g),
+             torch.empty((case.K, case.N), dtype=torch.bfloat16, device=dev).normal_(0, case.sigma_b, generator=g),
+             torch.empty((case.M, case.N), dtype=torch.bfloat16, device=dev)) for _ in range(sets)]
+    flops = 2.0 * case.M * case.N * case.K
+
+    def run(kind, k):
+        for i in range(k):
+            A, B, C = bufs[i % sets]
+            if kind == "cublas":
+                torch.matmul(A, B, out=C)
+            else:
+                tg.tile_gemm(A, B, C)
+
+    def timed(kind, k):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        run(kind, k)
+        e1.record()
+        torch.cuda.synchronize()
+        return flops / (e0.elapsed_time(e1) / k * 1e-3) / 1e12
+
+    out = {"note": "context only: torch.matmul (cuBLAS) is not on the product path"}
+    for kind in ("cublas", "tile_gemm", "cublas", "tile_gemm"):
+        time.sleep(pause)
+        run(kind, 5)
+        torch.cuda.synchronize()
+        out.setdefault(kind + "_burst_tflops", []).append(round(timed(kind, 20), 1))
+    for kind in ("tile_gemm", "cublas", "cublas", "tile_gemm"):
+        t_end = time.perf_counter() + 0.35
+        while time.perf_counter() < t_end:
+            run(kind, 16)
+            torch.cuda.synchronize()
+        k = max(16, int(seconds / 0.8e-3))
+        out.setdefault(kind + "_sustained_tflops", []).append(round(timed(kind, k), 1))
+    out["burst_ratio"] = round(max(out["tile_gemm_burst_tflops"]) / max(out["cublas_burst_tflops"]), 4)
+    out["sustained_ratio"] = round(sum(out["tile_gemm_sustained_tflops"]) / sum(out["cublas_sustained_tflops"]), 4)
+    del bufs
+    torch.cuda.empty_cache()
+    return out
+
+
 def bench_sustained(tg, torch, case, seconds, local_rank, tdist):
     """cfg3 back to back for >= `seconds`: the figure to hold against MEASURED_PEAKS.json's sustained
     cuBLAS number (a seconds-long loop under the power cap), with its own clock record."""
@@ -593,6 +643,9 @@ def run_cuda(args):
             "achieved": s_tf, "peak": peaks["bf16_tflops_sustained"], "frac": s_tf / peaks["bf16_tflops_sustained"],
             "unit": "TFLOP/s", "ms_per_step": s_ms, "steps": s_steps, "seconds": s_total * 1e-3, "clocks": s_clocks,
             "peak_source": f"{peaks['source']} cuBLAS bf16 back to back for seconds (MEASURED_PEAKS.json)"}
+
+    if rank == 0 and world == 1 and not (args.no_cublas_context or args.no_sustained or args.headline_only):
+        line["roofline"]["cublas_same_run"] = bench_cublas_context(tg, torch, case)
 
     if rank == 0 and not args.no_e2e:
         dt, h2d, d2h, _ = bench_e2e(tg, wl, torch, case, max(2, min(args.steps, 5)))
@@ -723,6 +776,7 @@ def main():
     ap.add_argument("--no-sweep", action="store_true", help="skip the f16/bf16 size sweep (SURVEY 8(f)1)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-sustained", action="store_true", help="skip the seconds-long back-to-back cfg3 leg")
+    ap.add_argument("--no-cublas-context", action="store_true", help="skip the same-run cuBLAS context figures (torch.matmul)")
     ap.add_argument("--sustained-seconds", type=float, default=2.5)
     ap.add_argument("--gemm-config", type=int, default=0, help="force a GEMM tile config (tile_gemm_set_tuning key 0)")
     ap.add_argument("--group-m", type=int, default=0, help="force the raster group height (tuning key 1)")
