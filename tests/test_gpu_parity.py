@@ -781,6 +781,60 @@ def test_skinny_normal_inputs_reproducible_and_agrees_with_the_tiled_gemm(M, out
     check_close(tiled, ref, S, K, out, f"tiled M={M} {out}")
 
 
+@pytest.mark.parametrize("M", [3, 8, 24])
+@pytest.mark.parametrize("static_b", [False, True])
+def test_skinny_chain_is_stream_ordered_under_pdl(M, static_b):
+    """C of one skinny-M GEMM is A of the next, launched back to back with programmatic dependent launch (weights
+    prefetched ahead of the dependency wait when they are immutable, activations behind it): the bits must equal
+    those of the same chain run with a synchronise after every launch, and every link must match the oracle on
+    the bits it was given.  Shapes alternate so that consecutive launches differ in cluster size."""
+    dims = [2048, 4096, 1024, 2048, 8192, 2048]
+    rng = np.random.default_rng(33 + M)
+    Ws = [wl.bits_to_torch(wl.f32_to_bf16_bits((rng.standard_normal((dims[i], dims[i + 1])) * dims[i] ** -0.5).astype(np.float32)), DEV)
+          for i in range(len(dims) - 1)]
+    x0 = wl.bits_to_torch(wl.f32_to_bf16_bits(rng.standard_normal((M, dims[0])).astype(np.float32)), DEV)
+    for i in range(len(Ws)):
+        assert tg.tile_gemm_query_plan(M, dims[i + 1], dims[i])["config"] == 5
+
+    def chain(sync):
+        xs = [x0] + [torch.empty((M, dims[i + 1]), dtype=torch.bfloat16, device=DEV) for i in range(len(Ws))]
+        for i in range(len(Ws)):
+            tg.tile_gemm(xs[i], Ws[i], xs[i + 1], static_b=static_b)
+            if sync:
+                torch.cuda.synchronize()
+        torch.cuda.synchronize()
+        return xs
+
+    want = chain(True)
+    for i in range(len(Ws)):
+        ref, S = oracle.gemm(wl.torch_to_bits(want[i]), wl.torch_to_bits(Ws[i]))
+        check_close(want[i + 1].float().cpu().numpy(), ref, S, dims[i], "bf16", f"skinny chain link {i}")
+    for rep in range(10):
+        got = chain(False)
+        for i in range(len(Ws) + 1):
+            assert torch.equal(got[i].view(torch.int16), want[i].view(torch.int16)), f"rep {rep} link {i}"
+
+
+def test_skinny_completes_next_to_a_kernel_that_holds_sms():
+    """The plan sizes the clusters for an empty device; with 100 SMs held by another kernel they arrive in waves
+    instead.  A slice only ever waits for the CTAs of its own cluster (which start together), so the launch still
+    completes, with the same bits."""
+    M, K, N = 8, 5120, 8192
+    a, b = wl.make_inputs_custom(M, N, K, "int4", seed=78)
+    ref, _ = oracle.gemm(a, b)
+    A, W = wl.bits_to_torch(a, DEV), wl.bits_to_torch(b, DEV)
+    assert tg.tile_gemm_query_plan(M, N, K)["split"] >= 2
+    blocker, worker = torch.cuda.Stream(), torch.cuda.Stream()
+    C = torch.full((M, N), float("nan"), dtype=torch.float32, device=DEV)
+    torch.cuda.synchronize()
+    tg.tile_gemm_debug_occupy(100, 20_000_000, stream=blocker)
+    for _ in range(3):
+        tg.tile_gemm(A, W, C, stream=worker, static_b=True)
+    worker.synchronize()
+    blocker.synchronize()
+    check_bit_exact(C.cpu().numpy(), ref, "skinny M next to a blocker")
+
+
 def test_skinny_32_row_box_for_few_rows_gives_the_same_bits():
     """The rows past M are TMA zero fill: a 32-row activation box (N = 32 of the MMA) on M = 8 changes nothing."""
     a, b = wl.make_inputs_custom(8, 1537 + 7, 2048, sigma_b=0.02, seed=76)
