@@ -458,7 +458,9 @@ GemmConfig choose_config(int64_t M, int64_t N, int64_t K, int sms) {
     if (t4 >= sms / 2 &&
         launch_us(M, N, K, 256, 512, 2, sms) + exposed4 <= launch_us(M, N, K, 256, 256, 2, sms) * 1.06)
         return kConfigs[4];
-    if (t3 >= sms / 2) return kConfigs[3];
+    // from four fifths of a wave of CTA pairs on, 256x256 pair tiles beat 128x256 single-CTA tiles (same-process A/B:
+    // 2048^3 980 vs 947 TF/s, 2048 x 2048 x 8192 1183 vs 1116, 1536 x 3072 x 2048 1036 vs 1013; level at K <= 1024)
+    if (t3 * 5 >= (int64_t)(sms / 2) * 4) return kConfigs[3];
     const int64_t t2 = ((M + 127) / 128) * ((N + 255) / 256);
     if (t2 * 4 >= (int64_t)sms * 3) return kConfigs[2];
     return kConfigs[1];

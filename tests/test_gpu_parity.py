@@ -717,6 +717,8 @@ def test_selector_plans_for_the_benchmarked_shapes():
     assert p["split"] * p["k_tiles_per_slice"] >= 400 > (p["split"] - 1) * p["k_tiles_per_slice"]
     p = plan(32768, 32768, 32768)
     assert p["lockstep_rounds"] >= 100 and p["lockstep_window"] == 32
+    assert plan(2048, 2048, 2048)["config"] == 3      # 64 pair tiles on 74 pairs: 256x256 pair tiles, not 128x256 single-CTA ones
+    assert plan(1536, 1536, 2048)["config"] == 1      # 36 pair tiles or 72 of 128x256: too few, 144 single-CTA tiles of 128x128
     p = plan(1024, 1024, 1024)            # below one wave but a short K loop: not cut
     assert p["split"] == 0 and p["a_box_rows"] == 128
     for M in (2, 8, 16):                  # skinny M: the weight-streaming kernel, K-sliced over clusters; A box only as tall as M needs
