@@ -394,7 +394,7 @@ def bench_launch_overhead(tg, torch, n_ops=1000, elems=2048):
 
 def bench_skinny(tg, wl, torch, ms_list, tdist, layers=8):
     """skinny M (decode with a few tokens in flight) on the four Qwen3-32B weight shapes:
-    the weight-streaming tensor-core kernel for M <= 32, the tiled GEMM with K slices above.  Weights are
+    the weight-streaming tensor-core kernel up to M = 48 (and M <= 64 on unsliced weights), else the tiled GEMM with K slices.  Weights are
     immutable (tile_gemm_static_b, as in the M = 1 leg).  HBM-bound: reported as GB/s of algorithmic bytes
     (weights once + activations + outputs), `layers` distinct weight sets; `per_shape_gbs` times each of
     the four shapes in a chain of its own (qkv, attn_out, gate_up, down)."""

@@ -85,7 +85,7 @@ extern "C" {
 /* execution paths (what the selector returns / what force_path accepts) */
 #define TILE_GEMM_PATH_AUTO 0         /* force_path only                                      */
 #define TILE_GEMM_PATH_GEMM_TMA 1     /* tcgen05 GEMM, A and B read in place through TMA: the tiled
-                                         persistent kernel, or for 2 <= M <= 32 the weight-streaming
+                                         persistent kernel, or for 2 <= M <= 64 the weight-streaming
                                          one (csrc/skinny_kernel.cuh); tile_gemm_query_plan says which */
 #define TILE_GEMM_PATH_GEMM_REPACK 2  /* same kernel after copying A and/or B to aligned rows */
 #define TILE_GEMM_PATH_GEMV 3         /* M == 1 (any alignment): HBM-bound weight-streaming kernel on
@@ -115,7 +115,7 @@ int tile_gemm_ex(const void* A, const void* B, void* C,
 /*
  * tile_gemm plus one promise from the caller: B holds weights -- no work that is
  * still in flight when this call's kernel starts (earlier in `stream` or on any
- * other stream) writes B.  The weight-streaming kernels (M == 1, and 2 <= M <= 32
+ * other stream) writes B.  The weight-streaming kernels (M == 1, and 2 <= M <= 64
  * with TMA-addressable operands) are launched with programmatic dependent launch
  * in either entry; with this promise they stream weight tiles
  * ahead of the wait on the previous kernel of the stream, so back-to-back
@@ -290,7 +290,7 @@ int tile_gemm_query_config(int64_t M, int64_t N, int64_t K, int out_dtype, int32
  * What the selector does with a GEMM shape (M >= 2, operands assumed TMA-addressable)
  * beyond the tile configuration:
  * out[0] = config id (1..4: the tiled kernel's configurations; 5: the weight-streaming
- * tensor-core kernel of 2 <= M <= 32, one CTA per 128 columns and K slice),
+ * tensor-core kernel of 2 <= M <= 64, one CTA per 128 columns and K slice),
  * out[1] = CTAs launched, out[2] = work units that are whole
  * tiles, out[3] = K slices per tile of the last, partial wave (config 5: per column
  * block; 0 = not cut), out[4] = k-tiles (of 64) per slice, out[5] = rounds the lockstep
@@ -352,10 +352,10 @@ int tile_gemm_debug_trace(unsigned long long* records, int64_t capacity);
  *          wait (tile_gemm_static_b only): n >= 1 means n - 1 tiles; automatic = 2.
  *   key 10 automatic cluster size of the weight-streaming kernels: per cent of the occupancy
  *          calculator's resident-cluster figure that the column blocks may fill; automatic = 88
- *          (M = 1) and 92 (2 <= M <= 32).
- *   key 11 weight-streaming tensor-core kernel of 2 <= M <= 32: bits 0-3: 1 = never (the tiled
+ *          (M = 1) and 92 (2 <= M <= 64).
+ *   key 11 weight-streaming tensor-core kernel of 2 <= M <= 64: bits 0-3: 1 = never (the tiled
  *          kernel takes every GEMM shape), 2 = wherever it can run; bits 8-15 = K slices per
- *          column block (1..8); bits 16-23 = 32: a 32-row activation box even for M <= 16.
+ *          column block (1..8); bits 16-23 = 32 or 64: an activation box of that many rows even for fewer.
  *   key 12 config 4 with clusters of two CTA pairs that share each B stage through TMA multicast
  *          (csrc/gemm_kernel.cuh, MC = 1): 1 = never, 2 = whenever the shape has two tile rows and
  *          runs on config 4; automatic = never (measured slower on this part: clusters of four

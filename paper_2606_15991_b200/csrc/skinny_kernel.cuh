@@ -1,4 +1,4 @@
-// skinny_tc_kernel: C = A * B for a FEW activation rows (M <= 32, "decode with some tokens in flight",
+// skinny_tc_kernel: C = A * B for a FEW activation rows (M <= 64, "decode with some tokens in flight",
 // SURVEY.md 8(f)2) -- a weight stream like the M = 1 kernel, with the arithmetic on the tensor cores.
 //
 // Same definition as everywhere: C[m][j] = sum_k A[m][k] * B[k][j], fp32
@@ -12,7 +12,7 @@
 //                                                             row-major K x N needs no transpose)
 //                                                  MMA "B" = the activations   (a_rows m x 16 k, K-major)
 //
-// so the tensor-core work is proportional to a_rows = 16 or 32 (M rounded up; the rows past M are
+// so the tensor-core work is proportional to a_rows = 16, 32 or 64 (M rounded up; the rows past M are
 // TMA zero fill), the accumulator is 128 TMEM lanes (n) x a_rows columns (m), and all four epilogue
 // warps hold live data.  Bounds: none in the K loop -- the N, K and M tails arrive as
 // zeros and the stores are clipped at (M, N).
@@ -35,14 +35,14 @@ constexpr int SKINNY_BK = 64;             // k rows per ring stage: one 128-byte
 constexpr int SKINNY_COLS = 128;          // weight columns per CTA = M of the MMA
 constexpr int SKINNY_GROUPS = 4;          // hand-over granularity: 32 columns
 constexpr int SKINNY_MAX_CLUSTER = 8;     // portable cluster size
-constexpr int SKINNY_MAX_ROWS = 32;
+constexpr int SKINNY_MAX_ROWS = 64;
 
 struct SkinnyParams {
     void* C;
     int64_t ldc;          // elements
     int32_t M, N, K;
     int32_t k_tiles;      // ceil(K / 64), >= gridDim.y
-    int32_t a_rows;       // 16 or 32: rows of the activation box = N of the MMA
+    int32_t a_rows;       // 16, 32 or 64: rows of the activation box = N of the MMA
     int32_t out_kind;     // 0: fp32, 1: bf16, 2: f16
     int32_t in_f16;
     int32_t flags;        // GEMV_FLAG_B_IMMUTABLE
@@ -112,7 +112,7 @@ skinny_tc_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_consta
     const uint32_t acc_bar = bar_base + 2 * STAGES * 8u;            // all MMAs of this CTA have completed
     const uint32_t recv_bar = acc_bar + 8u;                         // every partial sum this CTA combines has arrived
     volatile uint32_t* tmem_ptr_gen = reinterpret_cast<volatile uint32_t*>(smem_gen + L::bar_off(a_rows) + L::NUM_BARS * 8);
-    constexpr uint32_t TMEM_COLS = 32;                              // >= a_rows, the smallest allocation
+    const uint32_t TMEM_COLS = a_rows <= 32 ? 32u : 64u;            // >= a_rows, a power of two, 32 the smallest allocation
 
     // this slice's k-tiles: slice, slice + S, ...
     const int n_my = p.k_tiles > slice ? (p.k_tiles - slice + S - 1) / S : 0;

@@ -682,20 +682,23 @@ int setup_lockstep(GemmLaunch& gl, int dev, cudaStream_t s) {
 }
 
 // ------------------------------------------------------------------ skinny M: weight stream on the tensor cores
-// skinny_tc_kernel (skinny_kernel.cuh): 128 weight columns per CTA, a four-stage ring, two CTAs per SM.
+// skinny_tc_kernel (skinny_kernel.cuh): 128 weight columns per CTA, a three- or four-stage ring, two CTAs per SM.
 // Measured on B200 against the 256-column and the deeper-ring variants, and against the
-// tiled GEMM: it wins for M <= 32 on every decode shape; from M = 33 on the 128x128 tiles are level or ahead.
-constexpr int kSkinnyStages = 4;
+// tiled GEMM: it wins up to M = 48 on the decode shapes, and up to M = 64 where the column blocks run unsliced.
 constexpr int kSkinnyClusterMarginPct = 92, kSkinnyMinKTilesPerSlice = 4, kSkinnyL2PostTiles = 2;
-using SkinnyL = tg::SkinnySmem<kSkinnyStages>;
-// Two CTAs per SM by shared memory (<= 109 KB each).  The occupancy calculator is no help here: for a
+// Two CTAs per SM by shared memory (<= 112 KB each): a four-stage ring up to 32 activation rows, three stages for 33..64
+// (8 KB of activations per stage, and up to 32 KB of hand-over buffer).  The occupancy calculator is no help here: for a
 // kernel that allocates tensor memory it answers one CTA per SM (it cannot know how many columns), while
-// the hardware co-schedules two (32 of 512 columns each; ncu: launch__occupancy_limit_shared_mem = 2).  How
+// the hardware co-schedules two (32 or 64 of 512 columns each; ncu: launch__occupancy_limit_shared_mem = 2).  How
 // many CLUSTERS fit is a property of the GPC layout at two CTAs per SM, which the M = 1 kernel -- same
 // occupancy, no tensor memory -- gets from the calculator: gemv_cluster_capacity.
 constexpr int kSkinnyCtasPerSm = 2;
-static_assert(2 * (SkinnyL::total(tg::SKINNY_MAX_ROWS, tg::SKINNY_MAX_CLUSTER, tg::SKINNY_MAX_ROWS) + 1024) <= 228 * 1024,
-              "two skinny CTAs (and their 1 KB reserve each) must fit one SM's shared memory");
+constexpr uint32_t kSkinnySmemLimit = (228 * 1024) / 2 - 1024;   // per CTA at two per SM, less the 1 KB the driver reserves
+inline int skinny_stages(int a_rows) { return a_rows <= 32 ? 4 : 3; }
+inline uint32_t skinny_smem(int a_rows, int S, int mp) {
+    return a_rows <= 32 ? tg::SkinnySmem<4>::total(a_rows, S, mp) : tg::SkinnySmem<3>::total(a_rows, S, mp);
+}
+static_assert(tg::SkinnySmem<4>::total(32, tg::SKINNY_MAX_CLUSTER, 32) <= kSkinnySmemLimit, "two skinny CTAs must fit one SM's shared memory");
 int gemv_cluster_capacity(int cs, int dev, int sms);
 
 struct SkinnyPlan {
@@ -710,10 +713,11 @@ struct SkinnyPlan {
 // where a whole cluster's worth of slots is free (the M = 1 kernel's rule).
 SkinnyPlan plan_skinny(int64_t M, int64_t N, int64_t K, int dev, int sms) {
     SkinnyPlan sp;
-    sp.a_rows = M <= 16 ? 16 : 32;
+    sp.a_rows = M <= 16 ? 16 : M <= 32 ? 32 : 64;
     const int tune = g_tune[11].load();
     const int want_split = (tune >> 8) & 255, want_rows = (tune >> 16) & 255;
-    if (want_rows == 32) sp.a_rows = 32;
+    if ((want_rows == 32 || want_rows == 64) && want_rows > sp.a_rows) sp.a_rows = want_rows;
+    const int mp = (int)((M + 3) & ~int64_t(3));
     const int64_t k_tiles = (K + tg::SKINNY_BK - 1) / tg::SKINNY_BK;
     const int64_t cb = (N + tg::SKINNY_COLS - 1) / tg::SKINNY_COLS;
     const int64_t slots1 = (int64_t)sms * kSkinnyCtasPerSm;
@@ -722,17 +726,21 @@ SkinnyPlan plan_skinny(int64_t M, int64_t N, int64_t K, int dev, int sms) {
     sp.split = 1;
     int margin = g_tune[10].load();
     if (margin <= 0) margin = kSkinnyClusterMarginPct;
-    // 17..32 rows on weights wide enough to fill the CTA slots unsliced: the 128x128 tiles of the GEMM kernel re-read
-    // the activations less often and are ahead (measured on K = 5120, N = 51200: 6.45 vs 6.23 TB/s)
-    if (sp.a_rows == 32 && want_split == 0 && (tune & 15) != 2 && cb * 100 > slots1 * margin) return sp;
+    // Where the 128x128 tiles of the GEMM kernel are level or ahead (measured on the decode shapes; tuning
+    // key 11 mode 2 overrides): 17..32 rows on weights wide enough to fill the CTA slots unsliced (K = 5120, N = 51200:
+    // 6.45 vs 6.23 TB/s), and 49..64 rows on weights that have to be sliced (within +-3 %).
+    const bool unsliced = cb * 100 > slots1 * margin;
+    if (want_split == 0 && (tune & 15) != 2 && ((sp.a_rows == 32 && unsliced) || (M > 48 && !unsliced))) return sp;
     sp.ok = true;
     if (want_split > 0) {
         sp.split = (int)(want_split < k_tiles ? want_split : k_tiles);
         if (sp.split > tg::SKINNY_MAX_CLUSTER) sp.split = tg::SKINNY_MAX_CLUSTER;
+        while (sp.split > 1 && skinny_smem(sp.a_rows, sp.split, mp) > kSkinnySmemLimit) --sp.split;
         return sp;
     }
     for (int64_t cs = tg::SKINNY_MAX_CLUSTER; cs >= 2; --cs) {
         if (cs > k_tiles || k_tiles / cs < kSkinnyMinKTilesPerSlice) continue;
+        if (skinny_smem(sp.a_rows, (int)cs, mp) > kSkinnySmemLimit) continue;   // the hand-over buffer of 33..64 rows: up to 5 slices
         if (cb * cs * 100 > slots1 * margin) continue;
         if (cb * 100 > (int64_t)gemv_cluster_capacity((int)cs, dev, sms) * margin) continue;
         sp.split = (int)cs;
@@ -760,8 +768,7 @@ int run_skinny(const void* A, const void* B, void* C, int64_t M, int64_t N, int6
     if (rc) return rc;
     rc = get_tensor_map(&tx, A, 2, false, (uint64_t)K, (uint64_t)M, (uint64_t)lda * 2, 64u, (uint32_t)sp.a_rows, 128);
     if (rc) return rc;
-    auto kern = tg::skinny_tc_kernel<kSkinnyStages>;
-    const int smem = (int)SkinnyL::total(sp.a_rows, sp.split, (int)((M + 3) & ~int64_t(3)));
+    const int smem = (int)skinny_smem(sp.a_rows, sp.split, (int)((M + 3) & ~int64_t(3)));
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof cfg);
     cfg.gridDim = dim3((unsigned)sp.col_blocks, (unsigned)sp.split, 1);
@@ -786,11 +793,12 @@ int run_skinny(const void* A, const void* B, void* C, int64_t M, int64_t N, int6
     cfg.numAttrs = na;
     static bool configured[64] = {};
     if (!configured[dev]) {
-        CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)SkinnyL::total(tg::SKINNY_MAX_ROWS, tg::SKINNY_MAX_CLUSTER, tg::SKINNY_MAX_ROWS)));
+        CUDA_TRY(cudaFuncSetAttribute(tg::skinny_tc_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSkinnySmemLimit));
+        CUDA_TRY(cudaFuncSetAttribute(tg::skinny_tc_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSkinnySmemLimit));
         configured[dev] = true;
     }
-    CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, tw, tx, p));
+    if (skinny_stages(sp.a_rows) == 4) CUDA_TRY(cudaLaunchKernelEx(&cfg, tg::skinny_tc_kernel<4>, tw, tx, p));
+    else CUDA_TRY(cudaLaunchKernelEx(&cfg, tg::skinny_tc_kernel<3>, tw, tx, p));
     g_launches.fetch_add(1);
     return TILE_GEMM_OK;
 }

@@ -730,16 +730,18 @@ def test_selector_plans_for_the_benchmarked_shapes():
         p = plan(M, 51200, 5120)
         assert p["config"] == 5 and p["split"] == 0 and p["ctas"] == 400
     assert plan(32, 51200, 5120)["config"] == 1       # 17..32 rows on wide weights: the 128x128 tiles are ahead (measured)
-    for M in (40, 64):                    # from M = 33 on: the tiled kernel, K-sliced below one wave, A box as tall as M needs
-        p = plan(M, 5120, 25600)
-        assert p["config"] == 1 and p["full_units"] == 0 and p["split"] >= 2 and p["a_box_rows"] == 64 and p["ctas"] >= 100
-    for M in (64, 128):                   # one row of 128-tall tiles: never a CTA pair, 128x128 tiles on every SM
-        p = plan(M, 51200, 5120)
-        assert p["config"] == 1 and p["ctas"] == 148
+    p = plan(40, 5120, 25600)             # 33..48 rows: still the weight-streaming kernel (three-stage ring, 64-row box)
+    assert p["config"] == 5 and p["split"] >= 4 and p["a_box_rows"] == 64
+    p = plan(64, 5120, 25600)             # 49..64 rows on weights that must be sliced: the tiled kernel, K-sliced below one wave
+    assert p["config"] == 1 and p["full_units"] == 0 and p["split"] >= 2 and p["a_box_rows"] == 64 and p["ctas"] >= 100
+    p = plan(64, 51200, 5120)             # ... on weights that run unsliced: the weight-streaming kernel
+    assert p["config"] == 5 and p["split"] == 0 and p["ctas"] == 400
+    p = plan(128, 51200, 5120)            # one row of 128-tall tiles: never a CTA pair, 128x128 tiles on every SM
+    assert p["config"] == 1 and p["ctas"] == 148
     assert plan(129, 51200, 5120)["config"] in (3, 4)
 
 
-# ------------------------------------------------------------------ 2 <= M <= 32: the weight-streaming tensor-core kernel
+# ------------------------------------------------------------------ 2 <= M <= 64: the weight-streaming tensor-core kernel
 SKINNY_SHAPES = (((776, 1537), (0, 7, 3)), ((5120, 10240), (0, 0, 0)), ((64, 8), (8, 8, 0)), ((4104, 520), (8, 0, 8)),
                  ((1030, 130), (0, 6, 1)))
 
@@ -748,7 +750,7 @@ def _skinny_tune(mode=0, split=0, rows=0):
     tg.tile_gemm_set_tuning(tg.TUNE_SKINNY, mode | (split << 8) | (rows << 16))
 
 
-@pytest.mark.parametrize("M", [2, 3, 4, 5, 8, 13, 16, 17, 31, 32])
+@pytest.mark.parametrize("M", [2, 3, 4, 5, 8, 13, 16, 17, 31, 32, 33, 48, 57, 64])
 @pytest.mark.parametrize("split", [0, 1, 2, 3, 5, 7, 8])
 def test_skinny_integer_bit_exact_and_canary(M, split):
     """Every cluster size of the split-K reduce-scatter (1 = no cluster; 3, 5, 7: groups unevenly owned; 5..8: slices
@@ -764,7 +766,7 @@ def test_skinny_integer_bit_exact_and_canary(M, split):
         check_bit_exact(got.astype(np.float32), ref, f"skinny M={M} K={K} N={N} split={split}")
 
 
-@pytest.mark.parametrize("M", [2, 8, 24, 32])
+@pytest.mark.parametrize("M", [2, 8, 24, 32, 48])
 @pytest.mark.parametrize("out", ["f32", "bf16"])
 def test_skinny_normal_inputs_reproducible_and_agrees_with_the_tiled_gemm(M, out):
     K, N = 5120, 8192
@@ -783,7 +785,7 @@ def test_skinny_normal_inputs_reproducible_and_agrees_with_the_tiled_gemm(M, out
     check_close(tiled, ref, S, K, out, f"tiled M={M} {out}")
 
 
-@pytest.mark.parametrize("M", [3, 8, 24])
+@pytest.mark.parametrize("M", [3, 8, 24, 40])
 @pytest.mark.parametrize("static_b", [False, True])
 def test_skinny_chain_is_stream_ordered_under_pdl(M, static_b):
     """C of one skinny-M GEMM is A of the next, launched back to back with programmatic dependent launch (weights
