@@ -694,16 +694,19 @@ constexpr int kSkinnyClusterMarginPct = 92, kSkinnyMinKTilesPerSlice = 4, kSkinn
 // occupancy, no tensor memory -- gets from the calculator: gemv_cluster_capacity.
 constexpr int kSkinnyCtasPerSm = 2;
 constexpr uint32_t kSkinnySmemLimit = (228 * 1024) / 2 - 1024;   // per CTA at two per SM, less the 1 KB the driver reserves
-inline int skinny_stages(int a_rows) { return a_rows <= 32 ? 4 : 3; }
-inline uint32_t skinny_smem(int a_rows, int S, int mp) {
-    return a_rows <= 32 ? tg::SkinnySmem<4>::total(a_rows, S, mp) : tg::SkinnySmem<3>::total(a_rows, S, mp);
+// Ring depth: four stages, three where that buys a CTA -- 33..64 rows (two CTAs per SM at all), and 17..32 rows on column
+// blocks that run unsliced (61 KB: THREE CTAs per SM, so that e.g. the 400 column blocks of N = 51200 are one wave of the
+// 444 slots instead of 1.35 waves of 296; measured at M = 32: 6.18 vs 5.52 TB/s, tiled GEMM 5.90).
+inline int skinny_stages(int a_rows, bool unsliced) { return a_rows <= 16 ? 4 : a_rows == 32 ? (unsliced ? 3 : 4) : 3; }
+inline uint32_t skinny_smem(int stages, int a_rows, int S, int mp) {
+    return stages == 4 ? tg::SkinnySmem<4>::total(a_rows, S, mp) : tg::SkinnySmem<3>::total(a_rows, S, mp);
 }
 static_assert(tg::SkinnySmem<4>::total(32, tg::SKINNY_MAX_CLUSTER, 32) <= kSkinnySmemLimit, "two skinny CTAs must fit one SM's shared memory");
 int gemv_cluster_capacity(int cs, int dev, int sms);
 
 struct SkinnyPlan {
     bool ok = false;   // false: the tiled GEMM takes the shape
-    int split = 1, col_blocks = 0, a_rows = 16;
+    int split = 1, col_blocks = 0, a_rows = 16, stages = 4;
 };
 
 // K slices of a skinny launch (tuning key 11 bits 8-15 force them).  Column blocks that fill the CTA slots
@@ -727,20 +730,20 @@ SkinnyPlan plan_skinny(int64_t M, int64_t N, int64_t K, int dev, int sms) {
     int margin = g_tune[10].load();
     if (margin <= 0) margin = kSkinnyClusterMarginPct;
     // Where the 128x128 tiles of the GEMM kernel are level or ahead (measured on the decode shapes; tuning
-    // key 11 mode 2 overrides): 17..32 rows on weights wide enough to fill the CTA slots unsliced (K = 5120, N = 51200:
-    // 6.45 vs 6.23 TB/s), and 49..64 rows on weights that have to be sliced (within +-3 %).
+    // key 11 mode 2 overrides): 49..64 rows on weights that have to be sliced (within +-3 %).
     const bool unsliced = cb * 100 > slots1 * margin;
-    if (want_split == 0 && (tune & 15) != 2 && ((sp.a_rows == 32 && unsliced) || (M > 48 && !unsliced))) return sp;
+    if (want_split == 0 && (tune & 15) != 2 && M > 48 && !unsliced) return sp;
     sp.ok = true;
+    sp.stages = skinny_stages(sp.a_rows, unsliced && want_split <= 1);
     if (want_split > 0) {
         sp.split = (int)(want_split < k_tiles ? want_split : k_tiles);
         if (sp.split > tg::SKINNY_MAX_CLUSTER) sp.split = tg::SKINNY_MAX_CLUSTER;
-        while (sp.split > 1 && skinny_smem(sp.a_rows, sp.split, mp) > kSkinnySmemLimit) --sp.split;
+        while (sp.split > 1 && skinny_smem(sp.stages, sp.a_rows, sp.split, mp) > kSkinnySmemLimit) --sp.split;
         return sp;
     }
     for (int64_t cs = tg::SKINNY_MAX_CLUSTER; cs >= 2; --cs) {
         if (cs > k_tiles || k_tiles / cs < kSkinnyMinKTilesPerSlice) continue;
-        if (skinny_smem(sp.a_rows, (int)cs, mp) > kSkinnySmemLimit) continue;   // the hand-over buffer of 33..64 rows: up to 5 slices
+        if (skinny_smem(sp.stages, sp.a_rows, (int)cs, mp) > kSkinnySmemLimit) continue;   // the hand-over buffer of 33..64 rows: up to 5 slices
         if (cb * cs * 100 > slots1 * margin) continue;
         if (cb * 100 > (int64_t)gemv_cluster_capacity((int)cs, dev, sms) * margin) continue;
         sp.split = (int)cs;
@@ -768,7 +771,7 @@ int run_skinny(const void* A, const void* B, void* C, int64_t M, int64_t N, int6
     if (rc) return rc;
     rc = get_tensor_map(&tx, A, 2, false, (uint64_t)K, (uint64_t)M, (uint64_t)lda * 2, 64u, (uint32_t)sp.a_rows, 128);
     if (rc) return rc;
-    const int smem = (int)skinny_smem(sp.a_rows, sp.split, (int)((M + 3) & ~int64_t(3)));
+    const int smem = (int)skinny_smem(sp.stages, sp.a_rows, sp.split, (int)((M + 3) & ~int64_t(3)));
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof cfg);
     cfg.gridDim = dim3((unsigned)sp.col_blocks, (unsigned)sp.split, 1);
@@ -797,7 +800,7 @@ int run_skinny(const void* A, const void* B, void* C, int64_t M, int64_t N, int6
         CUDA_TRY(cudaFuncSetAttribute(tg::skinny_tc_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSkinnySmemLimit));
         configured[dev] = true;
     }
-    if (skinny_stages(sp.a_rows) == 4) CUDA_TRY(cudaLaunchKernelEx(&cfg, tg::skinny_tc_kernel<4>, tw, tx, p));
+    if (sp.stages == 4) CUDA_TRY(cudaLaunchKernelEx(&cfg, tg::skinny_tc_kernel<4>, tw, tx, p));
     else CUDA_TRY(cudaLaunchKernelEx(&cfg, tg::skinny_tc_kernel<3>, tw, tx, p));
     g_launches.fetch_add(1);
     return TILE_GEMM_OK;

@@ -729,7 +729,8 @@ def test_selector_plans_for_the_benchmarked_shapes():
     for M in (8, 16):                     # column blocks that fill the CTA slots run unsliced
         p = plan(M, 51200, 5120)
         assert p["config"] == 5 and p["split"] == 0 and p["ctas"] == 400
-    assert plan(32, 51200, 5120)["config"] == 1       # 17..32 rows on wide weights: the 128x128 tiles are ahead (measured)
+    p = plan(32, 51200, 5120)             # 17..32 rows unsliced: a three-stage ring, three CTAs per SM, one wave
+    assert p["config"] == 5 and p["split"] == 0 and p["ctas"] == 400 and p["a_box_rows"] == 32
     p = plan(40, 5120, 25600)             # 33..48 rows: still the weight-streaming kernel (three-stage ring, 64-row box)
     assert p["config"] == 5 and p["split"] >= 4 and p["a_box_rows"] == 64
     p = plan(64, 5120, 25600)             # 49..64 rows on weights that must be sliced: the tiled kernel, K-sliced below one wave
@@ -837,6 +838,23 @@ def test_skinny_completes_next_to_a_kernel_that_holds_sms():
     worker.synchronize()
     blocker.synchronize()
     check_bit_exact(C.cpu().numpy(), ref, "skinny M next to a blocker")
+
+
+@pytest.mark.parametrize("M", [8, 24, 32, 64])
+def test_skinny_unsliced_wide_weights(M):
+    """Column blocks that fill the CTA slots run unsliced, in several waves or (17..32 rows: three-stage ring) three
+    CTAs per SM: a ragged N just above 36864, integer inputs exact, canary intact."""
+    N, K = 36864 + 72, 328
+    p = tg.tile_gemm_query_plan(M, N, K)
+    assert p["config"] == 5 and p["split"] == 0 and p["ctas"] == 289
+    a, b = wl.make_inputs_custom(M, N, K, dist="int4", seed=79 + M)
+    ref, _ = oracle.gemm(a, b)
+    for out in ("f32", "bf16"):
+        got = run_case(a, b, out, pads=(0, 8, 8), what=f"skinny unsliced M={M}", static_b=True)
+        if out == "f32":
+            check_bit_exact(got.astype(np.float32), ref, f"skinny unsliced M={M}")
+        else:
+            assert np.array_equal(got, rne_bf16(ref))
 
 
 def test_skinny_32_row_box_for_few_rows_gives_the_same_bits():
