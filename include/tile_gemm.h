@@ -355,7 +355,8 @@ int tile_gemm_debug_trace(unsigned long long* records, int64_t capacity);
  *          (M = 1) and 92 (2 <= M <= 64).
  *   key 11 weight-streaming tensor-core kernel of 2 <= M <= 64: bits 0-3: 1 = never (the tiled
  *          kernel takes every GEMM shape), 2 = wherever it can run; bits 8-15 = K slices per
- *          column block (1..8); bits 16-23 = 32 or 64: an activation box of that many rows even for fewer.
+ *          column block (1..8); bits 16-23 = 32 or 64: an activation box of that many rows even for fewer;
+ *          bits 24-27 = 3 or 4: ring stages (4 only up to 32 rows).
  *   key 12 config 4 with clusters of two CTA pairs that share each B stage through TMA multicast
  *          (csrc/gemm_kernel.cuh, MC = 1): 1 = never, 2 = whenever the shape has two tile rows and
  *          runs on config 4; automatic = never (measured slower on this part: clusters of four

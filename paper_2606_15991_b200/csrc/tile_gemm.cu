@@ -735,6 +735,7 @@ SkinnyPlan plan_skinny(int64_t M, int64_t N, int64_t K, int dev, int sms) {
     if (want_split == 0 && (tune & 15) != 2 && M > 48 && !unsliced) return sp;
     sp.ok = true;
     sp.stages = skinny_stages(sp.a_rows, unsliced && want_split <= 1);
+    if (((tune >> 24) & 15) == 3 || (((tune >> 24) & 15) == 4 && sp.a_rows <= 32)) sp.stages = (tune >> 24) & 15;   // key 11 bits 24-27
     if (want_split > 0) {
         sp.split = (int)(want_split < k_tiles ? want_split : k_tiles);
         if (sp.split > tg::SKINNY_MAX_CLUSTER) sp.split = tg::SKINNY_MAX_CLUSTER;
