@@ -114,6 +114,10 @@ skinny_tc_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_consta
     volatile uint32_t* tmem_ptr_gen = reinterpret_cast<volatile uint32_t*>(smem_gen + L::bar_off(a_rows) + L::NUM_BARS * 8);
     const uint32_t TMEM_COLS = a_rows <= 32 ? 32u : 64u;            // >= a_rows, a power of two, 32 the smallest allocation
 
+    // the next kernel of the stream may be scheduled as soon as slots free up: everything of ours that it could
+    // disturb sits behind its own griddepcontrol.wait
+    griddep_launch_dependents();
+
     // this slice's k-tiles: slice, slice + S, ...
     const int n_my = p.k_tiles > slice ? (p.k_tiles - slice + S - 1) / S : 0;
 
@@ -151,7 +155,6 @@ skinny_tc_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_consta
     tc_fence_after();
     const uint32_t tmem_base = *tmem_ptr_gen;
     if (S > 1) cluster_arrive();   // "my barriers exist"; the matching wait sits in front of the first remote access
-    griddep_launch_dependents();
 
     if (warp == 4) {
         // ===== TMA producer: per k-tile two weight boxes (64 columns x 64 k, 128B-swizzled) and the
@@ -235,7 +238,7 @@ skinny_tc_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_consta
             mbar_arrive_expect_tx(recv_bar, (uint32_t)owned * (uint32_t)(S - 1) * (uint32_t)mp * 128u);
         }
         griddep_wait();   // C may still be in the previous kernel's use
-        mbar_wait_sleep(acc_bar, 0);
+        mbar_wait(acc_bar, 0);
         tc_fence_after();
         const uint32_t t_lane = tmem_base + ((warp * 32u) << 16);
         uint32_t v[16];
