@@ -238,6 +238,7 @@ skinny_tc_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_consta
             mbar_arrive_expect_tx(recv_bar, (uint32_t)owned * (uint32_t)(S - 1) * (uint32_t)mp * 128u);
         }
         griddep_wait();   // C may still be in the previous kernel's use
+        if (S > 1) cluster_wait();   // every peer's barriers exist (long since: this is off the critical path here)
         mbar_wait(acc_bar, 0);
         tc_fence_after();
         const uint32_t t_lane = tmem_base + ((warp * 32u) << 16);
@@ -252,7 +253,6 @@ skinny_tc_kernel(const __grid_constant__ CUtensorMap tmap_w, const __grid_consta
             }
         } else if (owner != slice) {
             // ---- push this warp's group to its owner: [source][slot][m / 4][lane][4 floats] ----
-            cluster_wait();   // the owner's barrier exists
             const uint32_t rbar = map_to_cta(recv_bar, (uint32_t)owner);
             const int src = slice < owner ? slice : slice - 1;
             const uint32_t dst0 = map_to_cta(recv_base + (uint32_t)((src * slots + slot) * (mp >> 2)) * 512u + lane * 16u, (uint32_t)owner);
