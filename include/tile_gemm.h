@@ -351,8 +351,7 @@ int tile_gemm_debug_trace(unsigned long long* records, int64_t capacity);
  *   key 9  weight tiles the weight-streaming kernels send as far as L2 right behind the dependency
  *          wait (tile_gemm_static_b only): n >= 1 means n - 1 tiles; automatic = 2.
  *   key 10 automatic cluster size of the weight-streaming kernels: per cent of the occupancy
- *          calculator's resident-cluster figure that the column blocks may fill; automatic = 88
- *          (M = 1) and 92 (2 <= M <= 64).
+ *          calculator's resident-cluster figure that the column blocks may fill; automatic = 92.
  *   key 11 weight-streaming tensor-core kernel of 2 <= M <= 64: bits 0-3: 1 = never (the tiled
  *          kernel takes every GEMM shape), 2 = wherever it can run; bits 8-15 = K slices per
  *          column block (1..8); bits 16-23 = 32 or 64: an activation box of that many rows even for fewer;

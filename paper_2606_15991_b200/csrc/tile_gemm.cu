@@ -975,8 +975,10 @@ int gemv_cluster_capacity(int cs, int dev, int sms) {
     return n;
 }
 
-// measured on B200: two units into L2 behind the dependency wait; clusters sized to 88 % of capacity
-constexpr int kGemvL2PostUnits = 2, kGemvClusterMarginPct = 88;
+// measured on B200: two units into L2 behind the dependency wait; clusters sized to 92 % of capacity
+// (same-process A/B of 80 / 88 / 92 / 96 / 100 %: 92 and 96 give N = 10240 six slices instead of five, +1.1 %; 100 % makes
+// every other launch of N = 8192 run in two waves, -17 %)
+constexpr int kGemvL2PostUnits = 2, kGemvClusterMarginPct = 92;
 
 // ring shapes of the split kernel: {columns per CTA, rows per stage, stages, CTAs per SM}
 struct GemvShape { int cols, tile_k, stages, occ; };
@@ -1018,7 +1020,7 @@ int run_gemv_split(const void* x, const void* B, void* y, int64_t N, int64_t K, 
     // Fix-up protocol (gemv_kernel.cuh; tuning key 8: 0 auto, 1 tickets, 2 tagged slots else tickets, 3 cluster
     // else tickets).  Cluster: default ring shape, one column block per CTA, S <= 8 -- and when the automatic S is
     // within reach (<= 10) it becomes the largest cluster size whose clusters all fit the device at once with
-    // slots to spare (key 10: per cent of the occupancy calculator's figure, default 88), because clusters of the
+    // slots to spare (key 10: per cent of the occupancy calculator's figure, default 92), because clusters of the
     // next kernel can only start where a whole cluster's worth of slots is free.
     const int fix_mode = g_tune[8].load();
     const bool cluster_ok = (fix_mode == 0 || fix_mode == 3) && shape == 2 && gx == col_blocks;
