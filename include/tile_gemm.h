@@ -77,7 +77,8 @@ extern "C" {
 #define TILE_GEMM_E_PATH 12       /* force_path unknown or not applicable to this shape    */
 #define TILE_GEMM_E_INTERNAL 13
 #define TILE_GEMM_E_IN_DTYPE 14   /* in_dtype is neither BF16 nor F16                       */
-#define TILE_GEMM_NUM_STATUS 15
+#define TILE_GEMM_E_LIMIT 15      /* tile_gemv_no_alloc: the request needs more than its fixed scratch */
+#define TILE_GEMM_NUM_STATUS 16
 
 /* internal flag behind tile_gemm_static_b */
 #define TILE_GEMM_FLAG_B_IMMUTABLE 1u
@@ -218,6 +219,76 @@ int tile_gemm_record_end(void* stream, void** step_out);
 int tile_gemm_replay(void* step, void* stream);
 int64_t tile_gemm_recorded_nodes(void* step);
 int tile_gemm_record_free(void* step);
+
+/*
+ * The M = 1 product  y = x * B  (the decode GEMV) for callers that
+ * must not, or cannot, allocate device memory.
+ *
+ * Why it exists.  tile_gemm keeps a grow-only workspace per stream and gets it from
+ * cudaMalloc the first time a shape needs one.  Some programs cannot afford that
+ * call: an inference server that hands every byte of HBM to its own pool at start-up
+ * (weights, KV cache) leaves nothing for a library's cudaMalloc to find; a plug-in
+ * running under a host whose memory policy forbids allocations after initialisation
+ * has no permission to make it; and a latency-bound decode loop cannot take the
+ * device-wide synchronisation and the unbounded duration that cudaMalloc / cudaFree
+ * bring with them.  For those callers this entry never calls cudaMalloc, cudaFree or
+ * any library routine that allocates device memory: its only scratch -- the fp32
+ * partial sums of the K slices and one arrival ticket per 256-column block -- lives
+ * in ONE array that is part of the library image itself,
+ * TILE_GEMV_NO_ALLOC_SCRATCH_BYTES (1 MiB + 4 KiB) per GPU, present from the moment
+ * a device loads the library until the process exits, whether or not this entry is
+ * ever called.  The caller passes x, B and y exactly as to tile_gemm.
+ *
+ * Operation: y[j] = round_out( sum_{k<K} x[k] * B[k*ldb + j] ), 0 <= j < N; x (K
+ * elements) and B (K x N, row stride ldb elements) hold in_dtype (TILE_GEMM_IN_BF16 /
+ * _F16), y holds out_dtype (TILE_GEMM_OUT_F32 / _BF16 / _F16); all three are DEVICE
+ * pointers on the current device, owned by the caller.  The kernel is the library's
+ * default M = 1 kernel (csrc/gemv_kernel.cuh: TMA ring over 256-column blocks,
+ * interleaved K slices, fp32 FMA) in its ticket hand-over: each slice stores its
+ * partial sums to the scratch array, and the slice that arrives last adds all of
+ * them in slice order and writes y.  The sum order is fixed by (N, K, slice count),
+ * so results are bitwise reproducible from call to call; they equal tile_gemm's bits
+ * when both run the same slice count and otherwise differ only by fp32 summation
+ * order (same tolerance; identical for integer-valued inputs whose sums are exact).
+ *
+ * `split`: 0 = automatic (as many K slices per column block as keep every CTA
+ * resident, at most what the scratch holds); > 0 = that many slices (values above
+ * ceil(K / 64) mean ceil(K / 64)).
+ *
+ * Limits -- a request beyond them fails with TILE_GEMM_E_LIMIT, says which limit, and
+ * enqueues nothing:
+ *   N <= TILE_GEMV_NO_ALLOC_MAX_N (262144 columns = 1024 blocks of 256: one ticket each);
+ *   ceil(N / 256) * slices <= TILE_GEMV_NO_ALLOC_MAX_TILES (1024 tiles of 256 partial sums).
+ * Further preconditions: those of tile_gemm with M = 1 (same codes), plus B 16-byte
+ * aligned with ldb a multiple of 8 (E_PATH otherwise: the repack path would need an
+ * allocated copy), split >= 0 (E_EXTENT).  x and y need only element alignment.
+ * N == 0 is a successful no-op, K == 0 writes zeros.
+ *
+ * Set-up on first use: the first call on each device looks up the device address of
+ * the scratch array (cudaGetSymbolAddress with that device current -- the array's
+ * name is only a host-side handle) and sets the kernel's shared-memory attribute;
+ * the first call for a given (B, N, K, ldb) encodes a TMA descriptor into a host-side
+ * cache.  Make that first call on a device before any stream capture begins.  Later
+ * calls do no set-up.
+ *
+ * Sharing: every call on a device -- whatever the stream or host thread -- uses the
+ * same array.  Each call clears the tickets it is about to use with a memset node
+ * queued on `stream` ahead of the kernel (the array keeps the previous call's
+ * contents; partial sums are always written before they are read) and launches
+ * without programmatic dependent launch, so calls queued on ONE stream are safe back
+ * to back.  Calls whose kernels can overlap on the GPU (different streams without
+ * an ordering between them, or several host threads feeding different streams) RACE
+ * on the scratch and produce wrong results: order them with events or keep them on
+ * one stream.  tile_gemm and the other entries never touch this array and may run
+ * concurrently with it.  Asynchronous on `stream`; tile_gemm_launch_count grows by one
+ * per call (the memset is not counted).
+ */
+#define TILE_GEMV_NO_ALLOC_MAX_N 262144
+#define TILE_GEMV_NO_ALLOC_MAX_TILES 1024
+#define TILE_GEMV_NO_ALLOC_SCRATCH_BYTES 1052672   /* 1024 * 256 * 4 partial sums + 1024 * 4 tickets */
+int tile_gemv_no_alloc(const void* x, const void* B, void* y,
+                       int64_t N, int64_t K, int64_t ldb,
+                       int in_dtype, int out_dtype, int split, void* stream);
 
 /*
  * Read-bandwidth probe of the measurement harness: adds the sum of

@@ -26,13 +26,18 @@ PATH_NAMES = {PATH_AUTO: "auto", PATH_GEMM_TMA: "gemm_tma", PATH_GEMM_REPACK: "g
               PATH_GEMV: "gemv", PATH_ZERO: "zero", PATH_NOOP: "noop"}
 
 (E_OK, E_NULL, E_EXTENT, E_LDA, E_LDB, E_LDC, E_DTYPE, E_ALIGN, E_ALIAS, E_OVERFLOW, E_DEVICE,
- E_CUDA, E_PATH, E_INTERNAL, E_IN_DTYPE) = range(15)
+ E_CUDA, E_PATH, E_INTERNAL, E_IN_DTYPE, E_LIMIT) = range(16)
 
 (TUNE_GEMM_CONFIG, TUNE_GEMM_GROUP_M, TUNE_GEMM_MAX_CTAS, TUNE_GEMV_SPLIT, TUNE_GEMV_VARIANT, TUNE_GEMV_SHAPE, TUNE_FLAGS,
  TUNE_ADD_SHAPE, TUNE_GEMV_FIXUP, TUNE_GEMV_L2_POST, TUNE_GEMV_CLUSTER_MARGIN, TUNE_SKINNY, TUNE_GEMM_MULTICAST) = range(13)
 NUM_TUNE_KEYS = 16
 
+NO_ALLOC_MAX_N = 262144           # TILE_GEMV_NO_ALLOC_MAX_N
+NO_ALLOC_MAX_TILES = 1024         # TILE_GEMV_NO_ALLOC_MAX_TILES
+NO_ALLOC_SCRATCH_BYTES = 1052672  # TILE_GEMV_NO_ALLOC_SCRATCH_BYTES
+
 EXPORTS = ("tile_gemm", "tile_gemm_ex", "tile_gemm_static_b", "tile_gemm_typed", "tile_gemm_swiglu", "tile_add_f32", "tile_read_probe_u32",
+           "tile_gemv_no_alloc",
            "tile_gemm_record_begin", "tile_gemm_record_end", "tile_gemm_replay", "tile_gemm_recorded_nodes",
            "tile_gemm_record_free", "tile_gemm_select", "tile_gemm_host",
            "tile_gemm_debug_owner_map", "tile_gemm_debug_trace", "tile_gemm_debug_occupy", "tile_gemm_query_config", "tile_gemm_query_plan", "tile_gemm_set_tuning",
@@ -85,6 +90,8 @@ def load_library():
     lib.tile_gemm_typed.restype = _int
     lib.tile_gemm_swiglu.argtypes = g + [_vp]
     lib.tile_gemm_swiglu.restype = _int
+    lib.tile_gemv_no_alloc.argtypes = [_vp, _vp, _vp, _i64, _i64, _i64, _int, _int, _int, _vp]
+    lib.tile_gemv_no_alloc.restype = _int
     lib.tile_read_probe_u32.argtypes = [_vp, _i64, _vp, _vp]
     lib.tile_read_probe_u32.restype = _int
     lib.tile_add_f32.argtypes = [_vp, _vp, _vp, _i64, _vp]
@@ -270,6 +277,47 @@ def tile_gemm_swiglu(X: torch.Tensor, Wgu: torch.Tensor, H: torch.Tensor | None 
                                              _ld(X), _ld(Wgu), _ld(H), od, _vp(_stream_handle(stream)))
     _check(st)
     return H
+
+
+def tile_gemv_no_alloc_raw(x: int, B: int, y: int, N, K, ldb, in_dtype, out_dtype, split: int = 0, stream: int = 0) -> int:
+    """Raw pointer form of tile_gemv_no_alloc; returns the status code instead of raising."""
+    return int(load_library().tile_gemv_no_alloc(_vp(x), _vp(B), _vp(y), N, K, ldb, int(in_dtype), int(out_dtype),
+                                                 int(split), _vp(stream)))
+
+
+def tile_gemv_no_alloc(x: torch.Tensor, B: torch.Tensor, y: torch.Tensor, split: int = 0, stream=None) -> torch.Tensor:
+    """y = x @ B for one activation row, through the entry point that allocates no device memory.
+
+    For programs that cannot call cudaMalloc once they are running -- a server whose own pool already
+    holds all of HBM, a host that forbids allocations after start-up, a decode loop that cannot absorb
+    cudaMalloc's device-wide synchronisation.  The kernel's split-K scratch is a fixed array inside the
+    library (NO_ALLOC_SCRATCH_BYTES per GPU, shared by every call on that GPU), so the caller supplies
+    all three tensors, `y` included: this wrapper creates none.
+
+    x: (K,) or (1, K); B: (K, N) row-major with a 16-byte aligned base and a row stride that is a
+    multiple of 8 elements; x and B both bf16 or both f16; y: (N,) or (1, N) float32, bfloat16 or
+    float16.  split = 0 lets the library choose the number of K slices.  Raises TileGemmError with
+    status E_LIMIT when N > NO_ALLOC_MAX_N or ceil(N / 256) * slices > NO_ALLOC_MAX_TILES.
+    Calls on one stream may follow each other freely; calls that could run at the same time on one GPU
+    (unordered streams) race on the shared scratch.  The first call on a device does the one-time
+    set-up and should come before any stream capture."""
+    if x.dtype != B.dtype or x.dtype not in (torch.bfloat16, torch.float16):
+        raise TypeError("x and B must both be torch.bfloat16 or both torch.float16")
+    if B.dim() != 2 or x.numel() != B.shape[0] or x.dim() > 2 or (x.dim() == 2 and x.shape[0] != 1):
+        raise ValueError("x must hold K elements ((K,) or (1, K)) for B of shape (K, N)")
+    K, N = B.shape
+    if y.dtype not in (torch.float32, torch.bfloat16, torch.float16) or y.numel() != N or y.dim() > 2 \
+            or (y.dim() == 2 and y.shape[0] != 1):
+        raise TypeError("y must be an (N,) or (1, N) float32, bfloat16 or float16 tensor")
+    if (x.numel() > 1 and x.stride(-1) != 1) or (y.numel() > 1 and y.stride(-1) != 1):
+        raise ValueError("x and y must have unit element stride")
+    od = {torch.float32: OUT_F32, torch.bfloat16: OUT_BF16, torch.float16: OUT_F16}[y.dtype]
+    with _on_device(x, B, y):
+        st = load_library().tile_gemv_no_alloc(_vp(x.data_ptr()), _vp(B.data_ptr()), _vp(y.data_ptr()), N, K, _ld(B),
+                                               IN_F16 if x.dtype == torch.float16 else IN_BF16, od, int(split),
+                                               _vp(_stream_handle(stream)))
+    _check(int(st))
+    return y
 
 
 def tile_read_probe_u32(buf: torch.Tensor, out_sum: torch.Tensor | None = None, stream=None) -> torch.Tensor:

@@ -53,6 +53,7 @@ const char* const kStatusNames[TILE_GEMM_NUM_STATUS] = {
     "path not applicable",
     "internal error",
     "unknown in_dtype",
+    "request exceeds the fixed scratch of tile_gemv_no_alloc",
 };
 
 std::atomic<int64_t> g_launches{0};
@@ -1719,6 +1720,120 @@ int tile_gemm_shutdown(void) {
     }
     g_maps.clear();
     return TILE_GEMM_OK;
+}
+
+}  // extern "C"
+
+// ====================================================================== M = 1 without any device allocation
+// tile_gemv_no_alloc (include/tile_gemm.h): the split-K M = 1 kernel in its ticket protocol, with the fp32 partial
+// sums and the tickets in the file-scope device array below instead of a cudaMalloc'ed workspace.  Nothing else in
+// the library touches this array and no other entry point is routed through this code.
+//
+// Every context that loads the library holds the array (1 MiB + 4 KiB) until the process exits.  Layout:
+//   [0, kNoAllocPartialBytes)                      float partials[tile][256], tile = column block * S + slice
+//   [kNoAllocPartialBytes, + 4 * MAX_TILES)        uint32_t tickets[column block]
+constexpr size_t kNoAllocPartialBytes = (size_t)TILE_GEMV_NO_ALLOC_MAX_TILES * tg::GEMV_COLS * sizeof(float);
+constexpr size_t kNoAllocTicketBytes = (size_t)TILE_GEMV_NO_ALLOC_MAX_TILES * sizeof(uint32_t);
+static_assert(kNoAllocPartialBytes + kNoAllocTicketBytes == TILE_GEMV_NO_ALLOC_SCRATCH_BYTES,
+              "the header states the size of the scratch array");
+static_assert(TILE_GEMV_NO_ALLOC_MAX_N == TILE_GEMV_NO_ALLOC_MAX_TILES * tg::GEMV_COLS, "one ticket per column block");
+
+static __device__ __align__(256) unsigned char g_no_alloc_scratch[TILE_GEMV_NO_ALLOC_SCRATCH_BYTES];
+
+namespace {
+// In host code `g_no_alloc_scratch` is only the handle the runtime registered for the symbol, not an address the
+// GPU can use: the device address is looked up once per device (with that device current) and kept here.
+std::mutex g_no_alloc_mu;
+void* g_no_alloc_ptr[64] = {};
+
+int no_alloc_scratch(int dev, unsigned char** out) {   // `dev` is the current device
+    std::lock_guard<std::mutex> lk(g_no_alloc_mu);
+    if (g_no_alloc_ptr[dev] == nullptr) {
+        void* ptr = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&ptr, g_no_alloc_scratch);
+        if (e != cudaSuccess || ptr == nullptr) {
+            cudaGetLastError();
+            return fail(TILE_GEMM_E_CUDA, "cudaGetSymbolAddress(no-alloc scratch) failed on device %d: %s (%d)", dev,
+                        cudaGetErrorString(e), (int)e);
+        }
+        g_no_alloc_ptr[dev] = ptr;
+    }
+    *out = (unsigned char*)g_no_alloc_ptr[dev];
+    return TILE_GEMM_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int tile_gemv_no_alloc(const void* x, const void* B, void* y, int64_t N, int64_t K, int64_t ldb, int in_dtype,
+                       int out_dtype, int split, void* stream) {
+    // ---- launch preconditions: those of tile_gemm at M = 1, then the ones the fixed scratch adds ----
+    Plan plan;
+    int rc = check_and_select(x, B, y, 1, N, K, K, ldb, N, in_dtype, out_dtype, &plan);
+    if (rc) return rc;
+    if (split < 0) return fail(TILE_GEMM_E_EXTENT, "negative K-slice count: split=%d", split);
+    if (N > TILE_GEMV_NO_ALLOC_MAX_N)
+        return fail(TILE_GEMM_E_LIMIT,
+                    "N=%lld is above TILE_GEMV_NO_ALLOC_MAX_N=%d, the widest output the fixed %d-byte scratch array "
+                    "has tickets for; use tile_gemm (which allocates its workspace) or split the columns over calls",
+                    (long long)N, TILE_GEMV_NO_ALLOC_MAX_N, TILE_GEMV_NO_ALLOC_SCRATCH_BYTES);
+    const int64_t col_blocks = (N + tg::GEMV_COLS - 1) / tg::GEMV_COLS;
+    const int64_t k_tiles = (K + 63) / 64;
+    if (split > 1 && col_blocks * (split < k_tiles ? split : k_tiles) > TILE_GEMV_NO_ALLOC_MAX_TILES)
+        return fail(TILE_GEMM_E_LIMIT,
+                    "split=%d over %lld column blocks needs %lld partial-sum tiles; the fixed scratch array holds "
+                    "TILE_GEMV_NO_ALLOC_MAX_TILES=%d (pass split = 0 for a count that fits)",
+                    split, (long long)col_blocks, (long long)(col_blocks * (split < k_tiles ? split : k_tiles)),
+                    TILE_GEMV_NO_ALLOC_MAX_TILES);
+    if (plan.path == TILE_GEMM_PATH_NOOP) return TILE_GEMM_OK;
+    if (K > 0 && !plan.b_tma)
+        return fail(TILE_GEMM_E_PATH,
+                    "tile_gemv_no_alloc reads B through TMA: B (%p) must be 16-byte aligned and ldb (%lld) a multiple "
+                    "of 8 (the repack path of tile_gemm would need an allocated copy)", B, (long long)ldb);
+    int dev = 0, sms = 0;
+    rc = current_device(&dev, &sms);
+    if (rc) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (K == 0) return run_zero(y, 1, N, N, plan.esize, s, sms);
+
+    // ---- plan: the default ring shape (256 columns, 64 rows per stage, 3 stages, 2 CTAs per SM) ----
+    const int64_t budget = (int64_t)sms * 2;
+    const int64_t gx = col_blocks < budget ? col_blocks : budget;
+    int64_t S = split;
+    if (S == 0) {
+        S = budget / gx;                                                    // as many slices as stay co-resident
+        const int64_t fit = TILE_GEMV_NO_ALLOC_MAX_TILES / col_blocks;     // >= 1: col_blocks <= MAX_TILES
+        if (S > fit) S = fit;
+    }
+    if (S > k_tiles) S = k_tiles;
+    if (S > 65535) S = 65535;
+    if (S < 1) S = 1;
+
+    tg::GemvSplitParams p;
+    memset(&p, 0, sizeof p);
+    p.x = (const uint16_t*)x;
+    p.y = y;
+    p.N = (int32_t)N;
+    p.K = (int32_t)K;
+    p.k_tiles = (int32_t)k_tiles;
+    p.col_blocks = (int32_t)col_blocks;
+    p.out_kind = out_dtype;
+    p.flags = (((uintptr_t)x) & 15) == 0 ? tg::GEMV_FLAG_X_TMA : 0;   // neither CLUSTER nor PACKED: tickets
+    p.l2_post = 0;
+    if (S > 1) {
+        unsigned char* scratch = nullptr;
+        rc = no_alloc_scratch(dev, &scratch);
+        if (rc) return rc;
+        p.partials = (float*)scratch;
+        p.tickets = (uint32_t*)(scratch + kNoAllocPartialBytes);
+        // The array keeps whatever the last call left.  Partial sums are written before they are read, the
+        // tickets must start at zero: clear the ones this launch draws, in stream order ahead of the kernel.
+        CUDA_TRY(cudaMemsetAsync(p.tickets, 0, (size_t)col_blocks * sizeof(uint32_t), s));
+    }
+    // no programmatic dependent launch: two calls in a row on one stream must not overlap on the shared scratch
+    return in_dtype == TILE_GEMM_IN_F16
+               ? launch_gemv_split<256, 64, 3, 2, true>(B, N, K, ldb, p, (int)gx, (int)S, false, s, dev)
+               : launch_gemv_split<256, 64, 3, 2, false>(B, N, K, ldb, p, (int)gx, (int)S, false, s, dev);
 }
 
 }  // extern "C"

@@ -21,7 +21,7 @@ A0, B0, C0 = 0x10000, 0x7000_0000_0000, 0x7100_0000_0000   # fake, well separate
 
 def test_library_exports_every_declared_symbol():
     header = open(os.path.join(ROOT, "include", "tile_gemm.h")).read()
-    declared = set(re.findall(r"\b(tile_(?:gemm|add|read)\w*)\s*\(", header))
+    declared = set(re.findall(r"\b(tile_(?:gemm|gemv|add|read)\w*)\s*\(", header))
     assert declared == set(tg.EXPORTS), declared ^ set(tg.EXPORTS)
     lib = tg.load_library()
     for name in declared:
@@ -29,8 +29,8 @@ def test_library_exports_every_declared_symbol():
 
 
 def test_status_strings_are_distinct():
-    names = [tg.tile_gemm_status_string(i) for i in range(15)]
-    assert len(set(names)) == 15 and names[0] == "ok"
+    names = [tg.tile_gemm_status_string(i) for i in range(16)]
+    assert len(set(names)) == 16 and names[0] == "ok"
     assert tg.tile_gemm_status_string(99) == "unknown status"
 
 
