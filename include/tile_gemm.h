@@ -201,7 +201,14 @@ int tile_add_f32(const float* x, const float* y, float* z, int64_t n, void* stre
  * The M == 1 kernels keep their programmatic-dependent-launch edges inside the
  * step.  `stream` must not be NULL (the legacy default stream cannot be captured)
  * and must not already be recording (E_PATH); record_end on a stream that is not
- * recording fails with E_PATH.  The capture uses cudaStreamCaptureModeRelaxed.
+ * recording fails with E_PATH.  The capture uses cudaStreamCaptureModeRelaxed (the
+ * step's workspaces are cudaMalloc'ed while the stream captures, which the stricter
+ * modes refuse).  Consequence for the caller: while the recording is open the runtime
+ * no longer rejects potentially unsafe calls (cudaMalloc, cudaMemcpy, a legacy-stream
+ * synchronisation, ...) made by this or any other host thread, as it would under the
+ * default global mode -- keep such calls from touching the recording stream's work
+ * yourself.  A recording that is still open at tile_gemm_shutdown is abandoned: its
+ * workspaces are freed, the stream's capture is left for the caller to end.
  * A failed call while recording leaves the capture open; still call record_end
  * (it reports the invalidated capture and releases what the recording held).
  * Library calls on a stream the CALLER captures itself (cudaStreamBeginCapture)
@@ -327,8 +334,9 @@ int tile_gemm_select(int64_t M, int64_t N, int64_t K,
  * host memory is needed for the copies to overlap.  This is the call bench.py's
  * `e2e` figure times.
  * Thread safety: the staging buffers, streams and events are kept per device and
- * the whole call runs under one process-wide lock -- concurrent callers are
- * serialised (they would share the PCIe link anyway), never mixed.
+ * the whole call runs under that device's lock -- concurrent callers on ONE GPU are
+ * serialised (they would share its PCIe link anyway), never mixed; callers on
+ * different GPUs do not wait for each other.
  */
 int tile_gemm_host(const void* A_host, const void* B_host, void* C_host,
                    int64_t M, int64_t N, int64_t K,

@@ -431,14 +431,23 @@ def tile_gemm_debug_occupy(ctas: int, ns: int, stream=None) -> None:
     _check(load_library().tile_gemm_debug_occupy(int(ctas), int(ns), _vp(_stream_handle(stream))))
 
 
+_trace_ref = None   # the tensor the library currently holds a raw pointer to (tile_gemm_debug_trace)
+
+
 def tile_gemm_debug_trace(records: torch.Tensor | None) -> None:
-    """records: int64 CUDA tensor of shape (capacity, 8) that the following M = 1 launches fill, or None to stop."""
+    """records: int64 CUDA tensor of shape (capacity, 8) that the following M = 1 and tiled-GEMM launches fill,
+    or None to stop.  The library keeps only the raw device pointer, so this module keeps the tensor alive
+    until tracing is switched off (or another buffer is set); launches made while a stream is recording or
+    capturing get no trace pointer."""
+    global _trace_ref
     if records is None:
         _check(load_library().tile_gemm_debug_trace(_vp(0), 0))
+        _trace_ref = None
         return
     if records.dtype != torch.int64 or records.dim() != 2 or records.shape[1] != 8 or not records.is_contiguous():
         raise TypeError("records must be a contiguous int64 tensor of shape (capacity, 8)")
     _check(load_library().tile_gemm_debug_trace(_vp(records.data_ptr()), records.shape[0]))
+    _trace_ref = records
 
 
 def tile_gemm_debug_owner_map(M, N, K, out_dtype=OUT_F32, ld_owner=None, stream=None, device="cuda"):

@@ -59,6 +59,15 @@ const char* const kStatusNames[TILE_GEMM_NUM_STATUS] = {
 std::atomic<int64_t> g_launches{0};
 std::atomic<unsigned long long*> g_trace{nullptr};   // tile_gemm_debug_trace
 std::atomic<int64_t> g_trace_cap{0};
+// The trace buffer a launch on `s` may write: none while `s` is capturing (a recorded step would keep the
+// raw address and write through it on every replay, long after the caller has dropped the buffer).
+unsigned long long* trace_for(cudaStream_t s) {
+    unsigned long long* t = g_trace.load();
+    if (!t) return nullptr;
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(s, &cs) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    return cs == cudaStreamCaptureStatusNone ? t : nullptr;
+}
 constexpr int kNumTune = 16;   // keys 0..11 are documented in include/tile_gemm.h
 std::atomic<int> g_tune[kNumTune];
 
@@ -280,14 +289,14 @@ std::unordered_map<uint64_t, WorkspaceSet> g_wsets;            // (device, strea
 std::unordered_map<uintptr_t, Recording*> g_recording;         // streams between record_begin and record_end
 std::vector<void*> g_retired;                                   // retired buffers of pinned per-stream sets
 
-// tile_gemm_host: one staging set per device, used under g_host_mu for the whole call
+// tile_gemm_host: one staging set per device, used under that device's own lock for the whole call
 struct HostStage {
+    std::mutex mu;
     Buf a, b, c;
     cudaStream_t in = nullptr, compute = nullptr, out = nullptr;   // copy-in, GEMMs, copy-out
     std::vector<cudaEvent_t> events;
 };
 HostStage g_host[64];
-std::mutex g_host_mu;
 
 int grow(Buf& b, size_t need) {
     if (b.n >= need) return TILE_GEMM_OK;
@@ -892,7 +901,7 @@ int run_gemm(const void* A, const void* B, void* C, int64_t M, int64_t N, int64_
     }
     rc = setup_lockstep(gl, dev, s);
     if (rc) return rc;
-    gl.p.trace = g_trace.load();                                   // tile_gemm_debug_trace: 4 words per cluster
+    gl.p.trace = trace_for(s);                                     // tile_gemm_debug_trace: 8 words per cluster
     gl.p.trace_cap = (int32_t)g_trace_cap.load();
     return launch_gemm(gl, ta, tb, tc, s, dev);
 }
@@ -976,6 +985,27 @@ int gemv_cluster_capacity(int cs, int dev, int sms) {
     return n;
 }
 
+// CTAs of one ring shape of the split kernel that the CURRENT context can hold at once, from the occupancy
+// calculator (it sees the shared-memory carve-out and the registers this build really uses) times the SM count;
+// cached per device.  The tagged-slot hand-over is only taken when the whole launch fits this figure: its
+// combiner CTAs poll for their column block's other slices, so those must be able to become resident.
+template <int COLS, int TILE_K, int STAGES, int MIN_CTAS, bool F16>
+int gemv_resident_ctas(int dev, int sms) {
+    static std::atomic<int> cache[64];
+    int v = cache[dev].load();
+    if (v != 0) return v > 0 ? v : 0;
+    using L = tg::GemvSplitSmem<COLS, TILE_K, STAGES>;
+    auto kern = tg::gemv_split_kernel<COLS, TILE_K, STAGES, MIN_CTAS, F16>;
+    int per_sm = 0;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L::TOTAL) != cudaSuccess ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, tg::GEMV_TMA_THREADS, (size_t)L::TOTAL) != cudaSuccess)
+        per_sm = 0;
+    cudaGetLastError();
+    v = per_sm > 0 ? per_sm * sms : -1;   // -1: unknown, treated as "nothing is provably resident"
+    cache[dev].store(v);
+    return v > 0 ? v : 0;
+}
+
 // measured on B200: two units into L2 behind the dependency wait; clusters sized to 92 % of capacity
 // (same-process A/B of 80 / 88 / 92 / 96 / 100 %: 92 and 96 give N = 10240 six slices instead of five, +1.1 %; 100 % makes
 // every other launch of N = 8192 run in two waves, -17 %)
@@ -1048,16 +1078,38 @@ int run_gemv_split(const void* x, const void* B, void* y, int64_t N, int64_t K, 
     p.out_kind = out_dtype;
     p.flags = (flags & TILE_GEMM_FLAG_B_IMMUTABLE) ? tg::GEMV_FLAG_B_IMMUTABLE : 0;
     if ((((uintptr_t)x) & 15) == 0 && (g_tune[6].load() & 2) == 0) p.flags |= tg::GEMV_FLAG_X_TMA;
-    p.trace = g_trace.load();
+    p.trace = trace_for(s);
     p.trace_cap = (int32_t)g_trace_cap.load();
     const int post = g_tune[9].load();                       // tuning key 9: n >= 1 -> n - 1 units
     p.l2_post = post > 0 ? post - 1 : kGemvL2PostUnits;
     if (split > 1) {
         int rc = TILE_GEMM_OK;
+        const bool f16_in = in_dtype == TILE_GEMM_IN_F16;
+        int64_t resident = 0;
+        if (!(cluster_ok && split <= tg::GEMV_MAX_CLUSTER) && (fix_mode == 0 || fix_mode == 2)) {
+#define TG_GEMV_RES(id, C, T, ST, O)                                                                  \
+    case id:                                                                                          \
+        resident = f16_in ? gemv_resident_ctas<C, T, ST, O, true>(dev, sms)                           \
+                          : gemv_resident_ctas<C, T, ST, O, false>(dev, sms);                         \
+        break;
+            switch (shape) {
+                TG_GEMV_RES(1, 256, 64, 2, 3)
+                TG_GEMV_RES(2, 256, 64, 3, 2)
+                TG_GEMV_RES(3, 256, 32, 3, 4)
+                TG_GEMV_RES(4, 512, 32, 3, 2)
+                TG_GEMV_RES(5, 512, 32, 2, 3)
+                TG_GEMV_RES(6, 512, 16, 4, 3)
+                TG_GEMV_RES(7, 1024, 16, 3, 2)
+                TG_GEMV_RES(8, 512, 16, 3, 4)
+            }
+#undef TG_GEMV_RES
+        }
         if (cluster_ok && split <= tg::GEMV_MAX_CLUSTER) {
             p.flags |= tg::GEMV_FLAG_CLUSTER;
-        } else if ((fix_mode == 0 || fix_mode == 2) && gx * split <= budget) {
+        } else if ((fix_mode == 0 || fix_mode == 2) && gx * split <= budget && gx * split <= resident) {
             // tagged slots: the designated combiner polls, so every CTA of the launch must fit the device at once
+            // -- by the nominal figure the plan was made with AND by what the occupancy calculator reports for this
+            // context.  Anything that is not provably one wave keeps the tickets, which cannot wait on anybody.
             rc = packed_workspace_for(dev, s, (size_t)col_blocks * split * gs.cols * 8, &p.packed);
             p.flags |= tg::GEMV_FLAG_PACKED;
         } else {
@@ -1497,11 +1549,12 @@ int tile_gemm_host(const void* A_host, const void* B_host, void* C_host, int64_t
     int dev = 0, sms = 0;
     rc = current_device(&dev, &sms);
     if (rc) return rc;
-    // One host call at a time (per process): the staging buffers, the three streams and the events of
-    // the current device are used for the whole call, and concurrent callers would only share the
-    // PCIe link anyway.  Other threads block here; they never see each other's staging data.
-    std::lock_guard<std::mutex> host_lk(g_host_mu);
+    // One host call at a time PER DEVICE: the staging buffers, the three streams and the events of the
+    // current device are used for the whole call.  Threads that target the same GPU block here (they
+    // would share its PCIe link anyway) and never see each other's staging data; threads on different
+    // GPUs share nothing and run side by side.
     HostStage& hs = g_host[dev];
+    std::lock_guard<std::mutex> host_lk(hs.mu);
     if (!hs.in) CUDA_TRY(cudaStreamCreateWithFlags(&hs.in, cudaStreamNonBlocking));
     if ((rc = grow(hs.a, (size_t)plan.a_bytes + 16))) return rc;
     if ((rc = grow(hs.b, (size_t)plan.b_bytes + 16))) return rc;
@@ -1701,10 +1754,17 @@ const char* tile_gemm_status_string(int status) {
 const char* tile_gemm_last_error(void) { return g_err; }
 
 int tile_gemm_shutdown(void) {
-    std::lock_guard<std::mutex> host_lk(g_host_mu);
+    for (HostStage& hs : g_host) hs.mu.lock();   // index order; tile_gemm_host holds at most one of them
     std::lock_guard<std::mutex> lk(g_mu);
     for (auto& kv : g_wsets) free_workspace_set(kv.second);
     g_wsets.clear();
+    // a step whose record_end never came: its private workspaces go too (the caller's capture, if it is
+    // still open, is the caller's to end; record_end on that stream now reports E_PATH)
+    for (auto& kv : g_recording) {
+        free_workspace_set(kv.second->ws);
+        delete kv.second;
+    }
+    g_recording.clear();
     for (void* q : g_retired) cudaFree(q);
     g_retired.clear();
     for (HostStage& hs : g_host) {
@@ -1719,6 +1779,7 @@ int tile_gemm_shutdown(void) {
         hs.events.clear();
     }
     g_maps.clear();
+    for (HostStage& hs : g_host) hs.mu.unlock();
     return TILE_GEMM_OK;
 }
 

@@ -203,3 +203,97 @@ def test_host_entry_from_two_threads():
     for t in threads:
         t.join()
     assert not errors, errors
+
+
+@pytest.mark.parametrize("fix,split", [(1, 10), (2, 10), (3, 4)])
+def test_gemv_trace_on_leaves_the_result_alone_and_fills_sane_records(fix, split):
+    """tile_gemm_debug_trace on an M = 1 launch in each hand-over protocol (tickets, tagged slots, cluster):
+    y keeps its bits, every CTA of the launch writes its record, the time stamps are ordered, and the
+    tiles the CTAs report add up to column blocks x k-tiles.  The binding holds the buffer while it is set."""
+    K, N = 2560, 2048                                   # 8 column blocks of 256, 40 k-tiles of 64
+    x, B, ref = _int_case(1, N, K, 411)
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMV_FIXUP, fix)
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMV_SPLIT, split)
+    y0 = tg.tile_gemm(x, B)
+    torch.cuda.synchronize()
+    rec = torch.zeros((128, 8), dtype=torch.int64, device=DEV)
+    tg.tile_gemm_debug_trace(rec)
+    assert tg._trace_ref is rec
+    try:
+        y1 = tg.tile_gemm(x, B)
+        torch.cuda.synchronize()
+    finally:
+        tg.tile_gemm_debug_trace(None)
+    assert tg._trace_ref is None
+    check_bit_exact(y1.cpu().numpy(), ref, f"traced GEMV, fix-up {fix}")
+    assert torch.equal(y0, y1)
+    r = rec.cpu().numpy()
+    ctas = 8 * split
+    used, rest = r[:ctas], r[ctas:]
+    assert (rest == 0).all(), "records past the launch's CTAs were written"
+    assert sorted((int(w) >> 16) & 0xFFFF | ((int(w) >> 32) << 16) for w in used[:, 0]) == \
+        sorted(bx | (by << 16) for by in range(split) for bx in range(8))
+    t = used[:, 1:6]
+    assert (t > 0).all() and (np.diff(t, axis=1) >= 0).all(), "time stamps out of order"
+    assert (t[:, 4] - t[:, 0] < 5_000_000).all(), "a CTA of a 10 MB GEMV took more than 5 ms"
+    assert int(used[:, 6].sum()) == 8 * 40
+    assert ((used[:, 7] >= t[:, 3]) & (used[:, 7] <= t[:, 4])).all(), "hand-over stamp outside [last tile, done]"
+    # a later launch without tracing leaves the buffer alone
+    rec.zero_()
+    tg.tile_gemm(x, B)
+    torch.cuda.synchronize()
+    assert (rec == 0).all()
+
+
+@pytest.mark.parametrize("cfg", [3, 4])
+def test_gemm_trace_on_leaves_the_result_alone_and_counts_the_k_tiles(cfg):
+    M, N, K = 1024, 1024, 1024
+    A, B, ref = _int_case(M, N, K, 412)
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMM_CONFIG, cfg)
+    tg.tile_gemm_set_tuning(tg.TUNE_GEMV_SPLIT, 1)      # whole tiles only
+    q = tg.tile_gemm_query_config(M, N, K)
+    tiles = -(-M // (q["BM"] * q["cta_group"])) * -(-N // q["BN"])
+    rec = torch.zeros((256, 8), dtype=torch.int64, device=DEV)
+    tg.tile_gemm_debug_trace(rec)
+    try:
+        C = tg.tile_gemm(A, B)
+        torch.cuda.synchronize()
+    finally:
+        tg.tile_gemm_debug_trace(None)
+    check_bit_exact(C.cpu().numpy(), ref, f"traced GEMM, config {cfg}")
+    r = rec.cpu().numpy()
+    live = r[r[:, 2] > 0]
+    assert len(live) == min(tiles, q["ctas"] // q["cta_group"])
+    assert (live[:, 1] <= live[:, 2]).all() and (live[:, 2] < 50_000_000).all()
+    assert int(live[:, 3].sum()) == tiles * (K // q["BK"])
+    assert int(live[:, 5].sum()) >= tiles and (live[:, 4] > 0).all()
+
+
+def test_recorded_step_takes_no_trace_pointer():
+    """A step recorded while tracing is on must not keep the trace buffer's address: after the buffer is gone
+    a replay would write into freed memory.  Launches under record_begin get a null trace pointer."""
+    x, B, ref = _int_case(1, 1536, 2560, 413)
+    A2, B2, ref2 = _int_case(256, 512, 512, 414)
+    y = torch.empty((1, 1536), dtype=torch.float32, device=DEV)
+    C2 = torch.empty((256, 512), dtype=torch.float32, device=DEV)
+    tg.tile_gemm(x, B, y)                                # workspaces exist before the recording
+    tg.tile_gemm(A2, B2, C2)
+    torch.cuda.synchronize()
+    s = torch.cuda.Stream()
+    rec = torch.zeros((256, 8), dtype=torch.int64, device=DEV)
+    tg.tile_gemm_debug_trace(rec)
+    try:
+        tg.tile_gemm_record_begin(s)
+        tg.tile_gemm(x, B, y, stream=s)
+        tg.tile_gemm(A2, B2, C2, stream=s)
+        step = tg.tile_gemm_record_end(s)
+    finally:
+        tg.tile_gemm_debug_trace(None)
+    y.fill_(float("nan"))
+    C2.fill_(float("nan"))
+    step.replay(s)
+    s.synchronize()
+    assert (rec == 0).all(), "a recorded launch wrote trace records"
+    check_bit_exact(y.cpu().numpy(), ref, "replayed GEMV")
+    check_bit_exact(C2.cpu().numpy(), ref2, "replayed GEMM")
+    step.free()
