@@ -605,6 +605,8 @@ def run_cuda(args):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback); use --impl reference for the oracle")
     rank, local_rank, world = tdist.init()
+    if world != args.gpus and rank == 0:
+        sys.stderr.write(f"bench.py: --gpus {args.gpus} but the launcher started {world} rank(s); reporting n_gpus = {world}\n")
     torch.cuda.set_device(local_rank)
     tg.load_library()
     if args.gemm_config:
@@ -754,7 +756,23 @@ def run_cuda(args):
     # final kilobytes of the line whatever the other legs print
     if gemv_rec is not None:
         line["read_probe"] = probe_rec
+        if gemv_rec["roofline"]["frac"] > 1.0:
+            note = ("above 1 because the peak is MEASURED_PEAKS.json's COPY bandwidth (read + write streams); a pure read "
+                    "stream runs faster on this part: the ceiling to read it against is frac_of_read_probe")
+            gemv_rec["roofline"]["frac_note"] = note
+            line["roofline"]["gemv"]["frac_note"] = note
         line["gemv"] = gemv_rec
+    # the steady-state figures once more, as short top-level records at the END of the line (the roofline object that
+    # holds the full versions is printed kilobytes earlier)
+    sus = line["roofline"].get("sustained")
+    if sus is not None:
+        line["sustained"] = {"achieved": round(sus["achieved"], 1), "peak": sus["peak"], "frac": round(sus["frac"], 4),
+                             "unit": "TFLOP/s", "seconds": round(sus["seconds"], 2),
+                             "sm_mhz": (sus.get("clocks") or {}).get("sm_mhz"), "reasons": (sus.get("clocks") or {}).get("reasons")}
+    ctx = line["roofline"].get("cublas_same_run")
+    if ctx is not None:
+        line["cublas_same_run"] = {"burst_ratio": ctx["burst_ratio"], "sustained_ratio": ctx["sustained_ratio"],
+                                   "note": "tile_gemm / torch.matmul on cfg3 in this run; context only"}
     if rank == 0:
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = cpu_baseline_leg()
@@ -762,6 +780,35 @@ def run_cuda(args):
     tdist.barrier()
     tdist.shutdown()
     return 0
+
+
+def spawn_ranks(n):
+    """`python bench.py --gpus N` with no torchrun environment: start the N ranks ourselves, exactly the way the
+    driver's torchrun form does (one process per GPU, rendezvous on 127.0.0.1), with this command line."""
+    import socket
+    import subprocess
+    with socket.socket() as sock:
+        sock.bind(("127.0.0.1", 0))
+        port = sock.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
+def run_rendezvous(args):
+    """The N > 1 plumbing without the kernels: every rank joins, the ranks meet at a barrier, and rank 0 prints how
+    many arrived and the max / sum of their rank numbers (what the timing scalars travel through)."""
+    from paper_2606_15991_b200 import dist as tdist
+    rank, local_rank, world = tdist.init()
+    tdist.barrier()
+    top = tdist.max_over_ranks(float(rank))
+    total = tdist.sum_over_ranks(float(rank + 1))
+    if rank == 0:
+        print(json.dumps({"rendezvous": world, "gpus_flag": args.gpus, "max_rank": top, "sum_rank_plus_1": total,
+                          "impl": args.impl}), flush=True)
+    tdist.barrier()
+    tdist.shutdown()
+    return 0 if world == args.gpus else 1
 
 
 def main():
@@ -781,8 +828,14 @@ def main():
     ap.add_argument("--sustained-seconds", type=float, default=2.5)
     ap.add_argument("--gemm-config", type=int, default=0, help="force a GEMM tile config (tile_gemm_set_tuning key 0)")
     ap.add_argument("--group-m", type=int, default=0, help="force the raster group height (tuning key 1)")
+    ap.add_argument("--rendezvous-only", action="store_true",
+                    help="start the ranks, rendezvous (NCCL on GPUs, gloo on a CPU box), print the world that met, and exit")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return spawn_ranks(args.gpus)
+    if args.rendezvous_only:
+        return run_rendezvous(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_cuda(args)

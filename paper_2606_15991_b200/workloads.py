@@ -136,15 +136,27 @@ def make_inputs_device(case: GemmCase, device="cuda"):
     return a, b
 
 
-def stratified_samples(M: int, N: int, block: int = 128, seed: int = 0):
+def make_int_inputs_device(M, N, K, seed=0, device="cuda", dtype=torch.bfloat16):
+    """Device-generated integer-valued inputs, uniform in [-4, 4] like "int4", for shapes whose host
+    generation would take longer than the test (weights of the decode shapes, the 32768^3 sweep point)."""
+    g = torch.Generator(device=device)
+    g.manual_seed(int(np.random.SeedSequence([int(seed), 7933]).generate_state(1)[0]))
+    a = torch.randint(-4, 5, (M, K), generator=g, device=device, dtype=torch.int8).to(dtype)
+    b = torch.randint(-4, 5, (K, N), generator=g, device=device, dtype=torch.int8).to(dtype)
+    return a, b
+
+
+def stratified_samples(M: int, N: int, block=128, seed: int = 0):
     """One seeded-uniform element inside every block x block cell of the output
-    (SURVEY.md 8(c) c13): every output tile is touched.  Returns (rows, cols)."""
+    (SURVEY.md 8(c) c13): every output tile is touched.  `block` may be a
+    (rows, columns) pair for rectangular cells.  Returns (rows, cols)."""
     rng = np.random.default_rng([int(seed), 104729])
-    bi = np.arange(0, M, block)
-    bj = np.arange(0, N, block)
+    block_m, block_n = (block, block) if isinstance(block, int) else block
+    bi = np.arange(0, M, block_m)
+    bj = np.arange(0, N, block_n)
     ii, jj = np.meshgrid(bi, bj, indexing="ij")
-    hi_i = np.minimum(ii + block, M) - ii
-    hi_j = np.minimum(jj + block, N) - jj
+    hi_i = np.minimum(ii + block_m, M) - ii
+    hi_j = np.minimum(jj + block_n, N) - jj
     rows = ii + (rng.random(ii.shape) * hi_i).astype(np.int64)
     cols = jj + (rng.random(jj.shape) * hi_j).astype(np.int64)
     return rows.ravel().astype(np.int64), cols.ravel().astype(np.int64)

@@ -2,6 +2,7 @@
 declares, launch preconditions and the selector behave as include/tile_gemm.h states (pure
 host, fake pointers, nothing dereferenced), the schedule function covers C exactly once, and
 the N>1 helpers work over gloo with world_size 2.  No compute call is made (no GPU here)."""
+import json
 import os
 import re
 import subprocess
@@ -229,7 +230,7 @@ def test_swiglu_preconditions_on_the_host():
 
 def test_selector_routes_a_few_rows_to_the_tensor_cores():
     # only M = 1 is the CUDA-core GEMV; from M = 2 on the tensor-core path (in place through TMA where A and B
-    # are 16-byte addressable -- the weight-streaming kernel up to M = 32 -- else after a repack)
+    # are 16-byte addressable -- the weight-streaming kernel up to M = 64 where its plan allows -- else after a repack)
     assert sel(1, 10240, 5120) == tg.PATH_GEMV
     for M in (2, 3, 4, 5, 32, 33):
         assert sel(M, 10240, 5120) == tg.PATH_GEMM_TMA
@@ -267,3 +268,23 @@ def test_truncation_model_on_the_hand_worked_cases():
         got = parity.tcgen05_accumulate_model(a, np.ones((len(v), 1)))[0, 0]
         assert got == want
 
+
+
+def test_bench_gpus_flag_starts_that_many_ranks():
+    """`python bench.py --gpus 2` without a torchrun environment (the driver's plain form) must start two ranks
+    itself: the self-spawn path re-launches the same command line under torch.distributed.run, the two ranks
+    rendezvous (gloo here, NCCL on a GPU box) and rank 0 reports the world that met.  --rendezvous-only stops
+    there, before any kernel, so this runs on the CPU box."""
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    env["PYTHONPATH"] = ROOT
+    res = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--rendezvous-only"],
+                         env=env, capture_output=True, text=True, timeout=300)
+    assert res.returncode == 0, res.stdout + res.stderr
+    lines = [json.loads(ln) for ln in res.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, res.stdout                      # rank 0 alone prints
+    assert lines[0]["rendezvous"] == 2 and lines[0]["gpus_flag"] == 2
+    assert lines[0]["max_rank"] == 1.0 and lines[0]["sum_rank_plus_1"] == 3.0
+    # one rank: no spawn, no process group
+    res = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--rendezvous-only"],
+                         env=env, capture_output=True, text=True, timeout=300)
+    assert res.returncode == 0 and json.loads(res.stdout.strip().splitlines()[-1])["rendezvous"] == 1
