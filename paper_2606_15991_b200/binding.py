@@ -1,4 +1,4 @@
-"""ctypes binding of libtilegemm.so (include/tile_gemm.h) -- argument marshalling only.
+"""ctypes binding of libtilegemm.so (include/tile_gemm.h, include/tile_gemm_debug.h) -- argument marshalling only.
 
 Every step of the path runs in the library's CUDA kernels.  There is no CPU
 fallback: if the shared library cannot be found or built, ``load_library``

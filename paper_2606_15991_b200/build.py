@@ -10,7 +10,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(CSRC, "libtilegemm.so")
 SOURCES = ["tile_gemm.cu"]
 HEADERS = ["ptx.cuh", "gemm_kernel.cuh", "gemv_kernel.cuh", "skinny_kernel.cuh", "aux_kernels.cuh", "add_kernel.cuh",
-           os.path.join("..", "..", "include", "tile_gemm.h")]
+           os.path.join("..", "..", "include", "tile_gemm.h"), os.path.join("..", "..", "include", "tile_gemm_debug.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
@@ -36,10 +36,18 @@ def needs_build() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
+def _defines() -> list:
+    """TILEGEMM_WATCHDOG=0 in the environment builds without the bounded-wait watchdog (csrc/ptx.cuh: every
+    mbarrier wait then spins without the %globaltimer check, printf and trap).  The default build keeps it:
+    measured cost on B200 see DESIGN.md "Watchdog"."""
+    wd = os.environ.get("TILEGEMM_WATCHDOG")
+    return [f"-DTILEGEMM_WATCHDOG={int(wd)}"] if wd not in (None, "") else []
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not needs_build():
         return LIB
-    cmd = [_nvcc()] + NVCC_FLAGS + ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
+    cmd = [_nvcc()] + NVCC_FLAGS + _defines() + ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
     res = subprocess.run(cmd, cwd=CSRC, capture_output=True, text=True)
     if verbose or res.returncode != 0:
         sys.stderr.write(res.stdout + res.stderr)

@@ -6,6 +6,7 @@
 // returns an error on failure".  Everything validated here is exactly what lets
 // the device K loops run without a single bounds check.
 #include "../../include/tile_gemm.h"
+#include "../../include/tile_gemm_debug.h"
 
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -68,7 +69,7 @@ unsigned long long* trace_for(cudaStream_t s) {
     if (cudaStreamIsCapturing(s, &cs) != cudaSuccess) { cudaGetLastError(); return nullptr; }
     return cs == cudaStreamCaptureStatusNone ? t : nullptr;
 }
-constexpr int kNumTune = 16;   // keys 0..11 are documented in include/tile_gemm.h
+constexpr int kNumTune = 16;   // keys 0..12 are documented in include/tile_gemm_debug.h
 std::atomic<int> g_tune[kNumTune];
 
 // ------------------------------------------------------------------ preconditions + selector

@@ -21,7 +21,7 @@ A0, B0, C0 = 0x10000, 0x7000_0000_0000, 0x7100_0000_0000   # fake, well separate
 
 
 def test_library_exports_every_declared_symbol():
-    header = open(os.path.join(ROOT, "include", "tile_gemm.h")).read()
+    header = "".join(open(os.path.join(ROOT, "include", h)).read() for h in ("tile_gemm.h", "tile_gemm_debug.h"))
     declared = set(re.findall(r"\b(tile_(?:gemm|gemv|add|read)\w*)\s*\(", header))
     assert declared == set(tg.EXPORTS), declared ^ set(tg.EXPORTS)
     lib = tg.load_library()
