@@ -91,11 +91,12 @@ int tile_gemm_debug_trace(unsigned long long* records, int64_t capacity);
  *   key 2  maximum number of CTAs of a GEMM launch; also caps the GEMV grids.
  *   key 3  K slices: of the M = 1 kernel's column blocks, and (1 = never, >= 2 = that
  *          many) of the tiled GEMM's partial last wave.
- *   key 4  M = 1 kernel: 1 = TMA ring + cluster split-K, 2 = 16-byte LDG, 3 = scalar LDG,
- *          4 = TMA ring + interleaved split-K with ticketed fix-up (the automatic choice when B
- *          is TMA-addressable).
- *   key 5  ring shape of kernel 4, 1..8 = {columns per CTA, rows per stage, stages, CTAs per SM}
- *          (table kGemvShapes in csrc/tile_gemm.cu).
+ *   key 4  M = 1 kernel: 2 = 16-byte LDG, 3 = scalar LDG (both with a thread-block-cluster split-K; 3 is what
+ *          weights that TMA cannot address get), 1 or 4 = TMA ring + interleaved split-K (the automatic
+ *          choice when B is TMA-addressable).
+ *   key 5  ring shape of the TMA-ring kernel {columns per CTA, rows per stage, stages, CTAs per SM}:
+ *          2 = {256, 64, 3, 2} (automatic), 4 = {512, 32, 3, 2}, 6 = {512, 16, 4, 3}; other values mean 2
+ *          (table kGemvShapes in csrc/tile_gemm.cu; the shapes that spilled were removed in round 3).
  *   key 6  flag bits: 0 = no programmatic dependent launch; 1 = kernel 4 reads x with global loads
  *          instead of through its TMA ring; 2 / 3 = GEMM lockstep producers forced on / off, bits
  *          8-15 = their window in k-tiles; 5 = full 128-row A box even for skinny M; 6 =

@@ -4,15 +4,17 @@
 // (decode roofline R = beta / (W + Kbar)): every weight is read exactly once, so
 // the kernels only have to keep enough bytes in flight and waste none.  No tensor cores.
 //
-//   gemv_tma_kernel : B rows are 16-byte addressable.  One producer warp streams 64(k) x 256(n)
-//                     tiles (32 KB) through a shared-memory ring with TMA + mbarriers; TMA zero
-//                     fill handles the K and N tails.  Eight consumer warps each own 8 rows of a
-//                     tile, lanes own 8 consecutive columns (one conflict-free 16-byte LDS per row).
+//   gemv_split_kernel : B rows are 16-byte addressable (the default, described at its definition below).  One
+//                     producer warp streams weight tiles through a shared-memory ring with TMA + mbarriers; TMA
+//                     zero fill handles the K and N tails.  Eight consumer warps each own rows of a tile,
+//                     lanes own 8 consecutive columns (one conflict-free 16-byte LDS per row).
 //   gemv_ldg_kernel : generic fallback (any alignment): direct global loads, 16-byte when VEC.
 //
-// Split-K: gridDim.y CTAs (one thread-block cluster along y) share a column block; partial sums
-// are combined through distributed shared memory in a fixed order (thread -> warp -> cluster
-// rank), so results are bitwise reproducible and need no global workspace or atomics.
+// Split-K of the fallback: gridDim.y CTAs (one thread-block cluster along y) share a column block; partial
+// sums are combined through distributed shared memory in a fixed order (thread -> warp -> cluster
+// rank), so results are bitwise reproducible and need no global workspace or atomics.  (Round 3 removed
+// gemv_tma_kernel, the round-1 TMA kernel with that same cluster reduction: the automatic path never
+// launched it once gemv_split_kernel existed.)
 #pragma once
 #include <cuda_fp16.h>
 
@@ -113,81 +115,6 @@ __device__ __forceinline__ void gemv_reduce_and_store(const float (&acc)[8], flo
         if (col < p.N) gemv_store(p.y, col, s, p.out_kind);
     }
     if (nsplit > 1) cluster_sync();   // peers may still be reading this CTA's `part`
-}
-
-template <int STAGES, bool F16>
-__global__ void __launch_bounds__(GEMV_TMA_THREADS)
-gemv_tma_kernel(const __grid_constant__ CUtensorMap tmap_b, const GemvParams p) {
-    extern __shared__ uint8_t smem_raw[];
-    const uint32_t smem_base = (smem_u32(smem_raw) + 127u) & ~127u;
-    uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
-    // layout: STAGES tiles | red [8][256] f32 | part [256] f32 | barriers
-    constexpr uint32_t RED_OFF = STAGES * GEMV_TILE_BYTES;
-    constexpr uint32_t PART_OFF = RED_OFF + GEMV_CONSUMER_WARPS * GEMV_COLS * 4;
-    constexpr uint32_t BAR_OFF = PART_OFF + GEMV_COLS * 4;
-    float* red = reinterpret_cast<float*>(smem_gen + RED_OFF);
-    float* part = reinterpret_cast<float*>(smem_gen + PART_OFF);
-    auto full_bar = [&](uint32_t s) { return smem_base + BAR_OFF + s * 8u; };
-    auto empty_bar = [&](uint32_t s) { return smem_base + BAR_OFF + (STAGES + s) * 8u; };
-
-    const uint32_t warp = threadIdx.x >> 5;
-    const uint32_t lane = threadIdx.x & 31;
-    const int n0 = (int)blockIdx.x * GEMV_COLS;
-    const int k_begin = (int)blockIdx.y * p.k_per_cta;
-    const int k_end = min(p.K, k_begin + p.k_per_cta);
-    const int ntiles = k_end > k_begin ? (k_end - k_begin + GEMV_TILE_K - 1) / GEMV_TILE_K : 0;
-
-    if (threadIdx.x == 0) {
-        prefetch_tmap(&tmap_b);
-        for (uint32_t s = 0; s < STAGES; ++s) {
-            mbar_init(full_bar(s), 1);
-            mbar_init(empty_bar(s), GEMV_CONSUMER_WARPS);
-        }
-        fence_mbar_init();
-    }
-    __syncthreads();
-
-    float acc[8];
-#pragma unroll
-    for (int e = 0; e < 8; ++e) acc[e] = 0.f;
-
-    if (warp == GEMV_CONSUMER_WARPS) {
-        // ===== producer =====
-        if (elect_one()) {
-            uint32_t stage = 0, phase = 0;
-            for (int it = 0; it < ntiles; ++it) {
-                mbar_wait(empty_bar(stage), phase ^ 1u);
-                mbar_arrive_expect_tx(full_bar(stage), GEMV_TILE_BYTES);
-                tma_load_2d(smem_base + stage * GEMV_TILE_BYTES, &tmap_b, full_bar(stage), n0,
-                            k_begin + it * GEMV_TILE_K);
-                if (++stage == STAGES) { stage = 0; phase ^= 1u; }
-            }
-        }
-        __syncwarp();
-    } else {
-        // ===== consumers: warp w owns rows 8w..8w+7 of every tile =====
-        auto load_x = [&](int it) -> float {
-            const int k = k_begin + it * GEMV_TILE_K + (int)warp * 8 + (int)(lane & 7u);
-            return (it < ntiles && k < p.K) ? in_bits_to_f32<F16>(__ldg(p.x + k)) : 0.f;
-        };
-        uint32_t stage = 0, phase = 0;
-        float xv_next = load_x(0);
-        for (int it = 0; it < ntiles; ++it) {
-            const float xv = xv_next;
-            xv_next = load_x(it + 1);
-            mbar_wait(full_bar(stage), phase);
-            const uint8_t* tile = smem_gen + stage * GEMV_TILE_BYTES + warp * 8u * (GEMV_COLS * 2) + lane * 16u;
-            uint4 w[8];
-#pragma unroll
-            for (int r = 0; r < 8; ++r) w[r] = *reinterpret_cast<const uint4*>(tile + r * (GEMV_COLS * 2));
-#pragma unroll
-            for (int r = 0; r < 8; ++r) fma8<F16>(acc, w[r], __shfl_sync(0xffffffffu, xv, r));
-            __syncwarp();
-            if (lane == 0) mbar_arrive(empty_bar(stage));
-            if (++stage == STAGES) { stage = 0; phase ^= 1u; }
-        }
-    }
-    gemv_reduce_and_store<GEMV_CONSUMER_WARPS>(acc, red, part, warp, lane, warp < GEMV_CONSUMER_WARPS, p, n0);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -527,8 +454,10 @@ gemv_split_kernel(const __grid_constant__ CUtensorMap tmap_b, const __grid_const
                             if ((++rounds & 0xfffu) == 0) {
                                 if (t0 == 0) t0 = global_timer_ns();
                                 else if (global_timer_ns() - t0 > 4000000000ull) {
+#if TILEGEMM_WATCHDOG >= 2
                                     printf("tilegemm watchdog: split-K slot wait timed out (block %d,%d thread %d)\n",
                                            (int)blockIdx.x, (int)blockIdx.y, (int)threadIdx.x);
+#endif
                                     __trap();
                                 }
                             }

@@ -200,7 +200,7 @@ def test_large_k_integer_bit_exact():
 
 
 # ------------------------------------------------------------------ GEMV variants
-@pytest.mark.parametrize("variant", [1, 2, 3, 4])
+@pytest.mark.parametrize("variant", [2, 3, 4])
 @pytest.mark.parametrize("split", [0, 1, 3, 8])
 def test_gemv_variants_integer_bit_exact(variant, split):
     tg.tile_gemm_set_tuning(tg.TUNE_GEMV_VARIANT, variant)
@@ -212,7 +212,7 @@ def test_gemv_variants_integer_bit_exact(variant, split):
         check_bit_exact(got, ref, f"gemv v{variant} s{split} K={K} N={N}")
 
 
-@pytest.mark.parametrize("shape", [1, 2, 3, 4, 5, 6, 7, 8])
+@pytest.mark.parametrize("shape", [2, 4, 6])
 @pytest.mark.parametrize("cap", [0, 1, 3, 7, 100])
 @pytest.mark.parametrize("nopdl", [0, 1])
 @pytest.mark.parametrize("fix", [0, 1])
